@@ -1,0 +1,552 @@
+// anm_oracle.cpp -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+//
+// A plain, slow, single-threaded fp64 CPU transport of 0.511 MeV annihilation photons through a
+// voxel phantom, written step by step from the paper (arxiv 2111.11687, "PAPER.md") in the
+// reading DESIGN.md lists.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+// --impl reference legs may call it.  It shares no code with paper_2111_11687_b200/ (the CUDA
+// path): only input arrays produced by anm_inputs/ are common to both.
+//
+// Deliberate algorithmic differences from the CUDA path (same distributions, different routes,
+// so that the two check each other):
+//   decay voxel   : inverse CDF, binary search on the fp64 cumulative activity   (CUDA: alias table)
+//   direction     : Marsaglia (1972), the paper's choice, PAPER.md:L65          (CUDA: cos/phi)
+//   tracking      : exact voxel-boundary stepping (3-D DDA)                      (CUDA: Woodcock)
+//   Klein-Nishina : plain rejection from the uniform envelope on epsilon         (CUDA: Kahn-style)
+//   arithmetic    : fp64 throughout, fp64 tallies                                (CUDA: fp32)
+//
+// Parity pins (tests/test_oracle_*.py, -m "not gpu"): P1 Philox known answers; P3 KN sampler vs
+// closed-form CDF and mean energy transfer; P4 flight vs brute-force line integrals of mu and
+// exp(-mu x); P5 energy conservation; P6 infinite medium; P7 first-collision kerma; P8 source
+// chi^2 / isotropy; P9 Rayleigh -> Thomson limit; P10 batch sigma calibration; P11 symmetry;
+// P12 unit conversion.  No function here is "parity unpinned".
+//
+// Units: cm, MeV, g/cm^3.  Linear voxel index = ix + nx*(iy + ny*iz).
+
+#include <cmath>
+#include <cstdint>
+#include <cstdlib>
+#include <cstring>
+#include <limits>
+#include <vector>
+
+namespace {
+
+const double kElectronMassMeV = 0.51099895;   // "0.511 MeV", PAPER.md:L65 (reading C9)
+const double kHcKeVAngstrom = 12.398419843;
+const double kTwoPi = 6.283185307179586476925;
+
+// ---------------------------------------------------------------------------------------------
+// Philox4x32-10 (Salmon et al. 2011): the counter-based generator north_star (d) names.
+// key = (seed lo, seed hi); counter = (history lo, history hi, block number, 0).
+// ---------------------------------------------------------------------------------------------
+inline void philox_round(uint32_t c[4], const uint32_t k[2]) {
+    const uint64_t p0 = (uint64_t)0xD2511F53u * c[0];
+    const uint64_t p1 = (uint64_t)0xCD9E8D57u * c[2];
+    const uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+    const uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+    const uint32_t n0 = hi1 ^ c[1] ^ k[0];
+    const uint32_t n1 = lo1;
+    const uint32_t n2 = hi0 ^ c[3] ^ k[1];
+    const uint32_t n3 = lo0;
+    c[0] = n0; c[1] = n1; c[2] = n2; c[3] = n3;
+}
+
+void philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+    uint32_t c[4] = {ctr[0], ctr[1], ctr[2], ctr[3]};
+    uint32_t k[2] = {key[0], key[1]};
+    for (int r = 0; r < 10; ++r) {
+        philox_round(c, k);
+        k[0] += 0x9E3779B9u;
+        k[1] += 0xBB67AE85u;
+    }
+    for (int i = 0; i < 4; ++i) out[i] = c[i];
+}
+
+struct Rng {
+    uint32_t key[2];
+    uint32_t ctr[4];
+    uint32_t buf[4];
+    int have;
+    void start(uint64_t seed, uint64_t history) {
+        key[0] = (uint32_t)seed; key[1] = (uint32_t)(seed >> 32);
+        ctr[0] = (uint32_t)history; ctr[1] = (uint32_t)(history >> 32); ctr[2] = 0; ctr[3] = 0;
+        have = 0;
+    }
+    uint32_t u32() {
+        if (have == 0) { philox4x32_10(ctr, key, buf); ctr[2] += 1; have = 4; }
+        return buf[4 - have--];
+    }
+    // uniform on (0,1): (r + 0.5) 2^-32 (reading C14)
+    double uniform() { return ((double)u32() + 0.5) * (1.0 / 4294967296.0); }
+    // 64 random bits -> uniform on [0,1) with 53-bit resolution (voxel pick needs > 32 bits)
+    double uniform64() {
+        const uint64_t hi = u32(), lo = u32();
+        return (double)(((hi << 32) | lo) >> 11) * (1.0 / 9007199254740992.0);
+    }
+};
+
+}  // namespace
+
+extern "C" {
+
+struct OrcTables {
+    int32_t n_materials, n_energy;
+    double lnE_min, dlnE;
+    const float *mu_pe, *mu_compton, *mu_rayleigh;   // [n_materials][n_energy] cm^2/g
+    int32_t n_x2, pad_;
+    const float *ray_x2;                              // [n_x2]
+    const float *ray_cum;                             // [n_materials][n_x2]
+};
+
+struct OrcProblem {
+    int32_t nx, ny, nz, pad0_;
+    double dx, dy, dz;                     // cm
+    const uint8_t* material;               // [V]
+    const float* density;                  // [V] g/cm^3
+    const double* cdf;                     // [V] cumulative activity (orc_build_cdf) or null
+    int32_t use_point_source, pad1_;
+    double px, py, pz;                     // cm
+    const uint8_t* labels;                 // [V] or null
+    int32_t n_organs;
+    int32_t photons_per_decay;             // 1 | 2
+    int32_t rayleigh_on;
+    int32_t tracking;                      // 0 exact DDA (the oracle); 1 Woodcock (cross-check only)
+    double photon_cutoff;                  // MeV, 0.010
+    double positron_ke;                    // MeV, 0 or 0.2498
+    uint64_t n_total;                      // N decays of the whole run
+    int32_t n_batches, pad2_;
+    uint64_t seed;
+    OrcTables t;
+};
+
+struct OrcStats {
+    double emitted, deposited, escaped, max_history_residual;
+    uint64_t n_histories, n_photons, n_crossings, n_collisions, n_pe, n_compton, n_rayleigh,
+        n_escaped, n_cutoff, n_virtual;
+};
+
+// ------------------------------------------------------------------ P1
+void orc_philox4x32_10(const uint32_t* ctr, const uint32_t* key, uint32_t* out) {
+    philox4x32_10(ctr, key, out);
+}
+
+// Table reader (reading C19): linear interpolation in ln E on a uniform ln E grid.
+double orc_interp(const float* row, int n, double lnE_min, double dlnE, double E) {
+    const double t = (std::log(E) - lnE_min) / dlnE;
+    int i = (int)std::floor(t);
+    if (i < 0) i = 0;
+    if (i > n - 2) i = n - 2;
+    const double f = t - (double)i;
+    return (1.0 - f) * (double)row[i] + f * (double)row[i + 1];
+}
+
+// PAPER.md:L65 "The probability density distribution of the decay events ... is constructed through
+// a linear conversion of the PET value": p_v = a_v / sum(a).  cdf[v] = a_0 + ... + a_v.
+void orc_build_cdf(const float* activity, uint64_t n_voxels, double* cdf) {
+    double run = 0.0;
+    for (uint64_t v = 0; v < n_voxels; ++v) { run += (double)activity[v]; cdf[v] = run; }
+}
+
+// Inverse CDF: the first voxel v with cdf[v] > u * total  (u in [0,1)); zero-activity voxels have
+// zero-width intervals and are never returned.
+uint64_t orc_pick_voxel(const double* cdf, uint64_t n_voxels, double u) {
+    const double target = u * cdf[n_voxels - 1];
+    uint64_t lo = 0, hi = n_voxels - 1;
+    while (lo < hi) {
+        const uint64_t mid = lo + (hi - lo) / 2;
+        if (cdf[mid] > target) hi = mid; else lo = mid + 1;
+    }
+    return lo;
+}
+
+}  // extern "C"
+
+namespace {
+
+// Marsaglia (1972): x1,x2 ~ U(-1,1) until s = x1^2+x2^2 < 1;
+// d = (2 x1 sqrt(1-s), 2 x2 sqrt(1-s), 1-2s).
+void isotropic_marsaglia(Rng& g, double d[3]) {
+    for (;;) {
+        const double x1 = 2.0 * g.uniform() - 1.0, x2 = 2.0 * g.uniform() - 1.0;
+        const double s = x1 * x1 + x2 * x2;
+        if (s >= 1.0) continue;
+        const double r = std::sqrt(1.0 - s);
+        d[0] = 2.0 * x1 * r; d[1] = 2.0 * x2 * r; d[2] = 1.0 - 2.0 * s;
+        return;
+    }
+}
+
+// Klein-Nishina ("Compton scattering ... explicitly considered"; reading C3: free
+// electron).  eps = E'/E in [1/(1+2a), 1], a = E/mc^2, density f(eps) ~ eps + 1/eps - sin^2(theta),
+// cos(theta) = 1 + 1/a - 1/(a eps).  Plain rejection: eps uniform, accept with f / (eps_min + 1/eps_min)
+// (f <= eps + 1/eps, which decreases on (0,1]).
+double kn_sample_eps(Rng& g, double E) {
+    const double a = E / kElectronMassMeV;
+    const double eps_min = 1.0 / (1.0 + 2.0 * a);
+    const double bound = eps_min + 1.0 / eps_min;
+    for (;;) {
+        const double eps = eps_min + (1.0 - eps_min) * g.uniform();
+        const double c = 1.0 + 1.0 / a - 1.0 / (a * eps);
+        const double f = eps + 1.0 / eps - (1.0 - c * c);
+        if (g.uniform() * bound <= f) return eps;
+    }
+}
+
+double interp_grid(const float* x, const float* y, int n, double xq) {
+    // piecewise-linear y(x) on an increasing grid; xq clamped to the grid
+    if (xq <= (double)x[0]) return (double)y[0];
+    if (xq >= (double)x[n - 1]) return (double)y[n - 1];
+    int lo = 0, hi = n - 1;
+    while (hi - lo > 1) { const int mid = (lo + hi) / 2; if ((double)x[mid] <= xq) lo = mid; else hi = mid; }
+    const double f = (xq - (double)x[lo]) / ((double)x[hi] - (double)x[lo]);
+    return (1.0 - f) * (double)y[lo] + f * (double)y[hi];
+}
+
+// Rayleigh (north_star "optional Rayleigh"; reading C4): form-factor sampling.  T = x_max^2 = (E/hc)^2.
+// Draw x^2 from the tabulated piecewise-linear cumulative A(x^2) restricted to [0, T]; cos = 1 - 2 x^2/T;
+// accept with probability (1 + cos^2)/2.
+double rayleigh_sample_cos(Rng& g, const OrcTables& t, int m, double E) {
+    const double xm = E * 1000.0 / kHcKeVAngstrom;
+    const double T = xm * xm;
+    const float* cum = t.ray_cum + (size_t)m * t.n_x2;
+    const double A_T = interp_grid(t.ray_x2, cum, t.n_x2, T);
+    for (;;) {
+        const double target = g.uniform() * A_T;
+        // invert the piecewise-linear cumulative
+        int lo = 0, hi = t.n_x2 - 1;
+        while (hi - lo > 1) { const int mid = (lo + hi) / 2; if ((double)cum[mid] <= target) lo = mid; else hi = mid; }
+        const double c0 = cum[lo], c1 = cum[hi];
+        double x2 = (double)t.ray_x2[lo];
+        if (c1 > c0) x2 += (target - c0) / (c1 - c0) * ((double)t.ray_x2[hi] - (double)t.ray_x2[lo]);
+        if (x2 > T) x2 = T;
+        const double c = 1.0 - 2.0 * x2 / T;
+        if (g.uniform() * 2.0 <= 1.0 + c * c) return c;
+    }
+}
+
+// Rotate unit vector d by polar angle (cos_t) and azimuth phi about itself.
+void rotate(const double d[3], double cos_t, double phi, double out[3]) {
+    const double sin_t = std::sqrt(std::fmax(0.0, 1.0 - cos_t * cos_t));
+    const double cp = std::cos(phi), sp = std::sin(phi);
+    const double u = d[0], v = d[1], w = d[2];
+    double o[3];
+    if (std::fabs(w) < 0.99999) {
+        const double s = std::sqrt(1.0 - w * w);
+        o[0] = u * cos_t + sin_t * (u * w * cp - v * sp) / s;
+        o[1] = v * cos_t + sin_t * (v * w * cp + u * sp) / s;
+        o[2] = w * cos_t - sin_t * s * cp;
+    } else {
+        const double sg = w > 0 ? 1.0 : -1.0;
+        o[0] = sin_t * cp; o[1] = sin_t * sp; o[2] = sg * cos_t;
+    }
+    const double n = std::sqrt(o[0] * o[0] + o[1] * o[1] + o[2] * o[2]);
+    out[0] = o[0] / n; out[1] = o[1] / n; out[2] = o[2] / n;
+}
+
+struct Xs { double pe[8], co[8], ra[8], tot[8]; };   // per material, at the current energy
+
+void load_xs(const OrcProblem& p, double E, Xs& xs) {
+    const OrcTables& t = p.t;
+    for (int m = 0; m < t.n_materials; ++m) {
+        xs.pe[m] = orc_interp(t.mu_pe + (size_t)m * t.n_energy, t.n_energy, t.lnE_min, t.dlnE, E);
+        xs.co[m] = orc_interp(t.mu_compton + (size_t)m * t.n_energy, t.n_energy, t.lnE_min, t.dlnE, E);
+        xs.ra[m] = p.rayleigh_on
+            ? orc_interp(t.mu_rayleigh + (size_t)m * t.n_energy, t.n_energy, t.lnE_min, t.dlnE, E) : 0.0;
+        xs.tot[m] = xs.pe[m] + xs.co[m] + xs.ra[m];
+    }
+}
+
+inline int64_t vox_index(const OrcProblem& p, const int i[3]) {
+    return (int64_t)i[0] + (int64_t)p.nx * ((int64_t)i[1] + (int64_t)p.ny * (int64_t)i[2]);
+}
+
+// Exact flight: spend optical depth tau walking voxel to voxel along d.
+// pos/vox are updated to the interaction point.  Returns 1 = collision, 0 = left the grid
+// (reading C13: outside iff coordinate < 0 or >= L).
+int flight_dda(const OrcProblem& p, const Xs& xs, double pos[3], const double d[3], int vox[3],
+               double tau, double* dist_out, uint64_t* crossings) {
+    const double h[3] = {p.dx, p.dy, p.dz};
+    const int n[3] = {p.nx, p.ny, p.nz};
+    double tmax[3], tdelta[3];
+    int step[3];
+    for (int a = 0; a < 3; ++a) {
+        if (d[a] > 0.0) {
+            step[a] = 1; tdelta[a] = h[a] / d[a];
+            tmax[a] = ((double)(vox[a] + 1) * h[a] - pos[a]) / d[a];
+        } else if (d[a] < 0.0) {
+            step[a] = -1; tdelta[a] = -h[a] / d[a];
+            tmax[a] = ((double)vox[a] * h[a] - pos[a]) / d[a];
+        } else {
+            step[a] = 0; tdelta[a] = std::numeric_limits<double>::infinity();
+            tmax[a] = std::numeric_limits<double>::infinity();
+        }
+        if (tmax[a] < 0.0) tmax[a] = 0.0;
+    }
+    double t = 0.0;
+    for (;;) {
+        int a = 0;
+        if (tmax[1] < tmax[a]) a = 1;
+        if (tmax[2] < tmax[a]) a = 2;
+        const int64_t v = vox_index(p, vox);
+        const double mu = (double)p.density[v] * xs.tot[p.material[v]];
+        const double seg = tmax[a] - t;
+        if (tau <= mu * seg) {
+            t += tau / mu;
+            for (int k = 0; k < 3; ++k) pos[k] += t * d[k];
+            *dist_out = t;
+            return 1;
+        }
+        tau -= mu * seg;
+        t = tmax[a];
+        vox[a] += step[a];
+        if (crossings) ++*crossings;
+        if (vox[a] < 0 || vox[a] >= n[a]) {
+            for (int k = 0; k < 3; ++k) pos[k] += t * d[k];
+            *dist_out = t;
+            return 0;
+        }
+        tmax[a] += tdelta[a];
+    }
+}
+
+// Woodcock delta tracking against a global majorant -- NOT the oracle's tracking; kept only as a
+// statistical cross-check of flight_dda (tests) and selected with OrcProblem.tracking = 1.
+int flight_woodcock(const OrcProblem& p, const Xs& xs, double majorant, Rng& g, double pos[3],
+                    const double d[3], int vox[3], double* dist_out, uint64_t* n_virtual) {
+    const double h[3] = {p.dx, p.dy, p.dz};
+    const int n[3] = {p.nx, p.ny, p.nz};
+    double t = 0.0;
+    for (;;) {
+        const double s = -std::log(g.uniform()) / majorant;
+        t += s;
+        for (int k = 0; k < 3; ++k) {
+            pos[k] += s * d[k];
+            vox[k] = (int)std::floor(pos[k] / h[k]);
+        }
+        for (int k = 0; k < 3; ++k)
+            if (vox[k] < 0 || vox[k] >= n[k]) { *dist_out = t; return 0; }
+        const int64_t v = vox_index(p, vox);
+        const double mu = (double)p.density[v] * xs.tot[p.material[v]];
+        if (g.uniform() * majorant < mu) { *dist_out = t; return 1; }
+        if (n_virtual) ++*n_virtual;
+    }
+}
+
+struct Tally {
+    double* batch;           // [V] energy of the current batch (MeV)
+    double deposited;        // this history
+};
+
+inline void deposit(Tally& ty, int64_t v, double e) { ty.batch[v] += e; ty.deposited += e; }
+
+struct Workspace {
+    std::vector<double> rho_max;   // per material, for the Woodcock cross-check
+};
+
+// One photon from (pos, d, E) until absorbed, below cutoff, or out of the grid.
+// fc_* : first-collision record (P7), may be null.
+void transport_photon(const OrcProblem& p, const Workspace& ws, Rng& g, double pos[3], double d[3],
+                      int vox[3], double E, Tally& ty, OrcStats& st, double* escaped,
+                      double* fc_dist, double* fc_dep) {
+    Xs xs;
+    load_xs(p, E, xs);
+    bool first = true;
+    ++st.n_photons;
+    for (;;) {
+        double dist = 0.0;
+        int hit;
+        if (p.tracking == 0) {
+            const double tau = -std::log(g.uniform());
+            hit = flight_dda(p, xs, pos, d, vox, tau, &dist, &st.n_crossings);
+        } else {
+            double maj = 0.0;
+            for (int m = 0; m < p.t.n_materials; ++m) maj = std::fmax(maj, ws.rho_max[m] * xs.tot[m]);
+            hit = flight_woodcock(p, xs, maj, g, pos, d, vox, &dist, &st.n_virtual);
+        }
+        if (!hit) {   // "photons are killed at the phantom boundary" (BASELINE.json cfg0)
+            *escaped += E;
+            ++st.n_escaped;
+            if (first && fc_dist) { *fc_dist = -1.0; *fc_dep = 0.0; }
+            return;
+        }
+        ++st.n_collisions;
+        const int64_t v = vox_index(p, vox);
+        const int m = p.material[v];
+        // interaction type proportional to the partial coefficients
+        const double u = g.uniform() * xs.tot[m];
+        double dep_here = 0.0;
+        bool alive = true;
+        if (u < xs.pe[m]) {
+            // photoelectric: all energy local (reading C5)
+            ++st.n_pe;
+            dep_here = E;
+            alive = false;
+        } else if (u < xs.pe[m] + xs.co[m]) {
+            ++st.n_compton;
+            const double a = E / kElectronMassMeV;
+            const double eps = kn_sample_eps(g, E);
+            const double cos_t = 1.0 + 1.0 / a - 1.0 / (a * eps);
+            const double phi = kTwoPi * g.uniform();
+            dep_here = E * (1.0 - eps);      // recoil electron deposited locally (north_star; reading C2)
+            E *= eps;
+            double nd[3];
+            rotate(d, cos_t, phi, nd);
+            d[0] = nd[0]; d[1] = nd[1]; d[2] = nd[2];
+            if (E < p.photon_cutoff) {       // below cutoff, remaining energy deposited locally
+                dep_here += E;
+                ++st.n_cutoff;
+                alive = false;
+            } else {
+                load_xs(p, E, xs);
+            }
+        } else {
+            ++st.n_rayleigh;
+            const double cos_t = rayleigh_sample_cos(g, p.t, m, E);
+            const double phi = kTwoPi * g.uniform();
+            double nd[3];
+            rotate(d, cos_t, phi, nd);
+            d[0] = nd[0]; d[1] = nd[1]; d[2] = nd[2];
+        }
+        if (dep_here > 0.0) deposit(ty, v, dep_here);
+        if (first && fc_dist) { *fc_dist = dist; *fc_dep = dep_here; }
+        first = false;
+        if (!alive) return;
+    }
+}
+
+void sample_source(const OrcProblem& p, Rng& g, double pos[3], double d[3], int vox[3]) {
+    const double h[3] = {p.dx, p.dy, p.dz};
+    if (p.use_point_source) {
+        pos[0] = p.px; pos[1] = p.py; pos[2] = p.pz;
+        for (int a = 0; a < 3; ++a) vox[a] = (int)std::floor(pos[a] / h[a]);   // reading C13
+    } else {
+        const uint64_t V = (uint64_t)p.nx * p.ny * p.nz;
+        const uint64_t v = orc_pick_voxel(p.cdf, V, g.uniform64());
+        vox[0] = (int)(v % (uint64_t)p.nx);
+        vox[1] = (int)((v / (uint64_t)p.nx) % (uint64_t)p.ny);
+        vox[2] = (int)(v / ((uint64_t)p.nx * (uint64_t)p.ny));
+        for (int a = 0; a < 3; ++a) pos[a] = ((double)vox[a] + g.uniform()) * h[a];   // uniform in the voxel (C11)
+    }
+    isotropic_marsaglia(g, d);
+}
+
+}  // namespace
+
+extern "C" {
+
+// ----------------------------------------------------------------- exposed pieces (pins)
+void orc_isotropic_many(uint64_t seed, uint64_t n, double* dirs /*[n][3]*/) {
+    for (uint64_t i = 0; i < n; ++i) { Rng g; g.start(seed, i); isotropic_marsaglia(g, dirs + 3 * i); }
+}
+
+void orc_kn_sample_many(double E, uint64_t seed, uint64_t n, double* eps) {
+    for (uint64_t i = 0; i < n; ++i) { Rng g; g.start(seed, i); eps[i] = kn_sample_eps(g, E); }
+}
+
+void orc_rayleigh_sample_many(const OrcTables* t, int material, double E, uint64_t seed, uint64_t n,
+                              double* cos_out) {
+    for (uint64_t i = 0; i < n; ++i) { Rng g; g.start(seed, i); cos_out[i] = rayleigh_sample_cos(g, *t, material, E); }
+}
+
+void orc_rotate(const double* d, double cos_t, double phi, double* out) { rotate(d, cos_t, phi, out); }
+
+void orc_sample_source_many(const OrcProblem* p, uint64_t h0, uint64_t n, double* pos /*[n][3]*/,
+                            double* dirs /*[n][3]*/, int64_t* voxel /*[n]*/) {
+    for (uint64_t i = 0; i < n; ++i) {
+        Rng g; g.start(p->seed, h0 + i);
+        int vox[3];
+        sample_source(*p, g, pos + 3 * i, dirs + 3 * i, vox);
+        voxel[i] = vox_index(*p, vox);
+    }
+}
+
+// One exact flight with a GIVEN optical depth tau from pos along d at energy E.  Returns 1 and the
+// interaction point/voxel/distance, or 0 (escaped; out_pos = exit point).
+int orc_flight(const OrcProblem* p, const double* pos, const double* d, double E, double tau,
+               double* out_pos, int64_t* out_voxel, double* out_dist) {
+    Xs xs;
+    load_xs(*p, E, xs);
+    const double h[3] = {p->dx, p->dy, p->dz};
+    double q[3] = {pos[0], pos[1], pos[2]};
+    int vox[3];
+    for (int a = 0; a < 3; ++a) vox[a] = (int)std::floor(q[a] / h[a]);
+    const int hit = flight_dda(*p, xs, q, d, vox, tau, out_dist, nullptr);
+    out_pos[0] = q[0]; out_pos[1] = q[1]; out_pos[2] = q[2];
+    *out_voxel = hit ? vox_index(*p, vox) : -1;
+    return hit;
+}
+
+// ----------------------------------------------------------------- the run
+// Histories [h0, h1) of a run of n_total decays in n_batches batches; h0 and h1 must be batch
+// boundaries (batch b = h / (n_total / n_batches); reading C15: n_total % n_batches == 0).
+//   sum[V], sumsq[V]       += per-batch voxel energies x_{b,i} and x_{b,i}^2 (MeV, MeV^2)
+//   organ_batch[B][n_organs+1] = sum over the organ's voxels of x_{b,i} / (rho_i V_vox)  (MeV/g); column 0 = unlabelled
+//   fc_dist/fc_dep[h1-h0]  first-collision distance (cm; -1 = escaped uncollided) and deposit of photon A (may be null)
+// Returns 0, or -1 on bad arguments.
+int orc_run(const OrcProblem* pp, uint64_t h0, uint64_t h1, double* sum, double* sumsq,
+            double* organ_batch, OrcStats* stats, double* fc_dist, double* fc_dep) {
+    const OrcProblem& p = *pp;
+    if (p.n_batches < 1 || p.n_total == 0 || p.n_total % (uint64_t)p.n_batches) return -1;
+    const uint64_t nb = p.n_total / (uint64_t)p.n_batches;
+    if (h0 % nb || h1 % nb || h1 < h0 || h1 > p.n_total) return -1;
+    if (!p.use_point_source && !p.cdf) return -1;
+    if (p.photons_per_decay != 1 && p.photons_per_decay != 2) return -1;
+    const uint64_t V = (uint64_t)p.nx * p.ny * p.nz;
+    const double vox_cm3 = p.dx * p.dy * p.dz;
+
+    Workspace ws;
+    ws.rho_max.assign(8, 0.0);
+    if (p.tracking == 1)
+        for (uint64_t v = 0; v < V; ++v)
+            ws.rho_max[p.material[v]] = std::fmax(ws.rho_max[p.material[v]], (double)p.density[v]);
+
+    std::vector<double> batch(V, 0.0);
+    Tally ty{batch.data(), 0.0};
+    OrcStats st;
+    std::memset(&st, 0, sizeof st);
+
+    for (uint64_t b = h0 / nb; b < h1 / nb; ++b) {
+        for (uint64_t h = b * nb; h < (b + 1) * nb; ++h) {
+            Rng g;
+            g.start(p.seed, h);
+            double pos[3], d[3];
+            int vox[3];
+            sample_source(p, g, pos, d, vox);
+            double emitted = 0.0, escaped = 0.0;
+            ty.deposited = 0.0;
+            if (p.positron_ke > 0.0) {   // constant positron kinetic energy deposited in the decay voxel (C10)
+                emitted += p.positron_ke;
+                deposit(ty, vox_index(p, vox), p.positron_ke);
+            }
+            // two photons of equal energy (0.511 MeV) in opposite directions
+            for (int k = 0; k < p.photons_per_decay; ++k) {
+                double q[3] = {pos[0], pos[1], pos[2]};
+                double dd[3] = {k == 0 ? d[0] : -d[0], k == 0 ? d[1] : -d[1], k == 0 ? d[2] : -d[2]};
+                int vv[3] = {vox[0], vox[1], vox[2]};
+                emitted += kElectronMassMeV;
+                const bool rec = (k == 0 && fc_dist != nullptr);
+                transport_photon(p, ws, g, q, dd, vv, kElectronMassMeV, ty, st, &escaped,
+                                 rec ? fc_dist + (h - h0) : nullptr, rec ? fc_dep + (h - h0) : nullptr);
+            }
+            st.emitted += emitted; st.deposited += ty.deposited; st.escaped += escaped;
+            const double res = std::fabs(ty.deposited + escaped - emitted);
+            if (res > st.max_history_residual) st.max_history_residual = res;
+            ++st.n_histories;
+        }
+        // fold the batch
+        double* ob = organ_batch ? organ_batch + (size_t)b * (size_t)(p.n_organs + 1) : nullptr;
+        for (uint64_t v = 0; v < V; ++v) {
+            const double x = batch[v];
+            if (x != 0.0) {
+                sum[v] += x;
+                sumsq[v] += x * x;
+                if (ob) ob[p.labels ? p.labels[v] : 0] += x / ((double)p.density[v] * vox_cm3);
+                batch[v] = 0.0;
+            }
+        }
+    }
+    if (stats) *stats = st;
+    return 0;
+}
+
+}  // extern "C"
