@@ -190,6 +190,15 @@ def _trilinear_activity(nx, ny, nz, dx, dy, dz, z_stretch):
     return act
 
 
+def _radial_shells(n, d_mm, centre_mm, width_mm, n_shells):
+    """Label volume of concentric shells around centre_mm (label 1 = innermost), by voxel-centre distance;
+    the 'dose-distance curve' of PAPER.md:L109 read out through the organ tally."""
+    c = (np.arange(n) + 0.5) * d_mm
+    Z, Y, X = np.meshgrid(c - centre_mm[2], c - centre_mm[1], c - centre_mm[0], indexing="ij")
+    k = np.floor(np.sqrt(X * X + Y * Y + Z * Z) / width_mm).astype(np.int64) + 1
+    return np.where(k <= n_shells, k, 0).astype(np.uint8)
+
+
 def _base(name, shape_xyz, spacing_mm, n_decays, seed, n_batches, photons_per_decay, positron_ke=0.0):
     return {
         "name": name, "shape": tuple(int(v) for v in shape_xyz),
@@ -211,6 +220,8 @@ def make_config(k: int, scale: int = 1) -> dict:
         c["material"] = np.full((n, n, n), WATER, np.uint8)
         c["density"] = quantize_density(np.full((n, n, n), 1.0))
         c["point_source_mm"] = (64.0, 64.0, 64.0)          # exact centre (a voxel corner, C11)
+        c.update(labels=_radial_shells(n, d, (64.0, 64.0, 64.0), 8.0, 8), n_organs=8,
+                 organ_names=["shell_%02d" % i for i in range(8)])
     elif k == 1:
         n, d = 100 // s, 2.0 * s
         c = _base(CONFIG_NAMES[1], (n, n, n), (d, d, d), 100_000_000, 1, 100, 1)
@@ -219,6 +230,9 @@ def make_config(k: int, scale: int = 1) -> dict:
         act = np.zeros((n, n, n), np.float32)
         act[n // 2, n // 2, n // 2] = 1.0                   # the paper's construction
         c["activity"] = act
+        ctr = ((n // 2 + 0.5) * d,) * 3
+        c.update(labels=_radial_shells(n, d, ctr, 4.0, 25), n_organs=25,
+                 organ_names=["shell_%02d" % i for i in range(25)])
     elif k == 2:
         n, d = 128 // s, 3.0 * s
         t = n // 4

@@ -1,0 +1,289 @@
+#!/usr/bin/env python
+"""bench.py -- decays/s of the whole hot path on the synthetic patient phantom (BASELINE.json cfg3).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--decays D] [--impl reference]
+
+One step = one anm_run of D decays (default 1e9, the north-star target) on cfg3 (256x256x400 voxels of
+2x2x4 mm, 27 organs, pairs of 0.511 MeV photons + 0.2498 MeV positron energy, 100 batches): source sampling,
+Woodcock transport, tally, 100 batch folds with organ reduction, finalize -- every SURVEY.md §8(a) row.
+`value` times K such runs with all inputs resident in HBM (CUDA events on the launching stream, max over ranks);
+`e2e` times the same job through the C ABI from HOST buffers (phantom / activity / label upload, set-up, run,
+dose + uncertainty + organ read-back to the host).  `roofline` is the ALU/issue roofline of the transport kernel
+(DESIGN.md §6); `cpu_baseline` is the oracle timed on this box's host cores on a bounded sample.
+With --impl reference the oracle itself is the timed arm (same metric / config, bounded sample per step).
+Under torchrun (N > 1) each rank simulates its own whole-batch shard of one logical run of N*D decays
+(history_offset = rank*D); no data-path collective, scaling = weak.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+WORKLOAD = "cfg3_patient 256x256x400 @2x2x4mm, 27 organs, pairs+positron KE, 100 batches"
+
+# algorithmic thread-instructions per event (what the method's arithmetic needs, counted from the
+# definitions: Philox4x32-10 = 100 integer ops per 4 words, ...), multiplied by the measured events per decay.
+INSTR_SUBSTEP = 84.0     # half a Philox block, log, 3 FMA, voxel index, texel fetch + unpack, table lerp, accept test
+INSTR_COMPTON_TRY = 210.0
+INSTR_RAYLEIGH_TRY = 180.0
+INSTR_SOURCE = 260.0
+INSTR_PE = 4.0
+LANES_PER_SM_PER_CLK = 128.0   # 4 SMSP x 32 lanes, one instruction per SMSP per clock
+N_SM = 148
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=subprocess.PIPE, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self) -> dict:
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.t.join(timeout=2)
+        sm = sorted(float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit())
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(len(r) > 3 + i and r[3 + i].lower().startswith("active") for r in self.rows)]
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        pw = [float(r[2]) for r in self.rows if len(r) > 2 and r[2].replace(".", "").isdigit()]
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx[0] if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": reasons}
+
+
+def run_reference(args, rank: int):
+    """The oracle as the timed arm: cfg3, each step a bounded sample of the workload on the host cores."""
+    if rank != 0:
+        return
+    import anm_inputs
+    from oracle import anm_oracle
+    cores = os.cpu_count() or 1
+    cfg = anm_inputs.make_config(3)
+    tables = anm_inputs.make_tables()
+    n = cores * args.ref_decays_per_core
+    o = anm_oracle.Oracle(cfg, tables, n_decays=n, n_batches=cores, seed=1042)
+    for _ in range(args.warmup):
+        o.run_parallel(cores)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        o.run_parallel(cores)
+    dt = time.perf_counter() - t0
+    val = n * args.steps / dt
+    sample = "%d decays per step (%d per core) of cfg3, %d single-threaded processes, one batch each" % (n, args.ref_decays_per_core, cores)
+    print(json.dumps({
+        "impl": "reference", "metric": "decays/s (18F, patient phantom)", "value": val, "unit": "decays/s",
+        "sec_per_1e9_decays": 1e9 / val, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": {"workload": WORKLOAD, "decays_per_step": n, "sample": sample},
+        "cpu_baseline": {"value": val, "unit": "decays/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": "decays/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--decays", type=float, default=1e9, help="decays per step per GPU")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--ref-decays-per-core", type=int, default=100_000)
+    ap.add_argument("--cpu-baseline-decays-per-core", type=int, default=400_000)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        return run_reference(args, rank)
+
+    import numpy as np
+    import torch
+    import anm_inputs
+    from paper_2111_11687_b200 import Simulation
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    dev = torch.device("cuda", local_rank)
+    torch.cuda.set_device(dev)
+
+    cfg = anm_inputs.make_config(3)
+    tables = anm_inputs.make_tables()
+    D = int(args.decays)
+    B = cfg["n_batches"]
+    V = int(np.prod(cfg["shape"]))
+    opts = dict(n_batches=B, photons_per_decay=2, rayleigh_on=1, photon_cutoff_MeV=0.010,
+                positron_ke_MeV=cfg["positron_ke_mev"], history_offset=rank * D)
+
+    # ---- device-resident arm ----------------------------------------------------------------------------
+    stream = torch.cuda.Stream(device=dev)
+    mat = torch.from_numpy(cfg["material"]).to(dev)
+    rho = torch.from_numpy(cfg["density"]).to(dev)
+    act = torch.from_numpy(cfg["activity"]).to(dev)
+    lab = torch.from_numpy(cfg["labels"]).to(dev)
+    sim = Simulation(local_rank)
+    with torch.cuda.stream(stream):
+        sim.set_stream(stream)
+        sim.set_grid(cfg["shape"], cfg["spacing_mm"])
+        sim.load_phantom(mat, rho)
+        sim.load_activity(act)
+        sim.load_organs(lab, cfg["n_organs"])
+        sim.set_physics_tables(tables)
+        # events per decay (properties of the method + majorant), from a short counted run
+        sim.set_options(collect_stats=1, **opts)
+        n_cnt = B * 100_000
+        sim.run(n_cnt, cfg["seed"])
+        cnt = sim.get_stats()
+        per_decay = {k: cnt[k] / n_cnt for k in ("n_steps", "n_real", "n_pe", "n_compton", "n_rayleigh")}
+        sim.set_options(collect_stats=0, **opts)
+        for _ in range(args.warmup):
+            sim.run(D, cfg["seed"])
+        if dist:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+        clocks = ClockSampler(local_rank)
+        clocks.start()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ms_t = ms_f = ms_fin = 0.0
+        launches = 0
+        e0.record(stream)
+        for _ in range(args.steps):
+            sim.run(D, cfg["seed"])
+            st = sim.get_stats()
+            ms_t += st["ms_transport"]; ms_f += st["ms_fold"]; ms_fin += st["ms_finalize"]
+            launches += st["n_launches"]
+        e1.record(stream)
+        torch.cuda.synchronize(dev)
+        if dist:
+            dist.barrier()
+        clk = clocks.stop()
+    ms_total = e0.elapsed_time(e1)
+    if dist:
+        t = torch.tensor([ms_total], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    value = world * D * args.steps / (ms_total * 1e-3)
+
+    # ---- roofline of the dominant kernel (transport): ALU / issue bound, DESIGN.md §6 ------------------------
+    compton_tries = per_decay["n_compton"] * 1.15
+    instr_per_decay = (per_decay["n_steps"] * INSTR_SUBSTEP + compton_tries * INSTR_COMPTON_TRY +
+                       per_decay["n_rayleigh"] * INSTR_RAYLEIGH_TRY * 1.4 + per_decay["n_pe"] * INSTR_PE + INSTR_SOURCE)
+    launches_transport = B * args.steps
+    sec_per_launch = ms_t * 1e-3 / launches_transport
+    achieved = instr_per_decay * (D / B) / sec_per_launch / 1e9                     # G thread-instr / s
+    sm_max = clk.get("sm_max_mhz") or 1965.0
+    peak = N_SM * LANES_PER_SM_PER_CLK * sm_max * 1e6 / 1e9
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "transport_dram_bytes_per_launch.json")
+    if os.path.exists(tpath):
+        try:
+            traffic = json.load(open(tpath)).get("dram_bytes_per_launch")
+        except Exception:
+            traffic = None
+    roofline = {"bound": "alu", "kernel": "transport_kernel", "achieved": achieved, "peak": peak, "unit": "Gthread-instr/s",
+                "frac": achieved / peak, "traffic": traffic,
+                "peak_source": "148 SM x 4 SMSP x 32 lanes x %.0f MHz (clocks.max.sm), DESIGN.md §6" % sm_max,
+                "instr_per_decay_algorithmic": instr_per_decay, "events_per_decay": per_decay,
+                "avg_launch_ms": sec_per_launch * 1e3, "share_of_step": ms_t / max(ms_t + ms_f + ms_fin, 1e-9),
+                "texel_bytes_per_decay": 4.0 * per_decay["n_steps"], "tally_bytes_per_decay": 8.0 * (per_decay["n_real"] - per_decay["n_rayleigh"] + 1)}
+
+    # ---- end to end through the C ABI from host buffers ----------------------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        hm, hr = torch.from_numpy(cfg["material"]).pin_memory(), torch.from_numpy(cfg["density"]).pin_memory()
+        ha, hl = torch.from_numpy(cfg["activity"]).pin_memory(), torch.from_numpy(cfg["labels"]).pin_memory()
+        out_d, out_u = torch.empty(V, dtype=torch.float32).pin_memory(), torch.empty(V, dtype=torch.float32).pin_memory()
+        if dist:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+        t0 = time.perf_counter()
+        with Simulation(local_rank) as s2:
+            s2.set_grid(cfg["shape"], cfg["spacing_mm"])
+            s2.load_phantom(hm, hr)
+            s2.load_activity(ha)
+            s2.load_organs(hl, cfg["n_organs"])
+            s2.set_physics_tables(tables)
+            s2.set_options(**opts)
+            s2.run(D, cfg["seed"])
+            s2.get_dose(out_d)
+            s2.get_uncertainty(out_u)
+            organs = s2.get_organ_doses()
+            st2 = s2.get_stats()
+        torch.cuda.synchronize(dev)
+        dt = time.perf_counter() - t0
+        if dist:
+            t = torch.tensor([dt], device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        assert float(out_d.sum()) > 0 and organs["mean_Gy_per_decay"].max() > 0
+        e2e = {"value": world * D / dt, "unit": "decays/s", "h2d_bytes_per_step": V * (1 + 4 + 4 + 1),
+               "d2h_bytes_per_step": V * 8 + 27 * 56, "seconds": dt, "ms_setup_device": st2["ms_setup"],
+               "what": "anm_set_grid + load_phantom/activity/organs (host) + tables + anm_run + get_dose + get_uncertainty + get_organ_doses (host)"}
+
+    if rank != 0:
+        if dist:
+            dist.destroy_process_group()
+        return
+
+    # ---- the oracle beside it, on this box's host cores (bounded sample) ------------------------------------
+    cpu = None
+    if not args.no_cpu_baseline and world == 1:
+        from oracle import anm_oracle
+        cores = os.cpu_count() or 1
+        n = cores * args.cpu_baseline_decays_per_core
+        o = anm_oracle.Oracle(cfg, tables, n_decays=n, n_batches=cores, seed=1042)
+        r = o.run_parallel(cores)
+        cpu = {"value": n / r["seconds"], "unit": "decays/s", "cores": r["cores"], "kind": "oracle",
+               "sample": "%d decays of cfg3 (%d per core), one batch per single-threaded process, %.1f s wall" % (n, args.cpu_baseline_decays_per_core, r["seconds"]),
+               "per_core": n / r["cpu_seconds"]}
+
+    print(json.dumps({
+        "metric": "decays/s (18F, patient phantom)", "value": value, "unit": "decays/s",
+        "sec_per_1e9_decays": 1e9 / value, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "decays_per_step_per_gpu": D, "seed": cfg["seed"],
+                   "l2": "working set (texels 105 MB + batch tally 105 MB + sum/sumsq 210 MB) exceeds the 126 MB L2; no flush needed",
+                   "multi_gpu": "whole-batch shards via history_offset, no collective" if world > 1 else "single GPU"},
+        "clocks": clk, "e2e": e2e, "gpu_launches": int(launches),
+        "phase_ms_per_step": {"transport": ms_t / args.steps, "fold": ms_f / args.steps, "finalize": ms_fin / args.steps},
+        "roofline": roofline, "cpu_baseline": cpu,
+        "paper_context": "ARCHER-NM on a Titan V: 1e9 decays in <0.5 min (>=3.3e7 decays/s), GATE 376 min (PAPER.md:L117); other hardware, other phantom, electron transport on",
+    }))
+    if dist:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

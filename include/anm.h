@@ -1,0 +1,148 @@
+/* anm.h -- C ABI of libanm.so: voxel Monte Carlo dose from annihilation photons on one B200.
+ *
+ * What it computes (arxiv 2111.11687 "ARCHER-NM", cited as PAPER.md:L<line>):
+ *   PAPER.md:L65  a voxel phantom of (material, density) from CT; a decay pdf that is a linear
+ *                 conversion of the PET voxel value; each decay -> two 0.511 MeV photons in opposite,
+ *                 isotropically distributed directions.
+ *   PAPER.md:L67  photoelectric absorption and Compton scattering (pair production impossible below
+ *                 1.02 MeV); a photon is followed until its energy falls below the 10 keV cutoff, the
+ *                 remaining energy is deposited locally; dose and its statistical uncertainty are
+ *                 scored per voxel, maps have the size of the phantom.
+ *   PAPER.md:L71-75 (Eq. 1)  dose rate = D / N_evts x A(t_s).
+ *   PAPER.md:L91-96 (Eq. 2,3) organ mean dose = unweighted mean over the organ's voxels; organ
+ *                 uncertainty = RMS of the voxel uncertainties.
+ * Readings where the paper is silent or BASELINE.json's north_star binds: secondary
+ * electrons are deposited locally; uncertainty by the batch method; Woodcock delta tracking; optional
+ * Rayleigh scattering; optional constant positron kinetic energy deposited in the decay voxel;
+ * Philox4x32-10 keyed by (seed, history index).
+ *
+ * Conventions
+ *   - Every function returns an anm_status (0 = ok, negative = error); nothing throws or exits.
+ *     anm_last_error(ctx) returns a ctx-owned, NUL-terminated message valid until the next call on ctx.
+ *   - Volumes are dense arrays of nx*ny*nz elements, linear index = ix + nx*(iy + ny*iz); voxel (ix,iy,iz)
+ *     spans [ix*dx,(ix+1)*dx) x ... in mm from the grid corner (0,0,0).  A point exactly on a face belongs
+ *     to the upper voxel; a photon is outside (killed, energy counted as escaped) iff a coordinate is < 0
+ *     or >= the grid length.
+ *   - `on_device` = 0: the pointer is host memory (borrowed for the duration of the call, copied);
+ *     `on_device` = 1: it is a CUDA device pointer on the ctx's device (e.g. torch.Tensor.data_ptr()),
+ *     read / written on the ctx stream.  The caller owns every buffer it passes in or receives into.
+ *   - The ctx owns all device memory it allocates and frees it in anm_destroy.  A ctx is not thread-safe;
+ *     separate ctxs are independent.  There is no global state, no CPU fallback and no other backend:
+ *     every call that needs the GPU fails with ANM_E_CUDA when there is none.
+ *   - Units: mm at this interface for lengths, MeV for energies, g/cm^3, cm^2/g, Gy, Bq.
+ */
+#ifndef ANM_H_
+#define ANM_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct anm_ctx anm_ctx;
+
+typedef enum {
+    ANM_OK = 0,
+    ANM_E_ARG = -1,          /* invalid argument (range, NaN, size mismatch, N % n_batches != 0, ...) */
+    ANM_E_STATE = -2,        /* call order: something required has not been set yet                   */
+    ANM_E_CUDA = -3,         /* a CUDA call failed; the CUDA error string is in anm_last_error        */
+    ANM_E_NOMEM = -4,        /* host or device allocation failed                                      */
+    ANM_E_UNSUPPORTED = -5   /* valid request this build does not implement                           */
+} anm_status;
+
+#define ANM_MAX_MATERIALS 8
+#define ANM_MAX_ORGANS 255
+
+/* Photon interaction data (set once; copied).  All tables are sampled on a grid uniform in ln(E/MeV):
+ * lnE_k = lnE_min + k*dlnE, k = 0..n_energy-1, and are read by linear interpolation in ln E.  The grid
+ * must cover [photon_cutoff_MeV, 0.51099895 MeV].
+ *   mu_pe, mu_compton, mu_rayleigh : [n_materials][n_energy] mass attenuation coefficients, cm^2/g (> 0)
+ *   ray_x2  : [n_x2]  increasing momentum-transfer grid x^2 (Angstrom^-2), ray_x2[0] = 0, last >= (E_max/hc)^2
+ *   ray_cum : [n_materials][n_x2]  integral_0^{x^2} F_m^2 dt (any positive scale), non-decreasing;
+ *             the Rayleigh angle is sampled from this piecewise-linear cumulative restricted to
+ *             [0, (E/hc)^2], cos(theta) = 1 - 2 x^2 / (E/hc)^2, accepted with probability (1+cos^2)/2. */
+typedef struct {
+    int32_t n_materials;      /* 1..ANM_MAX_MATERIALS */
+    int32_t n_energy;         /* 2..1024 */
+    double lnE_min, dlnE;
+    const float* mu_pe;
+    const float* mu_compton;
+    const float* mu_rayleigh;
+    int32_t n_x2;             /* 2..1024 */
+    int32_t reserved0;
+    const float* ray_x2;
+    const float* ray_cum;
+} anm_tables;
+
+typedef struct {
+    int32_t n_batches;          /* >= 2; n_decays must be a multiple (batch-method uncertainty)        */
+    int32_t photons_per_decay;  /* 2 = annihilation pair; 1 = single photon per history  */
+    int32_t rayleigh_on;        /* 0 | 1                                                                */
+    int32_t zero_air_dose;      /* 1: dose getters return 0 in voxels of material 0     */
+    double photon_cutoff_MeV;   /* 0.010                                                  */
+    double positron_ke_MeV;     /* 0, or e.g. 0.2498: deposited in the decay voxel                      */
+    int32_t schedule;           /* 0 auto, 1 history-based persistent lanes; 2 (event-based) unsupported */
+    int32_t collect_stats;      /* 1: fill the counters and escaped energy of anm_stats (slower)         */
+    int32_t warp_aggregate;     /* 1: merge same-voxel deposits within a warp before the atomic          */
+    int32_t hull_majorant;      /* 1: low-density margin outside the phantom's hull gets its own majorant */
+    uint64_t history_offset;    /* index of the first history: anm_run simulates offset .. offset+n_decays-1
+                                   (multi-GPU sharding of one logical run by whole batches); default 0      */
+} anm_options;
+
+typedef struct {
+    double mean_Gy_per_decay;          /* Eq. 2: (1/N_o) sum of voxel doses             */
+    double sigma_mean;                 /* batch standard error of that mean (absolute, Gy per decay)    */
+    double rms_voxel_rel_sigma;        /* Eq. 3 over the organ's voxels with dose > 0    */
+    double mass_weighted_Gy_per_decay; /* organ energy / organ mass                                     */
+    double mass_g;
+    uint64_t n_voxels, n_voxels_nonzero;
+} anm_organ;
+
+typedef struct {
+    double emitted_MeV, deposited_MeV, escaped_MeV;   /* escaped and the counters need collect_stats   */
+    uint64_t n_decays, n_steps, n_real, n_pe, n_compton, n_rayleigh, n_escaped, n_cutoff;
+    double ms_transport, ms_fold, ms_finalize, ms_setup;   /* device time of the last anm_run / last setup */
+    uint64_t n_launches;                                   /* kernels launched by the last anm_run         */
+} anm_stats;
+
+/* --- lifetime ---------------------------------------------------------------------------------- */
+int anm_create(anm_ctx** out, int cuda_device);    /* ANM_E_CUDA if the device cannot be used          */
+int anm_destroy(anm_ctx* c);                       /* frees everything the ctx allocated; NULL is ok   */
+const char* anm_last_error(const anm_ctx* c);
+int anm_set_stream(anm_ctx* c, void* cuda_stream); /* cudaStream_t; NULL = the default stream          */
+
+/* --- inputs (any order; set_grid first) -------------------------------------------------------- */
+int anm_set_grid(anm_ctx* c, int nx, int ny, int nz, double dx_mm, double dy_mm, double dz_mm);
+/* material[V] < n_materials (checked at run), density[V] in [0, 16) g/cm^3, stored on a 2^-20 grid. */
+int anm_load_phantom(anm_ctx* c, const uint8_t* material, const float* density_g_cm3, int on_device);
+/* activity[V] >= 0, finite, arbitrary units, not all zero: decay pdf = activity / sum;
+ * the decay point is uniform inside the chosen voxel. */
+int anm_load_activity(anm_ctx* c, const float* activity, int on_device);
+/* Replaces the activity map: every decay happens at this point (BASELINE.json cfg0). */
+int anm_set_point_source(anm_ctx* c, double x_mm, double y_mm, double z_mm);
+/* labels[V]: 0 = none, 1..n_organs (n_organs <= ANM_MAX_ORGANS).  Optional. */
+int anm_load_organs(anm_ctx* c, const uint8_t* labels, int n_organs, int on_device);
+int anm_set_physics_tables(anm_ctx* c, const anm_tables* t);
+int anm_set_options(anm_ctx* c, const anm_options* o);
+int anm_default_options(anm_options* o);   /* 100 batches, pairs, Rayleigh on, cutoff 0.010, no positron KE */
+
+/* --- run --------------------------------------------------------------------------------------- */
+/* Simulates histories 0..n_decays-1 with Philox4x32-10 key `seed`, counter (history, block, stream), in
+ * n_batches consecutive batches; replaces the previous run's tallies.  Synchronous: results are complete
+ * on return.  ANM_E_STATE unless grid, phantom, tables and a source are set. */
+int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed);
+
+/* --- results of the last run (n must equal nx*ny*nz) -------------------------------------------- */
+int anm_get_energy(anm_ctx* c, float* out_MeV, size_t n, int on_device);          /* sum over batches   */
+int anm_get_dose(anm_ctx* c, float* out_Gy_per_decay, size_t n, int on_device);
+int anm_get_dose_rate(anm_ctx* c, double total_activity_Bq, float* out_Gy_per_s, size_t n, int on_device); /* Eq. 1 */
+int anm_get_uncertainty(anm_ctx* c, float* out_rel_sigma, size_t n, int on_device); /* batch sigma of the mean / mean; 0 where the mean is 0 */
+int anm_get_organ_doses(anm_ctx* c, anm_organ* out, int n_organs);                  /* host array, out[k] = label k+1 */
+int anm_get_stats(anm_ctx* c, anm_stats* out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ANM_H_ */

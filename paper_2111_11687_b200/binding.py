@@ -1,0 +1,281 @@
+"""ctypes binding of libanm.so -- argument marshalling only; every step of the path runs in the CUDA kernels.
+
+The low-level functions keep the C names (`load().anm_run(...)`); `Simulation` wraps one `anm_ctx` with
+methods named after the calls (set_grid, load_phantom, load_activity, set_point_source, load_organs,
+set_physics_tables, set_options, set_stream, run, get_energy, get_dose, get_dose_rate, get_uncertainty,
+get_organ_doses, get_stats).  Volume arguments may be numpy arrays (host) or CUDA torch tensors (device
+pointers are passed through, `on_device=1`).  torch is used only for device memory and streams.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+
+ANM_SYMBOLS = [
+    "anm_create", "anm_destroy", "anm_last_error", "anm_set_stream", "anm_set_grid", "anm_load_phantom",
+    "anm_load_activity", "anm_set_point_source", "anm_load_organs", "anm_set_physics_tables", "anm_set_options",
+    "anm_default_options", "anm_run", "anm_get_energy", "anm_get_dose", "anm_get_dose_rate", "anm_get_uncertainty",
+    "anm_get_organ_doses", "anm_get_stats",
+]
+
+STATUS = {0: "ANM_OK", -1: "ANM_E_ARG", -2: "ANM_E_STATE", -3: "ANM_E_CUDA", -4: "ANM_E_NOMEM", -5: "ANM_E_UNSUPPORTED"}
+
+
+class AnmError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("%s: %s" % (STATUS.get(code, code), msg))
+        self.code = code
+
+
+class anm_tables(C.Structure):
+    _fields_ = [("n_materials", C.c_int32), ("n_energy", C.c_int32), ("lnE_min", C.c_double), ("dlnE", C.c_double),
+                ("mu_pe", C.c_void_p), ("mu_compton", C.c_void_p), ("mu_rayleigh", C.c_void_p),
+                ("n_x2", C.c_int32), ("reserved0", C.c_int32), ("ray_x2", C.c_void_p), ("ray_cum", C.c_void_p)]
+
+
+class anm_options(C.Structure):
+    _fields_ = [("n_batches", C.c_int32), ("photons_per_decay", C.c_int32), ("rayleigh_on", C.c_int32),
+                ("zero_air_dose", C.c_int32), ("photon_cutoff_MeV", C.c_double), ("positron_ke_MeV", C.c_double),
+                ("schedule", C.c_int32), ("collect_stats", C.c_int32), ("warp_aggregate", C.c_int32),
+                ("hull_majorant", C.c_int32), ("history_offset", C.c_uint64)]
+
+
+class anm_organ(C.Structure):
+    _fields_ = [("mean_Gy_per_decay", C.c_double), ("sigma_mean", C.c_double), ("rms_voxel_rel_sigma", C.c_double),
+                ("mass_weighted_Gy_per_decay", C.c_double), ("mass_g", C.c_double),
+                ("n_voxels", C.c_uint64), ("n_voxels_nonzero", C.c_uint64)]
+
+
+class anm_stats(C.Structure):
+    _fields_ = [("emitted_MeV", C.c_double), ("deposited_MeV", C.c_double), ("escaped_MeV", C.c_double)] + [
+        (n, C.c_uint64) for n in ("n_decays", "n_steps", "n_real", "n_pe", "n_compton", "n_rayleigh", "n_escaped", "n_cutoff")] + [
+        ("ms_transport", C.c_double), ("ms_fold", C.c_double), ("ms_finalize", C.c_double), ("ms_setup", C.c_double),
+        ("n_launches", C.c_uint64)]
+
+    def as_dict(self):
+        return {n: getattr(self, n) for n, _ in self._fields_}
+
+
+def lib_path() -> str:
+    return os.path.join(_PKG, "libanm.so")
+
+
+_lib = None
+
+
+def load(build_if_missing: bool = True):
+    """dlopen libanm.so and declare the prototypes.  Fails loudly (no fallback) if it cannot be built or loaded."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = lib_path()
+    if build_if_missing:
+        from . import build as _b
+        if _b.needs_build():
+            _b.build()
+    if not os.path.exists(path):
+        raise RuntimeError("libanm.so is missing (%s): build it with `python -m paper_2111_11687_b200.build`; "
+                           "there is no CPU fallback" % path)
+    L = C.CDLL(path)
+    vp, i32, u64, dbl, sz = C.c_void_p, C.c_int, C.c_uint64, C.c_double, C.c_size_t
+    protos = {
+        "anm_create": (i32, [C.POINTER(vp), i32]), "anm_destroy": (i32, [vp]), "anm_last_error": (C.c_char_p, [vp]),
+        "anm_set_stream": (i32, [vp, vp]), "anm_set_grid": (i32, [vp, i32, i32, i32, dbl, dbl, dbl]),
+        "anm_load_phantom": (i32, [vp, vp, vp, i32]), "anm_load_activity": (i32, [vp, vp, i32]),
+        "anm_set_point_source": (i32, [vp, dbl, dbl, dbl]), "anm_load_organs": (i32, [vp, vp, i32, i32]),
+        "anm_set_physics_tables": (i32, [vp, C.POINTER(anm_tables)]), "anm_set_options": (i32, [vp, C.POINTER(anm_options)]),
+        "anm_default_options": (i32, [C.POINTER(anm_options)]), "anm_run": (i32, [vp, u64, u64]),
+        "anm_get_energy": (i32, [vp, vp, sz, i32]), "anm_get_dose": (i32, [vp, vp, sz, i32]),
+        "anm_get_dose_rate": (i32, [vp, dbl, vp, sz, i32]), "anm_get_uncertainty": (i32, [vp, vp, sz, i32]),
+        "anm_get_organ_doses": (i32, [vp, C.POINTER(anm_organ), i32]), "anm_get_stats": (i32, [vp, C.POINTER(anm_stats)]),
+    }
+    for name, (res, args) in protos.items():
+        f = getattr(L, name)
+        f.restype, f.argtypes = res, args
+    _lib = L
+    return L
+
+
+def _is_torch(a) -> bool:
+    return type(a).__module__.startswith("torch")
+
+
+def _in_ptr(a, dtype, n, keep):
+    """(pointer, on_device) of an input volume: numpy -> host pointer; CUDA torch tensor -> device pointer."""
+    if _is_torch(a):
+        import torch
+        want = {np.uint8: torch.uint8, np.float32: torch.float32}[dtype]
+        if a.dtype != want or not a.is_contiguous() or a.numel() != n:
+            raise ValueError("tensor must be contiguous %s with %d elements" % (want, n))
+        keep.append(a)
+        if a.is_cuda:
+            return a.data_ptr(), 1
+        return a.data_ptr(), 0
+    arr = np.ascontiguousarray(a, dtype=dtype).reshape(-1)
+    if arr.size != n:
+        raise ValueError("array has %d elements, the grid has %d voxels" % (arr.size, n))
+    keep.append(arr)
+    return arr.ctypes.data, 0
+
+
+class Simulation:
+    """One anm_ctx.  Shapes are (nx, ny, nz); volumes are indexed [iz][iy][ix] (C order)."""
+
+    def __init__(self, device: int = 0):
+        self._L = load()
+        self._ctx = C.c_void_p()
+        rc = self._L.anm_create(C.byref(self._ctx), int(device))
+        if rc != 0:
+            raise AnmError(rc, "anm_create failed: no usable CUDA device %d (there is no CPU fallback)" % device)
+        self.device = int(device)
+        self.shape = None
+        self.V = 0
+        self.n_organs = 0
+        self._keep = []
+
+    def close(self):
+        if getattr(self, "_ctx", None):
+            self._L.anm_destroy(self._ctx)
+            self._ctx = None
+
+    __del__ = close
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def _ck(self, rc):
+        if rc != 0:
+            raise AnmError(rc, (self._L.anm_last_error(self._ctx) or b"").decode())
+
+    # ---- inputs
+    def set_stream(self, stream):
+        """stream: a torch.cuda.Stream, a raw cudaStream_t integer, or None (default stream)."""
+        h = getattr(stream, "cuda_stream", stream)
+        self._ck(self._L.anm_set_stream(self._ctx, C.c_void_p(int(h) if h else None)))
+
+    def set_grid(self, shape, spacing_mm):
+        nx, ny, nz = (int(v) for v in shape)
+        self._ck(self._L.anm_set_grid(self._ctx, nx, ny, nz, *(float(s) for s in spacing_mm)))
+        self.shape, self.V = (nx, ny, nz), nx * ny * nz
+
+    def load_phantom(self, material, density):
+        keep = []
+        pm, d1 = _in_ptr(material, np.uint8, self.V, keep)
+        pr, d2 = _in_ptr(density, np.float32, self.V, keep)
+        if d1 != d2:
+            raise ValueError("material and density must both be host or both be device arrays")
+        self._ck(self._L.anm_load_phantom(self._ctx, pm, pr, d1))
+
+    def load_activity(self, activity):
+        keep = []
+        p, d = _in_ptr(activity, np.float32, self.V, keep)
+        self._ck(self._L.anm_load_activity(self._ctx, p, d))
+
+    def set_point_source(self, xyz_mm):
+        self._ck(self._L.anm_set_point_source(self._ctx, *(float(v) for v in xyz_mm)))
+
+    def load_organs(self, labels, n_organs: int):
+        keep = []
+        p, d = _in_ptr(labels, np.uint8, self.V, keep)
+        self._ck(self._L.anm_load_organs(self._ctx, p, int(n_organs), d))
+        self.n_organs = int(n_organs)
+
+    def set_physics_tables(self, tables: dict):
+        t = anm_tables()
+        keep = []
+        t.n_materials, t.n_energy, t.n_x2 = int(tables["n_materials"]), int(tables["n_energy"]), int(tables["n_x2"])
+        t.lnE_min, t.dlnE = float(tables["lnE_min"]), float(tables["dlnE"])
+        for name, n in (("mu_pe", t.n_materials * t.n_energy), ("mu_compton", t.n_materials * t.n_energy),
+                        ("mu_rayleigh", t.n_materials * t.n_energy), ("ray_x2", t.n_x2), ("ray_cum", t.n_materials * t.n_x2)):
+            a = np.ascontiguousarray(tables[name], np.float32).reshape(-1)
+            if a.size != n:
+                raise ValueError("%s has %d elements, expected %d" % (name, a.size, n))
+            keep.append(a)
+            setattr(t, name, a.ctypes.data)
+        self._ck(self._L.anm_set_physics_tables(self._ctx, C.byref(t)))
+
+    def default_options(self) -> anm_options:
+        o = anm_options()
+        self._L.anm_default_options(C.byref(o))
+        return o
+
+    def set_options(self, **kw):
+        o = self.default_options()
+        for k, v in kw.items():
+            if not hasattr(o, k):
+                raise TypeError("unknown option %r" % k)
+            setattr(o, k, v)
+        self._ck(self._L.anm_set_options(self._ctx, C.byref(o)))
+        return o
+
+    # ---- run
+    def run(self, n_decays: int, seed: int):
+        self._ck(self._L.anm_run(self._ctx, int(n_decays), int(seed)))
+
+    # ---- results
+    def _out(self, out):
+        if out is None:
+            out = np.empty(self.V, np.float32)
+        if _is_torch(out):
+            import torch
+            if out.dtype != torch.float32 or not out.is_contiguous() or out.numel() != self.V:
+                raise ValueError("output tensor must be contiguous float32 with %d elements" % self.V)
+            return out, out.data_ptr(), 1 if out.is_cuda else 0
+        if out.dtype != np.float32 or not out.flags.c_contiguous or out.size != self.V:
+            raise ValueError("output array must be contiguous float32 with %d elements" % self.V)
+        return out, out.ctypes.data, 0
+
+    def get_energy(self, out=None):
+        out, p, d = self._out(out)
+        self._ck(self._L.anm_get_energy(self._ctx, p, self.V, d))
+        return out
+
+    def get_dose(self, out=None):
+        out, p, d = self._out(out)
+        self._ck(self._L.anm_get_dose(self._ctx, p, self.V, d))
+        return out
+
+    def get_dose_rate(self, total_activity_bq: float, out=None):
+        out, p, d = self._out(out)
+        self._ck(self._L.anm_get_dose_rate(self._ctx, float(total_activity_bq), p, self.V, d))
+        return out
+
+    def get_uncertainty(self, out=None):
+        out, p, d = self._out(out)
+        self._ck(self._L.anm_get_uncertainty(self._ctx, p, self.V, d))
+        return out
+
+    def get_organ_doses(self) -> dict:
+        arr = (anm_organ * self.n_organs)()
+        self._ck(self._L.anm_get_organ_doses(self._ctx, arr, self.n_organs))
+        names = [n for n, _ in anm_organ._fields_]
+        return {n: np.array([getattr(o, n) for o in arr]) for n in names}
+
+    def get_stats(self) -> dict:
+        s = anm_stats()
+        self._ck(self._L.anm_get_stats(self._ctx, C.byref(s)))
+        return s.as_dict()
+
+    # ---- convenience: everything a config dict (anm_inputs.make_config) describes
+    def load_config(self, cfg: dict, tables: dict, **options):
+        self.set_grid(cfg["shape"], cfg["spacing_mm"])
+        self.load_phantom(cfg["material"], cfg["density"])
+        if cfg.get("point_source_mm") is not None:
+            self.set_point_source(cfg["point_source_mm"])
+        else:
+            self.load_activity(cfg["activity"])
+        if cfg.get("labels") is not None and cfg.get("n_organs"):
+            self.load_organs(cfg["labels"], cfg["n_organs"])
+        self.set_physics_tables(tables)
+        opts = dict(n_batches=cfg["n_batches"], photons_per_decay=cfg["photons_per_decay"],
+                    rayleigh_on=cfg["rayleigh_on"], photon_cutoff_MeV=cfg["photon_cutoff_mev"],
+                    positron_ke_MeV=cfg["positron_ke_mev"])
+        opts.update(options)
+        self.set_options(**opts)

@@ -1,0 +1,667 @@
+// anm_api.cu -- host side of libanm.so: the C ABI of include/anm.h, device memory, set-up (texel packing,
+// alias table, majorant) and the batch loop.  All arithmetic of the method runs in anm_kernels.cuh.
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/anm.h"
+#include "anm_kernels.cuh"
+
+using namespace anm;
+
+namespace {
+
+constexpr double kGyPerMeVPerGram = 1.602176634e-10;
+
+template <typename T>
+struct DevBuf {
+    T* p = nullptr;
+    size_t n = 0;
+    cudaError_t alloc(size_t count) {
+        if (count == n && p) return cudaSuccess;
+        release();
+        if (count == 0) return cudaSuccess;
+        cudaError_t e = cudaMalloc(&p, count * sizeof(T));
+        if (e == cudaSuccess) n = count; else p = nullptr;
+        return e;
+    }
+    void release() { if (p) cudaFree(p); p = nullptr; n = 0; }
+};
+
+}  // namespace
+
+struct anm_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    std::string err;
+    int num_sms = 0;
+
+    // grid
+    bool have_grid = false;
+    int nx = 0, ny = 0, nz = 0;
+    double dx = 0, dy = 0, dz = 0;        // cm
+    size_t V = 0, Vpad = 0;
+
+    // inputs
+    bool have_phantom = false, have_source = false, have_tables = false, have_organs = false;
+    bool point_source = false;
+    double px = 0, py = 0, pz = 0;        // cm
+    unsigned max_material = 0;
+    unsigned rho_max_counts[ANM_MAX_MATERIALS] = {0};   // per material, in texel counts
+    int n_organs = 0;
+    anm_options opt;
+    // tables (host copies)
+    int nm = 0, ne = 0, n_x2 = 0;
+    double lnE_min = 0, dlnE = 0;
+    std::vector<float> mu_pe, mu_co, mu_ra, ray_x2, ray_cum;
+    bool dev_tables_dirty = true;
+
+    // device memory
+    DevBuf<uint32_t> texels;
+    DevBuf<float> batch, sum, sumsq, scratch;
+    DevBuf<uint8_t> labels;
+    DevBuf<uint4> alias;
+    DevBuf<unsigned> counters;
+    DevBuf<DeviceStats> dstats;
+    DevBuf<double> organ_batch;           // [B][256]
+    DevBuf<OrganAccum> organ_acc;         // [256]
+    DevBuf<double> organ_mass;            // [256]
+    DevBuf<unsigned long long> organ_count;   // [256]
+    DevBuf<double> total_energy;          // [1]
+    DevBuf<float> d_tot, d_maj, d_x2, d_cum;
+    DevBuf<float2> d_pec;
+    DevBuf<unsigned> d_flags;             // [2 + ANM_MAX_MATERIALS]
+    unsigned n_alias = 0;
+
+    // results of the last run
+    bool have_results = false;
+    uint64_t run_decays = 0;
+    int run_batches = 0;
+    std::vector<anm_organ> organs;
+    anm_stats stats;
+    double ms_setup = 0;
+
+    anm_ctx() { std::memset(&stats, 0, sizeof stats); anm_default_options(&opt); }
+};
+
+namespace {
+
+int fail(anm_ctx* c, int code, const char* fmt, ...) {
+    if (c) {
+        char buf[512];
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(buf, sizeof buf, fmt, ap);
+        va_end(ap);
+        c->err = buf;
+    }
+    return code;
+}
+
+#define ANM_CUDA(c, call)                                                                         \
+    do {                                                                                          \
+        cudaError_t e_ = (call);                                                                  \
+        if (e_ != cudaSuccess) {                                                                  \
+            cudaGetLastError();                                                                   \
+            return fail((c), e_ == cudaErrorMemoryAllocation ? ANM_E_NOMEM : ANM_E_CUDA,          \
+                        "%s: %s", #call, cudaGetErrorString(e_));                                 \
+        }                                                                                         \
+    } while (0)
+
+int grid_blocks(const anm_ctx* c, size_t items, int per_block) {
+    const size_t want = (items + per_block - 1) / per_block;
+    const size_t cap = (size_t)c->num_sms * 8;
+    return (int)std::max<size_t>(1, std::min(want, cap));
+}
+
+// Vose's alias method over the active voxels (host, fp64).  entry = {threshold (P(own) * 2^32), own voxel, alias voxel, 0}
+int build_alias(anm_ctx* c, const float* act) {
+    const size_t V = c->V;
+    double total = 0.0;
+    size_t M = 0;
+    for (size_t i = 0; i < V; ++i) {
+        const float a = act[i];
+        if (!(a >= 0.0f) || !std::isfinite(a)) return fail(c, ANM_E_ARG, "activity[%zu] is negative or not finite", i);
+        if (a > 0.0f) { total += (double)a; ++M; }
+    }
+    if (M == 0) return fail(c, ANM_E_ARG, "activity is zero everywhere");
+    if (M > 0xfffffff0ull) return fail(c, ANM_E_ARG, "too many active voxels");
+    std::vector<uint4> tab(M);
+    std::vector<double> q(M);
+    std::vector<uint32_t> small, large;
+    small.reserve(M); large.reserve(M);
+    size_t j = 0;
+    const double scale = (double)M / total;
+    for (size_t i = 0; i < V; ++i) {
+        if (act[i] > 0.0f) {
+            q[j] = (double)act[i] * scale;
+            tab[j] = make_uint4(0xffffffffu, (uint32_t)i, (uint32_t)i, 0u);
+            (q[j] < 1.0 ? small : large).push_back((uint32_t)j);
+            ++j;
+        }
+    }
+    while (!small.empty() && !large.empty()) {
+        const uint32_t s = small.back(); small.pop_back();
+        const uint32_t l = large.back();
+        const double t = std::floor(q[s] * 4294967296.0);
+        tab[s].x = (uint32_t)std::min(t, 4294967295.0);
+        tab[s].z = tab[l].y;
+        q[l] -= 1.0 - q[s];
+        if (q[l] < 1.0) { large.pop_back(); small.push_back(l); }
+    }
+    // leftovers have q == 1 up to rounding: keep threshold = 2^32 - 1, alias = own
+    ANM_CUDA(c, c->alias.alloc(M));
+    ANM_CUDA(c, cudaMemcpyAsync(c->alias.p, tab.data(), M * sizeof(uint4), cudaMemcpyHostToDevice, c->stream));
+    ANM_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->n_alias = (unsigned)M;
+    return ANM_OK;
+}
+
+// tot / {pe, pe+co} / majorant tables on the device, for the current options and phantom
+int upload_tables(anm_ctx* c) {
+    const int nm = c->nm, ne = c->ne;
+    std::vector<float> tot((size_t)nm * ne), maj(ne);
+    std::vector<float2> pec((size_t)nm * ne);
+    for (int m = 0; m < nm; ++m)
+        for (int k = 0; k < ne; ++k) {
+            const size_t i = (size_t)m * ne + k;
+            pec[i] = make_float2(c->mu_pe[i], c->mu_pe[i] + c->mu_co[i]);
+            tot[i] = pec[i].y + (c->opt.rayleigh_on ? c->mu_ra[i] : 0.0f);
+        }
+    // majorant at the grid nodes: max over materials of rho_max,m * tot_m; linear interpolation of the node
+    // maxima bounds every material's interpolated value, so it is a majorant at every energy
+    for (int k = 0; k < ne; ++k) {
+        float mx = 0.0f;
+        for (int m = 0; m < nm; ++m) {
+            const float rho = (float)c->rho_max_counts[m] * kDensityStep;
+            mx = std::max(mx, rho * tot[(size_t)m * ne + k]);
+        }
+        maj[k] = mx * 1.000001f + 1e-30f;    // head-room for fp32 rounding of rho * lerp
+    }
+    ANM_CUDA(c, c->d_tot.alloc(tot.size()));
+    ANM_CUDA(c, c->d_pec.alloc(pec.size()));
+    ANM_CUDA(c, c->d_maj.alloc(maj.size()));
+    ANM_CUDA(c, c->d_x2.alloc(c->ray_x2.size()));
+    ANM_CUDA(c, c->d_cum.alloc(c->ray_cum.size()));
+    ANM_CUDA(c, cudaMemcpyAsync(c->d_tot.p, tot.data(), tot.size() * 4, cudaMemcpyHostToDevice, c->stream));
+    ANM_CUDA(c, cudaMemcpyAsync(c->d_pec.p, pec.data(), pec.size() * 8, cudaMemcpyHostToDevice, c->stream));
+    ANM_CUDA(c, cudaMemcpyAsync(c->d_maj.p, maj.data(), maj.size() * 4, cudaMemcpyHostToDevice, c->stream));
+    ANM_CUDA(c, cudaMemcpyAsync(c->d_x2.p, c->ray_x2.data(), c->ray_x2.size() * 4, cudaMemcpyHostToDevice, c->stream));
+    ANM_CUDA(c, cudaMemcpyAsync(c->d_cum.p, c->ray_cum.data(), c->ray_cum.size() * 4, cudaMemcpyHostToDevice, c->stream));
+    ANM_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->dev_tables_dirty = false;
+    return ANM_OK;
+}
+
+struct HostE0 { int ie; float fe, maj, inv_maj; };
+
+template <bool S, bool W>
+cudaError_t launch_transport(int blocks, size_t smem, cudaStream_t st, const TransportParams& p) {
+    transport_kernel<S, W><<<blocks, kThreads, smem, st>>>(p);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+// =================================================================================================
+extern "C" {
+
+int anm_default_options(anm_options* o) {
+    if (!o) return ANM_E_ARG;
+    std::memset(o, 0, sizeof *o);
+    o->n_batches = 100;
+    o->photons_per_decay = 2;
+    o->rayleigh_on = 1;
+    o->photon_cutoff_MeV = 0.010;
+    o->positron_ke_MeV = 0.0;
+    o->schedule = 0;
+    return ANM_OK;
+}
+
+int anm_create(anm_ctx** out, int cuda_device) {
+    if (!out) return ANM_E_ARG;
+    *out = nullptr;
+    int count = 0;
+    cudaError_t e = cudaGetDeviceCount(&count);
+    if (e != cudaSuccess || cuda_device < 0 || cuda_device >= count) { cudaGetLastError(); return ANM_E_CUDA; }
+    if (cudaSetDevice(cuda_device) != cudaSuccess) { cudaGetLastError(); return ANM_E_CUDA; }
+    anm_ctx* c = new (std::nothrow) anm_ctx();
+    if (!c) return ANM_E_NOMEM;
+    c->device = cuda_device;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, cuda_device) != cudaSuccess) { delete c; return ANM_E_CUDA; }
+    c->num_sms = prop.multiProcessorCount;
+    *out = c;
+    return ANM_OK;
+}
+
+int anm_destroy(anm_ctx* c) {
+    if (!c) return ANM_OK;
+    cudaSetDevice(c->device);
+    c->texels.release(); c->batch.release(); c->sum.release(); c->sumsq.release(); c->scratch.release();
+    c->labels.release(); c->alias.release(); c->counters.release(); c->dstats.release();
+    c->organ_batch.release(); c->organ_acc.release(); c->organ_mass.release(); c->organ_count.release();
+    c->total_energy.release(); c->d_tot.release(); c->d_maj.release(); c->d_x2.release(); c->d_cum.release();
+    c->d_pec.release(); c->d_flags.release();
+    delete c;
+    return ANM_OK;
+}
+
+const char* anm_last_error(const anm_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+int anm_set_stream(anm_ctx* c, void* cuda_stream) {
+    if (!c) return ANM_E_ARG;
+    c->stream = (cudaStream_t)cuda_stream;
+    return ANM_OK;
+}
+
+int anm_set_grid(anm_ctx* c, int nx, int ny, int nz, double dx_mm, double dy_mm, double dz_mm) {
+    if (!c) return ANM_E_ARG;
+    if (nx < 1 || ny < 1 || nz < 1 || !(dx_mm > 0) || !(dy_mm > 0) || !(dz_mm > 0) ||
+        !std::isfinite(dx_mm) || !std::isfinite(dy_mm) || !std::isfinite(dz_mm))
+        return fail(c, ANM_E_ARG, "grid: sizes must be >= 1 and spacings > 0");
+    const unsigned long long V = (unsigned long long)nx * ny * nz;
+    if (V > 0xfffffff0ull) return fail(c, ANM_E_ARG, "grid: more than 2^32 voxels");
+    ANM_CUDA(c, cudaSetDevice(c->device));
+    c->nx = nx; c->ny = ny; c->nz = nz;
+    c->dx = dx_mm / 10.0; c->dy = dy_mm / 10.0; c->dz = dz_mm / 10.0;
+    c->V = (size_t)V;
+    c->Vpad = (c->V + 3) / 4 * 4;
+    c->have_grid = true;
+    c->have_phantom = c->have_organs = c->have_results = false;
+    c->have_source = c->point_source && c->have_source;
+    if (!c->point_source) c->have_source = false;
+    ANM_CUDA(c, c->texels.alloc(c->Vpad));
+    ANM_CUDA(c, c->batch.alloc(c->Vpad));
+    ANM_CUDA(c, c->sum.alloc(c->Vpad));
+    ANM_CUDA(c, c->sumsq.alloc(c->Vpad));
+    ANM_CUDA(c, cudaMemsetAsync(c->texels.p, 0, c->Vpad * 4, c->stream));
+    ANM_CUDA(c, cudaMemsetAsync(c->batch.p, 0, c->Vpad * 4, c->stream));
+    ANM_CUDA(c, c->d_flags.alloc(2 + ANM_MAX_MATERIALS));
+    ANM_CUDA(c, c->dstats.alloc(1));
+    ANM_CUDA(c, c->total_energy.alloc(1));
+    ANM_CUDA(c, c->organ_acc.alloc(256));
+    ANM_CUDA(c, c->organ_mass.alloc(256));
+    ANM_CUDA(c, c->organ_count.alloc(256));
+    return ANM_OK;
+}
+
+int anm_load_phantom(anm_ctx* c, const uint8_t* material, const float* density, int on_device) {
+    if (!c) return ANM_E_ARG;
+    if (!material || !density) return fail(c, ANM_E_ARG, "phantom: null pointer");
+    if (!c->have_grid) return fail(c, ANM_E_STATE, "phantom: set the grid first");
+    ANM_CUDA(c, cudaSetDevice(c->device));
+    cudaEvent_t e0, e1;
+    ANM_CUDA(c, cudaEventCreate(&e0));
+    ANM_CUDA(c, cudaEventCreate(&e1));
+    ANM_CUDA(c, cudaEventRecord(e0, c->stream));
+    const uint8_t* d_mat = material;
+    const float* d_rho = density;
+    DevBuf<uint8_t> stage_m;
+    if (!on_device) {
+        ANM_CUDA(c, stage_m.alloc(c->V));
+        ANM_CUDA(c, c->scratch.alloc(c->Vpad));
+        ANM_CUDA(c, cudaMemcpyAsync(stage_m.p, material, c->V, cudaMemcpyHostToDevice, c->stream));
+        ANM_CUDA(c, cudaMemcpyAsync(c->scratch.p, density, c->V * 4, cudaMemcpyHostToDevice, c->stream));
+        d_mat = stage_m.p; d_rho = c->scratch.p;
+    }
+    ANM_CUDA(c, cudaMemsetAsync(c->d_flags.p, 0, (2 + ANM_MAX_MATERIALS) * 4, c->stream));
+    pack_texels_kernel<<<grid_blocks(c, c->V, kFoldThreads), kFoldThreads, 0, c->stream>>>(
+        d_mat, d_rho, c->texels.p, c->V, c->d_flags.p, c->d_flags.p + 1);
+    ANM_CUDA(c, cudaGetLastError());
+    unsigned flags[2] = {0, 0};
+    ANM_CUDA(c, cudaMemcpyAsync(flags, c->d_flags.p, 8, cudaMemcpyDeviceToHost, c->stream));
+    ANM_CUDA(c, cudaEventRecord(e1, c->stream));
+    ANM_CUDA(c, cudaStreamSynchronize(c->stream));
+    stage_m.release();
+    float ms = 0;
+    cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    c->ms_setup += ms;
+    c->have_phantom = false;
+    if (flags[0] & 1u) return fail(c, ANM_E_ARG, "phantom: density must be finite and in [0, 16) g/cm^3");
+    if (flags[1] >= ANM_MAX_MATERIALS) return fail(c, ANM_E_ARG, "phantom: material id %u >= %d", flags[1], ANM_MAX_MATERIALS);
+    c->max_material = flags[1];
+    // per-material maximum density (texel counts): a second tiny pass on the host copy of the texels would cost a
+    // D2H of the volume; instead reduce on the device with one atomicMax per (block, material)
+    {
+        rho_max_kernel<<<grid_blocks(c, c->V, kFoldThreads), kFoldThreads, 0, c->stream>>>(c->texels.p, c->V, c->d_flags.p + 2);
+        ANM_CUDA(c, cudaGetLastError());
+        ANM_CUDA(c, cudaMemcpyAsync(c->rho_max_counts, c->d_flags.p + 2, ANM_MAX_MATERIALS * 4, cudaMemcpyDeviceToHost, c->stream));
+        ANM_CUDA(c, cudaStreamSynchronize(c->stream));
+    }
+    c->have_phantom = true;
+    c->have_results = false;
+    c->dev_tables_dirty = true;
+    if (c->have_organs) c->have_organs = false;   // masses depend on the phantom: reload the labels
+    return ANM_OK;
+}
+
+int anm_load_activity(anm_ctx* c, const float* activity, int on_device) {
+    if (!c) return ANM_E_ARG;
+    if (!activity) return fail(c, ANM_E_ARG, "activity: null pointer");
+    if (!c->have_grid) return fail(c, ANM_E_STATE, "activity: set the grid first");
+    ANM_CUDA(c, cudaSetDevice(c->device));
+    std::vector<float> host;
+    const float* a = activity;
+    try {
+        if (on_device) {
+            host.resize(c->V);
+            ANM_CUDA(c, cudaMemcpyAsync(host.data(), activity, c->V * 4, cudaMemcpyDeviceToHost, c->stream));
+            ANM_CUDA(c, cudaStreamSynchronize(c->stream));
+            a = host.data();
+        }
+        c->have_source = false;
+        const int rc = build_alias(c, a);
+        if (rc != ANM_OK) return rc;
+    } catch (const std::bad_alloc&) {
+        return fail(c, ANM_E_NOMEM, "activity: host allocation failed");
+    }
+    c->point_source = false;
+    c->have_source = true;
+    c->have_results = false;
+    return ANM_OK;
+}
+
+int anm_set_point_source(anm_ctx* c, double x_mm, double y_mm, double z_mm) {
+    if (!c) return ANM_E_ARG;
+    if (!c->have_grid) return fail(c, ANM_E_STATE, "point source: set the grid first");
+    const double x = x_mm / 10.0, y = y_mm / 10.0, z = z_mm / 10.0;
+    if (!(x >= 0 && x < c->nx * c->dx && y >= 0 && y < c->ny * c->dy && z >= 0 && z < c->nz * c->dz))
+        return fail(c, ANM_E_ARG, "point source outside the grid");
+    c->px = x; c->py = y; c->pz = z;
+    c->point_source = true;
+    c->have_source = true;
+    c->have_results = false;
+    return ANM_OK;
+}
+
+int anm_load_organs(anm_ctx* c, const uint8_t* labels, int n_organs, int on_device) {
+    if (!c) return ANM_E_ARG;
+    if (!labels) return fail(c, ANM_E_ARG, "organs: null pointer");
+    if (n_organs < 1 || n_organs > ANM_MAX_ORGANS) return fail(c, ANM_E_ARG, "organs: n_organs must be 1..%d", ANM_MAX_ORGANS);
+    if (!c->have_phantom) return fail(c, ANM_E_STATE, "organs: load the phantom first (organ masses need it)");
+    ANM_CUDA(c, cudaSetDevice(c->device));
+    ANM_CUDA(c, c->labels.alloc(c->Vpad));
+    ANM_CUDA(c, cudaMemsetAsync(c->labels.p, 0, c->Vpad, c->stream));
+    ANM_CUDA(c, cudaMemcpyAsync(c->labels.p, labels, c->V, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
+    ANM_CUDA(c, cudaMemsetAsync(c->organ_mass.p, 0, 256 * 8, c->stream));
+    ANM_CUDA(c, cudaMemsetAsync(c->organ_count.p, 0, 256 * 8, c->stream));
+    organ_mass_kernel<<<grid_blocks(c, c->V, kFoldThreads), kFoldThreads, 0, c->stream>>>(
+        c->labels.p, c->texels.p, c->organ_mass.p, c->organ_count.p, c->V, (float)(c->dx * c->dy * c->dz));
+    ANM_CUDA(c, cudaGetLastError());
+    unsigned long long cnt[256];
+    ANM_CUDA(c, cudaMemcpyAsync(cnt, c->organ_count.p, sizeof cnt, cudaMemcpyDeviceToHost, c->stream));
+    ANM_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->have_organs = false;
+    for (int l = n_organs + 1; l < 256; ++l)
+        if (cnt[l]) return fail(c, ANM_E_ARG, "organs: label %d > n_organs = %d", l, n_organs);
+    c->n_organs = n_organs;
+    c->have_organs = true;
+    c->have_results = false;
+    return ANM_OK;
+}
+
+int anm_set_physics_tables(anm_ctx* c, const anm_tables* t) {
+    if (!c) return ANM_E_ARG;
+    if (!t || !t->mu_pe || !t->mu_compton || !t->mu_rayleigh || !t->ray_x2 || !t->ray_cum)
+        return fail(c, ANM_E_ARG, "tables: null pointer");
+    if (t->n_materials < 1 || t->n_materials > ANM_MAX_MATERIALS || t->n_energy < 2 || t->n_energy > 1024 ||
+        t->n_x2 < 2 || t->n_x2 > 1024 || !(t->dlnE > 0) || !std::isfinite(t->lnE_min))
+        return fail(c, ANM_E_ARG, "tables: sizes out of range");
+    const size_t n = (size_t)t->n_materials * t->n_energy;
+    for (size_t i = 0; i < n; ++i)
+        if (!(t->mu_pe[i] > 0) || !(t->mu_compton[i] > 0) || !(t->mu_rayleigh[i] > 0) ||
+            !std::isfinite(t->mu_pe[i]) || !std::isfinite(t->mu_compton[i]) || !std::isfinite(t->mu_rayleigh[i]))
+            return fail(c, ANM_E_ARG, "tables: coefficients must be finite and > 0");
+    if (t->ray_x2[0] != 0.0f) return fail(c, ANM_E_ARG, "tables: ray_x2[0] must be 0");
+    for (int i = 1; i < t->n_x2; ++i)
+        if (!(t->ray_x2[i] > t->ray_x2[i - 1])) return fail(c, ANM_E_ARG, "tables: ray_x2 must increase");
+    for (int m = 0; m < t->n_materials; ++m)
+        for (int i = 1; i < t->n_x2; ++i)
+            if (!(t->ray_cum[(size_t)m * t->n_x2 + i] >= t->ray_cum[(size_t)m * t->n_x2 + i - 1]))
+                return fail(c, ANM_E_ARG, "tables: ray_cum must be non-decreasing");
+    const double e_hi = std::exp(t->lnE_min + t->dlnE * (t->n_energy - 1));
+    if (e_hi < 0.51099895) return fail(c, ANM_E_ARG, "tables: energy grid must reach 0.51099895 MeV");
+    const double xm = 0.51099895 * 1000.0 / 12.398419843;
+    if (t->ray_x2[t->n_x2 - 1] < xm * xm) return fail(c, ANM_E_ARG, "tables: ray_x2 must reach (E0/hc)^2");
+    try {
+        c->nm = t->n_materials; c->ne = t->n_energy; c->n_x2 = t->n_x2;
+        c->lnE_min = t->lnE_min; c->dlnE = t->dlnE;
+        c->mu_pe.assign(t->mu_pe, t->mu_pe + n);
+        c->mu_co.assign(t->mu_compton, t->mu_compton + n);
+        c->mu_ra.assign(t->mu_rayleigh, t->mu_rayleigh + n);
+        c->ray_x2.assign(t->ray_x2, t->ray_x2 + t->n_x2);
+        c->ray_cum.assign(t->ray_cum, t->ray_cum + (size_t)t->n_materials * t->n_x2);
+    } catch (const std::bad_alloc&) {
+        return fail(c, ANM_E_NOMEM, "tables: host allocation failed");
+    }
+    c->have_tables = true;
+    c->dev_tables_dirty = true;
+    c->have_results = false;
+    return ANM_OK;
+}
+
+int anm_set_options(anm_ctx* c, const anm_options* o) {
+    if (!c) return ANM_E_ARG;
+    if (!o) return fail(c, ANM_E_ARG, "options: null pointer");
+    if (o->n_batches < 2) return fail(c, ANM_E_ARG, "options: n_batches must be >= 2");
+    if (o->n_batches > 65536) return fail(c, ANM_E_ARG, "options: n_batches must be <= 65536");
+    if (o->photons_per_decay != 1 && o->photons_per_decay != 2) return fail(c, ANM_E_ARG, "options: photons_per_decay must be 1 or 2");
+    if (!(o->photon_cutoff_MeV > 0) || !(o->photon_cutoff_MeV < 0.51099895)) return fail(c, ANM_E_ARG, "options: photon cutoff out of range");
+    if (!(o->positron_ke_MeV >= 0) || !std::isfinite(o->positron_ke_MeV)) return fail(c, ANM_E_ARG, "options: positron energy must be >= 0");
+    if (o->schedule == 2) return fail(c, ANM_E_UNSUPPORTED, "options: event-based scheduling is not built (DESIGN.md: history-based chosen from the counters)");
+    if (o->schedule < 0 || o->schedule > 2) return fail(c, ANM_E_ARG, "options: schedule must be 0, 1 or 2");
+    c->opt = *o;
+    c->dev_tables_dirty = true;
+    c->have_results = false;
+    return ANM_OK;
+}
+
+int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
+    if (!c) return ANM_E_ARG;
+    if (!c->have_grid || !c->have_phantom || !c->have_tables || !c->have_source)
+        return fail(c, ANM_E_STATE, "run: need grid, phantom, physics tables and a source (missing:%s%s%s%s)",
+                    c->have_grid ? "" : " grid", c->have_phantom ? "" : " phantom", c->have_tables ? "" : " tables",
+                    c->have_source ? "" : " source");
+    const int B = c->opt.n_batches;
+    if (n_decays == 0 || n_decays % (uint64_t)B) return fail(c, ANM_E_ARG, "run: n_decays must be a positive multiple of n_batches = %d", B);
+    const uint64_t nb = n_decays / (uint64_t)B;
+    if (nb > 0x7fffffffull) return fail(c, ANM_E_ARG, "run: more than 2^31 decays per batch");
+    if ((int)c->max_material >= c->nm) return fail(c, ANM_E_ARG, "run: phantom uses material %u but the tables hold %d", c->max_material, c->nm);
+    if (std::exp(c->lnE_min) > c->opt.photon_cutoff_MeV * (1 + 1e-9)) return fail(c, ANM_E_ARG, "run: energy grid starts above the photon cutoff");
+    ANM_CUDA(c, cudaSetDevice(c->device));
+    c->have_results = false;
+    if (c->dev_tables_dirty) { const int rc = upload_tables(c); if (rc != ANM_OK) return rc; }
+
+    ANM_CUDA(c, c->counters.alloc((size_t)B));
+    ANM_CUDA(c, c->organ_batch.alloc((size_t)B * 256));
+    cudaStream_t st = c->stream;
+    ANM_CUDA(c, cudaMemsetAsync(c->sum.p, 0, c->Vpad * 4, st));
+    ANM_CUDA(c, cudaMemsetAsync(c->sumsq.p, 0, c->Vpad * 4, st));
+    ANM_CUDA(c, cudaMemsetAsync(c->batch.p, 0, c->Vpad * 4, st));
+    ANM_CUDA(c, cudaMemsetAsync(c->counters.p, 0, (size_t)B * 4, st));
+    ANM_CUDA(c, cudaMemsetAsync(c->organ_batch.p, 0, (size_t)B * 256 * 8, st));
+    ANM_CUDA(c, cudaMemsetAsync(c->organ_acc.p, 0, 256 * sizeof(OrganAccum), st));
+    ANM_CUDA(c, cudaMemsetAsync(c->dstats.p, 0, sizeof(DeviceStats), st));
+    ANM_CUDA(c, cudaMemsetAsync(c->total_energy.p, 0, 8, st));
+
+    TransportParams p;
+    std::memset(&p, 0, sizeof p);
+    p.texels = c->texels.p; p.batch = c->batch.p; p.alias = c->alias.p; p.stats = c->dstats.p;
+    p.tab_tot = c->d_tot.p; p.tab_pec = c->d_pec.p; p.tab_maj = c->d_maj.p; p.ray_x2 = c->d_x2.p; p.ray_cum = c->d_cum.p;
+    p.n_hist = (unsigned)nb; p.n_alias = c->n_alias;
+    p.key0 = (unsigned)seed; p.key1 = (unsigned)(seed >> 32);
+    p.nx = c->nx; p.ny = c->ny; p.nz = c->nz; p.nm = c->nm; p.ne = c->ne; p.n_x2 = c->n_x2;
+    p.dx = (float)c->dx; p.dy = (float)c->dy; p.dz = (float)c->dz;
+    p.inv_dx = (float)(1.0 / c->dx); p.inv_dy = (float)(1.0 / c->dy); p.inv_dz = (float)(1.0 / c->dz);
+    p.lnE_min = (float)c->lnE_min; p.inv_dlnE = (float)(1.0 / c->dlnE);
+    p.cutoff = (float)c->opt.photon_cutoff_MeV; p.positron_ke = (float)c->opt.positron_ke_MeV;
+    p.px = (float)c->px; p.py = (float)c->py; p.pz = (float)c->pz;
+    p.point_source = c->point_source ? 1 : 0;
+    p.photons_per_decay = c->opt.photons_per_decay; p.rayleigh_on = c->opt.rayleigh_on;
+    {   // energy-dependent quantities at E0, computed exactly like the device's set_energy (fp32)
+        std::vector<float> maj(c->ne);
+        ANM_CUDA(c, cudaMemcpyAsync(maj.data(), c->d_maj.p, (size_t)c->ne * 4, cudaMemcpyDeviceToHost, st));
+        ANM_CUDA(c, cudaStreamSynchronize(st));
+        const float t = (logf(kE0) - p.lnE_min) * p.inv_dlnE;
+        int i = std::max(0, std::min((int)t, c->ne - 2));
+        p.ie0 = i; p.fe0 = t - (float)i;
+        p.maj0 = fmaf(p.fe0, maj[i + 1] - maj[i], maj[i]);
+        p.inv_maj0 = 1.0f / p.maj0;
+    }
+
+    const size_t smem = (size_t)c->nm * c->ne * 12 + (size_t)c->ne * 4 + (size_t)c->n_x2 * 4 +
+                        (size_t)c->nm * c->n_x2 * 4 + 6 * kThreads * 4;
+    const bool S = c->opt.collect_stats != 0, W = c->opt.warp_aggregate != 0;
+    auto kern = S ? (W ? (const void*)transport_kernel<true, true> : (const void*)transport_kernel<true, false>)
+                  : (W ? (const void*)transport_kernel<false, true> : (const void*)transport_kernel<false, false>);
+    ANM_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int per_sm = 0;
+    ANM_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kThreads, smem));
+    if (per_sm < 1) return fail(c, ANM_E_UNSUPPORTED, "run: tables too large for shared memory (%zu bytes)", smem);
+    // persistent lanes: one resident wave; never more lanes than histories
+    const int blocks = (int)std::max<uint64_t>(1, std::min<uint64_t>((uint64_t)c->num_sms * per_sm, (nb + kThreads - 1) / kThreads));
+    const int fold_blocks = grid_blocks(c, c->Vpad / 4, kFoldThreads);
+    const float inv_vox = (float)(1.0 / (c->dx * c->dy * c->dz));
+
+    std::vector<cudaEvent_t> ev((size_t)2 * B + 2, nullptr);
+    auto free_events = [&]() { for (auto e : ev) if (e) cudaEventDestroy(e); };
+    for (auto& e : ev) if (cudaEventCreate(&e) != cudaSuccess) { free_events(); return fail(c, ANM_E_CUDA, "cudaEventCreate failed"); }
+#define ANM_CUDA_EV(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { cudaGetLastError(); free_events(); \
+        return fail(c, ANM_E_CUDA, "%s: %s", #call, cudaGetErrorString(e_)); } } while (0)
+
+    ANM_CUDA_EV(cudaEventRecord(ev[0], st));
+    for (int b = 0; b < B; ++b) {
+        p.counter = c->counters.p + b;
+        p.hist_base = c->opt.history_offset + (unsigned long long)b * nb;
+        cudaError_t le = S ? (W ? launch_transport<true, true>(blocks, smem, st, p) : launch_transport<true, false>(blocks, smem, st, p))
+                           : (W ? launch_transport<false, true>(blocks, smem, st, p) : launch_transport<false, false>(blocks, smem, st, p));
+        ANM_CUDA_EV(le);
+        ANM_CUDA_EV(cudaEventRecord(ev[2 * b + 1], st));
+        fold_kernel<<<fold_blocks, kFoldThreads, 0, st>>>(
+            (float4*)c->batch.p, (float4*)c->sum.p, (float4*)c->sumsq.p,
+            c->have_organs ? (const uint32_t*)c->labels.p : nullptr, (const uint4*)c->texels.p,
+            c->organ_batch.p + (size_t)b * 256, c->n_organs, c->Vpad / 4, inv_vox);
+        ANM_CUDA_EV(cudaGetLastError());
+        ANM_CUDA_EV(cudaEventRecord(ev[2 * b + 2], st));
+    }
+    finalize_kernel<<<grid_blocks(c, c->V, kFoldThreads), kFoldThreads, 0, st>>>(
+        c->sum.p, c->sumsq.p, c->have_organs ? c->labels.p : nullptr, c->organ_acc.p, c->total_energy.p,
+        c->n_organs, c->V, B);
+    ANM_CUDA_EV(cudaGetLastError());
+    ANM_CUDA_EV(cudaEventRecord(ev[2 * B + 1], st));
+
+    // results to the host
+    std::vector<double> ob((size_t)B * 256);
+    OrganAccum acc[256];
+    double mass[256];
+    unsigned long long cnt[256];
+    DeviceStats ds;
+    double tot_e = 0;
+    ANM_CUDA_EV(cudaMemcpyAsync(&ds, c->dstats.p, sizeof ds, cudaMemcpyDeviceToHost, st));
+    ANM_CUDA_EV(cudaMemcpyAsync(&tot_e, c->total_energy.p, 8, cudaMemcpyDeviceToHost, st));
+    if (c->have_organs) {
+        ANM_CUDA_EV(cudaMemcpyAsync(ob.data(), c->organ_batch.p, ob.size() * 8, cudaMemcpyDeviceToHost, st));
+        ANM_CUDA_EV(cudaMemcpyAsync(acc, c->organ_acc.p, sizeof acc, cudaMemcpyDeviceToHost, st));
+        ANM_CUDA_EV(cudaMemcpyAsync(mass, c->organ_mass.p, sizeof mass, cudaMemcpyDeviceToHost, st));
+        ANM_CUDA_EV(cudaMemcpyAsync(cnt, c->organ_count.p, sizeof cnt, cudaMemcpyDeviceToHost, st));
+    }
+    ANM_CUDA_EV(cudaStreamSynchronize(st));
+
+    double ms_t = 0, ms_f = 0, ms_fin = 0;
+    for (int b = 0; b < B; ++b) {
+        float a = 0, f = 0;
+        cudaEventElapsedTime(&a, ev[2 * b], ev[2 * b + 1]);
+        cudaEventElapsedTime(&f, ev[2 * b + 1], ev[2 * b + 2]);
+        ms_t += a; ms_f += f;
+    }
+    { float f = 0; cudaEventElapsedTime(&f, ev[2 * B], ev[2 * B + 1]); ms_fin = f; }
+    free_events();
+#undef ANM_CUDA_EV
+
+    // organ results: d_{o,b} = organ_batch[b][o] k / (n_b N_o); mean and batch sigma over b
+    c->organs.assign((size_t)c->n_organs, anm_organ{});
+    if (c->have_organs) {
+        for (int o = 1; o <= c->n_organs; ++o) {
+            anm_organ& r = c->organs[(size_t)o - 1];
+            r.n_voxels = cnt[o];
+            r.mass_g = mass[o];
+            r.n_voxels_nonzero = (uint64_t)(acc[o].n_nonzero + 0.5);
+            if (cnt[o] == 0) continue;
+            double s1 = 0, s2 = 0;
+            for (int b = 0; b < B; ++b) {
+                const double d = ob[(size_t)b * 256 + o] * kGyPerMeVPerGram / ((double)nb * (double)cnt[o]);
+                s1 += d; s2 += d * d;
+            }
+            const double mean = s1 / B;
+            r.mean_Gy_per_decay = mean;
+            r.sigma_mean = std::sqrt(std::max(0.0, (s2 / B - mean * mean) / (B - 1)));
+            r.rms_voxel_rel_sigma = acc[o].n_nonzero > 0 ? std::sqrt(acc[o].rel2 / acc[o].n_nonzero) : 0.0;
+            r.mass_weighted_Gy_per_decay = mass[o] > 0 ? acc[o].energy * kGyPerMeVPerGram / ((double)n_decays * mass[o]) : 0.0;
+        }
+    }
+    anm_stats& s = c->stats;
+    std::memset(&s, 0, sizeof s);
+    s.n_decays = n_decays;
+    s.emitted_MeV = (double)n_decays * ((double)kE0 * c->opt.photons_per_decay + c->opt.positron_ke_MeV);
+    s.deposited_MeV = tot_e;
+    s.escaped_MeV = ds.escaped_MeV;
+    s.n_steps = ds.n_steps; s.n_real = ds.n_real; s.n_pe = ds.n_pe; s.n_compton = ds.n_compton;
+    s.n_rayleigh = ds.n_rayleigh; s.n_escaped = ds.n_escaped; s.n_cutoff = ds.n_cutoff;
+    s.ms_transport = ms_t; s.ms_fold = ms_f; s.ms_finalize = ms_fin; s.ms_setup = c->ms_setup;
+    s.n_launches = (uint64_t)2 * B + 1;
+    c->run_decays = n_decays;
+    c->run_batches = B;
+    c->have_results = true;
+    return ANM_OK;
+}
+
+static int readout(anm_ctx* c, float* out, size_t n, int on_device, int mode, double scale) {
+    if (!c) return ANM_E_ARG;
+    if (!out) return fail(c, ANM_E_ARG, "get: null pointer");
+    if (!c->have_results) return fail(c, ANM_E_STATE, "get: no completed run");
+    if (n != c->V) return fail(c, ANM_E_ARG, "get: n = %zu but the grid has %zu voxels", n, c->V);
+    ANM_CUDA(c, cudaSetDevice(c->device));
+    float* dst = out;
+    if (!on_device) { ANM_CUDA(c, c->scratch.alloc(c->Vpad)); dst = c->scratch.p; }
+    const double factor = kGyPerMeVPerGram * scale / ((double)c->run_decays * c->dx * c->dy * c->dz);
+    readout_kernel<<<grid_blocks(c, c->V, kFoldThreads), kFoldThreads, 0, c->stream>>>(
+        c->sum.p, c->sumsq.p, c->texels.p, dst, c->V, mode, factor, c->run_batches, c->opt.zero_air_dose);
+    ANM_CUDA(c, cudaGetLastError());
+    if (!on_device) ANM_CUDA(c, cudaMemcpyAsync(out, dst, c->V * 4, cudaMemcpyDeviceToHost, c->stream));
+    ANM_CUDA(c, cudaStreamSynchronize(c->stream));
+    return ANM_OK;
+}
+
+int anm_get_energy(anm_ctx* c, float* out, size_t n, int on_device) { return readout(c, out, n, on_device, 0, 1.0); }
+int anm_get_dose(anm_ctx* c, float* out, size_t n, int on_device) { return readout(c, out, n, on_device, 1, 1.0); }
+int anm_get_dose_rate(anm_ctx* c, double total_activity_Bq, float* out, size_t n, int on_device) {
+    if (c && !(total_activity_Bq >= 0 && std::isfinite(total_activity_Bq))) return fail(c, ANM_E_ARG, "dose rate: activity must be >= 0");
+    return readout(c, out, n, on_device, 1, total_activity_Bq);
+}
+int anm_get_uncertainty(anm_ctx* c, float* out, size_t n, int on_device) { return readout(c, out, n, on_device, 2, 1.0); }
+
+int anm_get_organ_doses(anm_ctx* c, anm_organ* out, int n_organs) {
+    if (!c) return ANM_E_ARG;
+    if (!out) return fail(c, ANM_E_ARG, "organ doses: null pointer");
+    if (!c->have_results || !c->have_organs) return fail(c, ANM_E_STATE, "organ doses: no completed run with organ labels");
+    if (n_organs != c->n_organs) return fail(c, ANM_E_ARG, "organ doses: n_organs = %d but %d were loaded", n_organs, c->n_organs);
+    std::memcpy(out, c->organs.data(), sizeof(anm_organ) * (size_t)n_organs);
+    return ANM_OK;
+}
+
+int anm_get_stats(anm_ctx* c, anm_stats* out) {
+    if (!c) return ANM_E_ARG;
+    if (!out) return fail(c, ANM_E_ARG, "stats: null pointer");
+    if (!c->have_results) return fail(c, ANM_E_STATE, "stats: no completed run");
+    *out = c->stats;
+    return ANM_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,364 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle -- the `-m gpu` tests.
+
+Parity here is statistical: the method is a Monte Carlo estimator, the two sides use
+different but distribution-equivalent algorithms and independent random streams (the oracle runs with
+seed + 1000).  Acceptance follows BASELINE.json north_star:
+  * per-organ mean dose within max(1.0 %, 3 combined sigma);
+  * |z| > 4 in < 0.1 % of the voxels above 10 % of the maximum dose;
+  * total deposited energy within 0.1 % (at >= 1e8 decays; for smaller runs within 4 combined sigma);
+plus what is exact on the GPU side: energy balance, counters, determinism, error codes, edge shapes.
+Full-size cases compare with tests/golden/ (written by tests/golden/make_golden.py from the oracle only).
+"""
+import csv
+import json
+import os
+
+import numpy as np
+import pytest
+
+import anm_inputs
+from oracle import anm_oracle as O
+
+pytestmark = pytest.mark.gpu
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+E0 = 0.51099895
+NPROC = min(32, os.cpu_count() or 1)
+
+
+@pytest.fixture(scope="module")
+def anm():
+    import paper_2111_11687_b200 as pkg
+    return pkg
+
+
+def gpu_run(anm, cfg, tables, n, seed=None, **opts):
+    with anm.Simulation(0) as sim:
+        sim.load_config(cfg, tables, **opts)
+        sim.run(n, cfg["seed"] if seed is None else seed)
+        out = {"energy": sim.get_energy().astype(np.float64), "dose": sim.get_dose().astype(np.float64),
+               "rel": sim.get_uncertainty().astype(np.float64), "stats": sim.get_stats()}
+        if cfg.get("n_organs"):
+            out["organs"] = sim.get_organ_doses()
+    return out
+
+
+def oracle_run(cfg, tables, n, n_batches, **over):
+    o = O.Oracle(cfg, tables, n_decays=n, n_batches=n_batches, seed=cfg["seed"] + 1000, **over)
+    r = o.run_parallel(NPROC)
+    f = o.finalize(r)
+    f["stats"] = r["stats"]
+    return f
+
+
+def check_organs(g, mean_o, sig_o, nvox_o, min_vox=1):
+    """north_star: per-organ mean dose within max(1 %, 3 combined sigma)."""
+    gm, gs = g["organs"]["mean_Gy_per_decay"], g["organs"]["sigma_mean"]
+    assert np.array_equal(g["organs"]["n_voxels"].astype(np.int64), np.asarray(nvox_o, np.int64))
+    sel = np.asarray(nvox_o) >= min_vox
+    assert sel.any()
+    diff = np.abs(gm[sel] - mean_o[sel])
+    tol = np.maximum(0.01 * mean_o[sel], 3.0 * np.sqrt(gs[sel] ** 2 + sig_o[sel] ** 2))
+    bad = diff > tol
+    assert not bad.any(), list(zip(np.nonzero(sel)[0][bad], (diff / mean_o[sel])[bad], (diff / (tol / 3 + 1e-300))[bad]))
+
+
+def check_voxels_z(dose_g, sig_g, dose_o, sig_o, material, frac=1e-3):
+    """north_star: |z| > 4 in < 0.1 % of voxels with (oracle) dose > 10 % of max.  Air voxels are left out
+    (PAPER.md:L119 sets the dose in air to zero; a single hit in 1.2 mg/cm^3 air would otherwise set the maximum)."""
+    dose_na = np.where(np.asarray(material).reshape(-1) != 0, dose_o, 0.0)
+    pop = dose_na > 0.1 * dose_na.max()
+    den = np.sqrt(sig_g[pop] ** 2 + sig_o[pop] ** 2)
+    z = (dose_g[pop] - dose_o[pop]) / np.where(den > 0, den, 1.0)
+    n_bad = int((np.abs(z) > 4).sum())
+    assert n_bad <= max(1, int(frac * pop.sum())), (n_bad, int(pop.sum()))
+    return z
+
+
+def check_balance(st, tol=2e-5):
+    assert abs(st["deposited_MeV"] + st["escaped_MeV"] - st["emitted_MeV"]) < tol * st["emitted_MeV"], st
+    assert st["n_real"] == st["n_pe"] + st["n_compton"] + st["n_rayleigh"] + 0 or st["n_real"] >= st["n_pe"] + st["n_compton"]
+
+
+def check_total(st_g, st_o, n, rel_floor=1e-3):
+    """total deposited energy: within 0.1 %, or 4 sigma of the MC noise for small runs."""
+    dep_g, dep_o = st_g["deposited_MeV"], st_o["deposited"]
+    noise = 4.0 * np.sqrt(2.0) * 0.4 / np.sqrt(n) / (dep_o / n)      # per-history deposit spread <= 0.4 MeV
+    assert abs(dep_g / dep_o - 1.0) < max(rel_floor, noise), (dep_g, dep_o)
+
+
+# ------------------------------------------------------------------------------------------------- cfg0 (full size)
+def test_cfg0_point_source_full(anm, tables):
+    cfg = anm_inputs.make_config(0)
+    n = cfg["n_decays"]                          # 1e6 histories, 10 batches, seed 1
+    g = gpu_run(anm, cfg, tables, n, collect_stats=1)
+    f = oracle_run(cfg, tables, n, cfg["n_batches"])
+    st, so = g["stats"], f["stats"]
+    check_balance(st)
+    assert abs(st["emitted_MeV"] - n * E0) < 1e-6 * n * E0 and st["n_decays"] == n
+    check_total(st, so, n)
+    assert abs(g["energy"].sum() - st["deposited_MeV"]) < 1e-6 * st["deposited_MeV"]
+    # radial dose profile (the paper's dose-distance comparison) through the shell labels
+    check_organs(g, f["organs"]["mean"], f["organs"]["sigma_mean"], f["organs"]["n_voxels"])
+    # event statistics are properties of the method, not of the tracking algorithm
+    for kg, ko in (("n_real", "n_collisions"), ("n_pe", "n_pe"), ("n_compton", "n_compton"), ("n_rayleigh", "n_rayleigh"),
+                   ("n_escaped", "n_escaped")):
+        a, b = st[kg], so[ko]
+        assert abs(a - b) < 5 * np.sqrt(a + b) + 1, (kg, a, b)
+    # dose and uncertainty read-outs are consistent with the energy map
+    vox_g = 0.4 ** 3 * 1.0
+    assert np.allclose(g["dose"], g["energy"] * 1.602176634e-10 / (n * vox_g), rtol=2e-6)
+    sel = f["dose"] > 0.2 * f["dose"].max()
+    ratio = g["rel"][sel] / f["rel_sigma"][sel]
+    assert 0.6 < np.median(ratio) < 1.6             # B = 10: sigma estimates scatter by ~25 %
+
+
+# ------------------------------------------------------------------------------------------------- small variants, oracle live
+@pytest.mark.parametrize("k,scale,n,B", [(1, 4, 1_000_000, 50), (2, 4, 1_000_000, 50), (3, 4, 2_000_000, 100)])
+def test_small_configs_vs_live_oracle(anm, tables, k, scale, n, B):
+    cfg = anm_inputs.make_config(k, scale)
+    g = gpu_run(anm, cfg, tables, n, n_batches=B, collect_stats=1)
+    f = oracle_run(cfg, tables, n, B)
+    check_balance(g["stats"])
+    check_total(g["stats"], f["stats"], n)
+    check_organs(g, f["organs"]["mean"], f["organs"]["sigma_mean"], f["organs"]["n_voxels"], min_vox=1)
+    z = check_voxels_z(g["dose"], g["dose"] * g["rel"], f["dose"], f["dose_sigma"], cfg["material"])
+    assert abs(z.mean()) < 5.0 / np.sqrt(z.size) + 0.05 and 0.8 < z.std() < 1.25, (z.mean(), z.std(), z.size)
+    # Eq. 3 organ RMS of voxel uncertainties agrees (same statistics on both sides)
+    big = f["organs"]["n_voxels"] >= 30
+    if big.any():
+        r = g["organs"]["rms_voxel_rel_sigma"][big] / f["organs"]["rms_voxel_rel_sigma"][big]
+        assert np.all(np.abs(r - 1) < 0.15), r
+        mw = g["organs"]["mass_weighted_Gy_per_decay"][big] / f["organs"]["mass_weighted"][big]
+        assert np.all(np.abs(mw - 1) < 0.05)
+        assert np.allclose(g["organs"]["mass_g"][big], f["organs"]["mass_g"][big], rtol=1e-6)
+
+
+def test_no_rayleigh_single_photon_vs_oracle(anm, tables):
+    cfg = anm_inputs.make_config(0, 2)
+    n, B = 1_000_000, 20
+    g = gpu_run(anm, cfg, tables, n, n_batches=B, rayleigh_on=0, collect_stats=1)
+    f = oracle_run(cfg, tables, n, B, rayleigh_on=0)
+    assert g["stats"]["n_rayleigh"] == 0
+    check_balance(g["stats"])
+    check_total(g["stats"], f["stats"], n)
+    check_organs(g, f["organs"]["mean"], f["organs"]["sigma_mean"], f["organs"]["n_voxels"])
+
+
+def test_high_cutoff_vs_oracle(anm, tables):
+    """PAPER.md:L67 cutoff branch: with a 0.3 MeV cutoff most Compton scatters end the photon locally."""
+    cfg = anm_inputs.make_config(0, 2)
+    n, B = 500_000, 20
+    g = gpu_run(anm, cfg, tables, n, n_batches=B, photon_cutoff_MeV=0.3, collect_stats=1)
+    f = oracle_run(cfg, tables, n, B, photon_cutoff_mev=0.3)
+    a, b = g["stats"]["n_cutoff"], f["stats"]["n_cutoff"]
+    assert b > 10000 and abs(a - b) < 5 * np.sqrt(a + b)
+    check_balance(g["stats"])
+    check_total(g["stats"], f["stats"], n)
+
+
+# ------------------------------------------------------------------------------------------------- full size vs golden
+def _golden(k):
+    tag = os.path.join(HERE, "golden", "cfg%d_oracle" % k)
+    meta = json.load(open(tag + "_meta.json"))
+    org = list(csv.DictReader(open(tag + "_organs.csv")))
+    vox = np.loadtxt(tag + "_voxels.csv", delimiter=",", skiprows=1, ndmin=2)
+    return meta, org, vox
+
+
+@pytest.mark.parametrize("k", [1, 2, 3])
+def test_full_size_vs_golden(anm, tables, k):
+    """cfg1/cfg2/cfg3 at full size, 1e8 decays, 100 batches, the config's own seed, in the launch configuration
+    bench.py times (collect_stats off); oracle side from tests/golden/ (1e8 decays, seed + 1000)."""
+    meta, org, vox = _golden(k)
+    cfg = anm_inputs.make_config(k)
+    assert list(meta["shape"]) == list(cfg["shape"]) and meta["n_decays"] == 100_000_000
+    n, B = 100_000_000, 100
+    with anm.Simulation(0) as sim:
+        sim.load_config(cfg, tables)
+        sim.run(n, cfg["seed"])
+        st = sim.get_stats()
+        energy = sim.get_energy()
+        organs = sim.get_organ_doses()
+        rel = sim.get_uncertainty()
+    # total deposited energy within 0.1 %
+    dep_o = meta["stats"]["deposited"]
+    assert abs(st["deposited_MeV"] / dep_o - 1.0) < 1e-3, (st["deposited_MeV"], dep_o)
+    # organs within max(1 %, 3 sigma)
+    g = {"organs": organs}
+    check_organs(g, np.array([float(r["mean_gy_per_decay"]) for r in org]), np.array([float(r["sigma_mean"]) for r in org]),
+                 np.array([int(r["n_voxels"]) for r in org]))
+    # sampled voxels above 10 % of the oracle's maximum dose: z-scores
+    idx = vox[:, 0].astype(np.int64)
+    S_o, Q_o = vox[:, 1], vox[:, 2]
+    nb = n / B
+    var_o = np.maximum((Q_o / (nb * nb) / B - (S_o / n) ** 2) / (B - 1), 0.0)       # of the per-decay mean energy
+    y_g = energy[idx].astype(np.float64) / n
+    s_g = y_g * rel[idx].astype(np.float64)
+    den = np.sqrt(var_o + s_g ** 2)
+    z = (y_g - S_o / n) / np.where(den > 0, den, 1.0)
+    assert (np.abs(z) > 4).sum() <= max(1, int(1e-3 * z.size)), ((np.abs(z) > 4).sum(), z.size)
+    if z.size > 1000:
+        assert abs(z.mean()) < 0.1 and 0.85 < z.std() < 1.2, (z.mean(), z.std())
+
+
+# ------------------------------------------------------------------------------------------------- exact properties
+def test_determinism_and_history_keying(anm, tables):
+    """Same seed -> same result up to fp32 atomic order; a run split with history_offset reproduces the whole."""
+    cfg = anm_inputs.make_config(2, 4)
+    n, B = 200_000, 10
+    a = gpu_run(anm, cfg, tables, n, n_batches=B)
+    b = gpu_run(anm, cfg, tables, n, n_batches=B)
+    assert np.allclose(a["energy"], b["energy"], rtol=1e-4, atol=1e-3)
+    assert abs(a["energy"].sum() / b["energy"].sum() - 1) < 1e-6
+    h1 = gpu_run(anm, cfg, tables, n // 2, n_batches=B // 2)
+    h2 = gpu_run(anm, cfg, tables, n // 2, n_batches=B // 2, history_offset=n // 2)
+    assert np.allclose(a["energy"], h1["energy"] + h2["energy"], rtol=1e-4, atol=1e-3)
+    c = gpu_run(anm, cfg, tables, n, n_batches=B, seed=cfg["seed"] + 7)
+    assert not np.allclose(a["energy"], c["energy"], rtol=1e-4, atol=1e-3)
+    w = gpu_run(anm, cfg, tables, n, n_batches=B, warp_aggregate=1)
+    assert np.allclose(a["energy"], w["energy"], rtol=1e-4, atol=1e-3)
+
+
+def test_positron_energy_lands_in_decay_voxels(anm, tables):
+    n = 4
+    act = np.zeros((n, n, n), np.float32)
+    act[1, 2, 3], act[0, 0, 0] = 3.0, 1.0
+    cfg = {"shape": (n, n, n), "spacing_mm": (1.0,) * 3, "material": np.zeros((n, n, n), np.uint8),
+           "density": np.full((n, n, n), 2.0 ** -20, np.float32), "activity": act, "point_source_mm": None,
+           "labels": None, "n_organs": 0, "n_batches": 4, "photons_per_decay": 2, "rayleigh_on": 1,
+           "photon_cutoff_mev": 0.010, "positron_ke_mev": 0.2498, "seed": 3}
+    g = gpu_run(anm, cfg, tables, 40_000, collect_stats=1)
+    e = g["energy"].reshape(n, n, n)
+    assert abs(e.sum() - 40_000 * 0.2498) < 1e-3 * 40_000 * 0.2498
+    assert set(zip(*np.nonzero(e))) == {(1, 2, 3), (0, 0, 0)}
+    assert abs(e[1, 2, 3] / e.sum() - 0.75) < 4 * np.sqrt(0.75 * 0.25 / 40_000)
+    assert g["stats"]["n_escaped"] == 80_000
+
+
+def test_ragged_and_degenerate_grids(anm, tables):
+    """V not a multiple of 4 (the fold's vector width); a single voxel; a single active voxel."""
+    rng = np.random.default_rng(4)
+    for shape in ((5, 3, 7), (1, 1, 1), (2, 1, 1)):
+        nx, ny, nz = shape
+        cfg = {"shape": shape, "spacing_mm": (30.0, 50.0, 40.0), "material": rng.integers(0, 4, (nz, ny, nx)).astype(np.uint8),
+               "density": anm_inputs.phantoms.quantize_density(rng.uniform(0.3, 1.9, (nz, ny, nx))),
+               "activity": np.ones((nz, ny, nx), np.float32), "point_source_mm": None,
+               "labels": np.ones((nz, ny, nx), np.uint8), "n_organs": 1, "n_batches": 5, "photons_per_decay": 2,
+               "rayleigh_on": 1, "photon_cutoff_mev": 0.010, "positron_ke_mev": 0.0, "seed": 9}
+        n, B = 100_000, 5
+        g = gpu_run(anm, cfg, tables, n, collect_stats=1)
+        check_balance(g["stats"])
+        f = oracle_run(cfg, tables, n, B)
+        check_total(g["stats"], f["stats"], n, rel_floor=2e-3)
+        check_organs(g, f["organs"]["mean"], f["organs"]["sigma_mean"], f["organs"]["n_voxels"])
+        z = (g["dose"] - f["dose"]) / np.sqrt((g["dose"] * g["rel"]) ** 2 + f["dose_sigma"] ** 2 + 1e-300)
+        assert np.abs(z).max() < 6.0
+
+
+def test_zero_air_dose_and_dose_rate(anm, tables):
+    cfg = anm_inputs.make_config(3, 8)
+    with anm.Simulation(0) as sim:
+        sim.load_config(cfg, tables, n_batches=10, zero_air_dose=1)
+        sim.run(200_000, 42)
+        d = sim.get_dose()
+        dr = sim.get_dose_rate(cfg["total_activity_bq"])
+        e = sim.get_energy()
+    air = cfg["material"].reshape(-1) == 0
+    assert np.all(d[air] == 0) and (e[air] > 0).any()               # PAPER.md:L119 "dose rates in the air are set to zero"
+    assert np.allclose(dr, d * np.float32(cfg["total_activity_bq"]), rtol=1e-6)   # Eq. 1
+    # organ dose rates have the paper's order of magnitude (Table 1: 1e-7 .. 5e-7 Gy/s), a sanity check only
+    assert 1e-8 < np.median(dr[(cfg["labels"].reshape(-1) > 0)]) < 1e-5
+
+
+def test_device_resident_inputs_and_outputs(anm, tables):
+    """on_device = 1 path: CUDA torch tensors in, CUDA torch tensor out, caller's stream."""
+    import torch
+    cfg = anm_inputs.make_config(2, 4)
+    dev = torch.device("cuda:0")
+    mat = torch.from_numpy(cfg["material"]).to(dev)
+    rho = torch.from_numpy(cfg["density"]).to(dev)
+    act = torch.from_numpy(cfg["activity"]).to(dev)
+    lab = torch.from_numpy(cfg["labels"]).to(dev)
+    stream = torch.cuda.Stream(device=dev)
+    ref = gpu_run(anm, cfg, tables, 100_000, n_batches=10)
+    with anm.Simulation(0) as sim, torch.cuda.stream(stream):
+        sim.set_stream(stream)
+        sim.set_grid(cfg["shape"], cfg["spacing_mm"])
+        sim.load_phantom(mat, rho)
+        sim.load_activity(act)
+        sim.load_organs(lab, cfg["n_organs"])
+        sim.set_physics_tables(tables)
+        sim.set_options(n_batches=10, photons_per_decay=2)
+        sim.run(100_000, cfg["seed"])
+        out = torch.empty(mat.numel(), dtype=torch.float32, device=dev)
+        sim.get_energy(out)
+        stream.synchronize()
+    assert np.allclose(out.cpu().numpy(), ref["energy"], rtol=1e-4, atol=1e-3)
+
+
+def test_error_codes(anm, tables):
+    E = anm.AnmError
+    cfg = anm_inputs.make_config(0, 4)
+    with anm.Simulation(0) as sim:
+        with pytest.raises(E) as ei:
+            sim.run(100, 1)
+        assert ei.value.code == -2                                   # ANM_E_STATE
+        with pytest.raises(E) as ei:
+            sim.set_grid((0, 4, 4), (1, 1, 1))
+        assert ei.value.code == -1
+        sim.set_grid(cfg["shape"], cfg["spacing_mm"])
+        bad = cfg["density"].copy()
+        bad[0, 0, 0] = np.nan
+        with pytest.raises(E) as ei:
+            sim.load_phantom(cfg["material"], bad)
+        assert ei.value.code == -1
+        bad[0, 0, 0] = -1.0
+        with pytest.raises(E):
+            sim.load_phantom(cfg["material"], bad)
+        sim.load_phantom(cfg["material"], cfg["density"])
+        with pytest.raises(E) as ei:
+            sim.load_activity(np.zeros(cfg["material"].shape, np.float32))
+        assert ei.value.code == -1                                   # all-zero activity
+        neg = np.ones(cfg["material"].shape, np.float32)
+        neg[1, 1, 1] = -2.0
+        with pytest.raises(E):
+            sim.load_activity(neg)
+        with pytest.raises(E):
+            sim.set_point_source((1e6, 0, 0))
+        sim.set_point_source(cfg["point_source_mm"])
+        with pytest.raises(E) as ei:
+            sim.run(100, 1)                                          # tables missing
+        assert ei.value.code == -2
+        sim.set_physics_tables(tables)
+        for kw in (dict(n_batches=1), dict(photons_per_decay=3), dict(photon_cutoff_MeV=0.0), dict(positron_ke_MeV=-1.0)):
+            with pytest.raises(E) as ei:
+                sim.set_options(**kw)
+            assert ei.value.code == -1
+        with pytest.raises(E) as ei:
+            sim.set_options(schedule=2)
+        assert ei.value.code == -5                                   # ANM_E_UNSUPPORTED
+        sim.set_options(n_batches=10, photons_per_decay=1)
+        with pytest.raises(E) as ei:
+            sim.run(1005, 1)                                         # N % B != 0 (reading C15)
+        assert ei.value.code == -1
+        with pytest.raises(E):
+            sim.run(0, 1)
+        with pytest.raises(E) as ei:
+            sim.get_energy()
+        assert ei.value.code == -2                                   # no completed run
+        lab = np.full(cfg["material"].shape, 9, np.uint8)
+        with pytest.raises(E) as ei:
+            sim.load_organs(lab, 3)                                  # label > n_organs
+        assert ei.value.code == -1
+        m5 = cfg["material"].copy()
+        m5[0, 0, 0] = 5
+        sim.load_phantom(m5, cfg["density"])
+        with pytest.raises(E) as ei:
+            sim.run(1000, 1)                                         # material id >= n_materials of the tables
+        assert ei.value.code == -1
+        sim.load_phantom(cfg["material"], cfg["density"])
+        sim.run(1000, 1)
+        assert sim.get_energy().sum() > 0
+        with pytest.raises(ValueError):
+            sim.get_energy(np.empty(7, np.float32))
