@@ -83,10 +83,12 @@ typedef struct {
     int32_t zero_air_dose;      /* 1: dose getters return 0 in voxels of material 0     */
     double photon_cutoff_MeV;   /* 0.010                                                  */
     double positron_ke_MeV;     /* 0, or e.g. 0.2498: deposited in the decay voxel                      */
-    int32_t schedule;           /* 0 auto, 1 history-based persistent lanes; 2 (event-based) unsupported */
+    int32_t schedule;           /* 0 auto, 1 history-based persistent lanes, 2 event-based warp pool
+                                   (regenerate in place, compact by event type); same histories either way */
     int32_t collect_stats;      /* 1: fill the counters and escaped energy of anm_stats (slower)         */
-    int32_t warp_aggregate;     /* 1: merge same-voxel deposits within a warp before the atomic          */
-    int32_t hull_majorant;      /* 1: low-density margin outside the phantom's hull gets its own majorant */
+    int32_t warp_aggregate;     /* 1: merge same-voxel deposits within a warp before the atomic (schedule 1) */
+    int32_t hull_majorant;      /* 0 auto / 1 on: flights outside the bounding box of the dense voxels use the
+                                   low-density margin's own majorant and stop on the box surface; 2 off     */
     uint64_t history_offset;    /* index of the first history: anm_run simulates offset .. offset+n_decays-1
                                    (multi-GPU sharding of one logical run by whole batches); default 0      */
 } anm_options;

@@ -17,6 +17,7 @@ using namespace anm;
 namespace {
 
 constexpr double kGyPerMeVPerGram = 1.602176634e-10;
+constexpr int kAutoSchedule = 2;   // anm_options.schedule = 0: the warp event pool (1.4x schedule 1 on cfg3, profiles/)
 
 template <typename T>
 struct DevBuf {
@@ -53,6 +54,11 @@ struct anm_ctx {
     double px = 0, py = 0, pz = 0;        // cm
     unsigned max_material = 0;
     unsigned rho_max_counts[ANM_MAX_MATERIALS] = {0};   // per material, in texel counts
+    // hull box: voxel index range [lo, hi) enclosing every voxel denser than 5 % of the densest one, and the
+    // per-material maximum density outside it; hull_ok = the box exists and is worth using (anm_options.hull_majorant)
+    bool hull_ok = false;
+    unsigned hull_lo[3] = {0, 0, 0}, hull_hi[3] = {0, 0, 0};
+    unsigned rho_max_out_counts[ANM_MAX_MATERIALS] = {0};
     int n_organs = 0;
     anm_options opt;
     // tables (host copies)
@@ -73,9 +79,9 @@ struct anm_ctx {
     DevBuf<double> organ_mass;            // [256]
     DevBuf<unsigned long long> organ_count;   // [256]
     DevBuf<double> total_energy;          // [1]
-    DevBuf<float> d_tot, d_maj, d_x2, d_cum;
+    DevBuf<float> d_tot, d_maj, d_majo, d_x2, d_cum;
     DevBuf<float2> d_pec;
-    DevBuf<unsigned> d_flags;             // [2 + ANM_MAX_MATERIALS]
+    DevBuf<unsigned> d_flags;             // [2 + ANM_MAX_MATERIALS] + [6 + ANM_MAX_MATERIALS] for the hull pass
     unsigned n_alias = 0;
 
     // results of the last run
@@ -165,7 +171,7 @@ int build_alias(anm_ctx* c, const float* act) {
 // tot / {pe, pe+co} / majorant tables on the device, for the current options and phantom
 int upload_tables(anm_ctx* c) {
     const int nm = c->nm, ne = c->ne;
-    std::vector<float> tot((size_t)nm * ne), maj(ne);
+    std::vector<float> tot((size_t)nm * ne), maj(ne), majo(ne);
     std::vector<float2> pec((size_t)nm * ne);
     for (int m = 0; m < nm; ++m)
         for (int k = 0; k < ne; ++k) {
@@ -182,15 +188,21 @@ int upload_tables(anm_ctx* c) {
             mx = std::max(mx, rho * tot[(size_t)m * ne + k]);
         }
         maj[k] = mx * 1.000001f + 1e-30f;    // head-room for fp32 rounding of rho * lerp
+        float mo = 0.0f;                     // the same bound over the voxels outside the hull box
+        for (int m = 0; m < nm; ++m)
+            mo = std::max(mo, (float)c->rho_max_out_counts[m] * kDensityStep * tot[(size_t)m * ne + k]);
+        majo[k] = c->hull_ok ? mo * 1.000001f + 1e-30f : maj[k];
     }
     ANM_CUDA(c, c->d_tot.alloc(tot.size()));
     ANM_CUDA(c, c->d_pec.alloc(pec.size()));
     ANM_CUDA(c, c->d_maj.alloc(maj.size()));
+    ANM_CUDA(c, c->d_majo.alloc(majo.size()));
     ANM_CUDA(c, c->d_x2.alloc(c->ray_x2.size()));
     ANM_CUDA(c, c->d_cum.alloc(c->ray_cum.size()));
     ANM_CUDA(c, cudaMemcpyAsync(c->d_tot.p, tot.data(), tot.size() * 4, cudaMemcpyHostToDevice, c->stream));
     ANM_CUDA(c, cudaMemcpyAsync(c->d_pec.p, pec.data(), pec.size() * 8, cudaMemcpyHostToDevice, c->stream));
     ANM_CUDA(c, cudaMemcpyAsync(c->d_maj.p, maj.data(), maj.size() * 4, cudaMemcpyHostToDevice, c->stream));
+    ANM_CUDA(c, cudaMemcpyAsync(c->d_majo.p, majo.data(), majo.size() * 4, cudaMemcpyHostToDevice, c->stream));
     ANM_CUDA(c, cudaMemcpyAsync(c->d_x2.p, c->ray_x2.data(), c->ray_x2.size() * 4, cudaMemcpyHostToDevice, c->stream));
     ANM_CUDA(c, cudaMemcpyAsync(c->d_cum.p, c->ray_cum.data(), c->ray_cum.size() * 4, cudaMemcpyHostToDevice, c->stream));
     ANM_CUDA(c, cudaStreamSynchronize(c->stream));
@@ -200,10 +212,13 @@ int upload_tables(anm_ctx* c) {
 
 struct HostE0 { int ie; float fe, maj, inv_maj; };
 
-template <bool S, bool W>
-cudaError_t launch_transport(int blocks, size_t smem, cudaStream_t st, const TransportParams& p) {
-    transport_kernel<S, W><<<blocks, kThreads, smem, st>>>(p);
-    return cudaGetLastError();
+using TransportFn = void (*)(const TransportParams);
+
+// schedule 1 (history-based lanes) or 2 (warp-scope event pool), with / without counters and warp aggregation
+TransportFn pick_transport(int schedule, bool stats, bool wagg) {
+    if (schedule == 2) return stats ? transport_pool_kernel<true> : transport_pool_kernel<false>;
+    return stats ? (wagg ? transport_kernel<true, true> : transport_kernel<true, false>)
+                 : (wagg ? transport_kernel<false, true> : transport_kernel<false, false>);
 }
 
 }  // namespace
@@ -246,7 +261,7 @@ int anm_destroy(anm_ctx* c) {
     c->texels.release(); c->batch.release(); c->sum.release(); c->sumsq.release(); c->scratch.release();
     c->labels.release(); c->alias.release(); c->counters.release(); c->dstats.release();
     c->organ_batch.release(); c->organ_acc.release(); c->organ_mass.release(); c->organ_count.release();
-    c->total_energy.release(); c->d_tot.release(); c->d_maj.release(); c->d_x2.release(); c->d_cum.release();
+    c->total_energy.release(); c->d_tot.release(); c->d_maj.release(); c->d_majo.release(); c->d_x2.release(); c->d_cum.release();
     c->d_pec.release(); c->d_flags.release();
     delete c;
     return ANM_OK;
@@ -282,7 +297,7 @@ int anm_set_grid(anm_ctx* c, int nx, int ny, int nz, double dx_mm, double dy_mm,
     ANM_CUDA(c, c->sumsq.alloc(c->Vpad));
     ANM_CUDA(c, cudaMemsetAsync(c->texels.p, 0, c->Vpad * 4, c->stream));
     ANM_CUDA(c, cudaMemsetAsync(c->batch.p, 0, c->Vpad * 4, c->stream));
-    ANM_CUDA(c, c->d_flags.alloc(2 + ANM_MAX_MATERIALS));
+    ANM_CUDA(c, c->d_flags.alloc(2 + ANM_MAX_MATERIALS + 6 + ANM_MAX_MATERIALS));
     ANM_CUDA(c, c->dstats.alloc(1));
     ANM_CUDA(c, c->total_energy.alloc(1));
     ANM_CUDA(c, c->organ_acc.alloc(256));
@@ -310,7 +325,7 @@ int anm_load_phantom(anm_ctx* c, const uint8_t* material, const float* density, 
         ANM_CUDA(c, cudaMemcpyAsync(c->scratch.p, density, c->V * 4, cudaMemcpyHostToDevice, c->stream));
         d_mat = stage_m.p; d_rho = c->scratch.p;
     }
-    ANM_CUDA(c, cudaMemsetAsync(c->d_flags.p, 0, (2 + ANM_MAX_MATERIALS) * 4, c->stream));
+    ANM_CUDA(c, cudaMemsetAsync(c->d_flags.p, 0, (2 + ANM_MAX_MATERIALS + 6 + ANM_MAX_MATERIALS) * 4, c->stream));
     pack_texels_kernel<<<grid_blocks(c, c->V, kFoldThreads), kFoldThreads, 0, c->stream>>>(
         d_mat, d_rho, c->texels.p, c->V, c->d_flags.p, c->d_flags.p + 1);
     ANM_CUDA(c, cudaGetLastError());
@@ -334,6 +349,34 @@ int anm_load_phantom(anm_ctx* c, const uint8_t* material, const float* density, 
         ANM_CUDA(c, cudaGetLastError());
         ANM_CUDA(c, cudaMemcpyAsync(c->rho_max_counts, c->d_flags.p + 2, ANM_MAX_MATERIALS * 4, cudaMemcpyDeviceToHost, c->stream));
         ANM_CUDA(c, cudaStreamSynchronize(c->stream));
+    }
+    {   // hull box: bounding box of the voxels denser than 5 % of the densest voxel; outside it the majorant is
+        // that of the low-density margin (air around a patient).  Used only when the box is a proper part of the grid.
+        unsigned rmax = 0;
+        for (int m = 0; m < ANM_MAX_MATERIALS; ++m) rmax = std::max(rmax, c->rho_max_counts[m]);
+        unsigned* d_box = c->d_flags.p + 2 + ANM_MAX_MATERIALS;
+        const unsigned init[6] = {0xffffffffu, 0xffffffffu, 0xffffffffu, 0u, 0u, 0u};
+        ANM_CUDA(c, cudaMemcpyAsync(d_box, init, sizeof init, cudaMemcpyHostToDevice, c->stream));
+        hull_box_kernel<<<grid_blocks(c, (size_t)c->ny * c->nz, kFoldThreads / 32), kFoldThreads, 0, c->stream>>>(
+            c->texels.p, c->nx, c->ny, c->nz, rmax / 20u, d_box);
+        ANM_CUDA(c, cudaGetLastError());
+        unsigned box[6];
+        ANM_CUDA(c, cudaMemcpyAsync(box, d_box, sizeof box, cudaMemcpyDeviceToHost, c->stream));
+        ANM_CUDA(c, cudaStreamSynchronize(c->stream));
+        c->hull_ok = false;
+        std::memset(c->rho_max_out_counts, 0, sizeof c->rho_max_out_counts);
+        if (box[3] > box[0] && box[4] > box[1] && box[5] > box[2]) {
+            const double vol = (double)(box[3] - box[0]) * (box[4] - box[1]) * (box[5] - box[2]);
+            if (vol <= 0.9 * (double)c->V) {
+                rho_max_outside_kernel<<<grid_blocks(c, c->V, kFoldThreads), kFoldThreads, 0, c->stream>>>(
+                    c->texels.p, c->nx, c->ny, c->nz, box[0], box[1], box[2], box[3], box[4], box[5], d_box + 6);
+                ANM_CUDA(c, cudaGetLastError());
+                ANM_CUDA(c, cudaMemcpyAsync(c->rho_max_out_counts, d_box + 6, ANM_MAX_MATERIALS * 4, cudaMemcpyDeviceToHost, c->stream));
+                ANM_CUDA(c, cudaStreamSynchronize(c->stream));
+                for (int k = 0; k < 3; ++k) { c->hull_lo[k] = box[k]; c->hull_hi[k] = box[3 + k]; }
+                c->hull_ok = true;
+            }
+        }
     }
     c->have_phantom = true;
     c->have_results = false;
@@ -455,8 +498,9 @@ int anm_set_options(anm_ctx* c, const anm_options* o) {
     if (o->photons_per_decay != 1 && o->photons_per_decay != 2) return fail(c, ANM_E_ARG, "options: photons_per_decay must be 1 or 2");
     if (!(o->photon_cutoff_MeV > 0) || !(o->photon_cutoff_MeV < 0.51099895)) return fail(c, ANM_E_ARG, "options: photon cutoff out of range");
     if (!(o->positron_ke_MeV >= 0) || !std::isfinite(o->positron_ke_MeV)) return fail(c, ANM_E_ARG, "options: positron energy must be >= 0");
-    if (o->schedule == 2) return fail(c, ANM_E_UNSUPPORTED, "options: event-based scheduling is not built (DESIGN.md: history-based chosen from the counters)");
     if (o->schedule < 0 || o->schedule > 2) return fail(c, ANM_E_ARG, "options: schedule must be 0, 1 or 2");
+    if (o->hull_majorant < 0 || o->hull_majorant > 2) return fail(c, ANM_E_ARG, "options: hull_majorant must be 0, 1 or 2");
+    if (o->schedule == 2 && o->warp_aggregate) return fail(c, ANM_E_UNSUPPORTED, "options: warp_aggregate is a schedule-1 option");
     c->opt = *o;
     c->dev_tables_dirty = true;
     c->have_results = false;
@@ -505,6 +549,16 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     p.px = (float)c->px; p.py = (float)c->py; p.pz = (float)c->pz;
     p.point_source = c->point_source ? 1 : 0;
     p.photons_per_decay = c->opt.photons_per_decay; p.rayleigh_on = c->opt.rayleigh_on;
+    p.tab_maj_out = c->d_majo.p;
+    p.hull = (c->hull_ok && c->opt.hull_majorant != 2) ? 1 : 0;
+    if (p.hull) {
+        const double d[3] = {c->dx, c->dy, c->dz};
+        float lo[3], hi[3];
+        for (int k = 0; k < 3; ++k) { lo[k] = (float)(c->hull_lo[k] * d[k]); hi[k] = (float)(c->hull_hi[k] * d[k]); }
+        p.bx0 = lo[0]; p.by0 = lo[1]; p.bz0 = lo[2]; p.bx1 = hi[0]; p.by1 = hi[1]; p.bz1 = hi[2];
+        p.bx0m = nextafterf(lo[0], -INFINITY); p.by0m = nextafterf(lo[1], -INFINITY); p.bz0m = nextafterf(lo[2], -INFINITY);
+        p.bx1m = nextafterf(hi[0], -INFINITY); p.by1m = nextafterf(hi[1], -INFINITY); p.bz1m = nextafterf(hi[2], -INFINITY);
+    }
     {   // energy-dependent quantities at E0, computed exactly like the device's set_energy (fp32)
         std::vector<float> maj(c->ne);
         ANM_CUDA(c, cudaMemcpyAsync(maj.data(), c->d_maj.p, (size_t)c->ne * 4, cudaMemcpyDeviceToHost, st));
@@ -516,17 +570,19 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
         p.inv_maj0 = 1.0f / p.maj0;
     }
 
-    const size_t smem = (size_t)c->nm * c->ne * 12 + (size_t)c->ne * 4 + (size_t)c->n_x2 * 4 +
-                        (size_t)c->nm * c->n_x2 * 4 + 6 * kThreads * 4;
+    const int schedule = c->opt.schedule == 0 ? kAutoSchedule : c->opt.schedule;
+    const size_t smem_tables = (size_t)c->nm * c->ne * 12 + (size_t)c->ne * 8 + (size_t)c->n_x2 * 4 + (size_t)c->nm * c->n_x2 * 4;
+    const int threads = schedule == 2 ? kPoolThreads : kThreads;
+    const size_t smem = smem_tables + (schedule == 2 ? (size_t)kPoolWarps * kPoolWarpBytes : (size_t)6 * kThreads * 4);
     const bool S = c->opt.collect_stats != 0, W = c->opt.warp_aggregate != 0;
-    auto kern = S ? (W ? (const void*)transport_kernel<true, true> : (const void*)transport_kernel<true, false>)
-                  : (W ? (const void*)transport_kernel<false, true> : (const void*)transport_kernel<false, false>);
+    const TransportFn kern = pick_transport(schedule, S, W);
     ANM_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 0;
-    ANM_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kThreads, smem));
+    ANM_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem));
     if (per_sm < 1) return fail(c, ANM_E_UNSUPPORTED, "run: tables too large for shared memory (%zu bytes)", smem);
-    // persistent lanes: one resident wave; never more lanes than histories
-    const int blocks = (int)std::max<uint64_t>(1, std::min<uint64_t>((uint64_t)c->num_sms * per_sm, (nb + kThreads - 1) / kThreads));
+    // persistent lanes: one resident wave; never more photon slots than histories
+    const uint64_t per_block = schedule == 2 ? (uint64_t)kPoolWarps * kSlots : (uint64_t)kThreads;
+    const int blocks = (int)std::max<uint64_t>(1, std::min<uint64_t>((uint64_t)c->num_sms * per_sm, (nb + per_block - 1) / per_block));
     const int fold_blocks = grid_blocks(c, c->Vpad / 4, kFoldThreads);
     const float inv_vox = (float)(1.0 / (c->dx * c->dy * c->dz));
 
@@ -540,9 +596,8 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     for (int b = 0; b < B; ++b) {
         p.counter = c->counters.p + b;
         p.hist_base = c->opt.history_offset + (unsigned long long)b * nb;
-        cudaError_t le = S ? (W ? launch_transport<true, true>(blocks, smem, st, p) : launch_transport<true, false>(blocks, smem, st, p))
-                           : (W ? launch_transport<false, true>(blocks, smem, st, p) : launch_transport<false, false>(blocks, smem, st, p));
-        ANM_CUDA_EV(le);
+        kern<<<blocks, threads, smem, st>>>(p);
+        ANM_CUDA_EV(cudaGetLastError());
         ANM_CUDA_EV(cudaEventRecord(ev[2 * b + 1], st));
         fold_kernel<<<fold_blocks, kFoldThreads, 0, st>>>(
             (float4*)c->batch.p, (float4*)c->sum.p, (float4*)c->sumsq.p,

@@ -9,8 +9,12 @@ estimates are statistically independent -- and writes
   cfg<k>_oracle_organs.csv    per organ: Eq. 2 mean (Gy/decay), batch sigma of the mean, Eq. 3 RMS,
                               mass-weighted dose, voxel counts
   cfg<k>_oracle_voxels.csv    a seeded random sample of the non-air voxels (material != 0; the paper sets the
-                              dose in air to zero) with oracle dose > 10 % of their maximum:
-                              linear index, sum_b x, sum_b x^2 (MeV, MeV^2)  ->  per-voxel z-scores
+                              dose in air to zero) with oracle dose > 5 % of their maximum:
+                              linear index, sum_b x, sum_b x^2 (MeV, MeV^2)  ->  per-voxel z-scores.
+                              The 5 % pre-selection is deliberately wider than north_star's "> 10 % of max":
+                              the test applies the 10 % cut to the MEAN of the two estimates, which is
+                              uncorrelated with their difference; cutting on the oracle's own noisy value
+                              would select its upward fluctuations and bias z (regression to the mean).
 No value in these files comes from the CUDA path.
 """
 import argparse
@@ -32,7 +36,7 @@ def main():
     ap.add_argument("--cfg", type=int, required=True)
     ap.add_argument("--decays", type=float, default=1e8)
     ap.add_argument("--procs", type=int, default=os.cpu_count())
-    ap.add_argument("--sample", type=int, default=10000)
+    ap.add_argument("--sample", type=int, default=20000)
     a = ap.parse_args()
     cfg = anm_inputs.make_config(a.cfg)
     tables = anm_inputs.make_tables()
@@ -45,6 +49,7 @@ def main():
     meta = {"config": cfg["name"], "shape": cfg["shape"], "spacing_mm": cfg["spacing_mm"], "n_decays": n,
             "n_batches": 100, "seed": seed, "cores": r["cores"], "wall_seconds": r["seconds"],
             "stats": r["stats"], "max_dose_gy_per_decay_non_air": float(np.where(o.material != 0, f["dose"], 0.0).max()),
+            "voxel_preselection": "non-air, oracle dose > 0.05 * max_dose_gy_per_decay_non_air",
             "written_by": "tests/golden/make_golden.py (oracle only)"}
     json.dump(meta, open(tag + "_meta.json", "w"), indent=1)
     if "organs" in f:
@@ -56,7 +61,7 @@ def main():
                     i + 1, name, og["mean"][i], og["sigma_mean"][i], og["rms_voxel_rel_sigma"][i],
                     og["mass_weighted"][i], og["mass_g"][i], og["n_voxels"][i], og["n_voxels_nonzero"][i]))
     dose_na = np.where(o.material != 0, f["dose"], 0.0)
-    pop = np.nonzero(dose_na > 0.1 * dose_na.max())[0]
+    pop = np.nonzero(dose_na > 0.05 * dose_na.max())[0]
     rng = np.random.default_rng(2111)
     pick = np.sort(rng.choice(pop, size=min(a.sample, pop.size), replace=False))
     with open(tag + "_voxels.csv", "w") as fh:

@@ -64,10 +64,12 @@ def check_organs(g, mean_o, sig_o, nvox_o, min_vox=1):
 
 
 def check_voxels_z(dose_g, sig_g, dose_o, sig_o, material, frac=1e-3):
-    """north_star: |z| > 4 in < 0.1 % of voxels with (oracle) dose > 10 % of max.  Air voxels are left out
-    (PAPER.md:L119 sets the dose in air to zero; a single hit in 1.2 mg/cm^3 air would otherwise set the maximum)."""
-    dose_na = np.where(np.asarray(material).reshape(-1) != 0, dose_o, 0.0)
-    pop = dose_na > 0.1 * dose_na.max()
+    """north_star: |z| > 4 in < 0.1 % of voxels with dose > 10 % of max.  Air voxels are left out (PAPER.md:L119
+    sets the dose in air to zero; a single hit in 1.2 mg/cm^3 air would otherwise set the maximum).  The 10 % cut is
+    applied to the mean of the two estimates: that is uncorrelated with their difference, whereas a cut on either
+    side's own noisy value selects its upward fluctuations and biases z."""
+    not_air = np.asarray(material).reshape(-1) != 0
+    pop = not_air & (0.5 * (dose_g + dose_o) > 0.1 * np.where(not_air, dose_o, 0.0).max())
     den = np.sqrt(sig_g[pop] ** 2 + sig_o[pop] ** 2)
     z = (dose_g[pop] - dose_o[pop]) / np.where(den > 0, den, 1.0)
     n_bad = int((np.abs(z) > 4).sum())
@@ -188,10 +190,16 @@ def test_full_size_vs_golden(anm, tables, k):
     g = {"organs": organs}
     check_organs(g, np.array([float(r["mean_gy_per_decay"]) for r in org]), np.array([float(r["sigma_mean"]) for r in org]),
                  np.array([int(r["n_voxels"]) for r in org]))
-    # sampled voxels above 10 % of the oracle's maximum dose: z-scores
+    # sampled non-air voxels (pre-selected by the oracle at > 5 % of its maximum) whose dose, averaged over the two
+    # estimates, is above 10 % of the oracle's maximum: z-scores (the symmetric cut does not bias z)
     idx = vox[:, 0].astype(np.int64)
     S_o, Q_o = vox[:, 1], vox[:, 2]
     nb = n / B
+    vox_g = cfg["density"].reshape(-1)[idx].astype(np.float64) * float(np.prod(cfg["spacing_mm"])) * 1e-3
+    dose_mean = 0.5 * (energy[idx].astype(np.float64) + S_o) / n * 1.602176634e-10 / vox_g
+    keep = dose_mean > 0.1 * meta["max_dose_gy_per_decay_non_air"]
+    assert keep.sum() >= min(10, keep.size)
+    idx, S_o, Q_o = idx[keep], S_o[keep], Q_o[keep]
     var_o = np.maximum((Q_o / (nb * nb) / B - (S_o / n) ** 2) / (B - 1), 0.0)       # of the per-decay mean energy
     y_g = energy[idx].astype(np.float64) / n
     s_g = y_g * rel[idx].astype(np.float64)
@@ -218,6 +226,34 @@ def test_determinism_and_history_keying(anm, tables):
     assert not np.allclose(a["energy"], c["energy"], rtol=1e-4, atol=1e-3)
     w = gpu_run(anm, cfg, tables, n, n_batches=B, warp_aggregate=1)
     assert np.allclose(a["energy"], w["energy"], rtol=1e-4, atol=1e-3)
+
+
+@pytest.mark.parametrize("k,scale,n,B", [(3, 4, 400_000, 10), (0, 2, 200_000, 10), (2, 4, 200_000, 10)])
+def test_schedules_and_hull_run_the_same_histories(anm, tables, k, scale, n, B):
+    """Schedule 1 (history lanes) and 2 (warp event pool) consume the same Philox counters with the same per-event
+    arithmetic: identical counters, energies equal up to fp32 atomic order.  The hull majorant changes the flights
+    (different draws) but not the distribution: totals agree statistically, energy balance stays exact."""
+    cfg = anm_inputs.make_config(k, scale)
+    a = gpu_run(anm, cfg, tables, n, n_batches=B, collect_stats=1, schedule=1, hull_majorant=2)
+    b = gpu_run(anm, cfg, tables, n, n_batches=B, collect_stats=1, schedule=2, hull_majorant=2)
+    for key in ("n_steps", "n_real", "n_pe", "n_compton", "n_rayleigh", "n_escaped", "n_cutoff"):
+        assert a["stats"][key] == b["stats"][key], key
+    assert np.allclose(a["energy"], b["energy"], rtol=1e-4, atol=1e-3)
+    assert abs(a["stats"]["escaped_MeV"] / b["stats"]["escaped_MeV"] - 1) < 1e-5
+    for sched in (1, 2):
+        h = gpu_run(anm, cfg, tables, n, n_batches=B, collect_stats=1, schedule=sched, hull_majorant=1)
+        check_balance(h["stats"])
+        sd = 0.4 * np.sqrt(2.0 * n)                                  # per-history deposit spread <= 0.4 MeV
+        assert abs(h["stats"]["deposited_MeV"] - a["stats"]["deposited_MeV"]) < 5 * sd
+        for key in ("n_real", "n_pe", "n_compton", "n_escaped"):
+            x, y = h["stats"][key], a["stats"][key]
+            assert abs(x - y) < 6 * np.sqrt(x + y) + 1, (key, x, y)
+        if k == 3:
+            assert h["stats"]["n_steps"] < 0.95 * a["stats"]["n_steps"]    # fewer virtual collisions in the air margin
+    hs = [gpu_run(anm, cfg, tables, n, n_batches=B, collect_stats=1, schedule=s, hull_majorant=1) for s in (1, 2)]
+    for key in ("n_steps", "n_real", "n_pe", "n_compton", "n_rayleigh", "n_escaped", "n_cutoff"):
+        assert hs[0]["stats"][key] == hs[1]["stats"][key], key
+    assert np.allclose(hs[0]["energy"], hs[1]["energy"], rtol=1e-4, atol=1e-3)
 
 
 def test_positron_energy_lands_in_decay_voxels(anm, tables):
@@ -335,8 +371,12 @@ def test_error_codes(anm, tables):
             with pytest.raises(E) as ei:
                 sim.set_options(**kw)
             assert ei.value.code == -1
+        for kw in (dict(schedule=3), dict(hull_majorant=3)):
+            with pytest.raises(E) as ei:
+                sim.set_options(**kw)
+            assert ei.value.code == -1
         with pytest.raises(E) as ei:
-            sim.set_options(schedule=2)
+            sim.set_options(schedule=2, warp_aggregate=1)
         assert ei.value.code == -5                                   # ANM_E_UNSUPPORTED
         sim.set_options(n_batches=10, photons_per_decay=1)
         with pytest.raises(E) as ei:
