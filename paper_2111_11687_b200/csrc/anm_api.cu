@@ -554,20 +554,23 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     if (p.hull) {
         const double d[3] = {c->dx, c->dy, c->dz};
         float lo[3], hi[3];
-        for (int k = 0; k < 3; ++k) { lo[k] = (float)(c->hull_lo[k] * d[k]); hi[k] = (float)(c->hull_hi[k] * d[k]); }
+        // faces pushed outwards by 1e-3 voxel: far more than the fp32 rounding of x * inv_dx at the face, so a photon
+        // the test calls "outside" can never index a voxel of the box
+        for (int k = 0; k < 3; ++k) { lo[k] = (float)((c->hull_lo[k] - 1e-3) * d[k]); hi[k] = (float)((c->hull_hi[k] + 1e-3) * d[k]); }
         p.bx0 = lo[0]; p.by0 = lo[1]; p.bz0 = lo[2]; p.bx1 = hi[0]; p.by1 = hi[1]; p.bz1 = hi[2];
-        p.bx0m = nextafterf(lo[0], -INFINITY); p.by0m = nextafterf(lo[1], -INFINITY); p.bz0m = nextafterf(lo[2], -INFINITY);
-        p.bx1m = nextafterf(hi[0], -INFINITY); p.by1m = nextafterf(hi[1], -INFINITY); p.bz1m = nextafterf(hi[2], -INFINITY);
     }
     {   // energy-dependent quantities at E0, computed exactly like the device's set_energy (fp32)
-        std::vector<float> maj(c->ne);
+        std::vector<float> maj(c->ne), majo(c->ne);
         ANM_CUDA(c, cudaMemcpyAsync(maj.data(), c->d_maj.p, (size_t)c->ne * 4, cudaMemcpyDeviceToHost, st));
+        ANM_CUDA(c, cudaMemcpyAsync(majo.data(), c->d_majo.p, (size_t)c->ne * 4, cudaMemcpyDeviceToHost, st));
         ANM_CUDA(c, cudaStreamSynchronize(st));
         const float t = (logf(kE0) - p.lnE_min) * p.inv_dlnE;
         int i = std::max(0, std::min((int)t, c->ne - 2));
         p.ie0 = i; p.fe0 = t - (float)i;
         p.maj0 = fmaf(p.fe0, maj[i + 1] - maj[i], maj[i]);
         p.inv_maj0 = 1.0f / p.maj0;
+        p.majo0 = fmaf(p.fe0, majo[i + 1] - majo[i], majo[i]);
+        p.inv_majo0 = 1.0f / p.majo0;
     }
 
     const int schedule = c->opt.schedule == 0 ? kAutoSchedule : c->opt.schedule;

@@ -66,12 +66,12 @@ struct TransportParams {
     int point_source, photons_per_decay, rayleigh_on;
     // energy-dependent quantities at E0 (every photon starts there)
     int ie0; float fe0, maj0, inv_maj0;
-    // hull majorant (anm_options.hull_majorant): the axis-aligned box [b?0, b?1) cm encloses every voxel denser than
-    // the hull threshold; inside it flights use tab_maj, outside tab_maj_out (the low-density margin's own bound).
-    // A flight never crosses the box surface: it stops there and a fresh one starts (memoryless => exact).
+    // hull majorant (anm_options.hull_majorant): the axis-aligned box (b?0, b?1) cm encloses every voxel denser than
+    // the hull threshold (faces pushed outwards by a rounding margin).  A photon beyond a face and moving away from
+    // it flies against tab_maj_out (the bound of the voxels outside the box); every other photon against tab_maj.
     int hull;
     float bx0, bx1, by0, by1, bz0, bz1;      // faces (cm)
-    float bx0m, bx1m, by0m, by1m, bz0m, bz1m;   // nextafter(face, -inf): just below the face
+    float majo0, inv_majo0;                   // tab_maj_out at E0
     const float* tab_maj_out;    // [ne]
 };
 
@@ -133,64 +133,26 @@ struct FlyCounters { unsigned steps, real; };
 
 template <bool STATS>
 __device__ __forceinline__ int fly_substep(const TransportParams& p, const float* __restrict__ s_tot,
-                                           const float2* __restrict__ s_pec, const float* __restrict__ s_maj_out,
+                                           const float2* __restrict__ s_pec,
                                            float& x, float& y, float& z, const float u, const float v, const float w,
                                            const int ie, const float fe, const float maj, const float inv_maj,
+                                           const float maj_out, const float inv_maj_out,
                                            const unsigned r_s, const unsigned r_a, unsigned& vox, int& mat,
                                            FlyCounters& cnt) {
     const float nl = -__logf(u01(r_s));
-    float m_here = maj;
-    bool need_grid_test = true;
     if (STATS) ++cnt.steps;
-    if (p.hull) {
-        const bool in_box = x >= p.bx0 && x < p.bx1 && y >= p.by0 && y < p.by1 && z >= p.bz0 && z < p.bz1;
-        if (in_box) {
-            const float s = nl * inv_maj;
-            x = fmaf(s, u, x); y = fmaf(s, v, y); z = fmaf(s, w, z);
-            const bool still = x >= p.bx0 && x < p.bx1 && y >= p.by0 && y < p.by1 && z >= p.bz0 && z < p.bz1;
-            if (!still) {
-                // stop on the box surface: walk back along the ray to the first face crossed
-                const float tx = (x >= p.bx1) ? __fdividef(x - p.bx1, u) : (x < p.bx0) ? __fdividef(x - p.bx0, u) : 0.0f;
-                const float ty = (y >= p.by1) ? __fdividef(y - p.by1, v) : (y < p.by0) ? __fdividef(y - p.by0, v) : 0.0f;
-                const float tz = (z >= p.bz1) ? __fdividef(z - p.bz1, w) : (z < p.bz0) ? __fdividef(z - p.bz0, w) : 0.0f;
-                const float tb = fmaxf(tx, fmaxf(ty, tz));
-                x = fmaf(-tb, u, x); y = fmaf(-tb, v, y); z = fmaf(-tb, w, z);
-                if (tb == tx) x = (u > 0.0f) ? p.bx1 : p.bx0m;           // exactly outside through that face
-                else if (tb == ty) y = (v > 0.0f) ? p.by1 : p.by0m;
-                else z = (w > 0.0f) ? p.bz1 : p.bz0m;
-                const int ix = __float2int_rd(x * p.inv_dx), iy = __float2int_rd(y * p.inv_dy), iz = __float2int_rd(z * p.inv_dz);
-                if ((unsigned)ix >= (unsigned)p.nx || (unsigned)iy >= (unsigned)p.ny || (unsigned)iz >= (unsigned)p.nz)
-                    return FLY_ESCAPED;                                  // the box face is a grid face
-                return FLY_GO;
-            }
-            need_grid_test = false;
-        } else {
-            m_here = fmaf(fe, s_maj_out[ie + 1] - s_maj_out[ie], s_maj_out[ie]);
-            const float s = __fdividef(nl, m_here);
-            // slab test against the box
-            const float iu = __fdividef(1.0f, copysignf(fmaxf(fabsf(u), 1e-20f), u));
-            const float iv = __fdividef(1.0f, copysignf(fmaxf(fabsf(v), 1e-20f), v));
-            const float iw = __fdividef(1.0f, copysignf(fmaxf(fabsf(w), 1e-20f), w));
-            const float ax = (p.bx0 - x) * iu, bx = (p.bx1 - x) * iu;
-            const float ay = (p.by0 - y) * iv, by = (p.by1 - y) * iv;
-            const float az = (p.bz0 - z) * iw, bz = (p.bz1 - z) * iw;
-            const float t_in = fmaxf(fmaxf(fminf(ax, bx), fminf(ay, by)), fminf(az, bz));
-            const float t_out = fminf(fminf(fmaxf(ax, bx), fmaxf(ay, by)), fmaxf(az, bz));
-            if (t_in <= t_out && t_in >= 0.0f && t_in <= s) {            // reaches the box first: stop on its surface
-                x = fminf(fmaxf(fmaf(t_in, u, x), p.bx0), p.bx1m);
-                y = fminf(fmaxf(fmaf(t_in, v, y), p.by0), p.by1m);
-                z = fminf(fmaxf(fmaf(t_in, w, z), p.bz0), p.bz1m);
-                return FLY_GO;
-            }
-            x = fmaf(s, u, x); y = fmaf(s, v, y); z = fmaf(s, w, z);
-        }
-    } else {
-        const float s = nl * inv_maj;
-        x = fmaf(s, u, x); y = fmaf(s, v, y); z = fmaf(s, w, z);
-    }
+    // Hull majorant (reading C24), branch-free: a photon that is beyond a face of the hull box and moving
+    // away from it stays outside the (convex) box along its whole ray, so the majorant of the voxels outside the box
+    // bounds mu on every point it can reach; any other photon uses the global majorant, which is valid everywhere.
+    bool away = false;
+    if (p.hull)
+        away = (x >= p.bx1 && u >= 0.0f) || (x < p.bx0 && u <= 0.0f) || (y >= p.by1 && v >= 0.0f) ||
+               (y < p.by0 && v <= 0.0f) || (z >= p.bz1 && w >= 0.0f) || (z < p.bz0 && w <= 0.0f);
+    const float m_here = away ? maj_out : maj;
+    const float s = nl * (away ? inv_maj_out : inv_maj);
+    x = fmaf(s, u, x); y = fmaf(s, v, y); z = fmaf(s, w, z);
     const int ix = __float2int_rd(x * p.inv_dx), iy = __float2int_rd(y * p.inv_dy), iz = __float2int_rd(z * p.inv_dz);
-    if (need_grid_test &&
-        ((unsigned)ix >= (unsigned)p.nx || (unsigned)iy >= (unsigned)p.ny || (unsigned)iz >= (unsigned)p.nz))
+    if ((unsigned)ix >= (unsigned)p.nx || (unsigned)iy >= (unsigned)p.ny || (unsigned)iz >= (unsigned)p.nz)
         return FLY_ESCAPED;
     vox = (unsigned)ix + (unsigned)p.nx * ((unsigned)iy + (unsigned)p.ny * (unsigned)iz);
     const unsigned t = __ldg(p.texels + vox);
@@ -269,7 +231,7 @@ transport_kernel(const __grid_constant__ TransportParams p) {
 
     int state = ST_NEED, photon = 0, mat = 0, ie = 0;
     unsigned hl = 0, blk = 0, vox = 0;
-    float x = 0, y = 0, z = 0, u = 0, v = 0, w = 1, E = 0, fe = 0, maj = 1, inv_maj = 1;
+    float x = 0, y = 0, z = 0, u = 0, v = 0, w = 1, E = 0, fe = 0, maj = 1, inv_maj = 1, majo = 1, inv_majo = 1;
     unsigned pool_next = 0, pool_end = 0;   // warp-uniform
     bool exhausted = false;                 // warp-uniform
 
@@ -283,6 +245,8 @@ transport_kernel(const __grid_constant__ TransportParams p) {
         ie = i; fe = t - (float)i;
         maj = fmaf(fe, s_maj[i + 1] - s_maj[i], s_maj[i]);
         inv_maj = __fdividef(1.0f, maj);
+        majo = fmaf(fe, s_majo[i + 1] - s_majo[i], s_majo[i]);
+        inv_majo = __fdividef(1.0f, majo);
     };
 
     for (;;) {
@@ -317,9 +281,9 @@ transport_kernel(const __grid_constant__ TransportParams p) {
         bool dead = false;
         if (state == ST_FLY) {
             FlyCounters fc = {0u, 0u};
-            int code = fly_substep<STATS>(p, s_tot, s_pec, s_majo, x, y, z, u, v, w, ie, fe, maj, inv_maj, r.x, r.y, vox, mat, fc);
+            int code = fly_substep<STATS>(p, s_tot, s_pec, x, y, z, u, v, w, ie, fe, maj, inv_maj, majo, inv_majo, r.x, r.y, vox, mat, fc);
             if (code == FLY_GO)
-                code = fly_substep<STATS>(p, s_tot, s_pec, s_majo, x, y, z, u, v, w, ie, fe, maj, inv_maj, r.z, r.w, vox, mat, fc);
+                code = fly_substep<STATS>(p, s_tot, s_pec, x, y, z, u, v, w, ie, fe, maj, inv_maj, majo, inv_majo, r.z, r.w, vox, mat, fc);
             if (STATS) { c_steps += fc.steps; c_real += fc.real; }
             if (code == FLY_ESCAPED) { if (STATS) { esc += E; ++c_esc; } dead = true; }
             else if (code == FLY_PE) { if (STATS) ++c_pe; deposit<WAGG>(p.batch, vox, E); dead = true; }   // all energy local
@@ -375,7 +339,7 @@ transport_kernel(const __grid_constant__ TransportParams p) {
             stash[0 * kThreads] = x; stash[1 * kThreads] = y; stash[2 * kThreads] = z;
             stash[3 * kThreads] = u; stash[4 * kThreads] = v; stash[5 * kThreads] = w;
             if (p.positron_ke > 0.0f) deposit<WAGG>(p.batch, voxel, p.positron_ke);
-            E = kE0; ie = p.ie0; fe = p.fe0; maj = p.maj0; inv_maj = p.inv_maj0;
+            E = kE0; ie = p.ie0; fe = p.fe0; maj = p.maj0; inv_maj = p.inv_maj0; majo = p.majo0; inv_majo = p.inv_majo0;
             photon = 0; blk = 0; state = ST_FLY;
         }
 
@@ -384,7 +348,7 @@ transport_kernel(const __grid_constant__ TransportParams p) {
                 photon = 1; blk = 0; state = ST_FLY;
                 x = stash[0 * kThreads]; y = stash[1 * kThreads]; z = stash[2 * kThreads];
                 u = -stash[3 * kThreads]; v = -stash[4 * kThreads]; w = -stash[5 * kThreads];
-                E = kE0; ie = p.ie0; fe = p.fe0; maj = p.maj0; inv_maj = p.inv_maj0;
+                E = kE0; ie = p.ie0; fe = p.fe0; maj = p.maj0; inv_maj = p.inv_maj0; majo = p.majo0; inv_majo = p.inv_majo0;
             } else {
                 state = ST_NEED;
             }
@@ -423,9 +387,15 @@ transport_kernel(const __grid_constant__ TransportParams p) {
 // slots back.  A slot whose decay is complete waits for SOURCE, which hands it the next history index of the launch.
 // Same Philox counters and the same per-event arithmetic as schedule 1: the two schedules produce the same
 // histories; only the order of the fp32 atomics differs.
-constexpr int kPoolThreads = 256;
+#ifndef ANM_POOL_THREADS
+#define ANM_POOL_THREADS 1024
+#endif
+#ifndef ANM_POOL_MIN_BLOCKS
+#define ANM_POOL_MIN_BLOCKS 1
+#endif
+constexpr int kPoolThreads = ANM_POOL_THREADS;
 constexpr int kPoolWarps = kPoolThreads / 32;
-constexpr int kPoolMinBlocksPerSM = 3;
+constexpr int kPoolMinBlocksPerSM = ANM_POOL_MIN_BLOCKS;
 constexpr int kSlots = 64;                  // per warp
 constexpr int kRayleighBatch = 8;           // run the (rare) Rayleigh event once this many slots wait for it
 enum : int { F_X = 0, F_Y, F_Z, F_U, F_V, F_W, F_E, F_TV /* FLY: ln-E grid coordinate; COMPTON/RAYLEIGH: voxel */,
@@ -586,11 +556,13 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
             const float fe = t - (float)ie;
             const float maj = fmaf(fe, s_maj[ie + 1] - s_maj[ie], s_maj[ie]);
             const float inv_maj = __fdividef(1.0f, maj);
+            const float majo = fmaf(fe, s_majo[ie + 1] - s_majo[ie], s_majo[ie]);
+            const float inv_majo = __fdividef(1.0f, majo);
             unsigned vox = 0;
             int mat = 0;
-            int code = fly_substep<STATS>(p, s_tot, s_pec, s_majo, x, y, z, u, v, w, ie, fe, maj, inv_maj, r.x, r.y, vox, mat, fc);
+            int code = fly_substep<STATS>(p, s_tot, s_pec, x, y, z, u, v, w, ie, fe, maj, inv_maj, majo, inv_majo, r.x, r.y, vox, mat, fc);
             if (code == FLY_GO)
-                code = fly_substep<STATS>(p, s_tot, s_pec, s_majo, x, y, z, u, v, w, ie, fe, maj, inv_maj, r.z, r.w, vox, mat, fc);
+                code = fly_substep<STATS>(p, s_tot, s_pec, x, y, z, u, v, w, ie, fe, maj, inv_maj, majo, inv_majo, r.z, r.w, vox, mat, fc);
             if (code == FLY_GO) {
                 S[F_X * kSlots] = x; S[F_Y * kSlots] = y; S[F_Z * kSlots] = z;
                 SU[F_META * kSlots] = meta_next;
