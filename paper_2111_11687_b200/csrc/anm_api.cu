@@ -540,7 +540,10 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     p.texels = c->texels.p; p.batch = c->batch.p; p.alias = c->alias.p; p.stats = c->dstats.p;
     p.tab_tot = c->d_tot.p; p.tab_pec = c->d_pec.p; p.tab_maj = c->d_maj.p; p.ray_x2 = c->d_x2.p; p.ray_cum = c->d_cum.p;
     p.n_hist = (unsigned)nb; p.n_alias = c->n_alias;
-    p.key0 = (unsigned)seed; p.key1 = (unsigned)(seed >> 32);
+    for (int r = 0; r < 10; ++r) {      // Philox4x32-10 round keys
+        p.rk[2 * r] = (unsigned)seed + (unsigned)r * 0x9E3779B9u;
+        p.rk[2 * r + 1] = (unsigned)(seed >> 32) + (unsigned)r * 0xBB67AE85u;
+    }
     p.nx = c->nx; p.ny = c->ny; p.nz = c->nz; p.nm = c->nm; p.ne = c->ne; p.n_x2 = c->n_x2;
     p.dx = (float)c->dx; p.dy = (float)c->dy; p.dz = (float)c->dz;
     p.inv_dx = (float)(1.0 / c->dx); p.inv_dy = (float)(1.0 / c->dy); p.inv_dz = (float)(1.0 / c->dz);
@@ -552,25 +555,14 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     p.tab_maj_out = c->d_majo.p;
     p.hull = (c->hull_ok && c->opt.hull_majorant != 2) ? 1 : 0;
     if (p.hull) {
-        const double d[3] = {c->dx, c->dy, c->dz};
-        float lo[3], hi[3];
-        // faces pushed outwards by 1e-3 voxel: far more than the fp32 rounding of x * inv_dx at the face, so a photon
-        // the test calls "outside" can never index a voxel of the box
-        for (int k = 0; k < 3; ++k) { lo[k] = (float)((c->hull_lo[k] - 1e-3) * d[k]); hi[k] = (float)((c->hull_hi[k] + 1e-3) * d[k]); }
-        p.bx0 = lo[0]; p.by0 = lo[1]; p.bz0 = lo[2]; p.bx1 = hi[0]; p.by1 = hi[1]; p.bz1 = hi[2];
+        p.hx0 = (int)c->hull_lo[0]; p.hy0 = (int)c->hull_lo[1]; p.hz0 = (int)c->hull_lo[2];
+        p.hnx = (int)(c->hull_hi[0] - c->hull_lo[0]); p.hny = (int)(c->hull_hi[1] - c->hull_lo[1]);
+        p.hnz = (int)(c->hull_hi[2] - c->hull_lo[2]);
     }
-    {   // energy-dependent quantities at E0, computed exactly like the device's set_energy (fp32)
-        std::vector<float> maj(c->ne), majo(c->ne);
-        ANM_CUDA(c, cudaMemcpyAsync(maj.data(), c->d_maj.p, (size_t)c->ne * 4, cudaMemcpyDeviceToHost, st));
-        ANM_CUDA(c, cudaMemcpyAsync(majo.data(), c->d_majo.p, (size_t)c->ne * 4, cudaMemcpyDeviceToHost, st));
-        ANM_CUDA(c, cudaStreamSynchronize(st));
+    {   // ln-E grid coordinate of E0, in fp32 like the device's
         const float t = (logf(kE0) - p.lnE_min) * p.inv_dlnE;
-        int i = std::max(0, std::min((int)t, c->ne - 2));
+        const int i = std::max(0, std::min((int)t, c->ne - 2));
         p.ie0 = i; p.fe0 = t - (float)i;
-        p.maj0 = fmaf(p.fe0, maj[i + 1] - maj[i], maj[i]);
-        p.inv_maj0 = 1.0f / p.maj0;
-        p.majo0 = fmaf(p.fe0, majo[i + 1] - majo[i], majo[i]);
-        p.inv_majo0 = 1.0f / p.majo0;
     }
 
     const int schedule = c->opt.schedule == 0 ? kAutoSchedule : c->opt.schedule;

@@ -21,9 +21,16 @@
 // stream 0 = source, 1 = photon A, 2 = photon B.
 #pragma once
 #include <cstdint>
+#include <cstdio>
 #include <cuda_runtime.h>
 
 namespace anm {
+
+#ifdef ANM_TRACE
+#define ANM_TR(...) printf(__VA_ARGS__)
+#else
+#define ANM_TR(...) do {} while (0)
+#endif
 
 constexpr int kThreads = 256;
 constexpr int kMinBlocksPerSM = 4;
@@ -55,7 +62,7 @@ struct TransportParams {
     unsigned long long hist_base;   // global index of this launch's first history
     unsigned int n_hist;         // histories in this launch
     unsigned int n_alias;
-    unsigned int key0, key1;     // Philox key = seed
+    unsigned int rk[20];         // Philox round keys: rk[2r] = seed_lo + r*0x9E3779B9, rk[2r+1] = seed_hi + r*0xBB67AE85
     int nx, ny, nz;
     int nm, ne, n_x2;
     float dx, dy, dz;            // cm
@@ -64,26 +71,26 @@ struct TransportParams {
     float cutoff, positron_ke;
     float px, py, pz;            // point source (cm)
     int point_source, photons_per_decay, rayleigh_on;
-    // energy-dependent quantities at E0 (every photon starts there)
-    int ie0; float fe0, maj0, inv_maj0;
-    // hull majorant (anm_options.hull_majorant): the axis-aligned box (b?0, b?1) cm encloses every voxel denser than
-    // the hull threshold (faces pushed outwards by a rounding margin).  A photon beyond a face and moving away from
-    // it flies against tab_maj_out (the bound of the voxels outside the box); every other photon against tab_maj.
+    // ln-E grid coordinate of E0 (every photon starts there): ie0 + fe0
+    int ie0; float fe0;
+    // hull majorant (anm_options.hull_majorant): an axis-aligned box of voxels encloses every voxel denser than the
+    // hull threshold.  A photon that has left the box on a straight line flies against tab_maj_out (the bound of the
+    // voxels outside the box); every other photon against tab_maj (fly_substep).
     int hull;
-    float bx0, bx1, by0, by1, bz0, bz1;      // faces (cm)
-    float majo0, inv_majo0;                   // tab_maj_out at E0
+    int hx0, hy0, hz0, hnx, hny, hnz;         // the box in voxel indices: [hx0, hx0 + hnx) x ...
     const float* tab_maj_out;    // [ne]
 };
 
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint4 philox4x32_10(uint4 c, unsigned k0, unsigned k1) {
+// Philox4x32-10 (north_star (d)); rk[2r], rk[2r+1] = the key of round r (key + r * Weyl constants, computed on the
+// host: they sit in the constant bank and cost no instruction).
+__device__ __forceinline__ uint4 philox4x32_10(uint4 c, const TransportParams& p) {
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
-        const unsigned hi0 = __umulhi(0xD2511F53u, c.x), lo0 = 0xD2511F53u * c.x;
-        const unsigned hi1 = __umulhi(0xCD9E8D57u, c.z), lo1 = 0xCD9E8D57u * c.z;
-        c = make_uint4(hi1 ^ c.y ^ k0, lo1, hi0 ^ c.w ^ k1, lo0);
-        k0 += 0x9E3779B9u;
-        k1 += 0xBB67AE85u;
+        const unsigned long long p0 = (unsigned long long)0xD2511F53u * c.x;
+        const unsigned long long p1 = (unsigned long long)0xCD9E8D57u * c.z;
+        c = make_uint4((unsigned)(p1 >> 32) ^ c.y ^ p.rk[2 * r], (unsigned)p1,
+                       (unsigned)(p0 >> 32) ^ c.w ^ p.rk[2 * r + 1], (unsigned)p0);
     }
     return c;
 }
@@ -93,21 +100,23 @@ __device__ __forceinline__ float u01(unsigned r) {
     return fmaf(__uint2float_rn(r >> 8), 5.9604644775390625e-08f, 2.98023223876953125e-08f);
 }
 
+// The library is compiled with -fmad=false: every fused multiply-add below is written out, so the two schedules
+// (which inline these functions in different contexts) round identically and run bit-identical histories.
 __device__ __forceinline__ void rotate(float& u, float& v, float& w, float cos_t, float phi) {
-    const float sin_t = sqrtf(fmaxf(0.0f, 1.0f - cos_t * cos_t));
+    const float sin_t = sqrtf(fmaxf(0.0f, fmaf(-cos_t, cos_t, 1.0f)));
     float sp, cp;
     __sincosf(phi, &sp, &cp);
     float a, b, c;
     if (fabsf(w) < 0.99999f) {
-        const float s = sqrtf(1.0f - w * w);
+        const float s = sqrtf(fmaf(-w, w, 1.0f));
         const float k = __fdividef(sin_t, s);
-        a = u * cos_t + k * (u * w * cp - v * sp);
-        b = v * cos_t + k * (v * w * cp + u * sp);
-        c = w * cos_t - sin_t * s * cp;
+        a = fmaf(k, fmaf(u * w, cp, -(v * sp)), u * cos_t);
+        b = fmaf(k, fmaf(v * w, cp, u * sp), v * cos_t);
+        c = fmaf(-(sin_t * s), cp, w * cos_t);
     } else {
         a = sin_t * cp; b = sin_t * sp; c = copysignf(cos_t, w);
     }
-    const float n = rsqrtf(a * a + b * b + c * c);
+    const float n = rsqrtf(fmaf(a, a, fmaf(b, b, c * c)));
     u = a * n; v = b * n; w = c * n;
 }
 
@@ -125,59 +134,86 @@ __device__ __forceinline__ void deposit(float* __restrict__ batch, unsigned vox,
     }
 }
 
-// One Woodcock sub-step: exponential flight against the majorant of the region the photon
-// is in, then the real / virtual decision and the channel choice from one more uniform.
-enum : int { FLY_GO = 0, FLY_ESCAPED = 1, FLY_PE = 2, FLY_COMPTON = 3, FLY_RAYLEIGH = 4 };
+// One Woodcock sub-step: exponential flight against the majorant, voxel lookup, real / virtual
+// decision.  Returns FLY_GO (virtual), FLY_ESCAPED, or FLY_REAL with (mat, rho, rr) for select_channel.
+//
+// Hull majorant (reading C24), branch-free.  hull_bits: bit 0 = IN, the photon's last landing point (or its
+// start) was inside the hull box; bit 1 = AWAY, the photon is outside the box and has flown straight since a point
+// inside it.  A straight ray that has left a convex box never re-enters it, so an AWAY photon flies against the
+// majorant of the voxels outside the box; every other photon against the global majorant, which is valid everywhere.
+// A scatter clears AWAY (the caller does), a landing inside the box sets IN.
+enum : int { FLY_GO = 0, FLY_ESCAPED = 1, FLY_PE = 2, FLY_COMPTON = 3, FLY_RAYLEIGH = 4, FLY_REAL = 5 };
 
 struct FlyCounters { unsigned steps, real; };
 
 template <bool STATS>
 __device__ __forceinline__ int fly_substep(const TransportParams& p, const float* __restrict__ s_tot,
-                                           const float2* __restrict__ s_pec,
                                            float& x, float& y, float& z, const float u, const float v, const float w,
                                            const int ie, const float fe, const float maj, const float inv_maj,
                                            const float maj_out, const float inv_maj_out,
-                                           const unsigned r_s, const unsigned r_a, unsigned& vox, int& mat,
-                                           FlyCounters& cnt) {
+                                           const unsigned r_s, const unsigned r_a, unsigned& hull_bits,
+                                           unsigned& vox, int& mat, float& rho, float& rr, FlyCounters& cnt) {
     const float nl = -__logf(u01(r_s));
     if (STATS) ++cnt.steps;
-    // Hull majorant (reading C24), branch-free: a photon that is beyond a face of the hull box and moving
-    // away from it stays outside the (convex) box along its whole ray, so the majorant of the voxels outside the box
-    // bounds mu on every point it can reach; any other photon uses the global majorant, which is valid everywhere.
-    bool away = false;
-    if (p.hull)
-        away = (x >= p.bx1 && u >= 0.0f) || (x < p.bx0 && u <= 0.0f) || (y >= p.by1 && v >= 0.0f) ||
-               (y < p.by0 && v <= 0.0f) || (z >= p.bz1 && w >= 0.0f) || (z < p.bz0 && w <= 0.0f);
+    const bool away = (hull_bits & 2u) != 0u;
     const float m_here = away ? maj_out : maj;
     const float s = nl * (away ? inv_maj_out : inv_maj);
     x = fmaf(s, u, x); y = fmaf(s, v, y); z = fmaf(s, w, z);
     const int ix = __float2int_rd(x * p.inv_dx), iy = __float2int_rd(y * p.inv_dy), iz = __float2int_rd(z * p.inv_dz);
     if ((unsigned)ix >= (unsigned)p.nx || (unsigned)iy >= (unsigned)p.ny || (unsigned)iz >= (unsigned)p.nz)
         return FLY_ESCAPED;
+    if (p.hull) {
+        const bool in = (unsigned)(ix - p.hx0) < (unsigned)p.hnx && (unsigned)(iy - p.hy0) < (unsigned)p.hny &&
+                        (unsigned)(iz - p.hz0) < (unsigned)p.hnz;
+        hull_bits = in ? 1u : (hull_bits ? 2u : 0u);
+    }
     vox = (unsigned)ix + (unsigned)p.nx * ((unsigned)iy + (unsigned)p.ny * (unsigned)iz);
     const unsigned t = __ldg(p.texels + vox);
-    const int m = (int)(t >> 24);
-    const float rho = (float)(t & 0xffffffu) * kDensityStep;
-    const float* row = s_tot + m * p.ne + ie;
+    mat = (int)(t >> 24);
+    rho = (float)(t & 0xffffffu) * kDensityStep;
+    const float* row = s_tot + mat * p.ne + ie;
     const float mu = rho * fmaf(fe, row[1] - row[0], row[0]);
-    const float rr = u01(r_a) * m_here;
+    rr = u01(r_a) * m_here;
     if (rr >= mu) return FLY_GO;                     // virtual collision
     if (STATS) ++cnt.real;
-    const float2 a = s_pec[m * p.ne + ie], b = s_pec[m * p.ne + ie + 1];
-    if (rr < rho * fmaf(fe, b.x - a.x, a.x)) return FLY_PE;              // the same draw picks the channel
+    return FLY_REAL;
+}
+
+// A5: the draw that accepted the collision also picks the channel: rr < mu_pe -> photoelectric, < mu_pe + mu_compton ->
+// Compton, else Rayleigh.
+__device__ __forceinline__ int select_channel(const TransportParams& p, const float2* __restrict__ s_pec, const int mat,
+                                              const float rho, const int ie, const float fe, const float rr) {
+    const float2 a = s_pec[mat * p.ne + ie], b = s_pec[mat * p.ne + ie + 1];
+    if (rr < rho * fmaf(fe, b.x - a.x, a.x)) return FLY_PE;
     if (rr < rho * fmaf(fe, b.y - a.y, a.y) || !p.rayleigh_on) return FLY_COMPTON;
-    mat = m;
     return FLY_RAYLEIGH;
+}
+
+// Two Woodcock sub-steps from one Philox block (words x,y then z,w); stops at the first real collision or escape.
+template <bool STATS>
+__device__ __forceinline__ int fly_two(const TransportParams& p, const float* __restrict__ s_tot,
+                                       const float2* __restrict__ s_pec, float& x, float& y, float& z,
+                                       const float u, const float v, const float w, const int ie, const float fe,
+                                       const float maj, const float inv_maj, const float maj_out, const float inv_maj_out,
+                                       const uint4 r, unsigned& hull_bits, unsigned& vox, int& mat, FlyCounters& cnt) {
+    float rho = 0.0f, rr = 0.0f;
+    int code = fly_substep<STATS>(p, s_tot, x, y, z, u, v, w, ie, fe, maj, inv_maj, maj_out, inv_maj_out, r.x, r.y,
+                                  hull_bits, vox, mat, rho, rr, cnt);
+    if (code == FLY_GO)
+        code = fly_substep<STATS>(p, s_tot, x, y, z, u, v, w, ie, fe, maj, inv_maj, maj_out, inv_maj_out, r.z, r.w,
+                                  hull_bits, vox, mat, rho, rr, cnt);
+    if (code == FLY_REAL) code = select_channel(p, s_pec, mat, rho, ie, fe, rr);
+    return code;
 }
 
 // One Klein-Nishina try by composition-rejection on f(eps) = (1/eps + eps) g(eps).
 // Returns true when accepted; then eps = E'/E and t = 1 - cos(theta).
 __device__ __forceinline__ bool compton_try(const float E, const uint4 r, float& eps, float& t) {
     const float alpha = E * kInvE0;
-    const float eps0 = __fdividef(1.0f, 1.0f + 2.0f * alpha);
+    const float eps0 = __fdividef(1.0f, fmaf(2.0f, alpha, 1.0f));
     const float eps0sq = eps0 * eps0;
     const float a1 = -__logf(eps0);
-    const float a2 = a1 + 0.5f * (1.0f - eps0sq);
+    const float a2 = fmaf(0.5f, 1.0f - eps0sq, a1);
     const float u2 = u01(r.y);
     float epssq;
     if (a1 > a2 * u01(r.x)) { eps = __expf(-a1 * u2); epssq = eps * eps; }
@@ -204,8 +240,47 @@ __device__ __forceinline__ bool rayleigh_try(const float E, const uint4 r, const
     const float dc = cum[hi] - cum[lo];
     if (dc > 0.0f) x2 = fmaf(__fdividef(target - cum[lo], dc), s_x2[hi] - s_x2[lo], x2);
     x2 = fminf(x2, T);
-    c = 1.0f - 2.0f * __fdividef(x2, T);
-    return 2.0f * u01(r.y) <= 1.0f + c * c;
+    c = fmaf(-2.0f, __fdividef(x2, T), 1.0f);
+    return 2.0f * u01(r.y) <= fmaf(c, c, 1.0f);
+}
+
+__device__ __forceinline__ bool hull_in(const TransportParams& p, int ix, int iy, int iz) {
+    return p.hull && (unsigned)(ix - p.hx0) < (unsigned)p.hnx && (unsigned)(iy - p.hy0) < (unsigned)p.hny &&
+           (unsigned)(iz - p.hz0) < (unsigned)p.hnz;
+}
+
+// A2 + A3: the decay of history h: voxel pick (alias table, 64 random bits for the bin), uniform point in the voxel,
+// isotropic direction.  Philox stream 0, blocks 0 and 1.  Returns the decay voxel; in_box = hull_in(decay voxel).
+__device__ __forceinline__ unsigned sample_source(const TransportParams& p, const unsigned long long h, float& x, float& y,
+                                                  float& z, float& u, float& v, float& w, bool& in_box) {
+    const uint4 r = philox4x32_10(make_uint4((unsigned)h, (unsigned)(h >> 32), 0u, 0u), p);
+    const uint4 r2 = philox4x32_10(make_uint4((unsigned)h, (unsigned)(h >> 32), 1u, 0u), p);
+    unsigned voxel, ix, iy, iz;
+    if (p.point_source) {
+        x = p.px; y = p.py; z = p.pz;
+        ix = (unsigned)__float2int_rd(x * p.inv_dx); iy = (unsigned)__float2int_rd(y * p.inv_dy);
+        iz = (unsigned)__float2int_rd(z * p.inv_dz);
+        voxel = ix + (unsigned)p.nx * (iy + (unsigned)p.ny * iz);
+    } else {
+        const unsigned long long r64 = ((unsigned long long)r.x << 32) | r.y;
+        const unsigned j = (unsigned)__umul64hi(r64, (unsigned long long)p.n_alias);
+        const uint4 a = __ldg(p.alias + j);
+        voxel = (r.z < a.x) ? a.y : a.z;
+        const unsigned nxy = (unsigned)p.nx * (unsigned)p.ny;
+        iz = voxel / nxy;
+        const unsigned rem = voxel - iz * nxy;
+        iy = rem / (unsigned)p.nx; ix = rem - iy * (unsigned)p.nx;
+        x = ((float)ix + u01(r.w)) * p.dx;       // uniform inside the voxel
+        y = ((float)iy + u01(r2.x)) * p.dy;
+        z = ((float)iz + u01(r2.y)) * p.dz;
+    }
+    in_box = hull_in(p, (int)ix, (int)iy, (int)iz);
+    const float ct = fmaf(2.0f, u01(r2.z), -1.0f);    // isotropic direction
+    const float st = sqrtf(fmaxf(0.0f, fmaf(-ct, ct, 1.0f)));
+    float sp, cp;
+    __sincosf(kTwoPi * u01(r2.w), &sp, &cp);
+    u = st * cp; v = st * sp; w = ct;
+    return voxel;
 }
 
 template <bool STATS, bool WAGG>
@@ -230,24 +305,26 @@ transport_kernel(const __grid_constant__ TransportParams p) {
     float* stash = s_stash + threadIdx.x;
 
     int state = ST_NEED, photon = 0, mat = 0, ie = 0;
-    unsigned hl = 0, blk = 0, vox = 0;
+    unsigned hl = 0, blk = 0, vox = 0, hb = 0, hb_src = 0;
     float x = 0, y = 0, z = 0, u = 0, v = 0, w = 1, E = 0, fe = 0, maj = 1, inv_maj = 1, majo = 1, inv_majo = 1;
     unsigned pool_next = 0, pool_end = 0;   // warp-uniform
     bool exhausted = false;                 // warp-uniform
 
     float esc = 0.0f;
-    unsigned c_steps = 0, c_real = 0, c_pe = 0, c_co = 0, c_ra = 0, c_esc = 0, c_cut = 0;
+    unsigned c_pe = 0, c_co = 0, c_ra = 0, c_esc = 0, c_cut = 0;
+    FlyCounters fc = {0u, 0u};
 
-    auto set_energy = [&](float e) {
-        const float t = (__logf(e) - p.lnE_min) * p.inv_dlnE;
-        int i = (int)t;
-        i = max(0, min(i, p.ne - 2));
-        ie = i; fe = t - (float)i;
-        maj = fmaf(fe, s_maj[i + 1] - s_maj[i], s_maj[i]);
+    const float t0 = (float)p.ie0 + p.fe0;  // ln-E grid coordinate of E0
+    const float t_max = (float)(p.ne - 1) - 1.0f / 1024.0f;
+    // energy-dependent quantities from the ln-E grid coordinate t (the same arithmetic as schedule 2)
+    auto set_t = [&](float t) {
+        ie = (int)t; fe = t - (float)ie;
+        maj = fmaf(fe, s_maj[ie + 1] - s_maj[ie], s_maj[ie]);
         inv_maj = __fdividef(1.0f, maj);
-        majo = fmaf(fe, s_majo[i + 1] - s_majo[i], s_majo[i]);
+        majo = fmaf(fe, s_majo[ie + 1] - s_majo[ie], s_majo[ie]);
         inv_majo = __fdividef(1.0f, majo);
     };
+    auto set_energy = [&](float e) { set_t(fminf(fmaxf((__logf(e) - p.lnE_min) * p.inv_dlnE, 0.0f), t_max)); };
 
     for (;;) {
         // ---- hand out history indices --------------------------------------------------------
@@ -272,19 +349,26 @@ transport_kernel(const __grid_constant__ TransportParams p) {
         if (__all_sync(0xffffffffu, state == ST_DONE)) break;
         if (state == ST_NEED || state == ST_DONE) continue;
 
-        // ---- one Philox block per live lane ---------------------------------------------------
         const unsigned long long h = p.hist_base + hl;
-        const unsigned stream = (state == ST_SOURCE) ? 0u : 1u + (unsigned)photon;
-        const uint4 r = philox4x32_10(make_uint4((unsigned)h, (unsigned)(h >> 32), blk, stream), p.key0, p.key1);
-        ++blk;
-
         bool dead = false;
+        if (state == ST_SOURCE) {
+            bool in_box;
+            const unsigned voxel = sample_source(p, h, x, y, z, u, v, w, in_box);
+            stash[0 * kThreads] = x; stash[1 * kThreads] = y; stash[2 * kThreads] = z;
+            stash[3 * kThreads] = u; stash[4 * kThreads] = v; stash[5 * kThreads] = w;
+            if (p.positron_ke > 0.0f) deposit<WAGG>(p.batch, voxel, p.positron_ke);
+            E = kE0; set_t(t0);
+            hb_src = in_box ? 1u : 0u; hb = hb_src;
+            photon = 0; blk = 0; state = ST_FLY;
+            continue;
+        }
+
+        // ---- one Philox block per live photon --------------------------------------------------
+        const uint4 r = philox4x32_10(make_uint4((unsigned)h, (unsigned)(h >> 32), blk, 1u + (unsigned)photon), p);
+        ++blk;
         if (state == ST_FLY) {
-            FlyCounters fc = {0u, 0u};
-            int code = fly_substep<STATS>(p, s_tot, s_pec, x, y, z, u, v, w, ie, fe, maj, inv_maj, majo, inv_majo, r.x, r.y, vox, mat, fc);
-            if (code == FLY_GO)
-                code = fly_substep<STATS>(p, s_tot, s_pec, x, y, z, u, v, w, ie, fe, maj, inv_maj, majo, inv_majo, r.z, r.w, vox, mat, fc);
-            if (STATS) { c_steps += fc.steps; c_real += fc.real; }
+            const int code = fly_two<STATS>(p, s_tot, s_pec, x, y, z, u, v, w, ie, fe, maj, inv_maj, majo, inv_majo, r, hb, vox, mat, fc);
+            ANM_TR("S1 h=%llu ph=%d blk=%u FLY code=%d E=%.9g t=%d+%.9g pos=%.9g %.9g %.9g vox=%u hb=%u\n", h, photon, blk - 1, code, E, ie, fe, x, y, z, vox, hb);
             if (code == FLY_ESCAPED) { if (STATS) { esc += E; ++c_esc; } dead = true; }
             else if (code == FLY_PE) { if (STATS) ++c_pe; deposit<WAGG>(p.batch, vox, E); dead = true; }   // all energy local
             else if (code == FLY_COMPTON) state = ST_COMPTON;
@@ -295,60 +379,27 @@ transport_kernel(const __grid_constant__ TransportParams p) {
                 if (STATS) ++c_co;
                 float dep = E * (1.0f - eps);     // recoil electron deposited locally
                 E *= eps;
-                rotate(u, v, w, 1.0f - t, kTwoPi * u01(r.w));
                 if (E < p.cutoff) { dep += E; dead = true; if (STATS) ++c_cut; }
-                else { set_energy(E); state = ST_FLY; }
+                else { rotate(u, v, w, 1.0f - t, kTwoPi * u01(r.w)); set_energy(E); hb &= 1u; state = ST_FLY; }
                 deposit<WAGG>(p.batch, vox, dep);
             }
-        } else if (state == ST_RAYLEIGH) {
+        } else {   // ST_RAYLEIGH
             float c;
             if (rayleigh_try(E, r, s_x2, s_cum + mat * p.n_x2, p.n_x2, c)) {
                 if (STATS) ++c_ra;
                 rotate(u, v, w, c, kTwoPi * u01(r.z));
+                set_energy(E);      // E is unchanged; recomputed like schedule 2, whose slot held the voxel in its place
+                hb &= 1u;
                 state = ST_FLY;
             }
-        } else {   // ST_SOURCE
-            const uint4 r2 = philox4x32_10(make_uint4((unsigned)h, (unsigned)(h >> 32), 1u, 0u), p.key0, p.key1);
-            unsigned voxel;
-            if (p.point_source) {
-                x = p.px; y = p.py; z = p.pz;
-                voxel = 0;
-                if (p.positron_ke > 0.0f) {
-                    const int ix = __float2int_rd(x * p.inv_dx), iy = __float2int_rd(y * p.inv_dy),
-                              iz = __float2int_rd(z * p.inv_dz);
-                    voxel = (unsigned)ix + (unsigned)p.nx * ((unsigned)iy + (unsigned)p.ny * (unsigned)iz);
-                }
-            } else {
-                // alias table over the active voxels; 64 random bits pick the bin (n_alias can exceed 2^24)
-                const unsigned long long r64 = ((unsigned long long)r.x << 32) | r.y;
-                const unsigned j = (unsigned)__umul64hi(r64, (unsigned long long)p.n_alias);
-                const uint4 a = __ldg(p.alias + j);
-                voxel = (r.z < a.x) ? a.y : a.z;
-                const unsigned nxy = (unsigned)p.nx * (unsigned)p.ny;
-                const unsigned iz = voxel / nxy, rem = voxel - iz * nxy;
-                const unsigned iy = rem / (unsigned)p.nx, ix = rem - iy * (unsigned)p.nx;
-                x = ((float)ix + u01(r.w)) * p.dx;       // uniform inside the voxel
-                y = ((float)iy + u01(r2.x)) * p.dy;
-                z = ((float)iz + u01(r2.y)) * p.dz;
-            }
-            const float ct = 2.0f * u01(r2.z) - 1.0f;    // isotropic direction
-            const float st = sqrtf(fmaxf(0.0f, 1.0f - ct * ct));
-            float sp, cp;
-            __sincosf(kTwoPi * u01(r2.w), &sp, &cp);
-            u = st * cp; v = st * sp; w = ct;
-            stash[0 * kThreads] = x; stash[1 * kThreads] = y; stash[2 * kThreads] = z;
-            stash[3 * kThreads] = u; stash[4 * kThreads] = v; stash[5 * kThreads] = w;
-            if (p.positron_ke > 0.0f) deposit<WAGG>(p.batch, voxel, p.positron_ke);
-            E = kE0; ie = p.ie0; fe = p.fe0; maj = p.maj0; inv_maj = p.inv_maj0; majo = p.majo0; inv_majo = p.inv_majo0;
-            photon = 0; blk = 0; state = ST_FLY;
         }
 
         if (dead) {
             if (photon == 0 && p.photons_per_decay == 2) {   // the partner photon: same point, opposite direction
-                photon = 1; blk = 0; state = ST_FLY;
+                photon = 1; blk = 0; state = ST_FLY; hb = hb_src;
                 x = stash[0 * kThreads]; y = stash[1 * kThreads]; z = stash[2 * kThreads];
                 u = -stash[3 * kThreads]; v = -stash[4 * kThreads]; w = -stash[5 * kThreads];
-                E = kE0; ie = p.ie0; fe = p.fe0; maj = p.maj0; inv_maj = p.inv_maj0; majo = p.majo0; inv_majo = p.inv_majo0;
+                E = kE0; set_t(t0);
             } else {
                 state = ST_NEED;
             }
@@ -356,6 +407,7 @@ transport_kernel(const __grid_constant__ TransportParams p) {
     }
 
     if (STATS) {
+        unsigned c_steps = fc.steps, c_real = fc.real;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
             esc += __shfl_xor_sync(0xffffffffu, esc, o);
@@ -381,12 +433,14 @@ transport_kernel(const __grid_constant__ TransportParams p) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// Schedule 2: event-based at warp scope.  Each warp owns kSlots photon slots in shared memory (SoA, one word per
-// field per slot).  A trip: count the slots waiting for each event type (one redux), pick the type with the most
-// waiting slots, compact up to 32 of them (ballot + prefix), run that ONE event type with those lanes, write the
-// slots back.  A slot whose decay is complete waits for SOURCE, which hands it the next history index of the launch.
-// Same Philox counters and the same per-event arithmetic as schedule 1: the two schedules produce the same
-// histories; only the order of the fp32 atomics differs.
+// Schedule 2: event-based at warp scope.  Each warp owns kSlots decay slots in shared memory (SoA, one word per
+// field per slot; two banks of photon state, bank 0 = photon A, bank 1 = photon B, both written at the decay) and
+// four ring queues of slot numbers, one per event type (FLY, COMPTON, SOURCE = free, RAYLEIGH).  A trip: pick the
+// event type with the longest queue, pop up to 32 slots, run that ONE event with (nearly) all lanes active, push every
+// slot onto the queue of its next event (ballot + prefix popcount).  A slot whose decay is complete is free and waits
+// for SOURCE, which hands it the next history index of the launch: regenerate in place, compact by event type, no
+// global queues and no extra HBM traffic.  Same Philox counters and per-event arithmetic as schedule 1: the two
+// schedules produce the same histories; only the order of the fp32 atomics differs.
 #ifndef ANM_POOL_THREADS
 #define ANM_POOL_THREADS 1024
 #endif
@@ -396,12 +450,15 @@ transport_kernel(const __grid_constant__ TransportParams p) {
 constexpr int kPoolThreads = ANM_POOL_THREADS;
 constexpr int kPoolWarps = kPoolThreads / 32;
 constexpr int kPoolMinBlocksPerSM = ANM_POOL_MIN_BLOCKS;
-constexpr int kSlots = 64;                  // per warp
+constexpr int kSlots = 64;                  // per warp (a power of two: the queues are rings)
 constexpr int kRayleighBatch = 8;           // run the (rare) Rayleigh event once this many slots wait for it
+// photon bank fields (bank b at word offset b * kBankFields * kSlots)
 enum : int { F_X = 0, F_Y, F_Z, F_U, F_V, F_W, F_E, F_TV /* FLY: ln-E grid coordinate; COMPTON/RAYLEIGH: voxel */,
-             F_HL, F_META, F_SX, F_SY, F_SZ, F_SU, F_SV, F_SW, kSlotFields };
-// meta = state (bits 0-2) | photon (bit 3) | material (bits 4-6) | Philox block counter (bits 7-31)
-constexpr size_t kPoolWarpBytes = (size_t)kSlotFields * kSlots * 4 + 32;   // + the compaction list (one byte per lane)
+             kBankFields, F_HL = 2 * kBankFields, F_META, kSlotFields };
+// meta = photon (bit 0) | hull bits IN, AWAY (bits 1-2) | decay voxel inside the hull box (bit 3) | material (bits 4-6)
+//        | Philox block counter (bits 8-31)
+enum : int { Q_F = 0, Q_C = 1, Q_S = 2, Q_R = 3, Q_NONE = 4 };
+constexpr size_t kPoolWarpBytes = (size_t)kSlotFields * kSlots * 4 + 4 * kSlots;   // slots + the four queues (bytes)
 
 template <bool STATS>
 __global__ void __launch_bounds__(kPoolThreads, kPoolMinBlocksPerSM)
@@ -423,14 +480,14 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
     const unsigned lanemask_lt = (1u << lane) - 1u;
     float* slots = reinterpret_cast<float*>(s_pool + (size_t)(threadIdx.x >> 5) * kPoolWarpBytes);
     unsigned* slots_u = reinterpret_cast<unsigned*>(slots);
-    unsigned char* list = reinterpret_cast<unsigned char*>(slots + kSlotFields * kSlots);
+    unsigned char* q = reinterpret_cast<unsigned char*>(slots + kSlotFields * kSlots);   // [4][kSlots]
 #pragma unroll
-    for (int k = 0; k < kSlots / 32; ++k) slots_u[F_META * kSlots + lane + 32 * k] = ST_SOURCE;
+    for (int k = 0; k < kSlots / 32; ++k) q[Q_S * kSlots + lane + 32 * k] = (unsigned char)(lane + 32 * k);   // all free
     __syncthreads();
 
+    unsigned hF = 0, nF = 0, hC = 0, nC = 0, hS = 0, nS = kSlots, hR = 0, nR = 0;   // ring heads and lengths, warp-uniform
     unsigned pool_next = 0, pool_end = 0;   // warp-uniform
     bool exhausted = false;                 // warp-uniform
-    unsigned trip = 0;
     const float t0 = (float)p.ie0 + p.fe0;  // ln-E grid coordinate of E0
     const float t_max = (float)(p.ne - 1) - 1.0f / 1024.0f;
 
@@ -438,183 +495,176 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
     unsigned c_pe = 0, c_co = 0, c_ra = 0, c_esc = 0, c_cut = 0;
     FlyCounters fc = {0u, 0u};
 
-    for (;; ++trip) {
+    // push the slots whose next event is T onto ring T (all 32 lanes call it)
+#define ANM_PUSH(T, hT, nT)                                                                               \
+    do {                                                                                                   \
+        const unsigned b_ = __ballot_sync(0xffffffffu, next == (T));                                       \
+        if (next == (T)) q[(T) * kSlots + (((hT) + (nT) + __popc(b_ & lanemask_lt)) & (kSlots - 1))] = (unsigned char)slot; \
+        (nT) += __popc(b_);                                                                                \
+    } while (0)
+
+    for (;;) {
         __syncwarp();
-        // ---- vote: how many slots wait for each event type --------------------------------------------
-        const unsigned m0 = slots_u[F_META * kSlots + lane], m1 = slots_u[F_META * kSlots + lane + 32];
-        const int st0 = (int)(m0 & 7u), st1 = (int)(m1 & 7u);
-        // byte 0 FLY, byte 1 COMPTON, byte 2 SOURCE (and NEED), byte 3 RAYLEIGH; DONE counts nowhere
-        constexpr unsigned kShift = 16u | (16u << 5) | (0u << 10) | (8u << 15) | (24u << 20);
-        const unsigned inc0 = (st0 == ST_DONE) ? 0u : 1u << ((kShift >> (5 * st0)) & 31u);
-        const unsigned inc1 = (st1 == ST_DONE) ? 0u : 1u << ((kShift >> (5 * st1)) & 31u);
-        const unsigned tot = __reduce_add_sync(0xffffffffu, inc0 + inc1);
-        if (tot == 0u) break;
-        const unsigned nF = tot & 255u, nC = (tot >> 8) & 255u, nS = (tot >> 16) & 255u, nR = tot >> 24;
-        int X = ST_FLY;
+        // ---- pick the event type with the longest queue ------------------------------------------------
+        int X = Q_F;
         unsigned best = nF;
-        if (nC > best) { X = ST_COMPTON; best = nC; }
-        if (nS > best) { X = ST_SOURCE; best = nS; }
-        if (nR > best || nR >= (unsigned)kRayleighBatch) X = ST_RAYLEIGH;
-        // ---- compact the waiting slots; the half of the pool that goes first alternates ------------------
-        const bool h0 = (X == ST_SOURCE) ? (st0 <= ST_SOURCE) : (st0 == X);
-        const bool h1 = (X == ST_SOURCE) ? (st1 <= ST_SOURCE) : (st1 == X);
-        const unsigned b0 = __ballot_sync(0xffffffffu, h0), b1 = __ballot_sync(0xffffffffu, h1);
-        const bool flip = (trip & 1u) != 0u;
-        const unsigned r0 = __popc(b0 & lanemask_lt) + (flip ? __popc(b1) : 0u);
-        const unsigned r1 = __popc(b1 & lanemask_lt) + (flip ? 0u : __popc(b0));
-        if (h0 && r0 < 32u) list[r0] = (unsigned char)lane;
-        if (h1 && r1 < 32u) list[r1] = (unsigned char)(lane + 32u);
-        __syncwarp();
-        unsigned n = min((unsigned)(__popc(b0) + __popc(b1)), 32u);
+        if (nC > best) { X = Q_C; best = nC; }
+        if (!exhausted && nS > best) { X = Q_S; best = nS; }
+        if (nR > best || nR >= (unsigned)kRayleighBatch) { X = Q_R; best = nR; }
+        if (best == 0u) break;              // every slot is free and the launch has no history left
+        unsigned n = min(best, 32u);
+        unsigned head;
+        if (X == Q_F) head = hF; else if (X == Q_C) head = hC; else if (X == Q_S) head = hS; else head = hR;
         unsigned hl_new = 0;
-        if (X == ST_SOURCE) {                 // hand out history indices (warp-uniform bookkeeping)
-            if (pool_next == pool_end && !exhausted) {
+        if (X == Q_S) {                     // hand out history indices (warp-uniform bookkeeping)
+            if (pool_next == pool_end) {
                 unsigned base = 0;
                 if (lane == 0) base = atomicAdd(p.counter, kChunk);
                 base = __shfl_sync(0xffffffffu, base, 0);
                 pool_next = min(base, p.n_hist);
                 pool_end = min(base + kChunk, p.n_hist);
-                exhausted = (pool_next == pool_end);
+                if (pool_next == pool_end) { exhausted = true; continue; }
             }
-            const unsigned avail = pool_end - pool_next;
-            if (exhausted) {                  // nothing left in this launch: the waiting slots are finished
-                if (lane < n) slots_u[F_META * kSlots + list[lane]] = ST_DONE;
-                continue;
-            }
-            n = min(n, avail);
+            n = min(n, pool_end - pool_next);
             hl_new = pool_next + lane;
             pool_next += n;
         }
-        if (lane >= n) continue;
-        const unsigned slot = list[lane];
+        const unsigned slot = q[X * kSlots + ((head + lane) & (kSlots - 1))];
+        const bool active = lane < n;
         float* S = slots + slot;
         unsigned* SU = slots_u + slot;
+        int next = Q_NONE;
 
-        // a finished photon: start the partner (same point, opposite direction) or wait for a new history
+        // a finished photon: start the partner (bank 1, written at the decay) or free the slot
         auto photon_ends = [&](unsigned meta) {
-            if (!(meta & 8u) && p.photons_per_decay == 2) {
-                S[F_X * kSlots] = S[F_SX * kSlots]; S[F_Y * kSlots] = S[F_SY * kSlots]; S[F_Z * kSlots] = S[F_SZ * kSlots];
-                S[F_U * kSlots] = -S[F_SU * kSlots]; S[F_V * kSlots] = -S[F_SV * kSlots]; S[F_W * kSlots] = -S[F_SW * kSlots];
-                S[F_E * kSlots] = kE0; S[F_TV * kSlots] = t0;
-                SU[F_META * kSlots] = (unsigned)ST_FLY | 8u;
+            if (!(meta & 1u) && p.photons_per_decay == 2) {
+                SU[F_META * kSlots] = 1u | (meta & 8u) | ((meta & 8u) >> 2);   // photon B, block 0, IN = decay voxel's
+                next = Q_F;
             } else {
-                SU[F_META * kSlots] = ST_SOURCE;
+                next = Q_S;
             }
         };
 
-        if (X == ST_SOURCE) {
-            const unsigned long long h = p.hist_base + hl_new;
-            const uint4 r = philox4x32_10(make_uint4((unsigned)h, (unsigned)(h >> 32), 0u, 0u), p.key0, p.key1);
-            const uint4 r2 = philox4x32_10(make_uint4((unsigned)h, (unsigned)(h >> 32), 1u, 0u), p.key0, p.key1);
-            float x, y, z;
-            unsigned voxel;
-            if (p.point_source) {
-                x = p.px; y = p.py; z = p.pz;
-                voxel = 0;
-                if (p.positron_ke > 0.0f) {
-                    const int ix = __float2int_rd(x * p.inv_dx), iy = __float2int_rd(y * p.inv_dy), iz = __float2int_rd(z * p.inv_dz);
-                    voxel = (unsigned)ix + (unsigned)p.nx * ((unsigned)iy + (unsigned)p.ny * (unsigned)iz);
-                }
-            } else {
-                const unsigned long long r64 = ((unsigned long long)r.x << 32) | r.y;
-                const unsigned j = (unsigned)__umul64hi(r64, (unsigned long long)p.n_alias);
-                const uint4 a = __ldg(p.alias + j);
-                voxel = (r.z < a.x) ? a.y : a.z;
-                const unsigned nxy = (unsigned)p.nx * (unsigned)p.ny;
-                const unsigned iz = voxel / nxy, rem = voxel - iz * nxy;
-                const unsigned iy = rem / (unsigned)p.nx, ix = rem - iy * (unsigned)p.nx;
-                x = ((float)ix + u01(r.w)) * p.dx;
-                y = ((float)iy + u01(r2.x)) * p.dy;
-                z = ((float)iz + u01(r2.y)) * p.dz;
-            }
-            const float ct = 2.0f * u01(r2.z) - 1.0f;
-            const float st = sqrtf(fmaxf(0.0f, 1.0f - ct * ct));
-            float sp, cp;
-            __sincosf(kTwoPi * u01(r2.w), &sp, &cp);
-            const float u = st * cp, v = st * sp, w = ct;
-            S[F_X * kSlots] = x; S[F_Y * kSlots] = y; S[F_Z * kSlots] = z;
-            S[F_U * kSlots] = u; S[F_V * kSlots] = v; S[F_W * kSlots] = w;
-            S[F_SX * kSlots] = x; S[F_SY * kSlots] = y; S[F_SZ * kSlots] = z;
-            S[F_SU * kSlots] = u; S[F_SV * kSlots] = v; S[F_SW * kSlots] = w;
-            S[F_E * kSlots] = kE0; S[F_TV * kSlots] = t0;
-            SU[F_HL * kSlots] = hl_new;
-            SU[F_META * kSlots] = ST_FLY;
-            if (p.positron_ke > 0.0f) atomicAdd(p.batch + voxel, p.positron_ke);
-            continue;
-        }
-
-        const unsigned meta = SU[F_META * kSlots];
-        const unsigned long long h = p.hist_base + SU[F_HL * kSlots];
-        const uint4 r = philox4x32_10(make_uint4((unsigned)h, (unsigned)(h >> 32), meta >> 7, 1u + ((meta >> 3) & 1u)), p.key0, p.key1);
-        const unsigned meta_next = meta + 128u;    // block counter + 1
-
-        if (X == ST_FLY) {
-            float x = S[F_X * kSlots], y = S[F_Y * kSlots], z = S[F_Z * kSlots];
-            const float u = S[F_U * kSlots], v = S[F_V * kSlots], w = S[F_W * kSlots];
-            const float t = S[F_TV * kSlots];
-            const int ie = (int)t;
-            const float fe = t - (float)ie;
-            const float maj = fmaf(fe, s_maj[ie + 1] - s_maj[ie], s_maj[ie]);
-            const float inv_maj = __fdividef(1.0f, maj);
-            const float majo = fmaf(fe, s_majo[ie + 1] - s_majo[ie], s_majo[ie]);
-            const float inv_majo = __fdividef(1.0f, majo);
-            unsigned vox = 0;
-            int mat = 0;
-            int code = fly_substep<STATS>(p, s_tot, s_pec, x, y, z, u, v, w, ie, fe, maj, inv_maj, majo, inv_majo, r.x, r.y, vox, mat, fc);
-            if (code == FLY_GO)
-                code = fly_substep<STATS>(p, s_tot, s_pec, x, y, z, u, v, w, ie, fe, maj, inv_maj, majo, inv_majo, r.z, r.w, vox, mat, fc);
-            if (code == FLY_GO) {
-                S[F_X * kSlots] = x; S[F_Y * kSlots] = y; S[F_Z * kSlots] = z;
-                SU[F_META * kSlots] = meta_next;
-            } else if (code == FLY_COMPTON || code == FLY_RAYLEIGH) {
-                S[F_X * kSlots] = x; S[F_Y * kSlots] = y; S[F_Z * kSlots] = z;
-                SU[F_TV * kSlots] = vox;
-                SU[F_META * kSlots] = (meta_next & ~0x77u) | (code == FLY_COMPTON ? (unsigned)ST_COMPTON : (unsigned)ST_RAYLEIGH | ((unsigned)mat << 4));
-            } else {
-                const float E = S[F_E * kSlots];
-                if (code == FLY_PE) { if (STATS) ++c_pe; atomicAdd(p.batch + vox, E); }      // all energy local
-                else if (STATS) { esc += E; ++c_esc; }
-                photon_ends(meta);
-            }
-        } else if (X == ST_COMPTON) {
-            float E = S[F_E * kSlots];
-            float eps, t;
-            if (compton_try(E, r, eps, t)) {
-                if (STATS) ++c_co;
-                float u = S[F_U * kSlots], v = S[F_V * kSlots], w = S[F_W * kSlots];
-                const unsigned vox = SU[F_TV * kSlots];
-                float dep = E * (1.0f - eps);     // recoil electron deposited locally
-                E *= eps;
-                if (E < p.cutoff) {               // the rest is deposited locally
-                    dep += E;
-                    if (STATS) ++c_cut;
-                    photon_ends(meta);
+        if (X == Q_F) {
+            hF = (hF + n) & (kSlots - 1); nF -= n;
+            if (active) {
+                const unsigned meta = SU[F_META * kSlots];
+                const unsigned ph = meta & 1u;
+                const unsigned long long h = p.hist_base + SU[F_HL * kSlots];
+                const uint4 r = philox4x32_10(make_uint4((unsigned)h, (unsigned)(h >> 32), meta >> 8, 1u + ph), p);
+                float* Bk = S + ph * (kBankFields * kSlots);
+                float x = Bk[F_X * kSlots], y = Bk[F_Y * kSlots], z = Bk[F_Z * kSlots];
+                const float u = Bk[F_U * kSlots], v = Bk[F_V * kSlots], w = Bk[F_W * kSlots];
+                const float t = Bk[F_TV * kSlots];
+                const int ie = (int)t;
+                const float fe = t - (float)ie;
+                const float maj = fmaf(fe, s_maj[ie + 1] - s_maj[ie], s_maj[ie]);
+                const float inv_maj = __fdividef(1.0f, maj);
+                const float majo = fmaf(fe, s_majo[ie + 1] - s_majo[ie], s_majo[ie]);
+                const float inv_majo = __fdividef(1.0f, majo);
+                unsigned vox = 0, hb = (meta >> 1) & 3u;
+                int mat = 0;
+                const int code = fly_two<STATS>(p, s_tot, s_pec, x, y, z, u, v, w, ie, fe, maj, inv_maj, majo, inv_majo, r, hb, vox, mat, fc);
+                const unsigned meta_next = ((meta & ~0x76u) | (hb << 1)) + 256u;    // block counter + 1, new hull bits
+                ANM_TR("S2 h=%llu ph=%u blk=%u FLY code=%d E=%.9g t=%d+%.9g pos=%.9g %.9g %.9g vox=%u hb=%u\n", h, ph, meta >> 8, code, Bk[F_E * kSlots], ie, fe, x, y, z, vox, hb);
+                if (code == FLY_GO || code == FLY_COMPTON || code == FLY_RAYLEIGH) {
+                    Bk[F_X * kSlots] = x; Bk[F_Y * kSlots] = y; Bk[F_Z * kSlots] = z;
+                    if (code == FLY_GO) { SU[F_META * kSlots] = meta_next; next = Q_F; }
+                    else {
+                        reinterpret_cast<unsigned*>(Bk)[F_TV * kSlots] = vox;
+                        SU[F_META * kSlots] = meta_next | (code == FLY_RAYLEIGH ? (unsigned)mat << 4 : 0u);
+                        next = code == FLY_COMPTON ? Q_C : Q_R;
+                    }
                 } else {
-                    rotate(u, v, w, 1.0f - t, kTwoPi * u01(r.w));
-                    S[F_U * kSlots] = u; S[F_V * kSlots] = v; S[F_W * kSlots] = w;
-                    S[F_E * kSlots] = E;
-                    S[F_TV * kSlots] = fminf(fmaxf((__logf(E) - p.lnE_min) * p.inv_dlnE, 0.0f), t_max);
-                    SU[F_META * kSlots] = (meta_next & ~0x77u) | (unsigned)ST_FLY;
+                    const float E = Bk[F_E * kSlots];
+                    if (code == FLY_PE) { if (STATS) ++c_pe; atomicAdd(p.batch + vox, E); }      // all energy local
+                    else if (STATS) { esc += E; ++c_esc; }
+                    photon_ends(meta);
                 }
-                atomicAdd(p.batch + vox, dep);
-            } else {
-                SU[F_META * kSlots] = meta_next;
             }
-        } else {   // ST_RAYLEIGH
-            const float E = S[F_E * kSlots];
-            float c;
-            if (rayleigh_try(E, r, s_x2, s_cum + ((meta >> 4) & 7u) * p.n_x2, p.n_x2, c)) {
-                if (STATS) ++c_ra;
-                float u = S[F_U * kSlots], v = S[F_V * kSlots], w = S[F_W * kSlots];
-                rotate(u, v, w, c, kTwoPi * u01(r.z));
+            ANM_PUSH(Q_F, hF, nF); ANM_PUSH(Q_C, hC, nC); ANM_PUSH(Q_S, hS, nS); ANM_PUSH(Q_R, hR, nR);
+        } else if (X == Q_C) {
+            hC = (hC + n) & (kSlots - 1); nC -= n;
+            if (active) {
+                const unsigned meta = SU[F_META * kSlots];
+                const unsigned ph = meta & 1u;
+                const unsigned long long h = p.hist_base + SU[F_HL * kSlots];
+                const uint4 r = philox4x32_10(make_uint4((unsigned)h, (unsigned)(h >> 32), meta >> 8, 1u + ph), p);
+                float* Bk = S + ph * (kBankFields * kSlots);
+                float E = Bk[F_E * kSlots];
+                float eps, t;
+                if (compton_try(E, r, eps, t)) {
+                    if (STATS) ++c_co;
+                    const unsigned vox = reinterpret_cast<unsigned*>(Bk)[F_TV * kSlots];
+                    float dep = E * (1.0f - eps);     // recoil electron deposited locally
+                    E *= eps;
+                    if (E < p.cutoff) {               // the rest is deposited locally
+                        dep += E;
+                        if (STATS) ++c_cut;
+                        photon_ends(meta);
+                    } else {
+                        float u = Bk[F_U * kSlots], v = Bk[F_V * kSlots], w = Bk[F_W * kSlots];
+                        rotate(u, v, w, 1.0f - t, kTwoPi * u01(r.w));
+                        Bk[F_U * kSlots] = u; Bk[F_V * kSlots] = v; Bk[F_W * kSlots] = w;
+                        Bk[F_E * kSlots] = E;
+                        Bk[F_TV * kSlots] = fminf(fmaxf((__logf(E) - p.lnE_min) * p.inv_dlnE, 0.0f), t_max);
+                        SU[F_META * kSlots] = (meta & ~0x74u) + 256u;     // a scatter clears AWAY
+                        next = Q_F;
+                    }
+                    atomicAdd(p.batch + vox, dep);
+                } else {
+                    SU[F_META * kSlots] = meta + 256u;
+                    next = Q_C;
+                }
+            }
+            ANM_PUSH(Q_F, hF, nF); ANM_PUSH(Q_C, hC, nC); ANM_PUSH(Q_S, hS, nS);
+        } else if (X == Q_S) {
+            hS = (hS + n) & (kSlots - 1); nS -= n;
+            if (active) {
+                const unsigned long long h = p.hist_base + hl_new;
+                float x, y, z, u, v, w;
+                bool in_box;
+                const unsigned voxel = sample_source(p, h, x, y, z, u, v, w, in_box);
+                S[F_X * kSlots] = x; S[F_Y * kSlots] = y; S[F_Z * kSlots] = z;
                 S[F_U * kSlots] = u; S[F_V * kSlots] = v; S[F_W * kSlots] = w;
-                S[F_TV * kSlots] = fminf(fmaxf((__logf(E) - p.lnE_min) * p.inv_dlnE, 0.0f), t_max);
-                SU[F_META * kSlots] = (meta_next & ~0x77u) | (unsigned)ST_FLY;
-            } else {
-                SU[F_META * kSlots] = meta_next;
+                S[F_E * kSlots] = kE0; S[F_TV * kSlots] = t0;
+                float* B1 = S + kBankFields * kSlots;
+                B1[F_X * kSlots] = x; B1[F_Y * kSlots] = y; B1[F_Z * kSlots] = z;
+                B1[F_U * kSlots] = -u; B1[F_V * kSlots] = -v; B1[F_W * kSlots] = -w;
+                B1[F_E * kSlots] = kE0; B1[F_TV * kSlots] = t0;
+                SU[F_HL * kSlots] = hl_new;
+                SU[F_META * kSlots] = in_box ? (2u | 8u) : 0u;
+                if (p.positron_ke > 0.0f) atomicAdd(p.batch + voxel, p.positron_ke);
+                q[Q_F * kSlots + ((hF + nF + lane) & (kSlots - 1))] = (unsigned char)slot;
             }
+            nF += n;
+        } else {   // Q_R
+            hR = (hR + n) & (kSlots - 1); nR -= n;
+            if (active) {
+                const unsigned meta = SU[F_META * kSlots];
+                const unsigned ph = meta & 1u;
+                const unsigned long long h = p.hist_base + SU[F_HL * kSlots];
+                const uint4 r = philox4x32_10(make_uint4((unsigned)h, (unsigned)(h >> 32), meta >> 8, 1u + ph), p);
+                float* Bk = S + ph * (kBankFields * kSlots);
+                const float E = Bk[F_E * kSlots];
+                float c;
+                if (rayleigh_try(E, r, s_x2, s_cum + ((meta >> 4) & 7u) * p.n_x2, p.n_x2, c)) {
+                    if (STATS) ++c_ra;
+                    float u = Bk[F_U * kSlots], v = Bk[F_V * kSlots], w = Bk[F_W * kSlots];
+                    rotate(u, v, w, c, kTwoPi * u01(r.z));
+                    Bk[F_U * kSlots] = u; Bk[F_V * kSlots] = v; Bk[F_W * kSlots] = w;
+                    Bk[F_TV * kSlots] = fminf(fmaxf((__logf(E) - p.lnE_min) * p.inv_dlnE, 0.0f), t_max);
+                    SU[F_META * kSlots] = (meta & ~0x74u) + 256u;         // a scatter clears AWAY
+                    next = Q_F;
+                } else {
+                    SU[F_META * kSlots] = meta + 256u;
+                    next = Q_R;
+                }
+            }
+            ANM_PUSH(Q_F, hF, nF); ANM_PUSH(Q_R, hR, nR);
         }
     }
+#undef ANM_PUSH
 
     if (STATS) {
         unsigned c_steps = fc.steps, c_real = fc.real;
