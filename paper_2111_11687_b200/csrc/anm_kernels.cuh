@@ -165,7 +165,7 @@ __device__ __forceinline__ int fly_substep(const TransportParams& p, const float
     if (p.hull) {
         const bool in = (unsigned)(ix - p.hx0) < (unsigned)p.hnx && (unsigned)(iy - p.hy0) < (unsigned)p.hny &&
                         (unsigned)(iz - p.hz0) < (unsigned)p.hnz;
-        hull_bits = in ? 1u : (hull_bits ? 2u : 0u);
+        hull_bits = in ? 1u : ((hull_bits + 1u) & 2u);     // IN or AWAY -> AWAY; neither -> neither
     }
     vox = (unsigned)ix + (unsigned)p.nx * ((unsigned)iy + (unsigned)p.ny * (unsigned)iz);
     const unsigned t = __ldg(p.texels + vox);
@@ -180,13 +180,15 @@ __device__ __forceinline__ int fly_substep(const TransportParams& p, const float
 }
 
 // A5: the draw that accepted the collision also picks the channel: rr < mu_pe -> photoelectric, < mu_pe + mu_compton ->
-// Compton, else Rayleigh.
-__device__ __forceinline__ int select_channel(const TransportParams& p, const float2* __restrict__ s_pec, const int mat,
-                                              const float rho, const int ie, const float fe, const float rr) {
+// Compton, else Rayleigh.  Branch-free: every lane of the FLY event evaluates it, lanes without a real collision keep
+// their code.
+__device__ __forceinline__ int select_channel(const TransportParams& p, const float2* __restrict__ s_pec, const int code,
+                                              const int mat, const float rho, const int ie, const float fe, const float rr) {
     const float2 a = s_pec[mat * p.ne + ie], b = s_pec[mat * p.ne + ie + 1];
-    if (rr < rho * fmaf(fe, b.x - a.x, a.x)) return FLY_PE;
-    if (rr < rho * fmaf(fe, b.y - a.y, a.y) || !p.rayleigh_on) return FLY_COMPTON;
-    return FLY_RAYLEIGH;
+    const bool pe = rr < rho * fmaf(fe, b.x - a.x, a.x);
+    const bool co = rr < rho * fmaf(fe, b.y - a.y, a.y) || !p.rayleigh_on;
+    const int ch = pe ? FLY_PE : (co ? FLY_COMPTON : FLY_RAYLEIGH);
+    return code == FLY_REAL ? ch : code;
 }
 
 // Two Woodcock sub-steps from one Philox block (words x,y then z,w); stops at the first real collision or escape.
@@ -197,13 +199,13 @@ __device__ __forceinline__ int fly_two(const TransportParams& p, const float* __
                                        const float maj, const float inv_maj, const float maj_out, const float inv_maj_out,
                                        const uint4 r, unsigned& hull_bits, unsigned& vox, int& mat, FlyCounters& cnt) {
     float rho = 0.0f, rr = 0.0f;
+    mat = 0;
     int code = fly_substep<STATS>(p, s_tot, x, y, z, u, v, w, ie, fe, maj, inv_maj, maj_out, inv_maj_out, r.x, r.y,
                                   hull_bits, vox, mat, rho, rr, cnt);
     if (code == FLY_GO)
         code = fly_substep<STATS>(p, s_tot, x, y, z, u, v, w, ie, fe, maj, inv_maj, maj_out, inv_maj_out, r.z, r.w,
                                   hull_bits, vox, mat, rho, rr, cnt);
-    if (code == FLY_REAL) code = select_channel(p, s_pec, mat, rho, ie, fe, rr);
-    return code;
+    return select_channel(p, s_pec, code, mat, rho, ie, fe, rr);
 }
 
 // One Klein-Nishina try by composition-rejection on f(eps) = (1/eps + eps) g(eps).
@@ -264,7 +266,7 @@ __device__ __forceinline__ unsigned sample_source(const TransportParams& p, cons
     } else {
         const unsigned long long r64 = ((unsigned long long)r.x << 32) | r.y;
         const unsigned j = (unsigned)__umul64hi(r64, (unsigned long long)p.n_alias);
-        const uint4 a = __ldg(p.alias + j);
+        const uint4 a = __ldcs(p.alias + j);      // one use per decay, 16 B out of ~100 MB: evict-first, keep L2 for texels + tally
         voxel = (r.z < a.x) ? a.y : a.z;
         const unsigned nxy = (unsigned)p.nx * (unsigned)p.ny;
         iz = voxel / nxy;
@@ -495,13 +497,18 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
     unsigned c_pe = 0, c_co = 0, c_ra = 0, c_esc = 0, c_cut = 0;
     FlyCounters fc = {0u, 0u};
 
-    // push the slots whose next event is T onto ring T (all 32 lanes call it)
-#define ANM_PUSH(T, hT, nT)                                                                               \
-    do {                                                                                                   \
-        const unsigned b_ = __ballot_sync(0xffffffffu, next == (T));                                       \
-        if (next == (T)) q[(T) * kSlots + (((hT) + (nT) + __popc(b_ & lanemask_lt)) & (kSlots - 1))] = (unsigned char)slot; \
-        (nT) += __popc(b_);                                                                                \
-    } while (0)
+    // Push every processed slot onto the ring of its next event (all 32 lanes call it; idle lanes pass Q_NONE):
+    // one match groups the lanes by destination, the rank inside the group is the ring offset, one packed warp
+    // reduction counts the four groups.
+    auto push_all = [&](const int next, const unsigned slot) {
+        const unsigned same = __match_any_sync(0xffffffffu, next);
+        const unsigned rank = __popc(same & lanemask_lt);
+        const unsigned tails = ((hF + nF) & 255u) | (((hC + nC) & 255u) << 8) | (((hS + nS) & 255u) << 16) | (((hR + nR) & 255u) << 24);
+        if (next != Q_NONE)
+            q[next * kSlots + ((((tails >> (8 * next)) & 255u) + rank) & (kSlots - 1))] = (unsigned char)slot;
+        const unsigned cnt = __reduce_add_sync(0xffffffffu, next != Q_NONE ? 1u << (8 * next) : 0u);
+        nF += cnt & 255u; nC += (cnt >> 8) & 255u; nS += (cnt >> 16) & 255u; nR += cnt >> 24;
+    };
 
     for (;;) {
         __syncwarp();
@@ -565,24 +572,23 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                 unsigned vox = 0, hb = (meta >> 1) & 3u;
                 int mat = 0;
                 const int code = fly_two<STATS>(p, s_tot, s_pec, x, y, z, u, v, w, ie, fe, maj, inv_maj, majo, inv_majo, r, hb, vox, mat, fc);
-                const unsigned meta_next = ((meta & ~0x76u) | (hb << 1)) + 256u;    // block counter + 1, new hull bits
-                ANM_TR("S2 h=%llu ph=%u blk=%u FLY code=%d E=%.9g t=%d+%.9g pos=%.9g %.9g %.9g vox=%u hb=%u\n", h, ph, meta >> 8, code, Bk[F_E * kSlots], ie, fe, x, y, z, vox, hb);
-                if (code == FLY_GO || code == FLY_COMPTON || code == FLY_RAYLEIGH) {
-                    Bk[F_X * kSlots] = x; Bk[F_Y * kSlots] = y; Bk[F_Z * kSlots] = z;
-                    if (code == FLY_GO) { SU[F_META * kSlots] = meta_next; next = Q_F; }
-                    else {
-                        reinterpret_cast<unsigned*>(Bk)[F_TV * kSlots] = vox;
-                        SU[F_META * kSlots] = meta_next | (code == FLY_RAYLEIGH ? (unsigned)mat << 4 : 0u);
-                        next = code == FLY_COMPTON ? Q_C : Q_R;
-                    }
-                } else {
-                    const float E = Bk[F_E * kSlots];
-                    if (code == FLY_PE) { if (STATS) ++c_pe; atomicAdd(p.batch + vox, E); }      // all energy local
-                    else if (STATS) { esc += E; ++c_esc; }
-                    photon_ends(meta);
-                }
+                ANM_TR("S2 h=%llu ph=%u blk=%u FLY code=%d t=%d+%.9g pos=%.9g %.9g %.9g vox=%u hb=%u\n", h, ph, meta >> 8, code, ie, fe, x, y, z, vox, hb);
+                Bk[F_X * kSlots] = x; Bk[F_Y * kSlots] = y; Bk[F_Z * kSlots] = z;
+                // next event and slot header, branch-free: GO -> FLY; COMPTON / RAYLEIGH -> their queues, the voxel in
+                // place of the energy coordinate; PE / ESCAPED end the photon: start the partner (bank 1, written at
+                // the decay) or free the slot
+                const bool coll = code == FLY_COMPTON || code == FLY_RAYLEIGH;
+                const bool ended = code == FLY_PE || code == FLY_ESCAPED;
+                const bool partner = !ph && p.photons_per_decay == 2;
+                const unsigned meta_go = (((meta & ~0x76u) | (hb << 1)) + 256u) | (code == FLY_RAYLEIGH ? (unsigned)mat << 4 : 0u);
+                const unsigned meta_end = 1u | (meta & 8u) | ((meta & 8u) >> 2);   // photon B, block 0, IN = decay voxel's
+                SU[F_META * kSlots] = ended ? meta_end : meta_go;
+                if (coll) reinterpret_cast<unsigned*>(Bk)[F_TV * kSlots] = vox;
+                next = code == FLY_COMPTON ? Q_C : (code == FLY_RAYLEIGH ? Q_R : ((ended && !partner) ? Q_S : Q_F));
+                if (code == FLY_PE) { if (STATS) ++c_pe; atomicAdd(p.batch + vox, Bk[F_E * kSlots]); }      // all energy local
+                if (STATS && code == FLY_ESCAPED) { esc += Bk[F_E * kSlots]; ++c_esc; }
             }
-            ANM_PUSH(Q_F, hF, nF); ANM_PUSH(Q_C, hC, nC); ANM_PUSH(Q_S, hS, nS); ANM_PUSH(Q_R, hR, nR);
+            push_all(next, slot);
         } else if (X == Q_C) {
             hC = (hC + n) & (kSlots - 1); nC -= n;
             if (active) {
@@ -617,7 +623,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                     next = Q_C;
                 }
             }
-            ANM_PUSH(Q_F, hF, nF); ANM_PUSH(Q_C, hC, nC); ANM_PUSH(Q_S, hS, nS);
+            push_all(next, slot);
         } else if (X == Q_S) {
             hS = (hS + n) & (kSlots - 1); nS -= n;
             if (active) {
@@ -661,10 +667,9 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                     next = Q_R;
                 }
             }
-            ANM_PUSH(Q_F, hF, nF); ANM_PUSH(Q_R, hR, nR);
+            push_all(next, slot);
         }
     }
-#undef ANM_PUSH
 
     if (STATS) {
         unsigned c_steps = fc.steps, c_real = fc.real;
