@@ -134,78 +134,86 @@ __device__ __forceinline__ void deposit(float* __restrict__ batch, unsigned vox,
     }
 }
 
-// One Woodcock sub-step: exponential flight against the majorant, voxel lookup, real / virtual
-// decision.  Returns FLY_GO (virtual), FLY_ESCAPED, or FLY_REAL with (mat, rho, rr) for select_channel.
+// Woodcock flight: two sub-steps from one Philox block (words x,y then z,w), stopping at the
+// first real collision or escape.  A sub-step: exponential flight against the majorant, voxel lookup, real / virtual
+// decision from one more uniform, which also picks the channel.
+//
+// The second sub-step is evaluated speculatively, as if the first were a virtual collision: its landing point, voxel
+// index and majorant need no memory, so both texel loads are in flight together (one exposed L2 round trip per event
+// instead of two) and the event is branch-free.  The arithmetic of each sub-step is exactly the sequential one.
 //
 // Hull majorant (reading C24), branch-free.  hull_bits: bit 0 = IN, the photon's last landing point (or its
 // start) was inside the hull box; bit 1 = AWAY, the photon is outside the box and has flown straight since a point
 // inside it.  A straight ray that has left a convex box never re-enters it, so an AWAY photon flies against the
 // majorant of the voxels outside the box; every other photon against the global majorant, which is valid everywhere.
 // A scatter clears AWAY (the caller does), a landing inside the box sets IN.
-enum : int { FLY_GO = 0, FLY_ESCAPED = 1, FLY_PE = 2, FLY_COMPTON = 3, FLY_RAYLEIGH = 4, FLY_REAL = 5 };
+enum : int { FLY_GO = 0, FLY_ESCAPED = 1, FLY_PE = 2, FLY_COMPTON = 3, FLY_RAYLEIGH = 4 };
 
 struct FlyCounters { unsigned steps, real; };
 
-template <bool STATS>
-__device__ __forceinline__ int fly_substep(const TransportParams& p, const float* __restrict__ s_tot,
-                                           float& x, float& y, float& z, const float u, const float v, const float w,
-                                           const int ie, const float fe, const float maj, const float inv_maj,
-                                           const float maj_out, const float inv_maj_out,
-                                           const unsigned r_s, const unsigned r_a, unsigned& hull_bits,
-                                           unsigned& vox, int& mat, float& rho, float& rr, FlyCounters& cnt) {
+struct SubStep {        // one landing point
+    float x, y, z, m_here;
+    unsigned vox, hull_bits;
+    bool inside;        // inside the grid (else the photon has escaped)
+};
+
+__device__ __forceinline__ SubStep fly_land(const TransportParams& p, const float x, const float y, const float z,
+                                            const float u, const float v, const float w, const float maj,
+                                            const float inv_maj, const float maj_out, const float inv_maj_out,
+                                            const unsigned r_s, const unsigned hull_bits) {
+    SubStep o;
     const float nl = -__logf(u01(r_s));
-    if (STATS) ++cnt.steps;
     const bool away = (hull_bits & 2u) != 0u;
-    const float m_here = away ? maj_out : maj;
+    o.m_here = away ? maj_out : maj;
     const float s = nl * (away ? inv_maj_out : inv_maj);
-    x = fmaf(s, u, x); y = fmaf(s, v, y); z = fmaf(s, w, z);
-    const int ix = __float2int_rd(x * p.inv_dx), iy = __float2int_rd(y * p.inv_dy), iz = __float2int_rd(z * p.inv_dz);
-    if ((unsigned)ix >= (unsigned)p.nx || (unsigned)iy >= (unsigned)p.ny || (unsigned)iz >= (unsigned)p.nz)
-        return FLY_ESCAPED;
+    o.x = fmaf(s, u, x); o.y = fmaf(s, v, y); o.z = fmaf(s, w, z);
+    const int ix = __float2int_rd(o.x * p.inv_dx), iy = __float2int_rd(o.y * p.inv_dy), iz = __float2int_rd(o.z * p.inv_dz);
+    o.inside = (unsigned)ix < (unsigned)p.nx && (unsigned)iy < (unsigned)p.ny && (unsigned)iz < (unsigned)p.nz;
+    o.hull_bits = hull_bits;
     if (p.hull) {
         const bool in = (unsigned)(ix - p.hx0) < (unsigned)p.hnx && (unsigned)(iy - p.hy0) < (unsigned)p.hny &&
                         (unsigned)(iz - p.hz0) < (unsigned)p.hnz;
-        hull_bits = in ? 1u : ((hull_bits + 1u) & 2u);     // IN or AWAY -> AWAY; neither -> neither
+        o.hull_bits = in ? 1u : ((hull_bits + 1u) & 2u);     // IN or AWAY -> AWAY; neither -> neither
     }
-    vox = (unsigned)ix + (unsigned)p.nx * ((unsigned)iy + (unsigned)p.ny * (unsigned)iz);
-    const unsigned t = __ldg(p.texels + vox);
-    mat = (int)(t >> 24);
-    rho = (float)(t & 0xffffffu) * kDensityStep;
-    const float* row = s_tot + mat * p.ne + ie;
-    const float mu = rho * fmaf(fe, row[1] - row[0], row[0]);
-    rr = u01(r_a) * m_here;
-    if (rr >= mu) return FLY_GO;                     // virtual collision
-    if (STATS) ++cnt.real;
-    return FLY_REAL;
+    o.vox = (unsigned)ix + (unsigned)p.nx * ((unsigned)iy + (unsigned)p.ny * (unsigned)iz);
+    return o;
 }
 
-// A5: the draw that accepted the collision also picks the channel: rr < mu_pe -> photoelectric, < mu_pe + mu_compton ->
-// Compton, else Rayleigh.  Branch-free: every lane of the FLY event evaluates it, lanes without a real collision keep
-// their code.
-__device__ __forceinline__ int select_channel(const TransportParams& p, const float2* __restrict__ s_pec, const int code,
-                                              const int mat, const float rho, const int ie, const float fe, const float rr) {
-    const float2 a = s_pec[mat * p.ne + ie], b = s_pec[mat * p.ne + ie + 1];
-    const bool pe = rr < rho * fmaf(fe, b.x - a.x, a.x);
-    const bool co = rr < rho * fmaf(fe, b.y - a.y, a.y) || !p.rayleigh_on;
-    const int ch = pe ? FLY_PE : (co ? FLY_COMPTON : FLY_RAYLEIGH);
-    return code == FLY_REAL ? ch : code;
-}
-
-// Two Woodcock sub-steps from one Philox block (words x,y then z,w); stops at the first real collision or escape.
 template <bool STATS>
 __device__ __forceinline__ int fly_two(const TransportParams& p, const float* __restrict__ s_tot,
                                        const float2* __restrict__ s_pec, float& x, float& y, float& z,
                                        const float u, const float v, const float w, const int ie, const float fe,
                                        const float maj, const float inv_maj, const float maj_out, const float inv_maj_out,
                                        const uint4 r, unsigned& hull_bits, unsigned& vox, int& mat, FlyCounters& cnt) {
-    float rho = 0.0f, rr = 0.0f;
-    mat = 0;
-    int code = fly_substep<STATS>(p, s_tot, x, y, z, u, v, w, ie, fe, maj, inv_maj, maj_out, inv_maj_out, r.x, r.y,
-                                  hull_bits, vox, mat, rho, rr, cnt);
-    if (code == FLY_GO)
-        code = fly_substep<STATS>(p, s_tot, x, y, z, u, v, w, ie, fe, maj, inv_maj, maj_out, inv_maj_out, r.z, r.w,
-                                  hull_bits, vox, mat, rho, rr, cnt);
-    return select_channel(p, s_pec, code, mat, rho, ie, fe, rr);
+    const SubStep a = fly_land(p, x, y, z, u, v, w, maj, inv_maj, maj_out, inv_maj_out, r.x, hull_bits);
+    const unsigned ta = a.inside ? __ldg(p.texels + a.vox) : 0u;
+    const SubStep b = fly_land(p, a.x, a.y, a.z, u, v, w, maj, inv_maj, maj_out, inv_maj_out, r.z, a.hull_bits);
+    const bool b_inside = a.inside && b.inside;
+    const unsigned tb = b_inside ? __ldg(p.texels + b.vox) : 0u;
+    // real / virtual: u' * majorant < rho * (mu/rho)_tot(E)
+    const int mat_a = (int)(ta >> 24), mat_b = (int)(tb >> 24);
+    const float rho_a = (float)(ta & 0xffffffu) * kDensityStep, rho_b = (float)(tb & 0xffffffu) * kDensityStep;
+    const float* row_a = s_tot + mat_a * p.ne + ie;
+    const float* row_b = s_tot + mat_b * p.ne + ie;
+    const float rr_a = u01(r.y) * a.m_here, rr_b = u01(r.w) * b.m_here;
+    const bool real_a = a.inside && rr_a < rho_a * fmaf(fe, row_a[1] - row_a[0], row_a[0]);
+    const bool real_b = b_inside && rr_b < rho_b * fmaf(fe, row_b[1] - row_b[0], row_b[0]);
+    const bool first = real_a || !a.inside;            // the event ends at the first sub-step
+    if (STATS) { cnt.steps += first ? 1u : 2u; cnt.real += (real_a || (!first && real_b)) ? 1u : 0u; }
+    x = first ? a.x : b.x; y = first ? a.y : b.y; z = first ? a.z : b.z;
+    hull_bits = first ? a.hull_bits : b.hull_bits;
+    vox = first ? a.vox : b.vox;
+    mat = first ? mat_a : mat_b;
+    const float rho = first ? rho_a : rho_b, rr = first ? rr_a : rr_b;
+    const bool escaped = !a.inside || (!real_a && !b.inside);
+    const bool real = real_a || real_b;                // real_b implies a.inside; if real_a the first one counts
+    // A5: the draw that accepted the collision also picks the channel: rr < mu_pe -> photoelectric,
+    // < mu_pe + mu_compton -> Compton, else Rayleigh
+    const float2 c0 = s_pec[mat * p.ne + ie], c1 = s_pec[mat * p.ne + ie + 1];
+    const bool pe = rr < rho * fmaf(fe, c1.x - c0.x, c0.x);
+    const bool co = rr < rho * fmaf(fe, c1.y - c0.y, c0.y) || !p.rayleigh_on;
+    const int ch = pe ? FLY_PE : (co ? FLY_COMPTON : FLY_RAYLEIGH);
+    return escaped ? FLY_ESCAPED : (real ? ch : FLY_GO);
 }
 
 // One Klein-Nishina try by composition-rejection on f(eps) = (1/eps + eps) g(eps).
