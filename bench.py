@@ -11,8 +11,10 @@ Woodcock transport, tally, 100 batch folds with organ reduction, finalize -- eve
 dose + uncertainty + organ read-back to the host).  `roofline` is the ALU/issue roofline of the transport kernel
 (DESIGN.md §6); `cpu_baseline` is the oracle timed on this box's host cores on a bounded sample.
 With --impl reference the oracle itself is the timed arm (same metric / config, bounded sample per step).
-Under torchrun (N > 1) each rank simulates its own whole-batch shard of one logical run of N*D decays
-(history_offset = rank*D); no data-path collective, scaling = weak.
+Under torchrun (N > 1) the step is ONE logical run of N*D decays in N*100 batches: each rank simulates its own
+whole-batch shard (history_offset = rank*D, no collective during transport) and the step ends with the merge of
+the tallies (paper_2111_11687_b200.multi_gpu.run_sharded: in-place NCCL sum-all-reduce of the sum / sum-of-squares
+volumes + organ rows, finalize on the merged volumes); per-GPU work is fixed, scaling = weak.
 """
 from __future__ import annotations
 
@@ -143,8 +145,16 @@ def main():
     D = int(args.decays)
     B = cfg["n_batches"]
     V = int(np.prod(cfg["shape"]))
-    opts = dict(n_batches=B, photons_per_decay=2, rayleigh_on=1, photon_cutoff_MeV=0.010,
-                positron_ke_MeV=cfg["positron_ke_mev"], history_offset=rank * D)
+    phys = dict(photons_per_decay=2, rayleigh_on=1, photon_cutoff_MeV=0.010, positron_ke_MeV=cfg["positron_ke_mev"])
+    opts = dict(n_batches=B, history_offset=rank * D, **phys)
+    if world > 1:
+        from paper_2111_11687_b200.multi_gpu import run_sharded
+
+    def step(s):
+        if world > 1:
+            run_sharded(s, world * D, cfg["seed"], world * B, phys)      # this rank's shard + the NCCL merge
+        else:
+            s.run(D, cfg["seed"])
 
     # ---- device-resident arm ----------------------------------------------------------------------------
     stream = torch.cuda.Stream(device=dev)
@@ -168,7 +178,7 @@ def main():
         per_decay = {k: cnt[k] / n_cnt for k in ("n_steps", "n_real", "n_pe", "n_compton", "n_rayleigh")}
         sim.set_options(collect_stats=0, **opts)
         for _ in range(args.warmup):
-            sim.run(D, cfg["seed"])
+            step(sim)
         if dist:
             dist.barrier()
         torch.cuda.synchronize(dev)
@@ -179,7 +189,7 @@ def main():
         launches = 0
         e0.record(stream)
         for _ in range(args.steps):
-            sim.run(D, cfg["seed"])
+            step(sim)
             st = sim.get_stats()
             ms_t += st["ms_transport"]; ms_f += st["ms_fold"]; ms_fin += st["ms_finalize"]
             launches += st["n_launches"]
@@ -204,14 +214,16 @@ def main():
     achieved = instr_per_decay * (D / B) / sec_per_launch / 1e9                     # G thread-instr / s
     sm_max = clk.get("sm_max_mhz") or 1965.0
     peak = N_SM * LANES_PER_SM_PER_CLK * sm_max * 1e6 / 1e9
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "transport_dram_bytes_per_launch.json")
-    if os.path.exists(tpath):
-        try:
-            traffic = json.load(open(tpath)).get("dram_bytes_per_launch")
-        except Exception:
-            traffic = None
-    roofline = {"bound": "alu", "kernel": "transport_kernel", "achieved": achieved, "peak": peak, "unit": "Gthread-instr/s",
+    traffic = None          # dram__bytes_read.sum + dram__bytes_write.sum per launch, from the committed ncu capture
+    tdir = os.path.join(ROOT, "profiles")
+    for name in sorted(os.listdir(tdir) if os.path.isdir(tdir) else [], reverse=True):
+        if name.endswith("_transport_traffic.csv"):
+            import csv
+            rows = list(csv.DictReader(open(os.path.join(tdir, name))))
+            if rows and int(rows[-1]["decays_per_launch"]) == D // B:
+                traffic = int(rows[-1]["dram_bytes_read"]) + int(rows[-1]["dram_bytes_write"])
+            break
+    roofline = {"bound": "alu", "kernel": "transport_pool_kernel", "achieved": achieved, "peak": peak, "unit": "Gthread-instr/s",
                 "frac": achieved / peak, "traffic": traffic,
                 "peak_source": "148 SM x 4 SMSP x 32 lanes x %.0f MHz (clocks.max.sm), DESIGN.md §6" % sm_max,
                 "instr_per_decay_algorithmic": instr_per_decay, "events_per_decay": per_decay,
@@ -235,7 +247,7 @@ def main():
             s2.load_organs(hl, cfg["n_organs"])
             s2.set_physics_tables(tables)
             s2.set_options(**opts)
-            s2.run(D, cfg["seed"])
+            step(s2)
             s2.get_dose(out_d)
             s2.get_uncertainty(out_u)
             organs = s2.get_organ_doses()
@@ -275,7 +287,7 @@ def main():
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": WORKLOAD, "decays_per_step_per_gpu": D, "seed": cfg["seed"],
                    "l2": "working set (texels 105 MB + batch tally 105 MB + sum/sumsq 210 MB) exceeds the 126 MB L2; no flush needed",
-                   "multi_gpu": "whole-batch shards via history_offset, no collective" if world > 1 else "single GPU"},
+                   "multi_gpu": "one logical run of N*D decays: whole-batch shards via history_offset, NCCL sum-all-reduce of the tallies + merged finalize at the end of every step" if world > 1 else "single GPU"},
         "clocks": clk, "e2e": e2e, "gpu_launches": int(launches),
         "phase_ms_per_step": {"transport": ms_t / args.steps, "fold": ms_f / args.steps, "finalize": ms_fin / args.steps},
         "roofline": roofline, "cpu_baseline": cpu,

@@ -144,6 +144,27 @@ int anm_get_uncertainty(anm_ctx* c, float* out_rel_sigma, size_t n, int on_devic
 int anm_get_organ_doses(anm_ctx* c, anm_organ* out, int n_organs);                  /* host array, out[k] = label k+1 */
 int anm_get_stats(anm_ctx* c, anm_stats* out);
 
+/* --- one logical run over several GPUs ---------------------------------------
+ * Histories are independent and keyed by index (Philox counter = history index), so a run of N decays in B batches
+ * shards by whole batches: rank r sets anm_options.history_offset = (first batch of r) * N/B and n_batches = its own
+ * batch count, and calls anm_run on its N/B * n_batches decays.  The one exchange step is the merge of the tallies:
+ *
+ *   anm_get_tally_buffers  returns the ctx-owned DEVICE pointers of the last run's per-voxel sum and sum of squares
+ *                          over batches (n_floats = nx*ny*nz rounded up to a multiple of 4, fp32, MeV and MeV^2)
+ *                          and of its organ rows (n_rows = this run's n_batches rows of 256 fp64: row[b][label] =
+ *                          sum over the organ's voxels of x / (rho V_vox) in batch b).  The caller sum-all-reduces
+ *                          d_sum and d_sumsq IN PLACE across ranks (NCCL over NVLink) and gathers the organ rows of
+ *                          all ranks in batch order; the pointers stay valid until the next anm_run / anm_set_grid.
+ *   anm_merge              recomputes A11 (finalize) on the reduced volumes for the whole run: total_decays and
+ *                          total_batches are the logical run's; organ_rows_all is a HOST array [total_batches][256]
+ *                          (required when organ labels are loaded, else may be NULL); summed, if not NULL, is the
+ *                          caller's element-wise sum of every rank's anm_stats (counters and escaped energy).
+ *                          Afterwards every anm_get_* call on this ctx returns the merged result.
+ * ANM_E_STATE without a completed run; ANM_E_ARG if total_decays / total_batches differs from this run's decays per
+ * batch. */
+int anm_get_tally_buffers(anm_ctx* c, float** d_sum, float** d_sumsq, size_t* n_floats, double** d_organ_rows, int* n_rows);
+int anm_merge(anm_ctx* c, uint64_t total_decays, int total_batches, const double* organ_rows_all, const anm_stats* summed);
+
 #ifdef __cplusplus
 }
 #endif

@@ -19,7 +19,7 @@ ANM_SYMBOLS = [
     "anm_create", "anm_destroy", "anm_last_error", "anm_set_stream", "anm_set_grid", "anm_load_phantom",
     "anm_load_activity", "anm_set_point_source", "anm_load_organs", "anm_set_physics_tables", "anm_set_options",
     "anm_default_options", "anm_run", "anm_get_energy", "anm_get_dose", "anm_get_dose_rate", "anm_get_uncertainty",
-    "anm_get_organ_doses", "anm_get_stats",
+    "anm_get_organ_doses", "anm_get_stats", "anm_get_tally_buffers", "anm_merge",
 ]
 
 STATUS = {0: "ANM_OK", -1: "ANM_E_ARG", -2: "ANM_E_STATE", -3: "ANM_E_CUDA", -4: "ANM_E_NOMEM", -5: "ANM_E_UNSUPPORTED"}
@@ -92,6 +92,8 @@ def load(build_if_missing: bool = True):
         "anm_get_energy": (i32, [vp, vp, sz, i32]), "anm_get_dose": (i32, [vp, vp, sz, i32]),
         "anm_get_dose_rate": (i32, [vp, dbl, vp, sz, i32]), "anm_get_uncertainty": (i32, [vp, vp, sz, i32]),
         "anm_get_organ_doses": (i32, [vp, C.POINTER(anm_organ), i32]), "anm_get_stats": (i32, [vp, C.POINTER(anm_stats)]),
+        "anm_get_tally_buffers": (i32, [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(sz), C.POINTER(vp), C.POINTER(i32)]),
+        "anm_merge": (i32, [vp, u64, i32, vp, C.POINTER(anm_stats)]),
     }
     for name, (res, args) in protos.items():
         f = getattr(L, name)
@@ -262,6 +264,37 @@ class Simulation:
         s = anm_stats()
         self._ck(self._L.anm_get_stats(self._ctx, C.byref(s)))
         return s.as_dict()
+
+    # ---- one logical run over several GPUs (include/anm.h, "one logical run over several GPUs")
+    def get_tally_buffers(self):
+        """Zero-copy torch views of the ctx-owned device buffers: (sum f32[Vpad], sumsq f32[Vpad], organ_rows f64[B][256])."""
+        import torch
+        ps, pq, pr = C.c_void_p(), C.c_void_p(), C.c_void_p()
+        n, rows = C.c_size_t(), C.c_int()
+        self._ck(self._L.anm_get_tally_buffers(self._ctx, C.byref(ps), C.byref(pq), C.byref(n), C.byref(pr), C.byref(rows)))
+
+        class _View:   # the CUDA array interface is what torch.as_tensor reads: no copy, the ctx keeps ownership
+            def __init__(self, ptr, shape, typestr):
+                self.__cuda_array_interface__ = {"shape": shape, "typestr": typestr, "data": (int(ptr), False), "version": 3}
+
+        dev = torch.device("cuda", self.device)
+        return (torch.as_tensor(_View(ps.value, (n.value,), "<f4"), device=dev),
+                torch.as_tensor(_View(pq.value, (n.value,), "<f4"), device=dev),
+                torch.as_tensor(_View(pr.value, (rows.value, 256), "<f8"), device=dev))
+
+    def merge(self, total_decays: int, total_batches: int, organ_rows_all=None, summed_stats: dict | None = None):
+        rows = None
+        if organ_rows_all is not None:
+            rows = np.ascontiguousarray(organ_rows_all, np.float64)
+            if rows.shape != (int(total_batches), 256):
+                raise ValueError("organ_rows_all must be [total_batches][256]")
+        st = None
+        if summed_stats is not None:
+            st = anm_stats()
+            for k, v in summed_stats.items():
+                setattr(st, k, type(getattr(st, k))(v))
+        self._ck(self._L.anm_merge(self._ctx, int(total_decays), int(total_batches),
+                                   rows.ctypes.data if rows is not None else None, C.byref(st) if st is not None else None))
 
     # ---- convenience: everything a config dict (anm_inputs.make_config) describes
     def load_config(self, cfg: dict, tables: dict, **options):

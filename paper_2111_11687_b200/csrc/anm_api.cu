@@ -221,6 +221,58 @@ TransportFn pick_transport(int schedule, bool stats, bool wagg) {
                  : (wagg ? transport_kernel<false, true> : transport_kernel<false, false>);
 }
 
+// A11 on the current sum / sumsq volumes: finalize_kernel, then the organ arithmetic of SURVEY.md §8(c) step 7 on the
+// host over the B x 256 fp64 organ rows (rows_host, or the ctx's own device rows when null):
+// d_{o,b} = row[b][o] k / (n_b N_o); mean and batch sigma over b.  Fills c->organs and c->stats.deposited_MeV.
+int finalize_and_collect(anm_ctx* c, int B, uint64_t nb, uint64_t n_decays, const double* rows_host) {
+    cudaStream_t st = c->stream;
+    ANM_CUDA(c, cudaMemsetAsync(c->organ_acc.p, 0, 256 * sizeof(OrganAccum), st));
+    ANM_CUDA(c, cudaMemsetAsync(c->total_energy.p, 0, 8, st));
+    finalize_kernel<<<grid_blocks(c, c->V, kFoldThreads), kFoldThreads, 0, st>>>(
+        c->sum.p, c->sumsq.p, c->have_organs ? c->labels.p : nullptr, c->organ_acc.p, c->total_energy.p,
+        c->n_organs, c->V, B);
+    ANM_CUDA(c, cudaGetLastError());
+    std::vector<double> ob;
+    OrganAccum acc[256];
+    double mass[256];
+    unsigned long long cnt[256];
+    double tot_e = 0;
+    ANM_CUDA(c, cudaMemcpyAsync(&tot_e, c->total_energy.p, 8, cudaMemcpyDeviceToHost, st));
+    if (c->have_organs) {
+        if (!rows_host) {
+            ob.resize((size_t)B * 256);
+            ANM_CUDA(c, cudaMemcpyAsync(ob.data(), c->organ_batch.p, ob.size() * 8, cudaMemcpyDeviceToHost, st));
+            rows_host = ob.data();
+        }
+        ANM_CUDA(c, cudaMemcpyAsync(acc, c->organ_acc.p, sizeof acc, cudaMemcpyDeviceToHost, st));
+        ANM_CUDA(c, cudaMemcpyAsync(mass, c->organ_mass.p, sizeof mass, cudaMemcpyDeviceToHost, st));
+        ANM_CUDA(c, cudaMemcpyAsync(cnt, c->organ_count.p, sizeof cnt, cudaMemcpyDeviceToHost, st));
+    }
+    ANM_CUDA(c, cudaStreamSynchronize(st));
+    c->organs.assign((size_t)c->n_organs, anm_organ{});
+    if (c->have_organs) {
+        for (int o = 1; o <= c->n_organs; ++o) {
+            anm_organ& r = c->organs[(size_t)o - 1];
+            r.n_voxels = cnt[o];
+            r.mass_g = mass[o];
+            r.n_voxels_nonzero = (uint64_t)(acc[o].n_nonzero + 0.5);
+            if (cnt[o] == 0) continue;
+            double s1 = 0, s2 = 0;
+            for (int b = 0; b < B; ++b) {
+                const double d = rows_host[(size_t)b * 256 + o] * kGyPerMeVPerGram / ((double)nb * (double)cnt[o]);
+                s1 += d; s2 += d * d;
+            }
+            const double mean = s1 / B;
+            r.mean_Gy_per_decay = mean;
+            r.sigma_mean = std::sqrt(std::max(0.0, (s2 / B - mean * mean) / (B - 1)));
+            r.rms_voxel_rel_sigma = acc[o].n_nonzero > 0 ? std::sqrt(acc[o].rel2 / acc[o].n_nonzero) : 0.0;
+            r.mass_weighted_Gy_per_decay = mass[o] > 0 ? acc[o].energy * kGyPerMeVPerGram / ((double)n_decays * mass[o]) : 0.0;
+        }
+    }
+    c->stats.deposited_MeV = tot_e;
+    return ANM_OK;
+}
+
 }  // namespace
 
 // =================================================================================================
@@ -601,27 +653,13 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
         ANM_CUDA_EV(cudaGetLastError());
         ANM_CUDA_EV(cudaEventRecord(ev[2 * b + 2], st));
     }
-    finalize_kernel<<<grid_blocks(c, c->V, kFoldThreads), kFoldThreads, 0, st>>>(
-        c->sum.p, c->sumsq.p, c->have_organs ? c->labels.p : nullptr, c->organ_acc.p, c->total_energy.p,
-        c->n_organs, c->V, B);
-    ANM_CUDA_EV(cudaGetLastError());
-    ANM_CUDA_EV(cudaEventRecord(ev[2 * B + 1], st));
-
-    // results to the host
-    std::vector<double> ob((size_t)B * 256);
-    OrganAccum acc[256];
-    double mass[256];
-    unsigned long long cnt[256];
-    DeviceStats ds;
-    double tot_e = 0;
-    ANM_CUDA_EV(cudaMemcpyAsync(&ds, c->dstats.p, sizeof ds, cudaMemcpyDeviceToHost, st));
-    ANM_CUDA_EV(cudaMemcpyAsync(&tot_e, c->total_energy.p, 8, cudaMemcpyDeviceToHost, st));
-    if (c->have_organs) {
-        ANM_CUDA_EV(cudaMemcpyAsync(ob.data(), c->organ_batch.p, ob.size() * 8, cudaMemcpyDeviceToHost, st));
-        ANM_CUDA_EV(cudaMemcpyAsync(acc, c->organ_acc.p, sizeof acc, cudaMemcpyDeviceToHost, st));
-        ANM_CUDA_EV(cudaMemcpyAsync(mass, c->organ_mass.p, sizeof mass, cudaMemcpyDeviceToHost, st));
-        ANM_CUDA_EV(cudaMemcpyAsync(cnt, c->organ_count.p, sizeof cnt, cudaMemcpyDeviceToHost, st));
+    {
+        const int rc = finalize_and_collect(c, B, nb, n_decays, nullptr);
+        if (rc != ANM_OK) { free_events(); return rc; }
     }
+    ANM_CUDA_EV(cudaEventRecord(ev[2 * B + 1], st));
+    DeviceStats ds;
+    ANM_CUDA_EV(cudaMemcpyAsync(&ds, c->dstats.p, sizeof ds, cudaMemcpyDeviceToHost, st));
     ANM_CUDA_EV(cudaStreamSynchronize(st));
 
     double ms_t = 0, ms_f = 0, ms_fin = 0;
@@ -635,27 +673,7 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     free_events();
 #undef ANM_CUDA_EV
 
-    // organ results: d_{o,b} = organ_batch[b][o] k / (n_b N_o); mean and batch sigma over b
-    c->organs.assign((size_t)c->n_organs, anm_organ{});
-    if (c->have_organs) {
-        for (int o = 1; o <= c->n_organs; ++o) {
-            anm_organ& r = c->organs[(size_t)o - 1];
-            r.n_voxels = cnt[o];
-            r.mass_g = mass[o];
-            r.n_voxels_nonzero = (uint64_t)(acc[o].n_nonzero + 0.5);
-            if (cnt[o] == 0) continue;
-            double s1 = 0, s2 = 0;
-            for (int b = 0; b < B; ++b) {
-                const double d = ob[(size_t)b * 256 + o] * kGyPerMeVPerGram / ((double)nb * (double)cnt[o]);
-                s1 += d; s2 += d * d;
-            }
-            const double mean = s1 / B;
-            r.mean_Gy_per_decay = mean;
-            r.sigma_mean = std::sqrt(std::max(0.0, (s2 / B - mean * mean) / (B - 1)));
-            r.rms_voxel_rel_sigma = acc[o].n_nonzero > 0 ? std::sqrt(acc[o].rel2 / acc[o].n_nonzero) : 0.0;
-            r.mass_weighted_Gy_per_decay = mass[o] > 0 ? acc[o].energy * kGyPerMeVPerGram / ((double)n_decays * mass[o]) : 0.0;
-        }
-    }
+    const double tot_e = c->stats.deposited_MeV;
     anm_stats& s = c->stats;
     std::memset(&s, 0, sizeof s);
     s.n_decays = n_decays;
@@ -703,6 +721,41 @@ int anm_get_organ_doses(anm_ctx* c, anm_organ* out, int n_organs) {
     if (!c->have_results || !c->have_organs) return fail(c, ANM_E_STATE, "organ doses: no completed run with organ labels");
     if (n_organs != c->n_organs) return fail(c, ANM_E_ARG, "organ doses: n_organs = %d but %d were loaded", n_organs, c->n_organs);
     std::memcpy(out, c->organs.data(), sizeof(anm_organ) * (size_t)n_organs);
+    return ANM_OK;
+}
+
+// ---- multi-GPU merge ----------------------------------------------------------------
+int anm_get_tally_buffers(anm_ctx* c, float** d_sum, float** d_sumsq, size_t* n_floats, double** d_organ_rows, int* n_rows) {
+    if (!c) return ANM_E_ARG;
+    if (!d_sum || !d_sumsq || !n_floats || !d_organ_rows || !n_rows) return fail(c, ANM_E_ARG, "tally buffers: null pointer");
+    if (!c->have_results) return fail(c, ANM_E_STATE, "tally buffers: no completed run");
+    *d_sum = c->sum.p; *d_sumsq = c->sumsq.p; *n_floats = c->Vpad;
+    *d_organ_rows = c->organ_batch.p; *n_rows = c->run_batches;
+    return ANM_OK;
+}
+
+int anm_merge(anm_ctx* c, uint64_t total_decays, int total_batches, const double* organ_rows_all, const anm_stats* summed) {
+    if (!c) return ANM_E_ARG;
+    if (!c->have_results) return fail(c, ANM_E_STATE, "merge: no completed run");
+    if (total_batches < c->run_batches || total_batches < 2 || total_decays == 0 || total_decays % (uint64_t)total_batches)
+        return fail(c, ANM_E_ARG, "merge: total_decays must be a positive multiple of total_batches >= this run's batches");
+    const uint64_t nb = c->run_decays / (uint64_t)c->run_batches;
+    if (total_decays / (uint64_t)total_batches != nb)
+        return fail(c, ANM_E_ARG, "merge: every shard must use the same decays per batch (%llu here)", (unsigned long long)nb);
+    if (c->have_organs && !organ_rows_all) return fail(c, ANM_E_ARG, "merge: organ rows of all batches are required");
+    ANM_CUDA(c, cudaSetDevice(c->device));
+    const anm_stats mine = c->stats;
+    const int rc = finalize_and_collect(c, total_batches, nb, total_decays, organ_rows_all);
+    if (rc != ANM_OK) { c->have_results = false; return rc; }
+    anm_stats& s = c->stats;
+    const double dep = s.deposited_MeV;
+    if (summed) s = *summed; else { s = mine; s.escaped_MeV = 0; s.n_steps = s.n_real = s.n_pe = s.n_compton = s.n_rayleigh = s.n_escaped = s.n_cutoff = 0; }
+    s.n_launches += 1;     // the finalize launch of the merge
+    s.n_decays = total_decays;
+    s.emitted_MeV = (double)total_decays * ((double)kE0 * c->opt.photons_per_decay + c->opt.positron_ke_MeV);
+    s.deposited_MeV = dep;
+    c->run_decays = total_decays;
+    c->run_batches = total_batches;
     return ANM_OK;
 }
 
