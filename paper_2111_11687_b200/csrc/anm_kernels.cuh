@@ -495,7 +495,8 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
     for (int k = 0; k < kSlots / 32; ++k) q[Q_S * kSlots + lane + 32 * k] = (unsigned char)(lane + 32 * k);   // all free
     __syncthreads();
 
-    unsigned hF = 0, nF = 0, hC = 0, nC = 0, hS = 0, nS = kSlots, hR = 0, nR = 0;   // ring heads and lengths, warp-uniform
+    // ring heads and lengths, one byte per event type (byte Q_F .. Q_R), warp-uniform; all slots start free (Q_S)
+    unsigned heads = 0u, cnts = (unsigned)kSlots << (8 * Q_S);
     unsigned pool_next = 0, pool_end = 0;   // warp-uniform
     bool exhausted = false;                 // warp-uniform
     const float t0 = (float)p.ie0 + p.fe0;  // ln-E grid coordinate of E0
@@ -507,20 +508,20 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
 
     // Push every processed slot onto the ring of its next event (all 32 lanes call it; idle lanes pass Q_NONE):
     // one match groups the lanes by destination, the rank inside the group is the ring offset, one packed warp
-    // reduction counts the four groups.
+    // reduction counts the four groups (head + length per byte stays below 128: no carry between the bytes).
     auto push_all = [&](const int next, const unsigned slot) {
         const unsigned same = __match_any_sync(0xffffffffu, next);
         const unsigned rank = __popc(same & lanemask_lt);
-        const unsigned tails = ((hF + nF) & 255u) | (((hC + nC) & 255u) << 8) | (((hS + nS) & 255u) << 16) | (((hR + nR) & 255u) << 24);
+        const unsigned sh = 8u * (unsigned)(next & 3);
         if (next != Q_NONE)
-            q[next * kSlots + ((((tails >> (8 * next)) & 255u) + rank) & (kSlots - 1))] = (unsigned char)slot;
-        const unsigned cnt = __reduce_add_sync(0xffffffffu, next != Q_NONE ? 1u << (8 * next) : 0u);
-        nF += cnt & 255u; nC += (cnt >> 8) & 255u; nS += (cnt >> 16) & 255u; nR += cnt >> 24;
+            q[next * kSlots + ((((heads + cnts) >> sh) + rank) & (kSlots - 1))] = (unsigned char)slot;
+        cnts += __reduce_add_sync(0xffffffffu, next != Q_NONE ? 1u << sh : 0u);
     };
 
     for (;;) {
         __syncwarp();
         // ---- pick the event type with the longest queue ------------------------------------------------
+        const unsigned nF = cnts & 255u, nC = (cnts >> 8) & 255u, nS = (cnts >> 16) & 255u, nR = cnts >> 24;
         int X = Q_F;
         unsigned best = nF;
         if (nC > best) { X = Q_C; best = nC; }
@@ -528,8 +529,6 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
         if (nR > best || nR >= (unsigned)kRayleighBatch) { X = Q_R; best = nR; }
         if (best == 0u) break;              // every slot is free and the launch has no history left
         unsigned n = min(best, 32u);
-        unsigned head;
-        if (X == Q_F) head = hF; else if (X == Q_C) head = hC; else if (X == Q_S) head = hS; else head = hR;
         unsigned hl_new = 0;
         if (X == Q_S) {                     // hand out history indices (warp-uniform bookkeeping)
             if (pool_next == pool_end) {
@@ -544,6 +543,10 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
             hl_new = pool_next + lane;
             pool_next += n;
         }
+        const unsigned shX = 8u * (unsigned)X;
+        const unsigned head = heads >> shX;
+        heads = (heads + (n << shX)) & (0x01010101u * (unsigned)(kSlots - 1));     // pop n slots
+        cnts -= n << shX;
         const unsigned slot = q[X * kSlots + ((head + lane) & (kSlots - 1))];
         const bool active = lane < n;
         float* S = slots + slot;
@@ -561,7 +564,6 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
         };
 
         if (X == Q_F) {
-            hF = (hF + n) & (kSlots - 1); nF -= n;
             if (active) {
                 const unsigned meta = SU[F_META * kSlots];
                 const unsigned ph = meta & 1u;
@@ -598,7 +600,6 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
             }
             push_all(next, slot);
         } else if (X == Q_C) {
-            hC = (hC + n) & (kSlots - 1); nC -= n;
             if (active) {
                 const unsigned meta = SU[F_META * kSlots];
                 const unsigned ph = meta & 1u;
@@ -633,7 +634,6 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
             }
             push_all(next, slot);
         } else if (X == Q_S) {
-            hS = (hS + n) & (kSlots - 1); nS -= n;
             if (active) {
                 const unsigned long long h = p.hist_base + hl_new;
                 float x, y, z, u, v, w;
@@ -649,11 +649,10 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                 SU[F_HL * kSlots] = hl_new;
                 SU[F_META * kSlots] = in_box ? (2u | 8u) : 0u;
                 if (p.positron_ke > 0.0f) atomicAdd(p.batch + voxel, p.positron_ke);
-                q[Q_F * kSlots + ((hF + nF + lane) & (kSlots - 1))] = (unsigned char)slot;
+                q[Q_F * kSlots + ((heads + cnts + lane) & (kSlots - 1))] = (unsigned char)slot;
             }
-            nF += n;
+            cnts += n;
         } else {   // Q_R
-            hR = (hR + n) & (kSlots - 1); nR -= n;
             if (active) {
                 const unsigned meta = SU[F_META * kSlots];
                 const unsigned ph = meta & 1u;
