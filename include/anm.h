@@ -144,6 +144,15 @@ int anm_get_uncertainty(anm_ctx* c, float* out_rel_sigma, size_t n, int on_devic
 int anm_get_organ_doses(anm_ctx* c, anm_organ* out, int n_organs);                  /* host array, out[k] = label k+1 */
 int anm_get_stats(anm_ctx* c, anm_stats* out);
 
+/* --- inspection ---------------------------------------------------------------------------------
+ * The decay-voxel sampler of the loaded activity map: n_entries buckets of four uint32
+ * {threshold, own voxel, alias voxel, 0}; a decay picks a bucket uniformly and takes `own` iff a 32-bit uniform is
+ * below `threshold`, else `alias`, so P(voxel v) = [sum over buckets owning v of threshold/2^32 + sum over buckets
+ * aliasing v of (1 - threshold/2^32)] / n_entries = activity[v] / sum(activity).  out == NULL only returns the
+ * count; otherwise out is a HOST array with room for capacity_entries * 4 uint32.  ANM_E_STATE without an
+ * activity map (point-source mode has no table). */
+int anm_get_alias_table(anm_ctx* c, uint32_t* out, size_t capacity_entries, size_t* n_entries);
+
 /* --- one logical run over several GPUs ---------------------------------------
  * Histories are independent and keyed by index (Philox counter = history index), so a run of N decays in B batches
  * shards by whole batches: rank r sets anm_options.history_offset = (first batch of r) * N/B and n_batches = its own

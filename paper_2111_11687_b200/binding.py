@@ -19,7 +19,7 @@ ANM_SYMBOLS = [
     "anm_create", "anm_destroy", "anm_last_error", "anm_set_stream", "anm_set_grid", "anm_load_phantom",
     "anm_load_activity", "anm_set_point_source", "anm_load_organs", "anm_set_physics_tables", "anm_set_options",
     "anm_default_options", "anm_run", "anm_get_energy", "anm_get_dose", "anm_get_dose_rate", "anm_get_uncertainty",
-    "anm_get_organ_doses", "anm_get_stats", "anm_get_tally_buffers", "anm_merge",
+    "anm_get_organ_doses", "anm_get_stats", "anm_get_tally_buffers", "anm_merge", "anm_get_alias_table",
 ]
 
 STATUS = {0: "ANM_OK", -1: "ANM_E_ARG", -2: "ANM_E_STATE", -3: "ANM_E_CUDA", -4: "ANM_E_NOMEM", -5: "ANM_E_UNSUPPORTED"}
@@ -94,6 +94,7 @@ def load(build_if_missing: bool = True):
         "anm_get_organ_doses": (i32, [vp, C.POINTER(anm_organ), i32]), "anm_get_stats": (i32, [vp, C.POINTER(anm_stats)]),
         "anm_get_tally_buffers": (i32, [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(sz), C.POINTER(vp), C.POINTER(i32)]),
         "anm_merge": (i32, [vp, u64, i32, vp, C.POINTER(anm_stats)]),
+        "anm_get_alias_table": (i32, [vp, vp, sz, C.POINTER(sz)]),
     }
     for name, (res, args) in protos.items():
         f = getattr(L, name)
@@ -264,6 +265,14 @@ class Simulation:
         s = anm_stats()
         self._ck(self._L.anm_get_stats(self._ctx, C.byref(s)))
         return s.as_dict()
+
+    def get_alias_table(self) -> np.ndarray:
+        """uint32 [n_entries][4] = {threshold, own voxel, alias voxel, 0} of the loaded activity map."""
+        n = C.c_size_t()
+        self._ck(self._L.anm_get_alias_table(self._ctx, None, 0, C.byref(n)))
+        out = np.empty((n.value, 4), np.uint32)
+        self._ck(self._L.anm_get_alias_table(self._ctx, out.ctypes.data, n.value, C.byref(n)))
+        return out
 
     # ---- one logical run over several GPUs (include/anm.h, "one logical run over several GPUs")
     def get_tally_buffers(self):

@@ -11,6 +11,12 @@
 
 #include "../../include/anm.h"
 #include "anm_kernels.cuh"
+#include "anm_alias.cuh"
+
+#include <cub/device/device_scan.cuh>
+#include <cub/device/device_select.cuh>
+#include <thrust/iterator/counting_iterator.h>
+#include <thrust/iterator/transform_iterator.h>
 
 using namespace anm;
 
@@ -125,45 +131,87 @@ int grid_blocks(const anm_ctx* c, size_t items, int per_block) {
     return (int)std::max<size_t>(1, std::min(want, cap));
 }
 
-// Vose's alias method over the active voxels (host, fp64).  entry = {threshold (P(own) * 2^32), own voxel, alias voxel, 0}
-int build_alias(anm_ctx* c, const float* act) {
+// Alias table over the active voxels, built on the device (anm_alias.cuh): statistics pass, stable selection of the
+// light / heavy voxel indices and prefix sums of their weights (CUB device primitives), one thread per bucket.
+// d_act: activity[V] on the device.
+int build_alias(anm_ctx* c, const float* d_act) {
     const size_t V = c->V;
+    cudaStream_t st = c->stream;
+    const int blocks = grid_blocks(c, V, kAliasThreads);
+    DevBuf<double> bsum, L, H;
+    DevBuf<unsigned long long> bcnt;
+    DevBuf<uint32_t> lidx, hidx;
+    DevBuf<unsigned char> temp;
+    DevBuf<unsigned> nsel;
+    struct Cleanup { DevBuf<double>&a, &b, &d; DevBuf<unsigned long long>& e; DevBuf<uint32_t>&f, &g; DevBuf<unsigned char>& h; DevBuf<unsigned>& i;
+                     ~Cleanup() { a.release(); b.release(); d.release(); e.release(); f.release(); g.release(); h.release(); i.release(); } }
+        cleanup{bsum, L, H, bcnt, lidx, hidx, temp, nsel};
+    ANM_CUDA(c, bsum.alloc((size_t)blocks));
+    ANM_CUDA(c, bcnt.alloc((size_t)blocks));
+    ANM_CUDA(c, nsel.alloc(2));
+    ANM_CUDA(c, cudaMemsetAsync(c->d_flags.p, 0, 4, st));
+    activity_stats_kernel<<<blocks, kAliasThreads, 0, st>>>(d_act, V, bsum.p, bcnt.p, c->d_flags.p);
+    ANM_CUDA(c, cudaGetLastError());
+    std::vector<double> hs((size_t)blocks);
+    std::vector<unsigned long long> hc((size_t)blocks);
+    unsigned flags = 0;
+    ANM_CUDA(c, cudaMemcpyAsync(hs.data(), bsum.p, (size_t)blocks * 8, cudaMemcpyDeviceToHost, st));
+    ANM_CUDA(c, cudaMemcpyAsync(hc.data(), bcnt.p, (size_t)blocks * 8, cudaMemcpyDeviceToHost, st));
+    ANM_CUDA(c, cudaMemcpyAsync(&flags, c->d_flags.p, 4, cudaMemcpyDeviceToHost, st));
+    ANM_CUDA(c, cudaStreamSynchronize(st));
+    if (flags & 1u) return fail(c, ANM_E_ARG, "activity holds a negative or non-finite value");
     double total = 0.0;
-    size_t M = 0;
-    for (size_t i = 0; i < V; ++i) {
-        const float a = act[i];
-        if (!(a >= 0.0f) || !std::isfinite(a)) return fail(c, ANM_E_ARG, "activity[%zu] is negative or not finite", i);
-        if (a > 0.0f) { total += (double)a; ++M; }
-    }
+    unsigned long long M = 0;
+    for (int b = 0; b < blocks; ++b) { total += hs[(size_t)b]; M += hc[(size_t)b]; }
     if (M == 0) return fail(c, ANM_E_ARG, "activity is zero everywhere");
     if (M > 0xfffffff0ull) return fail(c, ANM_E_ARG, "too many active voxels");
-    std::vector<uint4> tab(M);
-    std::vector<double> q(M);
-    std::vector<uint32_t> small, large;
-    small.reserve(M); large.reserve(M);
-    size_t j = 0;
     const double scale = (double)M / total;
-    for (size_t i = 0; i < V; ++i) {
-        if (act[i] > 0.0f) {
-            q[j] = (double)act[i] * scale;
-            tab[j] = make_uint4(0xffffffffu, (uint32_t)i, (uint32_t)i, 0u);
-            (q[j] < 1.0 ? small : large).push_back((uint32_t)j);
-            ++j;
-        }
+
+    // stable selection of the light (w <= 1) and heavy (w > 1) voxel indices
+    ANM_CUDA(c, lidx.alloc((size_t)M));
+    ANM_CUDA(c, hidx.alloc((size_t)M));
+    thrust::counting_iterator<uint32_t> vox(0u);
+    const AliasIsLight is_light{d_act, scale};
+    const AliasIsHeavy is_heavy{d_act, scale};
+    size_t tb1 = 0, tb2 = 0, tb3 = 0;
+    const long long nV = (long long)V;
+    ANM_CUDA(c, cub::DeviceSelect::If(nullptr, tb1, vox, lidx.p, nsel.p, nV, is_light, st));
+    ANM_CUDA(c, cub::DeviceSelect::If(nullptr, tb2, vox, hidx.p, nsel.p + 1, nV, is_heavy, st));
+    {   // scan scratch size: bounded by the larger of the two item counts (<= M)
+        auto w = thrust::make_transform_iterator(thrust::counting_iterator<uint32_t>(0u), AliasWeight{d_act, lidx.p, scale});
+        ANM_CUDA(c, cub::DeviceScan::InclusiveSum(nullptr, tb3, w, (double*)nullptr, (long long)M, st));
     }
-    while (!small.empty() && !large.empty()) {
-        const uint32_t s = small.back(); small.pop_back();
-        const uint32_t l = large.back();
-        const double t = std::floor(q[s] * 4294967296.0);
-        tab[s].x = (uint32_t)std::min(t, 4294967295.0);
-        tab[s].z = tab[l].y;
-        q[l] -= 1.0 - q[s];
-        if (q[l] < 1.0) { large.pop_back(); small.push_back(l); }
+    ANM_CUDA(c, temp.alloc(std::max(tb1, std::max(tb2, tb3))));
+    size_t tb = temp.n;
+    ANM_CUDA(c, cub::DeviceSelect::If(temp.p, tb, vox, lidx.p, nsel.p, nV, is_light, st));
+    tb = temp.n;
+    ANM_CUDA(c, cub::DeviceSelect::If(temp.p, tb, vox, hidx.p, nsel.p + 1, nV, is_heavy, st));
+    unsigned n_lh[2] = {0, 0};
+    ANM_CUDA(c, cudaMemcpyAsync(n_lh, nsel.p, 8, cudaMemcpyDeviceToHost, st));
+    ANM_CUDA(c, cudaStreamSynchronize(st));
+    const unsigned nl = n_lh[0], nh = n_lh[1];
+    if ((unsigned long long)nl + nh != M) return fail(c, ANM_E_CUDA, "alias: selection counted %u + %u voxels, expected %llu", nl, nh, M);
+
+    // exclusive prefix sums with the total in the last element: L[0..nl], H[0..nh]
+    ANM_CUDA(c, L.alloc((size_t)nl + 1));
+    ANM_CUDA(c, H.alloc((size_t)nh + 1));
+    ANM_CUDA(c, cudaMemsetAsync(L.p, 0, 8, st));
+    ANM_CUDA(c, cudaMemsetAsync(H.p, 0, 8, st));
+    if (nl) {
+        auto w = thrust::make_transform_iterator(thrust::counting_iterator<uint32_t>(0u), AliasWeight{d_act, lidx.p, scale});
+        tb = temp.n;
+        ANM_CUDA(c, cub::DeviceScan::InclusiveSum(temp.p, tb, w, L.p + 1, (long long)nl, st));
     }
-    // leftovers have q == 1 up to rounding: keep threshold = 2^32 - 1, alias = own
-    ANM_CUDA(c, c->alias.alloc(M));
-    ANM_CUDA(c, cudaMemcpyAsync(c->alias.p, tab.data(), M * sizeof(uint4), cudaMemcpyHostToDevice, c->stream));
-    ANM_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (nh) {
+        auto w = thrust::make_transform_iterator(thrust::counting_iterator<uint32_t>(0u), AliasWeight{d_act, hidx.p, scale});
+        tb = temp.n;
+        ANM_CUDA(c, cub::DeviceScan::InclusiveSum(temp.p, tb, w, H.p + 1, (long long)nh, st));
+    }
+    ANM_CUDA(c, c->alias.alloc((size_t)M));
+    alias_build_kernel<<<(unsigned)((M + kAliasThreads - 1) / kAliasThreads), kAliasThreads, 0, st>>>(
+        d_act, scale, lidx.p, hidx.p, L.p, H.p, nl, nh, c->alias.p);
+    ANM_CUDA(c, cudaGetLastError());
+    ANM_CUDA(c, cudaStreamSynchronize(st));
     c->n_alias = (unsigned)M;
     return ANM_OK;
 }
@@ -442,21 +490,30 @@ int anm_load_activity(anm_ctx* c, const float* activity, int on_device) {
     if (!activity) return fail(c, ANM_E_ARG, "activity: null pointer");
     if (!c->have_grid) return fail(c, ANM_E_STATE, "activity: set the grid first");
     ANM_CUDA(c, cudaSetDevice(c->device));
-    std::vector<float> host;
-    const float* a = activity;
-    try {
-        if (on_device) {
-            host.resize(c->V);
-            ANM_CUDA(c, cudaMemcpyAsync(host.data(), activity, c->V * 4, cudaMemcpyDeviceToHost, c->stream));
-            ANM_CUDA(c, cudaStreamSynchronize(c->stream));
-            a = host.data();
-        }
-        c->have_source = false;
-        const int rc = build_alias(c, a);
-        if (rc != ANM_OK) return rc;
-    } catch (const std::bad_alloc&) {
-        return fail(c, ANM_E_NOMEM, "activity: host allocation failed");
+    const float* d_act = activity;
+    if (!on_device) {
+        ANM_CUDA(c, c->scratch.alloc(c->Vpad));
+        ANM_CUDA(c, cudaMemcpyAsync(c->scratch.p, activity, c->V * 4, cudaMemcpyHostToDevice, c->stream));
+        d_act = c->scratch.p;
     }
+    c->have_source = false;
+    cudaEvent_t e0, e1;
+    ANM_CUDA(c, cudaEventCreate(&e0));
+    ANM_CUDA(c, cudaEventCreate(&e1));
+    cudaEventRecord(e0, c->stream);
+    int rc;
+    try {
+        rc = build_alias(c, d_act);
+    } catch (const std::bad_alloc&) {
+        rc = fail(c, ANM_E_NOMEM, "activity: host allocation failed");
+    }
+    cudaEventRecord(e1, c->stream);
+    cudaEventSynchronize(e1);
+    float ms = 0;
+    cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    c->ms_setup += ms;
+    if (rc != ANM_OK) return rc;
     c->point_source = false;
     c->have_source = true;
     c->have_results = false;
@@ -721,6 +778,19 @@ int anm_get_organ_doses(anm_ctx* c, anm_organ* out, int n_organs) {
     if (!c->have_results || !c->have_organs) return fail(c, ANM_E_STATE, "organ doses: no completed run with organ labels");
     if (n_organs != c->n_organs) return fail(c, ANM_E_ARG, "organ doses: n_organs = %d but %d were loaded", n_organs, c->n_organs);
     std::memcpy(out, c->organs.data(), sizeof(anm_organ) * (size_t)n_organs);
+    return ANM_OK;
+}
+
+int anm_get_alias_table(anm_ctx* c, uint32_t* out, size_t capacity_entries, size_t* n_entries) {
+    if (!c) return ANM_E_ARG;
+    if (!n_entries) return fail(c, ANM_E_ARG, "alias table: null pointer");
+    if (!c->have_source || c->point_source) return fail(c, ANM_E_STATE, "alias table: no activity map is loaded");
+    *n_entries = c->n_alias;
+    if (!out) return ANM_OK;
+    if (capacity_entries < c->n_alias) return fail(c, ANM_E_ARG, "alias table: %zu entries needed, room for %zu", (size_t)c->n_alias, capacity_entries);
+    ANM_CUDA(c, cudaSetDevice(c->device));
+    ANM_CUDA(c, cudaMemcpyAsync(out, c->alias.p, (size_t)c->n_alias * sizeof(uint4), cudaMemcpyDeviceToHost, c->stream));
+    ANM_CUDA(c, cudaStreamSynchronize(c->stream));
     return ANM_OK;
 }
 

@@ -402,3 +402,48 @@ def test_error_codes(anm, tables):
         assert sim.get_energy().sum() > 0
         with pytest.raises(ValueError):
             sim.get_energy(np.empty(7, np.float32))
+
+
+# ------------------------------------------------------------------------------------------------- A0: alias table
+@pytest.mark.parametrize("case", ["cfg3", "uniform", "spiky", "single", "two"])
+def test_alias_table_reproduces_the_activity_pdf(anm, case):
+    """The device-built alias table is exact: every active voxel owns one bucket and the probabilities reconstructed
+    from the buckets equal activity / sum(activity) to fp64 rounding + the 2^-32 threshold grid."""
+    rng = np.random.default_rng(5)
+    if case == "cfg3":
+        cfg = anm_inputs.make_config(3, 4)
+        shape, act = cfg["shape"], cfg["activity"].reshape(-1).astype(np.float32)
+    else:
+        shape = (37, 29, 23)                                         # V = 24679, not a multiple of anything useful
+        V = int(np.prod(shape))
+        act = np.zeros(V, np.float32)
+        if case == "uniform":
+            act[rng.random(V) < 0.4] = 3.0                           # all weights equal the mean: no heavy item
+        elif case == "spiky":
+            act[:] = rng.lognormal(0.0, 2.0, V).astype(np.float32)
+            act[rng.random(V) < 0.3] = 0.0
+            act[rng.integers(0, V, 5)] = 1e6
+        elif case == "single":
+            act[12345] = 2.5
+        else:
+            act[7], act[V - 1] = 1.0, 1e-9
+    V = act.size
+    with anm.Simulation(0) as sim:
+        sim.set_grid(shape, (2.0, 2.0, 2.0))
+        sim.load_activity(act)
+        tab = sim.get_alias_table()
+    active = np.flatnonzero(act > 0)
+    assert tab.shape == (active.size, 4)
+    assert np.array_equal(np.sort(tab[:, 1]), active)                # one bucket per active voxel
+    assert np.all(act[tab[:, 2]] > 0) and np.all(tab[:, 3] == 0)
+    p_own = tab[:, 0].astype(np.float64) / 2.0 ** 32
+    p = np.zeros(V)
+    np.add.at(p, tab[:, 1], p_own)
+    np.add.at(p, tab[:, 2], 1.0 - p_own)
+    p /= active.size
+    want = act.astype(np.float64) / act.astype(np.float64).sum()
+    # every bucket that owns or aliases v contributes one floor() on the table's 2^-32 threshold grid
+    touch = np.bincount(tab[:, 1], minlength=V) + np.bincount(tab[:, 2], minlength=V)
+    tol = (touch + 1.0) / 2.0 ** 32 / active.size + 1e-13 * want.max()
+    assert np.all(np.abs(p - want) < tol), float(np.max(np.abs(p - want) / tol))
+    assert abs(p.sum() - 1.0) < 1e-9
