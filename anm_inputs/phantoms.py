@@ -211,6 +211,18 @@ def _base(name, shape_xyz, spacing_mm, n_decays, seed, n_batches, photons_per_de
     }
 
 
+def make_patient_on_grid(shape_xyz, spacing_mm, n_decays: int = 1_000_000_000) -> dict:
+    """The cfg3 analytic patient sampled on an arbitrary grid (body axis stretched to the grid's height), e.g. the
+    paper's PET grid 168 x 168 x 219 at 4.063 x 4.063 x 5 mm."""
+    nx, ny, nz = (int(v) for v in shape_xyz)
+    sp = tuple(float(v) for v in spacing_mm)
+    c = _base("patient_%dx%dx%d" % (nx, ny, nz), (nx, ny, nz), sp, n_decays, 42, 100, 2, positron_ke=0.2498)
+    mat, rho, lab, act = _patient_volume(nx, ny, nz, *sp, z_stretch=(nz * sp[2]) / _BODY_Z)
+    c.update(material=mat, density=rho, activity=act, labels=lab, n_organs=27, organ_names=list(ORGAN_NAMES))
+    c["scale"] = 1
+    return c
+
+
 def make_config(k: int, scale: int = 1) -> dict:
     """Build config k (0..4) of BASELINE.json; `scale` coarsens the grid (tests)."""
     s = int(scale)

@@ -107,7 +107,27 @@ typedef struct {
     uint64_t n_decays, n_steps, n_real, n_pe, n_compton, n_rayleigh, n_escaped, n_cutoff;
     double ms_transport, ms_fold, ms_finalize, ms_setup;   /* device time of the last anm_run / last setup */
     uint64_t n_launches;                                   /* kernels launched by the last anm_run         */
+    double ms_load_ct, ms_load_pet;                        /* device time of the last anm_load_ct / anm_load_pet
+                                                              resample kernels (also counted in ms_setup)   */
 } anm_stats;
+
+/* HU -> (material, density) conversion curve ("Hounsfield unit (HU)-to-density conversion curve";
+ * four materials "each having a density specified by the HU").  A continuous piecewise-linear density over
+ * n_nodes HU nodes, one material per HU interval:
+ *   density(h)  = linear interpolation of (hu[k], rho[k]); rho[0] below hu[0], rho[n_nodes-1] above the last node
+ *   material(h) = material[k] for hu[k] <= h < hu[k+1]; material[0] below hu[0]; material[n_nodes-2] at and above
+ *                 the last node (material[n_nodes-1] is ignored)
+ * hu must increase strictly, rho in [0, 16) g/cm^3, material < ANM_MAX_MATERIALS.  hu_outside is the HU assumed
+ * where the simulation grid reaches beyond the CT image (air). */
+#define ANM_MAX_RAMP_NODES 16
+typedef struct {
+    int32_t n_nodes;          /* 2..ANM_MAX_RAMP_NODES */
+    int32_t reserved0;
+    double hu[ANM_MAX_RAMP_NODES];
+    double rho[ANM_MAX_RAMP_NODES];
+    int32_t material[ANM_MAX_RAMP_NODES];
+    double hu_outside;
+} anm_hu_ramp;
 
 /* --- lifetime ---------------------------------------------------------------------------------- */
 int anm_create(anm_ctx** out, int cuda_device);    /* ANM_E_CUDA if the device cannot be used          */
@@ -119,6 +139,30 @@ int anm_set_stream(anm_ctx* c, void* cuda_stream); /* cudaStream_t; NULL = the d
 int anm_set_grid(anm_ctx* c, int nx, int ny, int nz, double dx_mm, double dy_mm, double dz_mm);
 /* material[V] < n_materials (checked at run), density[V] in [0, 16) g/cm^3, stored on a 2^-20 grid. */
 int anm_load_phantom(anm_ctx* c, const uint8_t* material, const float* density_g_cm3, int on_device);
+/* --- image front end: the scanner's images instead of ready-made volumes ---------------
+ * anm_load_ct replaces anm_load_phantom: a CT image of int16 HU on ITS OWN grid (cnx*cny*cnz voxels of
+ * cdx x cdy x cdz mm, x fastest, its corner at (ox, oy, oz) mm in the simulation grid's frame) is resampled to the
+ * simulation grid ("The CT images are resampled to obtain the same size as the PET images") -- the
+ * value of a simulation voxel is the volume-weighted MEAN of the piecewise-constant HU image over that voxel, with
+ * ramp->hu_outside wherever the voxel reaches beyond the image -- and converted to (material, density) by `ramp`
+ * (NULL = anm_default_hu_ramp), densities rounded to the 2^-20 g/cm^3 texel grid.  One fused kernel; fp64 weights
+ * and accumulation.  ANM_E_ARG for a bad ramp or sizes; ANM_E_STATE before anm_set_grid.
+ * anm_get_phantom returns the (material, density) volumes the ctx holds (after anm_load_ct or anm_load_phantom). */
+int anm_default_hu_ramp(anm_hu_ramp* r);   /* air / lung / water / compact bone; numbers approximate */
+int anm_load_ct(anm_ctx* c, const int16_t* hu, int cnx, int cny, int cnz, double cdx_mm, double cdy_mm, double cdz_mm,
+                double ox_mm, double oy_mm, double oz_mm, const anm_hu_ramp* ramp, int on_device);
+int anm_get_phantom(anm_ctx* c, uint8_t* material, float* density_g_cm3, size_t n, int on_device);
+/* anm_load_pet replaces anm_load_activity: a PET image of float32 Bq/mL on its own grid (same conventions; 0 outside
+ * the image) is resampled by the same volume-weighted mean and converted linearly ("linear conversion
+ * of the PET value"): activity of a simulation voxel [Bq] = mean concentration x voxel volume [mL].  The decay pdf is
+ * built from it as in anm_load_activity.  *total_activity_Bq (may be NULL) receives the sum = the whole-body activity
+ * A(t_s) of Eq. 1 for anm_get_dose_rate; out_activity_Bq (may be NULL; n = nx*ny*nz floats, host
+ * or device like the input) receives the activity volume.  ANM_E_ARG for negative / non-finite values or an image
+ * that leaves the grid without activity. */
+int anm_load_pet(anm_ctx* c, const float* bq_per_ml, int pnx, int pny, int pnz, double pdx_mm, double pdy_mm, double pdz_mm,
+                 double ox_mm, double oy_mm, double oz_mm, int on_device, double* total_activity_Bq,
+                 float* out_activity_Bq, size_t n);
+
 /* activity[V] >= 0, finite, arbitrary units, not all zero: decay pdf = activity / sum;
  * the decay point is uniform inside the chosen voxel. */
 int anm_load_activity(anm_ctx* c, const float* activity, int on_device);
@@ -142,7 +186,7 @@ int anm_get_dose(anm_ctx* c, float* out_Gy_per_decay, size_t n, int on_device);
 int anm_get_dose_rate(anm_ctx* c, double total_activity_Bq, float* out_Gy_per_s, size_t n, int on_device); /* Eq. 1 */
 int anm_get_uncertainty(anm_ctx* c, float* out_rel_sigma, size_t n, int on_device); /* batch sigma of the mean / mean; 0 where the mean is 0 */
 int anm_get_organ_doses(anm_ctx* c, anm_organ* out, int n_organs);                  /* host array, out[k] = label k+1 */
-int anm_get_stats(anm_ctx* c, anm_stats* out);
+int anm_get_stats(anm_ctx* c, anm_stats* out);    /* before a completed run: zeros except the ms_setup / ms_load_* timings */
 
 /* --- inspection ---------------------------------------------------------------------------------
  * The decay-voxel sampler of the loaded activity map: n_entries buckets of four uint32

@@ -20,6 +20,7 @@ ANM_SYMBOLS = [
     "anm_load_activity", "anm_set_point_source", "anm_load_organs", "anm_set_physics_tables", "anm_set_options",
     "anm_default_options", "anm_run", "anm_get_energy", "anm_get_dose", "anm_get_dose_rate", "anm_get_uncertainty",
     "anm_get_organ_doses", "anm_get_stats", "anm_get_tally_buffers", "anm_merge", "anm_get_alias_table",
+    "anm_default_hu_ramp", "anm_load_ct", "anm_get_phantom", "anm_load_pet",
 ]
 
 STATUS = {0: "ANM_OK", -1: "ANM_E_ARG", -2: "ANM_E_STATE", -3: "ANM_E_CUDA", -4: "ANM_E_NOMEM", -5: "ANM_E_UNSUPPORTED"}
@@ -54,10 +55,38 @@ class anm_stats(C.Structure):
     _fields_ = [("emitted_MeV", C.c_double), ("deposited_MeV", C.c_double), ("escaped_MeV", C.c_double)] + [
         (n, C.c_uint64) for n in ("n_decays", "n_steps", "n_real", "n_pe", "n_compton", "n_rayleigh", "n_escaped", "n_cutoff")] + [
         ("ms_transport", C.c_double), ("ms_fold", C.c_double), ("ms_finalize", C.c_double), ("ms_setup", C.c_double),
-        ("n_launches", C.c_uint64)]
+        ("n_launches", C.c_uint64), ("ms_load_ct", C.c_double), ("ms_load_pet", C.c_double)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
+
+
+ANM_MAX_RAMP_NODES = 16
+
+
+class anm_hu_ramp(C.Structure):
+    _fields_ = [("n_nodes", C.c_int32), ("reserved0", C.c_int32), ("hu", C.c_double * ANM_MAX_RAMP_NODES),
+                ("rho", C.c_double * ANM_MAX_RAMP_NODES), ("material", C.c_int32 * ANM_MAX_RAMP_NODES),
+                ("hu_outside", C.c_double)]
+
+    @classmethod
+    def from_dict(cls, ramp: dict) -> "anm_hu_ramp":
+        r = cls()
+        n = len(ramp["hu"])
+        if n > ANM_MAX_RAMP_NODES or len(ramp["rho"]) != n or len(ramp["material"]) != n - 1:
+            raise ValueError("ramp: need n HU nodes, n densities and n - 1 materials, n <= %d" % ANM_MAX_RAMP_NODES)
+        r.n_nodes = n
+        for k in range(n):
+            r.hu[k], r.rho[k] = float(ramp["hu"][k]), float(ramp["rho"][k])
+        for k in range(n - 1):
+            r.material[k] = int(ramp["material"][k])
+        r.hu_outside = float(ramp["hu_outside"])
+        return r
+
+    def as_dict(self) -> dict:
+        n = self.n_nodes
+        return {"hu": [self.hu[k] for k in range(n)], "rho": [self.rho[k] for k in range(n)],
+                "material": [self.material[k] for k in range(n - 1)], "hu_outside": self.hu_outside}
 
 
 def lib_path() -> str:
@@ -95,6 +124,10 @@ def load(build_if_missing: bool = True):
         "anm_get_tally_buffers": (i32, [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(sz), C.POINTER(vp), C.POINTER(i32)]),
         "anm_merge": (i32, [vp, u64, i32, vp, C.POINTER(anm_stats)]),
         "anm_get_alias_table": (i32, [vp, vp, sz, C.POINTER(sz)]),
+        "anm_default_hu_ramp": (i32, [C.POINTER(anm_hu_ramp)]),
+        "anm_load_ct": (i32, [vp, vp, i32, i32, i32, dbl, dbl, dbl, dbl, dbl, dbl, C.POINTER(anm_hu_ramp), i32]),
+        "anm_get_phantom": (i32, [vp, vp, vp, sz, i32]),
+        "anm_load_pet": (i32, [vp, vp, i32, i32, i32, dbl, dbl, dbl, dbl, dbl, dbl, i32, C.POINTER(dbl), vp, sz]),
     }
     for name, (res, args) in protos.items():
         f = getattr(L, name)
@@ -111,7 +144,7 @@ def _in_ptr(a, dtype, n, keep):
     """(pointer, on_device) of an input volume: numpy -> host pointer; CUDA torch tensor -> device pointer."""
     if _is_torch(a):
         import torch
-        want = {np.uint8: torch.uint8, np.float32: torch.float32}[dtype]
+        want = {np.uint8: torch.uint8, np.float32: torch.float32, np.int16: torch.int16}[dtype]
         if a.dtype != want or not a.is_contiguous() or a.numel() != n:
             raise ValueError("tensor must be contiguous %s with %d elements" % (want, n))
         keep.append(a)
@@ -180,6 +213,50 @@ class Simulation:
         keep = []
         p, d = _in_ptr(activity, np.float32, self.V, keep)
         self._ck(self._L.anm_load_activity(self._ctx, p, d))
+
+    def load_ct(self, hu, shape, spacing_mm, offset_mm=(0.0, 0.0, 0.0), ramp: dict | None = None):
+        """CT image of int16 HU on its own grid (shape = (cnx, cny, cnz), [iz][iy][ix]) -> the phantom (anm_load_ct)."""
+        cn = tuple(int(v) for v in shape)
+        keep = []
+        p, d = _in_ptr(hu, np.int16, cn[0] * cn[1] * cn[2], keep)
+        r = anm_hu_ramp.from_dict(ramp) if ramp is not None else None
+        self._ck(self._L.anm_load_ct(self._ctx, p, *cn, *(float(v) for v in spacing_mm), *(float(v) for v in offset_mm),
+                                     C.byref(r) if r is not None else None, d))
+
+    def load_pet(self, bq_per_ml, shape, spacing_mm, offset_mm=(0.0, 0.0, 0.0), out_activity=None) -> float:
+        """PET image of float32 Bq/mL on its own grid -> the decay pdf (anm_load_pet).  Returns A(t_s) in Bq;
+        out_activity (numpy float32 [V] for host input, CUDA tensor for device input) receives Bq per voxel."""
+        pn = tuple(int(v) for v in shape)
+        keep = []
+        p, d = _in_ptr(bq_per_ml, np.float32, pn[0] * pn[1] * pn[2], keep)
+        total = C.c_double(0.0)
+        po, n = None, 0
+        if out_activity is not None:
+            if _is_torch(out_activity):
+                po, d_out = _in_ptr(out_activity, np.float32, self.V, keep)
+            else:
+                if not (isinstance(out_activity, np.ndarray) and out_activity.dtype == np.float32 and
+                        out_activity.flags.c_contiguous and out_activity.size == self.V):
+                    raise ValueError("out_activity must be a C-contiguous float32 array with one element per voxel")
+                po, d_out = out_activity.ctypes.data, 0
+            if d_out != d:
+                raise ValueError("out_activity must live in the same memory space as the image")
+            n = self.V
+        self._ck(self._L.anm_load_pet(self._ctx, p, *pn, *(float(v) for v in spacing_mm), *(float(v) for v in offset_mm),
+                                      d, C.byref(total), po, n))
+        return float(total.value)
+
+    def get_phantom(self):
+        """(material uint8 [nz][ny][nx], density float32) the ctx holds, on the host."""
+        nx, ny, nz = self.shape
+        m, r = np.empty(self.V, np.uint8), np.empty(self.V, np.float32)
+        self._ck(self._L.anm_get_phantom(self._ctx, m.ctypes.data, r.ctypes.data, self.V, 0))
+        return m.reshape(nz, ny, nx), r.reshape(nz, ny, nx)
+
+    def default_hu_ramp(self) -> dict:
+        r = anm_hu_ramp()
+        self._ck(self._L.anm_default_hu_ramp(C.byref(r)))
+        return r.as_dict()
 
     def set_point_source(self, xyz_mm):
         self._ck(self._L.anm_set_point_source(self._ctx, *(float(v) for v in xyz_mm)))

@@ -12,6 +12,7 @@
 #include "../../include/anm.h"
 #include "anm_kernels.cuh"
 #include "anm_alias.cuh"
+#include "anm_frontend.cuh"
 
 #include <cub/device/device_scan.cuh>
 #include <cub/device/device_select.cuh>
@@ -96,7 +97,7 @@ struct anm_ctx {
     int run_batches = 0;
     std::vector<anm_organ> organs;
     anm_stats stats;
-    double ms_setup = 0;
+    double ms_setup = 0, ms_load_ct = 0, ms_load_pet = 0;
 
     anm_ctx() { std::memset(&stats, 0, sizeof stats); anm_default_options(&opt); }
 };
@@ -406,6 +407,8 @@ int anm_set_grid(anm_ctx* c, int nx, int ny, int nz, double dx_mm, double dy_mm,
     return ANM_OK;
 }
 
+static int phantom_setup(anm_ctx* c);
+
 int anm_load_phantom(anm_ctx* c, const uint8_t* material, const float* density, int on_device) {
     if (!c) return ANM_E_ARG;
     if (!material || !density) return fail(c, ANM_E_ARG, "phantom: null pointer");
@@ -442,6 +445,12 @@ int anm_load_phantom(anm_ctx* c, const uint8_t* material, const float* density, 
     if (flags[0] & 1u) return fail(c, ANM_E_ARG, "phantom: density must be finite and in [0, 16) g/cm^3");
     if (flags[1] >= ANM_MAX_MATERIALS) return fail(c, ANM_E_ARG, "phantom: material id %u >= %d", flags[1], ANM_MAX_MATERIALS);
     c->max_material = flags[1];
+    return phantom_setup(c);
+}
+
+// after the texels are written and c->max_material is set: per-material maximum density, hull box (shared by
+// anm_load_phantom and anm_load_ct)
+static int phantom_setup(anm_ctx* c) {
     // per-material maximum density (texel counts): a second tiny pass on the host copy of the texels would cost a
     // D2H of the volume; instead reduce on the device with one atomicMax per (block, material)
     {
@@ -514,6 +523,184 @@ int anm_load_activity(anm_ctx* c, const float* activity, int on_device) {
     cudaEventDestroy(e0); cudaEventDestroy(e1);
     c->ms_setup += ms;
     if (rc != ANM_OK) return rc;
+    c->point_source = false;
+    c->have_source = true;
+    c->have_results = false;
+    return ANM_OK;
+}
+
+
+// ---- image front end (anm_frontend.cuh) -----------------------------------------------
+
+int anm_default_hu_ramp(anm_hu_ramp* r) {
+    if (!r) return ANM_E_ARG;
+    std::memset(r, 0, sizeof *r);
+    // air / lung / soft tissue as water / compact bone; node values of the usual four-segment CT
+    // ramp, restated from memory and therefore approximate (reading C27)
+    const double hu[5] = {-1024.0, -974.0, -724.0, 101.0, 1976.0};
+    const double rho[5] = {0.001, 0.044, 0.302, 1.101, 2.088};
+    const int mat[4] = {0, 1, 2, 3};
+    r->n_nodes = 5;
+    for (int k = 0; k < 5; ++k) { r->hu[k] = hu[k]; r->rho[k] = rho[k]; }
+    for (int k = 0; k < 4; ++k) r->material[k] = mat[k];
+    r->hu_outside = -1024.0;
+    return ANM_OK;
+}
+
+static int check_image_grid(anm_ctx* c, const char* what, int n0, int n1, int n2, double d0, double d1, double d2,
+                            double o0, double o1, double o2) {
+    if (n0 < 1 || n1 < 1 || n2 < 1 || !(d0 > 0) || !(d1 > 0) || !(d2 > 0) || !std::isfinite(d0) || !std::isfinite(d1) ||
+        !std::isfinite(d2) || !std::isfinite(o0) || !std::isfinite(o1) || !std::isfinite(o2))
+        return fail(c, ANM_E_ARG, "%s: image sizes must be >= 1, spacings > 0, offsets finite", what);
+    if ((unsigned long long)n0 * n1 * n2 > 0x7fffffff0ull) return fail(c, ANM_E_ARG, "%s: image too large", what);
+    return ANM_OK;
+}
+
+static ResampleParams resample_params(const anm_ctx* c, int n0, int n1, int n2, double d0, double d1, double d2,
+                                      double o0, double o1, double o2, double fill, double scale) {
+    ResampleParams p;
+    p.nx = c->nx; p.ny = c->ny; p.nz = c->nz;
+    p.dx = c->dx * 10.0; p.dy = c->dy * 10.0; p.dz = c->dz * 10.0;
+    p.snx = n0; p.sny = n1; p.snz = n2; p.sdx = d0; p.sdy = d1; p.sdz = d2;
+    p.ox = o0; p.oy = o1; p.oz = o2; p.fill = fill; p.scale = scale;
+    return p;
+}
+
+int anm_load_ct(anm_ctx* c, const int16_t* hu, int cnx, int cny, int cnz, double cdx_mm, double cdy_mm, double cdz_mm,
+                double ox_mm, double oy_mm, double oz_mm, const anm_hu_ramp* ramp, int on_device) {
+    if (!c) return ANM_E_ARG;
+    if (!hu) return fail(c, ANM_E_ARG, "ct: null pointer");
+    if (!c->have_grid) return fail(c, ANM_E_STATE, "ct: set the grid first");
+    { const int rc = check_image_grid(c, "ct", cnx, cny, cnz, cdx_mm, cdy_mm, cdz_mm, ox_mm, oy_mm, oz_mm); if (rc != ANM_OK) return rc; }
+    anm_hu_ramp def;
+    if (!ramp) { anm_default_hu_ramp(&def); ramp = &def; }
+    if (ramp->n_nodes < 2 || ramp->n_nodes > ANM_MAX_RAMP_NODES) return fail(c, ANM_E_ARG, "ct: ramp needs 2..%d nodes", ANM_MAX_RAMP_NODES);
+    RampParams rp;
+    std::memset(&rp, 0, sizeof rp);
+    rp.n_nodes = ramp->n_nodes;
+    for (int k = 0; k < ramp->n_nodes; ++k) {
+        if (!std::isfinite(ramp->hu[k]) || (k > 0 && !(ramp->hu[k] > ramp->hu[k - 1]))) return fail(c, ANM_E_ARG, "ct: ramp HU nodes must be finite and increase");
+        if (!(ramp->rho[k] >= 0.0) || !(ramp->rho[k] < 16.0)) return fail(c, ANM_E_ARG, "ct: ramp densities must be in [0, 16) g/cm^3");
+        if (k < ramp->n_nodes - 1 && (ramp->material[k] < 0 || ramp->material[k] >= ANM_MAX_MATERIALS)) return fail(c, ANM_E_ARG, "ct: ramp material id out of range");
+        rp.hu[k] = ramp->hu[k]; rp.rho[k] = ramp->rho[k]; rp.material[k] = ramp->material[k];
+    }
+    if (!std::isfinite(ramp->hu_outside)) return fail(c, ANM_E_ARG, "ct: hu_outside must be finite");
+    rp.hu_outside = ramp->hu_outside;
+    ANM_CUDA(c, cudaSetDevice(c->device));
+    const size_t n_src = (size_t)cnx * cny * cnz;
+    DevBuf<int16_t> stage;
+    const int16_t* d_src = hu;
+    if (!on_device) {
+        ANM_CUDA(c, stage.alloc(n_src));
+        ANM_CUDA(c, cudaMemcpyAsync(stage.p, hu, n_src * 2, cudaMemcpyHostToDevice, c->stream));
+        d_src = stage.p;
+    }
+    c->have_phantom = false;
+    cudaEvent_t e0, e1;
+    ANM_CUDA(c, cudaEventCreate(&e0));
+    ANM_CUDA(c, cudaEventCreate(&e1));
+    ANM_CUDA(c, cudaMemsetAsync(c->d_flags.p, 0, (2 + ANM_MAX_MATERIALS + 6 + ANM_MAX_MATERIALS) * 4, c->stream));
+    const ResampleParams p = resample_params(c, cnx, cny, cnz, cdx_mm, cdy_mm, cdz_mm, ox_mm, oy_mm, oz_mm, ramp->hu_outside, 1.0);
+    ANM_CUDA(c, cudaEventRecord(e0, c->stream));
+    resample_kernel<int16_t, RS_CT><<<grid_blocks(c, c->V, kResampleThreads), kResampleThreads, 0, c->stream>>>(
+        d_src, p, rp, c->texels.p, nullptr, nullptr, nullptr, c->d_flags.p, c->d_flags.p + 1);
+    ANM_CUDA(c, cudaGetLastError());
+    ANM_CUDA(c, cudaEventRecord(e1, c->stream));
+    unsigned flags[2] = {0, 0};
+    ANM_CUDA(c, cudaMemcpyAsync(flags, c->d_flags.p, 8, cudaMemcpyDeviceToHost, c->stream));
+    ANM_CUDA(c, cudaStreamSynchronize(c->stream));
+    stage.release();
+    float ms = 0;
+    cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    c->ms_setup += ms; c->ms_load_ct = ms;
+    c->max_material = flags[1];
+    return phantom_setup(c);
+}
+
+int anm_get_phantom(anm_ctx* c, uint8_t* material, float* density, size_t n, int on_device) {
+    if (!c) return ANM_E_ARG;
+    if (!material || !density) return fail(c, ANM_E_ARG, "get_phantom: null pointer");
+    if (!c->have_phantom) return fail(c, ANM_E_STATE, "get_phantom: no phantom loaded");
+    if (n != c->V) return fail(c, ANM_E_ARG, "get_phantom: n = %zu but the grid has %zu voxels", n, c->V);
+    ANM_CUDA(c, cudaSetDevice(c->device));
+    DevBuf<uint8_t> dm;
+    DevBuf<float> dr;
+    uint8_t* pm = material; float* pr = density;
+    if (!on_device) { ANM_CUDA(c, dm.alloc(c->V)); ANM_CUDA(c, dr.alloc(c->V)); pm = dm.p; pr = dr.p; }
+    unpack_texels_kernel<<<grid_blocks(c, c->V, kResampleThreads), kResampleThreads, 0, c->stream>>>(c->texels.p, pm, pr, c->V);
+    ANM_CUDA(c, cudaGetLastError());
+    if (!on_device) {
+        ANM_CUDA(c, cudaMemcpyAsync(material, pm, c->V, cudaMemcpyDeviceToHost, c->stream));
+        ANM_CUDA(c, cudaMemcpyAsync(density, pr, c->V * 4, cudaMemcpyDeviceToHost, c->stream));
+    }
+    ANM_CUDA(c, cudaStreamSynchronize(c->stream));
+    dm.release(); dr.release();
+    return ANM_OK;
+}
+
+int anm_load_pet(anm_ctx* c, const float* bq_per_ml, int pnx, int pny, int pnz, double pdx_mm, double pdy_mm, double pdz_mm,
+                 double ox_mm, double oy_mm, double oz_mm, int on_device, double* total_activity_Bq,
+                 float* out_activity_Bq, size_t n) {
+    if (!c) return ANM_E_ARG;
+    if (!bq_per_ml) return fail(c, ANM_E_ARG, "pet: null pointer");
+    if (!c->have_grid) return fail(c, ANM_E_STATE, "pet: set the grid first");
+    if (out_activity_Bq && n != c->V) return fail(c, ANM_E_ARG, "pet: n = %zu but the grid has %zu voxels", n, c->V);
+    { const int rc = check_image_grid(c, "pet", pnx, pny, pnz, pdx_mm, pdy_mm, pdz_mm, ox_mm, oy_mm, oz_mm); if (rc != ANM_OK) return rc; }
+    ANM_CUDA(c, cudaSetDevice(c->device));
+    const size_t n_src = (size_t)pnx * pny * pnz;
+    DevBuf<float> stage;
+    DevBuf<double> d_total;
+    const float* d_src = bq_per_ml;
+    if (!on_device) {
+        ANM_CUDA(c, stage.alloc(n_src));
+        ANM_CUDA(c, cudaMemcpyAsync(stage.p, bq_per_ml, n_src * 4, cudaMemcpyHostToDevice, c->stream));
+        d_src = stage.p;
+    }
+    ANM_CUDA(c, c->scratch.alloc(c->Vpad));
+    ANM_CUDA(c, d_total.alloc(1));
+    ANM_CUDA(c, cudaMemsetAsync(d_total.p, 0, 8, c->stream));
+    ANM_CUDA(c, cudaMemsetAsync(c->d_flags.p, 0, 8, c->stream));
+    c->have_source = false;
+    cudaEvent_t e0, e1, e2;
+    ANM_CUDA(c, cudaEventCreate(&e0));
+    ANM_CUDA(c, cudaEventCreate(&e1));
+    ANM_CUDA(c, cudaEventCreate(&e2));
+    const double vox_ml = c->dx * c->dy * c->dz;     // cm^3 = mL
+    const ResampleParams p = resample_params(c, pnx, pny, pnz, pdx_mm, pdy_mm, pdz_mm, ox_mm, oy_mm, oz_mm, 0.0, vox_ml);
+    RampParams rp;
+    std::memset(&rp, 0, sizeof rp);
+    float* d_copy = (out_activity_Bq && on_device) ? out_activity_Bq : nullptr;
+    cudaEventRecord(e0, c->stream);
+    resample_kernel<float, RS_PET><<<grid_blocks(c, c->V, kResampleThreads), kResampleThreads, 0, c->stream>>>(
+        d_src, p, rp, nullptr, c->scratch.p, d_copy, d_total.p, c->d_flags.p, c->d_flags.p + 1);
+    ANM_CUDA(c, cudaGetLastError());
+    cudaEventRecord(e1, c->stream);
+    unsigned flags = 0;
+    double total = 0.0;
+    ANM_CUDA(c, cudaMemcpyAsync(&flags, c->d_flags.p, 4, cudaMemcpyDeviceToHost, c->stream));
+    ANM_CUDA(c, cudaMemcpyAsync(&total, d_total.p, 8, cudaMemcpyDeviceToHost, c->stream));
+    if (out_activity_Bq && !on_device)
+        ANM_CUDA(c, cudaMemcpyAsync(out_activity_Bq, c->scratch.p, c->V * 4, cudaMemcpyDeviceToHost, c->stream));
+    ANM_CUDA(c, cudaStreamSynchronize(c->stream));
+    stage.release(); d_total.release();
+    float ms = 0;
+    cudaEventElapsedTime(&ms, e0, e1);
+    c->ms_load_pet = ms;
+    if (flags & 1u) { cudaEventDestroy(e0); cudaEventDestroy(e1); cudaEventDestroy(e2); return fail(c, ANM_E_ARG, "pet: values must be finite and >= 0"); }
+    int rc;
+    try {
+        rc = build_alias(c, c->scratch.p);
+    } catch (const std::bad_alloc&) {
+        rc = fail(c, ANM_E_NOMEM, "pet: host allocation failed");
+    }
+    cudaEventRecord(e2, c->stream);
+    cudaEventSynchronize(e2);
+    cudaEventElapsedTime(&ms, e0, e2);
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaEventDestroy(e2);
+    c->ms_setup += ms;
+    if (rc != ANM_OK) return rc;
+    if (total_activity_Bq) *total_activity_Bq = total;
     c->point_source = false;
     c->have_source = true;
     c->have_results = false;
@@ -740,6 +927,7 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     s.n_steps = ds.n_steps; s.n_real = ds.n_real; s.n_pe = ds.n_pe; s.n_compton = ds.n_compton;
     s.n_rayleigh = ds.n_rayleigh; s.n_escaped = ds.n_escaped; s.n_cutoff = ds.n_cutoff;
     s.ms_transport = ms_t; s.ms_fold = ms_f; s.ms_finalize = ms_fin; s.ms_setup = c->ms_setup;
+    s.ms_load_ct = c->ms_load_ct; s.ms_load_pet = c->ms_load_pet;
     s.n_launches = (uint64_t)2 * B + 1;
     c->run_decays = n_decays;
     c->run_batches = B;
@@ -832,8 +1020,9 @@ int anm_merge(anm_ctx* c, uint64_t total_decays, int total_batches, const double
 int anm_get_stats(anm_ctx* c, anm_stats* out) {
     if (!c) return ANM_E_ARG;
     if (!out) return fail(c, ANM_E_ARG, "stats: null pointer");
-    if (!c->have_results) return fail(c, ANM_E_STATE, "stats: no completed run");
-    *out = c->stats;
+    if (c->have_results) *out = c->stats;
+    else std::memset(out, 0, sizeof *out);     // before a run: only the set-up timings are meaningful
+    out->ms_setup = c->ms_setup; out->ms_load_ct = c->ms_load_ct; out->ms_load_pet = c->ms_load_pet;
     return ANM_OK;
 }
 

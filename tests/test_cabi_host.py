@@ -37,7 +37,8 @@ def test_struct_sizes_match_header():
     assert C.sizeof(binding.anm_tables) == 8 + 16 + 24 + 8 + 16
     assert C.sizeof(binding.anm_options) == 16 + 16 + 16 + 8
     assert C.sizeof(binding.anm_organ) == 5 * 8 + 2 * 8
-    assert C.sizeof(binding.anm_stats) == 3 * 8 + 8 * 8 + 4 * 8 + 8
+    assert C.sizeof(binding.anm_stats) == 3 * 8 + 8 * 8 + 4 * 8 + 8 + 2 * 8
+    assert C.sizeof(binding.anm_hu_ramp) == 8 + 16 * 8 + 16 * 8 + 16 * 4 + 8
 
 
 def test_default_options():
@@ -47,6 +48,18 @@ def test_default_options():
     assert (o.n_batches, o.photons_per_decay, o.rayleigh_on) == (100, 2, 1)
     assert abs(o.photon_cutoff_MeV - 0.010) < 1e-15 and o.positron_ke_MeV == 0.0 and o.history_offset == 0
     assert lib.anm_default_options(None) == -1
+
+
+def test_default_hu_ramp_matches_the_input_module():
+    """include/anm.h's default HU ramp and anm_inputs.DEFAULT_HU_RAMP (which the oracle is handed) hold the same numbers."""
+    import anm_inputs
+    lib = binding.load()
+    r = binding.anm_hu_ramp()
+    assert lib.anm_default_hu_ramp(C.byref(r)) == 0
+    assert r.as_dict() == {k: list(v) if isinstance(v, list) else v for k, v in anm_inputs.DEFAULT_HU_RAMP.items()}
+    assert lib.anm_default_hu_ramp(None) == -1
+    back = binding.anm_hu_ramp.from_dict(anm_inputs.DEFAULT_HU_RAMP).as_dict()
+    assert back == r.as_dict()
 
 
 def test_no_gpu_is_a_loud_error():
