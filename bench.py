@@ -118,6 +118,7 @@ def main():
     ap.add_argument("--cpu-baseline-decays-per-core", type=int, default=400_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-frontend", action="store_true", help="skip the image front-end timing (anm_load_ct / anm_load_pet)")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -263,6 +264,36 @@ def main():
                "d2h_bytes_per_step": V * 8 + 27 * 56, "seconds": dt, "ms_setup_device": st2["ms_setup"],
                "what": "anm_set_grid + load_phantom/activity/organs (host) + tables + anm_run + get_dose + get_uncertainty + get_organ_doses (host)"}
 
+    # ---- image front end: set-up, not part of decays/s; HBM roofline of its two kernels -------
+    frontend = None
+    if not args.no_frontend and world == 1:
+        img = anm_inputs.make_ct_pet(cfg, ct_shape=(512, 512, 400))          # 1 x 1 x 4 mm CT over the cfg3 grid
+        hu_d = torch.from_numpy(img["ct_hu"]).to(dev)
+        pet_d = torch.from_numpy(img["pet_bqml"]).to(dev)
+        with Simulation(local_rank) as s3:
+            s3.set_grid(cfg["shape"], cfg["spacing_mm"])
+            ms_ct, ms_pet = [], []
+            for _ in range(5):
+                s3.load_ct(hu_d, img["ct_shape"], img["ct_spacing_mm"], img["ct_offset_mm"])
+                s3.load_pet(pet_d, img["pet_shape"], img["pet_spacing_mm"], img["pet_offset_mm"])
+                st3 = s3.get_stats()
+                ms_ct.append(st3["ms_load_ct"]); ms_pet.append(st3["ms_load_pet"])
+        peaks = {}
+        try:
+            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        except Exception:
+            pass
+        hbm = float(peaks.get("hbm_gbs", 6500.0))
+        b_ct = hu_d.numel() * 2 + V * 4
+        b_pet = pet_d.numel() * 4 + V * 4
+        frontend = {"workload": "CT 512x512x400 int16 HU @1x1x4mm + PET 256x256x400 Bq/mL -> cfg3 grid",
+                    "load_ct_ms": min(ms_ct[1:]), "load_ct_bytes": b_ct, "load_ct_gbs": b_ct / (min(ms_ct[1:]) * 1e-3) / 1e9,
+                    "load_pet_ms": min(ms_pet[1:]), "load_pet_bytes": b_pet, "load_pet_gbs": b_pet / (min(ms_pet[1:]) * 1e-3) / 1e9,
+                    "hbm_peak_gbs": hbm, "peak_source": "MEASURED_PEAKS.json hbm_gbs" if peaks else "fallback 6500 GB/s",
+                    "load_ct_frac": b_ct / (min(ms_ct[1:]) * 1e-3) / 1e9 / hbm,
+                    "load_pet_frac": b_pet / (min(ms_pet[1:]) * 1e-3) / 1e9 / hbm}
+        del hu_d, pet_d
+
     if rank != 0:
         if dist:
             dist.destroy_process_group()
@@ -290,7 +321,7 @@ def main():
                    "multi_gpu": "one logical run of N*D decays: whole-batch shards via history_offset, NCCL sum-all-reduce of the tallies + merged finalize at the end of every step" if world > 1 else "single GPU"},
         "clocks": clk, "e2e": e2e, "gpu_launches": int(launches),
         "phase_ms_per_step": {"transport": ms_t / args.steps, "fold": ms_f / args.steps, "finalize": ms_fin / args.steps},
-        "roofline": roofline, "cpu_baseline": cpu,
+        "roofline": roofline, "cpu_baseline": cpu, "frontend": frontend,
         "paper_context": "ARCHER-NM on a Titan V: 1e9 decays in <0.5 min (>=3.3e7 decays/s), GATE 376 min (PAPER.md:L117); other hardware, other phantom, electron transport on",
     }))
     if dist:

@@ -53,6 +53,7 @@ struct anm_ctx {
     bool have_grid = false;
     int nx = 0, ny = 0, nz = 0;
     double dx = 0, dy = 0, dz = 0;        // cm
+    double dx_mm = 0, dy_mm = 0, dz_mm = 0;   // as given to anm_set_grid
     size_t V = 0, Vpad = 0;
 
     // inputs
@@ -386,6 +387,7 @@ int anm_set_grid(anm_ctx* c, int nx, int ny, int nz, double dx_mm, double dy_mm,
     ANM_CUDA(c, cudaSetDevice(c->device));
     c->nx = nx; c->ny = ny; c->nz = nz;
     c->dx = dx_mm / 10.0; c->dy = dy_mm / 10.0; c->dz = dz_mm / 10.0;
+    c->dx_mm = dx_mm; c->dy_mm = dy_mm; c->dz_mm = dz_mm;
     c->V = (size_t)V;
     c->Vpad = (c->V + 3) / 4 * 4;
     c->have_grid = true;
@@ -560,10 +562,46 @@ static ResampleParams resample_params(const anm_ctx* c, int n0, int n1, int n2, 
                                       double o0, double o1, double o2, double fill, double scale) {
     ResampleParams p;
     p.nx = c->nx; p.ny = c->ny; p.nz = c->nz;
-    p.dx = c->dx * 10.0; p.dy = c->dy * 10.0; p.dz = c->dz * 10.0;
+    p.dx = c->dx_mm; p.dy = c->dy_mm; p.dz = c->dz_mm;
     p.snx = n0; p.sny = n1; p.snz = n2; p.sdx = d0; p.sdy = d1; p.sdz = d2;
+    p.inv_dx = 1.0 / p.dx; p.inv_dy = 1.0 / p.dy; p.inv_dz = 1.0 / p.dz;
+    p.inv_sdx = 1.0 / d0; p.inv_sdy = 1.0 / d1; p.inv_sdz = 1.0 / d2;
     p.ox = o0; p.oy = o1; p.oz = o2; p.fill = fill; p.scale = scale;
     return p;
+}
+
+// The overlap geometry of one axis (anm_frontend.cuh): destination voxel i = [i d, (i+1) d) against the source voxels
+// [off + j sd, off + (j+1) sd), j = 0..sn-1.  fp64 on the host; nx + ny + nz entries per image.
+static void axis_overlap_table(AxisOverlap* out, int n, double d, int sn, double sd, double off) {
+    for (int i = 0; i < n; ++i) {
+        AxisOverlap o;
+        const double a = (double)i * d, b = (double)(i + 1) * d;
+        const double f0 = std::floor((a - off) / sd), f1 = std::ceil((b - off) / sd) - 1.0;
+        o.j0 = (int)std::max(0.0, std::min(f0, (double)sn));          // may end up > j1: empty
+        o.j1 = (int)std::min((double)(sn - 1), std::max(f1, -1.0));
+        const double lo0 = off + (double)o.j0 * sd, hi0 = off + (double)(o.j0 + 1) * sd;
+        const double lo1 = off + (double)o.j1 * sd, hi1 = off + (double)(o.j1 + 1) * sd;
+        o.w_first = std::max(0.0, std::min(b, hi0) - std::max(a, lo0)) / d;
+        o.w_last = std::max(0.0, std::min(b, hi1) - std::max(a, lo1)) / d;
+        o.inside = std::max(0.0, std::min(b, off + (double)sn * sd) - std::max(a, off)) / d;
+        out[i] = o;
+    }
+}
+
+// one destination row (iy, iz) per block and trip; a few resident waves
+static int resample_blocks(const anm_ctx* c) {
+    return (int)std::max<size_t>(1, std::min<size_t>((size_t)c->ny * c->nz, (size_t)c->num_sms * 16));
+}
+
+static int upload_overlap_tables(anm_ctx* c, const ResampleParams& p, DevBuf<AxisOverlap>& tab) {
+    std::vector<AxisOverlap> h((size_t)p.nx + p.ny + p.nz);
+    axis_overlap_table(h.data(), p.nx, p.dx, p.snx, p.sdx, p.ox);
+    axis_overlap_table(h.data() + p.nx, p.ny, p.dy, p.sny, p.sdy, p.oy);
+    axis_overlap_table(h.data() + p.nx + p.ny, p.nz, p.dz, p.snz, p.sdz, p.oz);
+    ANM_CUDA(c, tab.alloc(h.size()));
+    ANM_CUDA(c, cudaMemcpyAsync(tab.p, h.data(), h.size() * sizeof(AxisOverlap), cudaMemcpyHostToDevice, c->stream));
+    ANM_CUDA(c, cudaStreamSynchronize(c->stream));     // h goes out of scope
+    return ANM_OK;
 }
 
 int anm_load_ct(anm_ctx* c, const int16_t* hu, int cnx, int cny, int cnz, double cdx_mm, double cdy_mm, double cdz_mm,
@@ -586,6 +624,7 @@ int anm_load_ct(anm_ctx* c, const int16_t* hu, int cnx, int cny, int cnz, double
     }
     if (!std::isfinite(ramp->hu_outside)) return fail(c, ANM_E_ARG, "ct: hu_outside must be finite");
     rp.hu_outside = ramp->hu_outside;
+    for (int k = 0; k + 1 < ramp->n_nodes; ++k) rp.inv_dhu[k] = 1.0 / (ramp->hu[k + 1] - ramp->hu[k]);
     ANM_CUDA(c, cudaSetDevice(c->device));
     const size_t n_src = (size_t)cnx * cny * cnz;
     DevBuf<int16_t> stage;
@@ -601,15 +640,17 @@ int anm_load_ct(anm_ctx* c, const int16_t* hu, int cnx, int cny, int cnz, double
     ANM_CUDA(c, cudaEventCreate(&e1));
     ANM_CUDA(c, cudaMemsetAsync(c->d_flags.p, 0, (2 + ANM_MAX_MATERIALS + 6 + ANM_MAX_MATERIALS) * 4, c->stream));
     const ResampleParams p = resample_params(c, cnx, cny, cnz, cdx_mm, cdy_mm, cdz_mm, ox_mm, oy_mm, oz_mm, ramp->hu_outside, 1.0);
+    DevBuf<AxisOverlap> tab;
+    { const int rc = upload_overlap_tables(c, p, tab); if (rc != ANM_OK) { stage.release(); tab.release(); return rc; } }
     ANM_CUDA(c, cudaEventRecord(e0, c->stream));
-    resample_kernel<int16_t, RS_CT><<<grid_blocks(c, c->V, kResampleThreads), kResampleThreads, 0, c->stream>>>(
-        d_src, p, rp, c->texels.p, nullptr, nullptr, nullptr, c->d_flags.p, c->d_flags.p + 1);
+    resample_kernel<int16_t, RS_CT><<<resample_blocks(c), kResampleThreads, 0, c->stream>>>(
+        d_src, tab.p, p, rp, c->texels.p, nullptr, nullptr, nullptr, c->d_flags.p, c->d_flags.p + 1);
     ANM_CUDA(c, cudaGetLastError());
     ANM_CUDA(c, cudaEventRecord(e1, c->stream));
     unsigned flags[2] = {0, 0};
     ANM_CUDA(c, cudaMemcpyAsync(flags, c->d_flags.p, 8, cudaMemcpyDeviceToHost, c->stream));
     ANM_CUDA(c, cudaStreamSynchronize(c->stream));
-    stage.release();
+    stage.release(); tab.release();
     float ms = 0;
     cudaEventElapsedTime(&ms, e0, e1);
     cudaEventDestroy(e0); cudaEventDestroy(e1);
@@ -671,9 +712,19 @@ int anm_load_pet(anm_ctx* c, const float* bq_per_ml, int pnx, int pny, int pnz, 
     RampParams rp;
     std::memset(&rp, 0, sizeof rp);
     float* d_copy = (out_activity_Bq && on_device) ? out_activity_Bq : nullptr;
-    cudaEventRecord(e0, c->stream);
-    resample_kernel<float, RS_PET><<<grid_blocks(c, c->V, kResampleThreads), kResampleThreads, 0, c->stream>>>(
-        d_src, p, rp, nullptr, c->scratch.p, d_copy, d_total.p, c->d_flags.p, c->d_flags.p + 1);
+    DevBuf<AxisOverlap> tab;
+    const bool same_grid = pnx == c->nx && pny == c->ny && pnz == c->nz && ox_mm == 0.0 && oy_mm == 0.0 && oz_mm == 0.0 &&
+                           pdx_mm == p.dx && pdy_mm == p.dy && pdz_mm == p.dz;
+    if (same_grid) {     // the PET grid is the simulation grid -> one streaming pass
+        cudaEventRecord(e0, c->stream);
+        pet_same_grid_kernel<<<grid_blocks(c, c->V / 4 + 1, kResampleThreads), kResampleThreads, 0, c->stream>>>(
+            d_src, vox_ml, c->scratch.p, d_copy, c->V, d_total.p, c->d_flags.p);
+    } else {
+        { const int rc = upload_overlap_tables(c, p, tab); if (rc != ANM_OK) { stage.release(); tab.release(); d_total.release(); return rc; } }
+        cudaEventRecord(e0, c->stream);
+        resample_kernel<float, RS_PET><<<resample_blocks(c), kResampleThreads, 0, c->stream>>>(
+            d_src, tab.p, p, rp, nullptr, c->scratch.p, d_copy, d_total.p, c->d_flags.p, c->d_flags.p + 1);
+    }
     ANM_CUDA(c, cudaGetLastError());
     cudaEventRecord(e1, c->stream);
     unsigned flags = 0;
@@ -683,7 +734,7 @@ int anm_load_pet(anm_ctx* c, const float* bq_per_ml, int pnx, int pny, int pnz, 
     if (out_activity_Bq && !on_device)
         ANM_CUDA(c, cudaMemcpyAsync(out_activity_Bq, c->scratch.p, c->V * 4, cudaMemcpyDeviceToHost, c->stream));
     ANM_CUDA(c, cudaStreamSynchronize(c->stream));
-    stage.release(); d_total.release();
+    stage.release(); d_total.release(); tab.release();
     float ms = 0;
     cudaEventElapsedTime(&ms, e0, e1);
     c->ms_load_pet = ms;

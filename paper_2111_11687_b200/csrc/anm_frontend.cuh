@@ -28,6 +28,7 @@ constexpr int kResampleThreads = 256;
 struct RampParams {
     int n_nodes;
     double hu[kMaxRampNodes], rho[kMaxRampNodes];
+    double inv_dhu[kMaxRampNodes];      // 1 / (hu[k+1] - hu[k])
     int material[kMaxRampNodes];
     double hu_outside;
 };
@@ -35,8 +36,10 @@ struct RampParams {
 struct ResampleParams {
     int nx, ny, nz;          // destination (simulation) grid
     double dx, dy, dz;       // mm
+    double inv_dx, inv_dy, inv_dz;
     int snx, sny, snz;       // source image
     double sdx, sdy, sdz;    // mm
+    double inv_sdx, inv_sdy, inv_sdz;
     double ox, oy, oz;       // position of the source image's corner in the destination frame, mm
     double fill;             // value of the field outside the source image
     double scale;            // PET: voxel volume in mL
@@ -44,26 +47,17 @@ struct ResampleParams {
 
 // One axis of a destination voxel [a, b): the source indices j0..j1 that overlap it (may be empty: j1 < j0) and their
 // weights = overlap length / (b - a).  Only the first and the last source voxel can be cut by the destination voxel's
-// faces; every one in between lies wholly inside it and weighs sd / (b - a).  `inside` = the fraction of [a, b) that
-// lies inside the image.
+// faces; every one in between lies wholly inside it and weighs w_mid = sd / (b - a) (one number per axis).  `inside` =
+// the fraction of [a, b) that lies inside the image.  The weights are separable, so the three tables (nx + ny + nz
+// entries, filled on the host in fp64 by axis_overlap_table in anm_api.cu) are all the geometry the kernel needs:
+// per voxel it loads three entries and streams the source voxels under it.
 struct AxisOverlap {
     int j0, j1;
-    double w_first, w_mid, w_last, inside;
-    __device__ __forceinline__ double w(int j) const { return j == j0 ? w_first : (j == j1 ? w_last : w_mid); }
+    double w_first, w_last, inside;
 };
 
-__device__ __forceinline__ AxisOverlap axis_overlap(int i, double d, int sn, double sd, double off) {
-    AxisOverlap o;
-    const double a = (double)i * d, b = (double)(i + 1) * d, inv_d = 1.0 / d;
-    o.j0 = max(0, (int)floor((a - off) / sd));
-    o.j1 = min(sn - 1, (int)ceil((b - off) / sd) - 1);
-    const double lo0 = off + (double)o.j0 * sd, hi0 = off + (double)(o.j0 + 1) * sd;
-    const double lo1 = off + (double)o.j1 * sd, hi1 = off + (double)(o.j1 + 1) * sd;
-    o.w_first = fmax(0.0, fmin(b, hi0) - fmax(a, lo0)) * inv_d;
-    o.w_last = fmax(0.0, fmin(b, hi1) - fmax(a, lo1)) * inv_d;
-    o.w_mid = sd * inv_d;
-    o.inside = fmax(0.0, fmin(b, off + (double)sn * sd) - fmax(a, off)) * inv_d;
-    return o;
+__device__ __forceinline__ double axis_w(const AxisOverlap& o, double w_mid, int j) {
+    return j == o.j0 ? o.w_first : (j == o.j1 ? o.w_last : w_mid);
 }
 
 enum : int { RS_CT = 0, RS_PET = 1 };
@@ -73,40 +67,46 @@ enum : int { RS_CT = 0, RS_PET = 1 };
 //              flags bit 0 set if a source value under a destination voxel is negative or not finite
 template <typename T, int MODE>
 __global__ void __launch_bounds__(kResampleThreads)
-resample_kernel(const T* __restrict__ src, const __grid_constant__ ResampleParams p, const __grid_constant__ RampParams ramp,
+resample_kernel(const T* __restrict__ src, const AxisOverlap* __restrict__ tab, const __grid_constant__ ResampleParams p, const __grid_constant__ RampParams ramp,
                 uint32_t* __restrict__ out_texels, float* __restrict__ out_act, float* __restrict__ out_copy,
                 double* __restrict__ total, unsigned* __restrict__ flags, unsigned* __restrict__ max_mat) {
-    const size_t V = (size_t)p.nx * p.ny * p.nz;
+    const double wmx = p.sdx * p.inv_dx, wmy = p.sdy * p.inv_dy, wmz = p.sdz * p.inv_dz;
     double local_total = 0.0;
     unsigned bad = 0, mm = 0;
-    for (size_t idx = (size_t)blockIdx.x * kResampleThreads + threadIdx.x; idx < V; idx += (size_t)gridDim.x * kResampleThreads) {
-        const int ix = (int)(idx % (size_t)p.nx), iy = (int)((idx / (size_t)p.nx) % (size_t)p.ny), iz = (int)(idx / ((size_t)p.nx * p.ny));
-        const AxisOverlap X = axis_overlap(ix, p.dx, p.snx, p.sdx, p.ox);
-        const AxisOverlap Y = axis_overlap(iy, p.dy, p.sny, p.sdy, p.oy);
-        const AxisOverlap Z = axis_overlap(iz, p.dz, p.snz, p.sdz, p.oz);
+    // a thread keeps its x column(s) and walks down the destination rows (iy, iz) its block owns: the X entry is loaded
+    // once per column, the Y and Z entries of a row are block-uniform (broadcast loads, no index division)
+    const unsigned rows = (unsigned)p.ny * (unsigned)p.nz;
+    for (unsigned ux = threadIdx.x; ux < (unsigned)p.nx; ux += kResampleThreads) {
+      const AxisOverlap X = tab[ux];
+      for (unsigned row_id = blockIdx.x; row_id < rows; row_id += gridDim.x) {
+        const unsigned uz = row_id / (unsigned)p.ny, uy = row_id - uz * (unsigned)p.ny;
+        const AxisOverlap Y = tab[(unsigned)p.nx + uy];
+        const AxisOverlap Z = tab[(unsigned)p.nx + (unsigned)p.ny + uz];
+        const double inside_yz = Z.inside * Y.inside;
+        const size_t idx = (size_t)row_id * (unsigned)p.nx + ux;
         double acc = 0.0;
         for (int c = Z.j0; c <= Z.j1; ++c) {
-            const double wz = Z.w(c);
+            const double wz = axis_w(Z, wmz, c);
             for (int b = Y.j0; b <= Y.j1; ++b) {
-                const double wzy = wz * Y.w(b);
+                const double wzy = wz * axis_w(Y, wmy, b);
                 const T* row = src + ((size_t)c * p.sny + b) * (size_t)p.snx;
                 double racc = 0.0;
                 for (int a = X.j0; a <= X.j1; ++a) {
                     const double v = (double)__ldg(row + a);
                     if (MODE == RS_PET && !(v >= 0.0 && v < 1e300)) bad = 1;
-                    racc = fma(X.w(a), v, racc);
+                    racc = fma(axis_w(X, wmx, a), v, racc);
                 }
                 acc = fma(wzy, racc, acc);
             }
         }
-        const double mean = acc + (1.0 - Z.inside * Y.inside * X.inside) * p.fill;
+        const double mean = acc + (1.0 - inside_yz * X.inside) * p.fill;
         if (MODE == RS_CT) {
             // HU -> (material, density): interval k with hu[k] <= mean < hu[k+1], clamped at both ends
             int k = 0;
 #pragma unroll 1
             for (int n = 1; n < ramp.n_nodes - 1; ++n) if (mean >= ramp.hu[n]) k = n;
             const double hc = fmin(fmax(mean, ramp.hu[0]), ramp.hu[ramp.n_nodes - 1]);
-            const double f = (hc - ramp.hu[k]) / (ramp.hu[k + 1] - ramp.hu[k]);
+            const double f = (hc - ramp.hu[k]) * ramp.inv_dhu[k];
             const double rho = ramp.rho[k] + f * (ramp.rho[k + 1] - ramp.rho[k]);
             const unsigned m = (unsigned)ramp.material[k];
             const double counts = fmin(rint(rho * 1048576.0), 16777215.0);
@@ -118,6 +118,7 @@ resample_kernel(const T* __restrict__ src, const __grid_constant__ ResampleParam
             if (out_copy) out_copy[idx] = a;
             local_total += mean * p.scale;
         }
+      }
     }
     if (MODE == RS_CT) {
         atomicMax(max_mat, mm);
@@ -134,6 +135,52 @@ resample_kernel(const T* __restrict__ src, const __grid_constant__ ResampleParam
         }
         if (bad) atomicOr(flags, 1u);
     }
+}
+
+// PET image already on the simulation grid (the paper's case: the CT is resampled to the PET grid, so the
+// PET grid IS the simulation grid): the mean over a voxel is the voxel's own value, so the front end is one streaming
+// pass  activity = Bq/mL x mL  with the fp64 block-reduced total and the same validation.  n4 = ceil(V / 4) float4s
+// (the buffers are padded to a multiple of 4 by anm_set_grid; the padding of src is not read: tail handled by V).
+__global__ void __launch_bounds__(kResampleThreads)
+pet_same_grid_kernel(const float* __restrict__ src, double scale, float* __restrict__ out_act, float* __restrict__ out_copy,
+                     size_t V, double* __restrict__ total, unsigned* __restrict__ flags) {
+    double local_total = 0.0;
+    unsigned bad = 0;
+    const size_t n4 = V / 4;
+    const bool aligned = ((reinterpret_cast<size_t>(src) | reinterpret_cast<size_t>(out_copy)) & 15u) == 0;
+    const size_t stride = (size_t)gridDim.x * kResampleThreads, tid = (size_t)blockIdx.x * kResampleThreads + threadIdx.x;
+    auto one = [&](float v) -> float {
+        if (!(v >= 0.0f && v < 3.0e38f)) bad = 1;
+        const double a = (double)v * scale;
+        local_total += a;
+        return (float)a;
+    };
+    size_t done = 0;
+    if (aligned) {
+        for (size_t i = tid; i < n4; i += stride) {
+            const float4 v = __ldcs(reinterpret_cast<const float4*>(src) + i);
+            const float4 a = make_float4(one(v.x), one(v.y), one(v.z), one(v.w));
+            reinterpret_cast<float4*>(out_act)[i] = a;
+            if (out_copy) reinterpret_cast<float4*>(out_copy)[i] = a;
+        }
+        done = n4 * 4;
+    }
+    for (size_t i = done + tid; i < V; i += stride) {
+        const float a = one(src[i]);
+        out_act[i] = a;
+        if (out_copy) out_copy[i] = a;
+    }
+    __shared__ double s_tot[kResampleThreads / 32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) local_total += __shfl_xor_sync(0xffffffffu, local_total, o);
+    if ((threadIdx.x & 31) == 0) s_tot[threadIdx.x >> 5] = local_total;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < kResampleThreads / 32; ++w) t += s_tot[w];
+        if (t != 0.0) atomicAdd(total, t);
+    }
+    if (bad) atomicOr(flags, 1u);
 }
 
 // inspection: texels -> material u8 + density f32
