@@ -16,3 +16,4 @@ from .materials import MATERIALS, MATERIAL_IDS, electrons_per_gram  # noqa: F401
 from .tables import make_tables, sigma_kn_per_electron, E0_MEV  # noqa: F401
 from .phantoms import make_config, make_patient_on_grid, ORGAN_NAMES, CONFIG_NAMES  # noqa: F401
 from .images import DEFAULT_HU_RAMP, make_ct_pet, density_to_hu  # noqa: F401
+from .electrons import make_electron_tables, bethe_collision_stopping, ELECTRON_CUTOFF_MEV  # noqa: F401

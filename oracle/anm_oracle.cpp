@@ -117,12 +117,17 @@ struct OrcProblem {
     int32_t n_batches, pad2_;
     uint64_t seed;
     OrcTables t;
+    // secondary-electron transport (PAPER.md:L67 electron cutoff 200 keV; reading C28)
+    int32_t electron_on, n_t;              // n_t points of the kinetic-energy grid T_k = t_min + k dt
+    double electron_cutoff;                // MeV; must equal t_min (the range table is "range above the cutoff")
+    double t_min, dt;
+    const float* e_range;                  // [n_materials][n_t] residual CSDA range above the cutoff, g/cm^2
 };
 
 struct OrcStats {
     double emitted, deposited, escaped, max_history_residual;
     uint64_t n_histories, n_photons, n_crossings, n_collisions, n_pe, n_compton, n_rayleigh,
-        n_escaped, n_cutoff, n_virtual;
+        n_escaped, n_cutoff, n_virtual, n_electrons, n_electron_crossings;
 };
 
 // ------------------------------------------------------------------ P1
@@ -343,6 +348,93 @@ struct Workspace {
     std::vector<double> rho_max;   // per material, for the Woodcock cross-check
 };
 
+// ---------------------------------------------------------------------------------------------
+// Secondary electrons ("A photon or an electron is transported ... until its energy falls below
+// cutoff energy ... its remaining energy is deposited locally.  The cutoff energies for photons and electrons are
+// set to 10 keV and 200 keV").  The paper does not describe its electron physics; reading C28: continuous
+// slowing down along a STRAIGHT line in the electron's initial direction, no angular deflection, no secondaries.
+//   residual range above the cutoff in material m:  r = R_m(T)  [g/cm^2], R_m piecewise linear on the T grid;
+//   after a chord of length l in a voxel of density rho:  r' = r - rho l,  T' = R_m^{-1}(r')  (the exact inverse of
+//   that piecewise-linear function);  T - T' is deposited in the voxel;
+//   r' <= 0: the electron reaches the cutoff inside this voxel: all of T is deposited here (the slowing down to the
+//   cutoff plus the cutoff energy itself, "deposited locally").
+// An electron that leaves the grid carries its remaining energy out (counted as escaped).
+// ---------------------------------------------------------------------------------------------
+double e_range_of(const OrcProblem& p, int m, double T) {          // R_m(T)
+    const float* R = p.e_range + (size_t)m * p.n_t;
+    double x = (T - p.t_min) / p.dt;
+    if (x <= 0.0) return 0.0;
+    int k = (int)std::floor(x);
+    if (k > p.n_t - 2) k = p.n_t - 2;                              // (set-up checks that the grid covers T)
+    return (double)R[k] + (x - (double)k) * ((double)R[k + 1] - (double)R[k]);
+}
+
+double e_energy_of(const OrcProblem& p, int m, double r) {         // R_m^{-1}(r)
+    const float* R = p.e_range + (size_t)m * p.n_t;
+    if (r <= 0.0) return p.t_min;
+    int k = 0;
+    while (k < p.n_t - 2 && (double)R[k + 1] <= r) ++k;            // segment with R[k] <= r < R[k+1]
+    const double f = (r - (double)R[k]) / ((double)R[k + 1] - (double)R[k]);
+    return p.t_min + ((double)k + f) * p.dt;
+}
+
+// Walk one electron from pos (inside voxel vox) along unit vector e with kinetic energy T > cutoff.
+// dep(v, energy) is called once per voxel that receives energy.  Returns the energy carried out of the grid (0 if
+// the electron stopped inside).
+template <class Dep>
+double electron_walk(const OrcProblem& p, const double pos[3], const double e[3], const int vox0[3], double T,
+                     Dep dep, uint64_t* crossings) {
+    const double h[3] = {p.dx, p.dy, p.dz};
+    const int n[3] = {p.nx, p.ny, p.nz};
+    int vox[3] = {vox0[0], vox0[1], vox0[2]};
+    double tmax[3], tdelta[3];
+    int step[3];
+    for (int a = 0; a < 3; ++a) {                                  // the same voxel-boundary stepping as flight_dda
+        if (e[a] > 0.0) { step[a] = 1; tdelta[a] = h[a] / e[a]; tmax[a] = ((double)(vox[a] + 1) * h[a] - pos[a]) / e[a]; }
+        else if (e[a] < 0.0) { step[a] = -1; tdelta[a] = -h[a] / e[a]; tmax[a] = ((double)vox[a] * h[a] - pos[a]) / e[a]; }
+        else { step[a] = 0; tdelta[a] = tmax[a] = std::numeric_limits<double>::infinity(); }
+        if (tmax[a] < 0.0) tmax[a] = 0.0;
+    }
+    double t = 0.0;
+    for (;;) {
+        int a = 0;
+        if (tmax[1] < tmax[a]) a = 1;
+        if (tmax[2] < tmax[a]) a = 2;
+        const int64_t v = vox_index(p, vox);
+        const int m = p.material[v];
+        const double rho = (double)p.density[v];
+        const double chord = tmax[a] - t;
+        const double r = e_range_of(p, m, T);
+        if (rho * chord >= r) { dep(v, T); return 0.0; }           // reaches the cutoff here: everything local
+        const double T_new = e_energy_of(p, m, r - rho * chord);
+        if (T > T_new) dep(v, T - T_new);
+        T = T_new;
+        t = tmax[a];
+        vox[a] += step[a];
+        if (crossings) ++*crossings;
+        if (vox[a] < 0 || vox[a] >= n[a]) return T;
+        tmax[a] += tdelta[a];
+    }
+}
+
+// Direction of the Compton recoil electron: momentum conservation, p_e = k - k' with photon momenta k = E d / c,
+// k' = eps E d' / c.  (Textbook check: cot(phi_e) = (1 + alpha) tan(theta / 2).)
+void compton_electron_direction(double E, double eps, const double d[3], const double d_new[3], double out[3]) {
+    double pe[3] = {E * d[0] - E * eps * d_new[0], E * d[1] - E * eps * d_new[1], E * d[2] - E * eps * d_new[2]};
+    const double nrm = std::sqrt(pe[0] * pe[0] + pe[1] * pe[1] + pe[2] * pe[2]);
+    for (int a = 0; a < 3; ++a) out[a] = nrm > 0.0 ? pe[a] / nrm : d[a];
+}
+
+// Energy T set free as an electron at pos in voxel vox with direction e: transported if the option is on and T is
+// above the electron cutoff, else deposited on the spot (north_star's reading C2).
+void release_electron(const OrcProblem& p, const double pos[3], const double e[3], const int vox[3], double T,
+                      Tally& ty, OrcStats& st, double* escaped) {
+    if (!(T > 0.0)) return;
+    if (!p.electron_on || T <= p.electron_cutoff) { deposit(ty, vox_index(p, vox), T); return; }
+    ++st.n_electrons;
+    *escaped += electron_walk(p, pos, e, vox, T, [&](int64_t v, double x) { deposit(ty, v, x); }, &st.n_electron_crossings);
+}
+
 // One photon from (pos, d, E) until absorbed, below cutoff, or out of the grid.
 // fc_* : first-collision record (P7), may be null.
 void transport_photon(const OrcProblem& p, const Workspace& ws, Rng& g, double pos[3], double d[3],
@@ -374,12 +466,14 @@ void transport_photon(const OrcProblem& p, const Workspace& ws, Rng& g, double p
         const int m = p.material[v];
         // interaction type proportional to the partial coefficients
         const double u = g.uniform() * xs.tot[m];
-        double dep_here = 0.0;
+        double dep_here = 0.0, dep_first = 0.0;   // dep_here: photon energy left on the spot; dep_first: energy transferred
         bool alive = true;
         if (u < xs.pe[m]) {
-            // photoelectric: all energy local (reading C5)
+            // photoelectric: all energy to one electron moving in the photon's direction (reading C5: no
+            // fluorescence, binding energy neglected; C28); deposited locally unless electron transport is on
             ++st.n_pe;
-            dep_here = E;
+            release_electron(p, pos, d, vox, E, ty, st, escaped);
+            dep_first = E;
             alive = false;
         } else if (u < xs.pe[m] + xs.co[m]) {
             ++st.n_compton;
@@ -387,13 +481,20 @@ void transport_photon(const OrcProblem& p, const Workspace& ws, Rng& g, double p
             const double eps = kn_sample_eps(g, E);
             const double cos_t = 1.0 + 1.0 / a - 1.0 / (a * eps);
             const double phi = kTwoPi * g.uniform();
-            dep_here = E * (1.0 - eps);      // recoil electron deposited locally (north_star; reading C2)
-            E *= eps;
+            const double T = E * (1.0 - eps);   // recoil electron: deposited locally (north_star; reading C2) ...
             double nd[3];
             rotate(d, cos_t, phi, nd);
+            {   // ... or transported (C28) along its momentum
+                double pe[3];
+                compton_electron_direction(E, eps, d, nd, pe);
+                release_electron(p, pos, pe, vox, T, ty, st, escaped);
+            }
+            dep_first = T;
+            E *= eps;
             d[0] = nd[0]; d[1] = nd[1]; d[2] = nd[2];
             if (E < p.photon_cutoff) {       // below cutoff, remaining energy deposited locally
                 dep_here += E;
+                dep_first += E;
                 ++st.n_cutoff;
                 alive = false;
             } else {
@@ -408,7 +509,7 @@ void transport_photon(const OrcProblem& p, const Workspace& ws, Rng& g, double p
             d[0] = nd[0]; d[1] = nd[1]; d[2] = nd[2];
         }
         if (dep_here > 0.0) deposit(ty, v, dep_here);
-        if (first && fc_dist) { *fc_dist = dist; *fc_dep = dep_here; }
+        if (first && fc_dist) { *fc_dist = dist; *fc_dep = dep_first; }
         first = false;
         if (!alive) return;
     }
@@ -476,6 +577,23 @@ int orc_flight(const OrcProblem* p, const double* pos, const double* d, double E
     return hit;
 }
 
+// Electron pins: R_m(T), its inverse, and one walk.  out_voxel/out_dep receive up to cap (voxel, energy) pairs in
+// path order; returns the number of pairs, *escaped = energy carried out of the grid.
+void orc_compton_electron_direction(double E, double eps, const double* d, const double* d_new, double* out) {
+    compton_electron_direction(E, eps, d, d_new, out);
+}
+double orc_e_range(const OrcProblem* p, int m, double T) { return e_range_of(*p, m, T); }
+double orc_e_energy(const OrcProblem* p, int m, double r) { return e_energy_of(*p, m, r); }
+int orc_electron_walk(const OrcProblem* p, const double* pos, const double* e, double T, int64_t* out_voxel,
+                      double* out_dep, int cap, double* escaped) {
+    const double h[3] = {p->dx, p->dy, p->dz};
+    int vox[3];
+    for (int a = 0; a < 3; ++a) vox[a] = (int)std::floor(pos[a] / h[a]);
+    int n = 0;
+    *escaped = electron_walk(*p, pos, e, vox, T, [&](int64_t v, double x) { if (n < cap) { out_voxel[n] = v; out_dep[n] = x; } ++n; }, nullptr);
+    return n;
+}
+
 // ----------------------------------------------------------------- the run
 // Histories [h0, h1) of a run of n_total decays in n_batches batches; h0 and h1 must be batch
 // boundaries (batch b = h / (n_total / n_batches); reading C15: n_total % n_batches == 0).
@@ -491,6 +609,8 @@ int orc_run(const OrcProblem* pp, uint64_t h0, uint64_t h1, double* sum, double*
     if (h0 % nb || h1 % nb || h1 < h0 || h1 > p.n_total) return -1;
     if (!p.use_point_source && !p.cdf) return -1;
     if (p.photons_per_decay != 1 && p.photons_per_decay != 2) return -1;
+    if (p.electron_on && (!p.e_range || p.n_t < 2 || !(p.dt > 0.0) || p.electron_cutoff != p.t_min ||
+                          p.t_min + p.dt * (p.n_t - 1) < 2.0 * kElectronMassMeV / 3.0)) return -1;
     const uint64_t V = (uint64_t)p.nx * p.ny * p.nz;
     const double vox_cm3 = p.dx * p.dy * p.dz;
 

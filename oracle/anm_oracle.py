@@ -55,14 +55,17 @@ class OrcProblem(C.Structure):
                 ("rayleigh_on", C.c_int32), ("tracking", C.c_int32),
                 ("photon_cutoff", C.c_double), ("positron_ke", C.c_double),
                 ("n_total", C.c_uint64), ("n_batches", C.c_int32), ("pad2_", C.c_int32),
-                ("seed", C.c_uint64), ("t", OrcTables)]
+                ("seed", C.c_uint64), ("t", OrcTables),
+                ("electron_on", C.c_int32), ("n_t", C.c_int32), ("electron_cutoff", C.c_double),
+                ("t_min", C.c_double), ("dt", C.c_double), ("e_range", C.c_void_p)]
 
 
 class OrcStats(C.Structure):
     _fields_ = [("emitted", C.c_double), ("deposited", C.c_double), ("escaped", C.c_double),
                 ("max_history_residual", C.c_double)] + [
         (n, C.c_uint64) for n in ("n_histories", "n_photons", "n_crossings", "n_collisions", "n_pe",
-                                  "n_compton", "n_rayleigh", "n_escaped", "n_cutoff", "n_virtual")]
+                                  "n_compton", "n_rayleigh", "n_escaped", "n_cutoff", "n_virtual",
+                                  "n_electrons", "n_electron_crossings")]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
@@ -89,6 +92,13 @@ def lib():
         L.orc_flight.restype = C.c_int
         L.orc_flight.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_double,
                                  C.c_void_p, C.c_void_p, C.c_void_p]
+        L.orc_compton_electron_direction.argtypes = [C.c_double, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.orc_e_range.restype = C.c_double
+        L.orc_e_range.argtypes = [C.c_void_p, C.c_int, C.c_double]
+        L.orc_e_energy.restype = C.c_double
+        L.orc_e_energy.argtypes = [C.c_void_p, C.c_int, C.c_double]
+        L.orc_electron_walk.restype = C.c_int
+        L.orc_electron_walk.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
         L.orc_run.restype = C.c_int
         L.orc_run.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64] + [C.c_void_p] * 6
         _lib = L
@@ -165,6 +175,15 @@ class Oracle:
         p.positron_ke = float(get("positron_ke_mev"))
         p.n_total, p.n_batches, p.seed = self.n_decays, self.n_batches, int(get("seed"))
         p.t = tables_struct(tables, self._keep)
+        # secondary-electron transport (NEXT-2): electron_tables = anm_inputs.make_electron_tables()
+        et = over.get("electron_tables")
+        p.electron_on = int(bool(over.get("electron_on", et is not None)))
+        if et is not None:
+            rng = np.ascontiguousarray(et["range"], np.float32)
+            assert rng.shape == (tables["n_materials"], et["n_t"])
+            self._keep.append(rng)
+            p.n_t, p.t_min, p.dt, p.e_range = int(et["n_t"]), float(et["t_min"]), float(et["dt"]), _ptr(rng)
+            p.electron_cutoff = float(over.get("electron_cutoff_mev", et["t_min"]))
         self.p = p
         self.tables = tables
 
@@ -228,6 +247,21 @@ class Oracle:
                 "organ_batch": np.frombuffer(sh_ob, np.float64).reshape(B, no).copy(), "stats": stats,
                 "seconds": wall, "cpu_seconds": sum(r[1] for r in res), "cores": n_procs,
                 "n_decays_run": self.n_decays}
+
+    # ------------------------------------------------------------------ electron pins
+    def electron_range(self, m: int, T: float) -> float:
+        return float(lib().orc_e_range(C.byref(self.p), int(m), float(T)))
+
+    def electron_energy(self, m: int, r: float) -> float:
+        return float(lib().orc_e_energy(C.byref(self.p), int(m), float(r)))
+
+    def electron_walk(self, pos_cm, direction, T: float, cap: int = 4096):
+        """One CSDA straight-line walk: ([(voxel, MeV), ...] in path order, escaped MeV)."""
+        pos = np.asarray(pos_cm, np.float64); d = np.asarray(direction, np.float64)
+        vox = np.zeros(cap, np.int64); dep = np.zeros(cap, np.float64); esc = C.c_double(0.0)
+        n = lib().orc_electron_walk(C.byref(self.p), _ptr(pos), _ptr(d), float(T), _ptr(vox), _ptr(dep), cap, C.byref(esc))
+        assert n <= cap
+        return list(zip(vox[:n].tolist(), dep[:n].tolist())), float(esc.value)
 
     # ------------------------------------------------------------------ post-processing
     def finalize(self, r: dict, total_activity_bq: float | None = None) -> dict:
