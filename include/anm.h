@@ -91,7 +91,28 @@ typedef struct {
                                    low-density margin's own majorant and stop on the box surface; 2 off     */
     uint64_t history_offset;    /* index of the first history: anm_run simulates offset .. offset+n_decays-1
                                    (multi-GPU sharding of one logical run by whole batches); default 0      */
+    int32_t electron_transport; /* 0: secondary electrons deposited where they are set free (north_star);
+                                   1: Compton / photo-electrons above the electron cutoff are transported
+                                   (needs anm_set_electron_tables; schedule 0 or 2 only)      */
+    int32_t reserved0;
 } anm_options;
+
+/* Electron data for anm_options.electron_transport ("The cutoff energies for
+ * photons and electrons are set to 10 keV and 200 keV"; reading C28): continuous slowing down along a
+ * straight line in the electron's initial direction (Compton: its momentum k - k'; photoelectric: the photon's
+ * direction), no deflection, no secondaries.  range[m][k] = residual CSDA mass range ABOVE THE CUTOFF (g/cm^2) at the
+ * kinetic energy t_min + k*dt (MeV): t_min IS the electron cutoff, range[m][0] = 0, strictly increasing in k, read
+ * by linear interpolation and inverted as that piecewise-linear function; the grid must reach 2/3 * 0.51099895 MeV
+ * (the Compton edge of an annihilation photon).  Crossing a voxel of density rho along a chord l takes rho*l off the
+ * residual range; the energy difference is deposited in the voxel; when the range runs out inside a voxel the whole
+ * remaining energy (cutoff energy included, "deposited locally") goes there; an electron that leaves the grid carries
+ * its energy out (counted in escaped_MeV). */
+typedef struct {
+    int32_t n_materials;      /* must cover the phantom's material ids */
+    int32_t n_t;              /* 2..1024 */
+    double t_min, dt;         /* MeV */
+    const float* range;       /* [n_materials][n_t] */
+} anm_electron_tables;
 
 typedef struct {
     double mean_Gy_per_decay;          /* Eq. 2: (1/N_o) sum of voxel doses             */
@@ -105,6 +126,7 @@ typedef struct {
 typedef struct {
     double emitted_MeV, deposited_MeV, escaped_MeV;   /* escaped and the counters need collect_stats   */
     uint64_t n_decays, n_steps, n_real, n_pe, n_compton, n_rayleigh, n_escaped, n_cutoff;
+    uint64_t n_electrons;                                  /* electrons transported (collect_stats)         */
     double ms_transport, ms_fold, ms_finalize, ms_setup;   /* device time of the last anm_run / last setup */
     uint64_t n_launches;                                   /* kernels launched by the last anm_run         */
     double ms_load_ct, ms_load_pet;                        /* device time of the last anm_load_ct / anm_load_pet
@@ -171,6 +193,7 @@ int anm_set_point_source(anm_ctx* c, double x_mm, double y_mm, double z_mm);
 /* labels[V]: 0 = none, 1..n_organs (n_organs <= ANM_MAX_ORGANS).  Optional. */
 int anm_load_organs(anm_ctx* c, const uint8_t* labels, int n_organs, int on_device);
 int anm_set_physics_tables(anm_ctx* c, const anm_tables* t);
+int anm_set_electron_tables(anm_ctx* c, const anm_electron_tables* t);   /* host struct, copied */
 int anm_set_options(anm_ctx* c, const anm_options* o);
 int anm_default_options(anm_options* o);   /* 100 batches, pairs, Rayleigh on, cutoff 0.010, no positron KE */
 
@@ -196,6 +219,12 @@ int anm_get_stats(anm_ctx* c, anm_stats* out);    /* before a completed run: zer
  * count; otherwise out is a HOST array with room for capacity_entries * 4 uint32.  ANM_E_STATE without an
  * activity map (point-source mode has no table). */
 int anm_get_alias_table(anm_ctx* c, uint32_t* out, size_t capacity_entries, size_t* n_entries);
+
+/* Parity hook of the electron walk: the n given electrons {x, y, z (mm), ex, ey, ez (unit vector), T (MeV)} (HOST
+ * array of 7 n floats, T above the cutoff, start points inside the grid) are walked by the same device function the
+ * transport kernel calls; out_MeV (HOST, nx*ny*nz floats) receives the energy each voxel got, *escaped_MeV the
+ * energy carried out of the grid.  Needs grid, phantom and electron tables; leaves the run state untouched. */
+int anm_trace_electrons(anm_ctx* c, const float* electrons, size_t n, float* out_MeV, size_t n_voxels, double* escaped_MeV);
 
 /* --- one logical run over several GPUs ---------------------------------------
  * Histories are independent and keyed by index (Philox counter = history index), so a run of N decays in B batches

@@ -21,6 +21,7 @@ ANM_SYMBOLS = [
     "anm_default_options", "anm_run", "anm_get_energy", "anm_get_dose", "anm_get_dose_rate", "anm_get_uncertainty",
     "anm_get_organ_doses", "anm_get_stats", "anm_get_tally_buffers", "anm_merge", "anm_get_alias_table",
     "anm_default_hu_ramp", "anm_load_ct", "anm_get_phantom", "anm_load_pet",
+    "anm_set_electron_tables", "anm_trace_electrons",
 ]
 
 STATUS = {0: "ANM_OK", -1: "ANM_E_ARG", -2: "ANM_E_STATE", -3: "ANM_E_CUDA", -4: "ANM_E_NOMEM", -5: "ANM_E_UNSUPPORTED"}
@@ -42,7 +43,13 @@ class anm_options(C.Structure):
     _fields_ = [("n_batches", C.c_int32), ("photons_per_decay", C.c_int32), ("rayleigh_on", C.c_int32),
                 ("zero_air_dose", C.c_int32), ("photon_cutoff_MeV", C.c_double), ("positron_ke_MeV", C.c_double),
                 ("schedule", C.c_int32), ("collect_stats", C.c_int32), ("warp_aggregate", C.c_int32),
-                ("hull_majorant", C.c_int32), ("history_offset", C.c_uint64)]
+                ("hull_majorant", C.c_int32), ("history_offset", C.c_uint64),
+                ("electron_transport", C.c_int32), ("reserved0", C.c_int32)]
+
+
+class anm_electron_tables(C.Structure):
+    _fields_ = [("n_materials", C.c_int32), ("n_t", C.c_int32), ("t_min", C.c_double), ("dt", C.c_double),
+                ("range", C.c_void_p)]
 
 
 class anm_organ(C.Structure):
@@ -53,7 +60,7 @@ class anm_organ(C.Structure):
 
 class anm_stats(C.Structure):
     _fields_ = [("emitted_MeV", C.c_double), ("deposited_MeV", C.c_double), ("escaped_MeV", C.c_double)] + [
-        (n, C.c_uint64) for n in ("n_decays", "n_steps", "n_real", "n_pe", "n_compton", "n_rayleigh", "n_escaped", "n_cutoff")] + [
+        (n, C.c_uint64) for n in ("n_decays", "n_steps", "n_real", "n_pe", "n_compton", "n_rayleigh", "n_escaped", "n_cutoff", "n_electrons")] + [
         ("ms_transport", C.c_double), ("ms_fold", C.c_double), ("ms_finalize", C.c_double), ("ms_setup", C.c_double),
         ("n_launches", C.c_uint64), ("ms_load_ct", C.c_double), ("ms_load_pet", C.c_double)]
 
@@ -124,6 +131,8 @@ def load(build_if_missing: bool = True):
         "anm_get_tally_buffers": (i32, [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(sz), C.POINTER(vp), C.POINTER(i32)]),
         "anm_merge": (i32, [vp, u64, i32, vp, C.POINTER(anm_stats)]),
         "anm_get_alias_table": (i32, [vp, vp, sz, C.POINTER(sz)]),
+        "anm_set_electron_tables": (i32, [vp, C.POINTER(anm_electron_tables)]),
+        "anm_trace_electrons": (i32, [vp, vp, sz, vp, sz, C.POINTER(dbl)]),
         "anm_default_hu_ramp": (i32, [C.POINTER(anm_hu_ramp)]),
         "anm_load_ct": (i32, [vp, vp, i32, i32, i32, dbl, dbl, dbl, dbl, dbl, dbl, C.POINTER(anm_hu_ramp), i32]),
         "anm_get_phantom": (i32, [vp, vp, vp, sz, i32]),
@@ -280,6 +289,25 @@ class Simulation:
             keep.append(a)
             setattr(t, name, a.ctypes.data)
         self._ck(self._L.anm_set_physics_tables(self._ctx, C.byref(t)))
+
+    def set_electron_tables(self, et: dict):
+        """et = anm_inputs.make_electron_tables(): {"n_materials", "n_t", "t_min", "dt", "range" [nm][n_t]}."""
+        t = anm_electron_tables()
+        rng = np.ascontiguousarray(et["range"], np.float32).reshape(-1)
+        t.n_materials, t.n_t, t.t_min, t.dt = int(et["n_materials"]), int(et["n_t"]), float(et["t_min"]), float(et["dt"])
+        if rng.size != t.n_materials * t.n_t:
+            raise ValueError("range must hold n_materials * n_t values")
+        t.range = rng.ctypes.data
+        self._ck(self._L.anm_set_electron_tables(self._ctx, C.byref(t)))
+
+    def trace_electrons(self, electrons):
+        """electrons: [n][7] = x, y, z (mm), unit direction, T (MeV).  Returns (energy per voxel [nz][ny][nx], escaped MeV)."""
+        e = np.ascontiguousarray(electrons, np.float32).reshape(-1, 7)
+        nx, ny, nz = self.shape
+        out = np.zeros(self.V, np.float32)
+        esc = C.c_double(0.0)
+        self._ck(self._L.anm_trace_electrons(self._ctx, e.ctypes.data, e.shape[0], out.ctypes.data, self.V, C.byref(esc)))
+        return out.reshape(nz, ny, nx), float(esc.value)
 
     def default_options(self) -> anm_options:
         o = anm_options()

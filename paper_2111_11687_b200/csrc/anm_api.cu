@@ -74,6 +74,11 @@ struct anm_ctx {
     double lnE_min = 0, dlnE = 0;
     std::vector<float> mu_pe, mu_co, mu_ra, ray_x2, ray_cum;
     bool dev_tables_dirty = true;
+    // electron tables (host copy + device)
+    bool have_etables = false;
+    int e_nm = 0, e_nt = 0;
+    double e_tmin = 0, e_dt = 0;
+    std::vector<float> e_range;
 
     // device memory
     DevBuf<uint32_t> texels;
@@ -87,7 +92,7 @@ struct anm_ctx {
     DevBuf<double> organ_mass;            // [256]
     DevBuf<unsigned long long> organ_count;   // [256]
     DevBuf<double> total_energy;          // [1]
-    DevBuf<float> d_tot, d_maj, d_majo, d_x2, d_cum;
+    DevBuf<float> d_tot, d_maj, d_majo, d_x2, d_cum, d_erange;
     DevBuf<float2> d_pec;
     DevBuf<unsigned> d_flags;             // [2 + ANM_MAX_MATERIALS] + [6 + ANM_MAX_MATERIALS] for the hull pass
     unsigned n_alias = 0;
@@ -265,8 +270,10 @@ struct HostE0 { int ie; float fe, maj, inv_maj; };
 using TransportFn = void (*)(const TransportParams);
 
 // schedule 1 (history-based lanes) or 2 (warp-scope event pool), with / without counters and warp aggregation
-TransportFn pick_transport(int schedule, bool stats, bool wagg) {
-    if (schedule == 2) return stats ? transport_pool_kernel<true> : transport_pool_kernel<false>;
+TransportFn pick_transport(int schedule, bool stats, bool wagg, bool elec) {
+    if (schedule == 2)
+        return elec ? (stats ? transport_pool_kernel<true, true> : transport_pool_kernel<false, true>)
+                    : (stats ? transport_pool_kernel<true, false> : transport_pool_kernel<false, false>);
     return stats ? (wagg ? transport_kernel<true, true> : transport_kernel<true, false>)
                  : (wagg ? transport_kernel<false, true> : transport_kernel<false, false>);
 }
@@ -837,6 +844,79 @@ int anm_set_physics_tables(anm_ctx* c, const anm_tables* t) {
     return ANM_OK;
 }
 
+// electron part of the kernel parameters (zeros when no tables are set)
+static void fill_electron_params(const anm_ctx* c, TransportParams& p) {
+    p.e_range = c->have_etables ? c->d_erange.p : nullptr;
+    p.n_t = c->e_nt;
+    p.t_min = (float)c->e_tmin; p.e_dt = (float)c->e_dt; p.e_inv_dt = c->e_dt > 0 ? (float)(1.0 / c->e_dt) : 0.0f;
+}
+
+int anm_set_electron_tables(anm_ctx* c, const anm_electron_tables* t) {
+    if (!c) return ANM_E_ARG;
+    if (!t || !t->range) return fail(c, ANM_E_ARG, "electron tables: null pointer");
+    if (t->n_materials < 1 || t->n_materials > ANM_MAX_MATERIALS || t->n_t < 2 || t->n_t > 1024 || !(t->dt > 0) ||
+        !(t->t_min > 0) || !std::isfinite(t->t_min) || !std::isfinite(t->dt))
+        return fail(c, ANM_E_ARG, "electron tables: sizes out of range");
+    if (t->t_min + t->dt * (t->n_t - 1) < 2.0 * 0.51099895 / 3.0) return fail(c, ANM_E_ARG, "electron tables: the grid must reach the Compton edge 0.3407 MeV");
+    for (int m = 0; m < t->n_materials; ++m) {
+        const float* R = t->range + (size_t)m * t->n_t;
+        if (R[0] != 0.0f) return fail(c, ANM_E_ARG, "electron tables: range[m][0] must be 0 (t_min is the cutoff)");
+        for (int k = 1; k < t->n_t; ++k)
+            if (!(R[k] > R[k - 1]) || !std::isfinite(R[k])) return fail(c, ANM_E_ARG, "electron tables: range must increase strictly");
+    }
+    ANM_CUDA(c, cudaSetDevice(c->device));
+    try { c->e_range.assign(t->range, t->range + (size_t)t->n_materials * t->n_t); }
+    catch (const std::bad_alloc&) { return fail(c, ANM_E_NOMEM, "electron tables: host allocation failed"); }
+    c->e_nm = t->n_materials; c->e_nt = t->n_t; c->e_tmin = t->t_min; c->e_dt = t->dt;
+    ANM_CUDA(c, c->d_erange.alloc(c->e_range.size()));
+    ANM_CUDA(c, cudaMemcpyAsync(c->d_erange.p, c->e_range.data(), c->e_range.size() * 4, cudaMemcpyHostToDevice, c->stream));
+    ANM_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->have_etables = true;
+    c->have_results = false;
+    return ANM_OK;
+}
+
+int anm_trace_electrons(anm_ctx* c, const float* electrons, size_t n, float* out_MeV, size_t n_voxels, double* escaped_MeV) {
+    if (!c) return ANM_E_ARG;
+    if (!electrons || !out_MeV || !escaped_MeV || n == 0 || n > 0x7fffffffu) return fail(c, ANM_E_ARG, "trace: null pointer or bad count");
+    if (!c->have_grid || !c->have_phantom || !c->have_etables) return fail(c, ANM_E_STATE, "trace: need grid, phantom and electron tables");
+    if (n_voxels != c->V) return fail(c, ANM_E_ARG, "trace: n_voxels = %zu but the grid has %zu voxels", n_voxels, c->V);
+    if ((int)c->max_material >= c->e_nm) return fail(c, ANM_E_ARG, "trace: phantom uses material %u but the electron tables hold %d", c->max_material, c->e_nm);
+    std::vector<float> in(electrons, electrons + 7 * n);
+    for (size_t i = 0; i < n; ++i) {
+        float* e = in.data() + 7 * i;
+        e[0] *= 0.1f; e[1] *= 0.1f; e[2] *= 0.1f;       // mm -> cm
+        if (!(e[0] >= 0 && e[0] < c->nx * c->dx && e[1] >= 0 && e[1] < c->ny * c->dy && e[2] >= 0 && e[2] < c->nz * c->dz))
+            return fail(c, ANM_E_ARG, "trace: electron %zu starts outside the grid", i);
+        if (!(e[6] > c->e_tmin) || !(e[6] <= c->e_tmin + c->e_dt * (c->e_nt - 1))) return fail(c, ANM_E_ARG, "trace: electron %zu energy outside the table", i);
+        const double n2 = (double)e[3] * e[3] + (double)e[4] * e[4] + (double)e[5] * e[5];
+        if (!(std::fabs(n2 - 1.0) < 1e-3)) return fail(c, ANM_E_ARG, "trace: electron %zu direction is not a unit vector", i);
+    }
+    ANM_CUDA(c, cudaSetDevice(c->device));
+    DevBuf<float> d_in, d_vol;
+    DevBuf<double> d_esc;
+    struct Rel { DevBuf<float>&a, &b; DevBuf<double>& d; ~Rel() { a.release(); b.release(); d.release(); } } rel{d_in, d_vol, d_esc};
+    ANM_CUDA(c, d_in.alloc(in.size()));
+    ANM_CUDA(c, d_vol.alloc(c->Vpad));
+    ANM_CUDA(c, d_esc.alloc(1));
+    ANM_CUDA(c, cudaMemcpyAsync(d_in.p, in.data(), in.size() * 4, cudaMemcpyHostToDevice, c->stream));
+    ANM_CUDA(c, cudaMemsetAsync(d_vol.p, 0, c->Vpad * 4, c->stream));
+    ANM_CUDA(c, cudaMemsetAsync(d_esc.p, 0, 8, c->stream));
+    TransportParams p;
+    std::memset(&p, 0, sizeof p);
+    p.texels = c->texels.p; p.batch = d_vol.p;
+    p.nx = c->nx; p.ny = c->ny; p.nz = c->nz;
+    p.dx = (float)c->dx; p.dy = (float)c->dy; p.dz = (float)c->dz;
+    p.inv_dx = (float)(1.0 / c->dx); p.inv_dy = (float)(1.0 / c->dy); p.inv_dz = (float)(1.0 / c->dz);
+    fill_electron_params(c, p);
+    electron_trace_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(p, d_in.p, (unsigned)n, d_esc.p);
+    ANM_CUDA(c, cudaGetLastError());
+    ANM_CUDA(c, cudaMemcpyAsync(out_MeV, d_vol.p, c->V * 4, cudaMemcpyDeviceToHost, c->stream));
+    ANM_CUDA(c, cudaMemcpyAsync(escaped_MeV, d_esc.p, 8, cudaMemcpyDeviceToHost, c->stream));
+    ANM_CUDA(c, cudaStreamSynchronize(c->stream));
+    return ANM_OK;
+}
+
 int anm_set_options(anm_ctx* c, const anm_options* o) {
     if (!c) return ANM_E_ARG;
     if (!o) return fail(c, ANM_E_ARG, "options: null pointer");
@@ -848,6 +928,8 @@ int anm_set_options(anm_ctx* c, const anm_options* o) {
     if (o->schedule < 0 || o->schedule > 2) return fail(c, ANM_E_ARG, "options: schedule must be 0, 1 or 2");
     if (o->hull_majorant < 0 || o->hull_majorant > 2) return fail(c, ANM_E_ARG, "options: hull_majorant must be 0, 1 or 2");
     if (o->schedule == 2 && o->warp_aggregate) return fail(c, ANM_E_UNSUPPORTED, "options: warp_aggregate is a schedule-1 option");
+    if (o->electron_transport != 0 && o->electron_transport != 1) return fail(c, ANM_E_ARG, "options: electron_transport must be 0 or 1");
+    if (o->electron_transport && o->schedule == 1) return fail(c, ANM_E_UNSUPPORTED, "options: electron transport runs in the event-pool schedule (0 or 2)");
     c->opt = *o;
     c->dev_tables_dirty = true;
     c->have_results = false;
@@ -866,6 +948,10 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     if (nb > 0x7fffffffull) return fail(c, ANM_E_ARG, "run: more than 2^31 decays per batch");
     if ((int)c->max_material >= c->nm) return fail(c, ANM_E_ARG, "run: phantom uses material %u but the tables hold %d", c->max_material, c->nm);
     if (std::exp(c->lnE_min) > c->opt.photon_cutoff_MeV * (1 + 1e-9)) return fail(c, ANM_E_ARG, "run: energy grid starts above the photon cutoff");
+    if (c->opt.electron_transport) {
+        if (!c->have_etables) return fail(c, ANM_E_STATE, "run: electron_transport needs anm_set_electron_tables");
+        if ((int)c->max_material >= c->e_nm) return fail(c, ANM_E_ARG, "run: phantom uses material %u but the electron tables hold %d", c->max_material, c->e_nm);
+    }
     ANM_CUDA(c, cudaSetDevice(c->device));
     c->have_results = false;
     if (c->dev_tables_dirty) { const int rc = upload_tables(c); if (rc != ANM_OK) return rc; }
@@ -900,6 +986,7 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     p.point_source = c->point_source ? 1 : 0;
     p.photons_per_decay = c->opt.photons_per_decay; p.rayleigh_on = c->opt.rayleigh_on;
     p.tab_maj_out = c->d_majo.p;
+    fill_electron_params(c, p);
     p.hull = (c->hull_ok && c->opt.hull_majorant != 2) ? 1 : 0;
     if (p.hull) {
         p.hx0 = (int)c->hull_lo[0]; p.hy0 = (int)c->hull_lo[1]; p.hz0 = (int)c->hull_lo[2];
@@ -917,7 +1004,8 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     const int threads = schedule == 2 ? kPoolThreads : kThreads;
     const size_t smem = smem_tables + (schedule == 2 ? (size_t)kPoolWarps * kPoolWarpBytes : (size_t)6 * kThreads * 4);
     const bool S = c->opt.collect_stats != 0, W = c->opt.warp_aggregate != 0;
-    const TransportFn kern = pick_transport(schedule, S, W);
+    const bool EL = c->opt.electron_transport != 0;
+    const TransportFn kern = pick_transport(schedule, S, W, EL);
     ANM_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 0;
     ANM_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem));
@@ -976,7 +1064,7 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     s.deposited_MeV = tot_e;
     s.escaped_MeV = ds.escaped_MeV;
     s.n_steps = ds.n_steps; s.n_real = ds.n_real; s.n_pe = ds.n_pe; s.n_compton = ds.n_compton;
-    s.n_rayleigh = ds.n_rayleigh; s.n_escaped = ds.n_escaped; s.n_cutoff = ds.n_cutoff;
+    s.n_rayleigh = ds.n_rayleigh; s.n_escaped = ds.n_escaped; s.n_cutoff = ds.n_cutoff; s.n_electrons = ds.n_electrons;
     s.ms_transport = ms_t; s.ms_fold = ms_f; s.ms_finalize = ms_fin; s.ms_setup = c->ms_setup;
     s.ms_load_ct = c->ms_load_ct; s.ms_load_pet = c->ms_load_pet;
     s.n_launches = (uint64_t)2 * B + 1;
@@ -1058,7 +1146,7 @@ int anm_merge(anm_ctx* c, uint64_t total_decays, int total_batches, const double
     if (rc != ANM_OK) { c->have_results = false; return rc; }
     anm_stats& s = c->stats;
     const double dep = s.deposited_MeV;
-    if (summed) s = *summed; else { s = mine; s.escaped_MeV = 0; s.n_steps = s.n_real = s.n_pe = s.n_compton = s.n_rayleigh = s.n_escaped = s.n_cutoff = 0; }
+    if (summed) s = *summed; else { s = mine; s.escaped_MeV = 0; s.n_steps = s.n_real = s.n_pe = s.n_compton = s.n_rayleigh = s.n_escaped = s.n_cutoff = s.n_electrons = 0; }
     s.n_launches += 1;     // the finalize launch of the merge
     s.n_decays = total_decays;
     s.emitted_MeV = (double)total_decays * ((double)kE0 * c->opt.photons_per_decay + c->opt.positron_ke_MeV);

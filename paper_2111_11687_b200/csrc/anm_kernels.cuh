@@ -45,7 +45,7 @@ enum : int { ST_NEED = 0, ST_SOURCE = 1, ST_FLY = 2, ST_COMPTON = 3, ST_RAYLEIGH
 
 struct DeviceStats {   // accumulated with atomics at kernel exit (collect_stats only)
     double escaped_MeV;
-    unsigned long long n_steps, n_real, n_pe, n_compton, n_rayleigh, n_escaped, n_cutoff;
+    unsigned long long n_steps, n_real, n_pe, n_compton, n_rayleigh, n_escaped, n_cutoff, n_electrons;
 };
 
 struct TransportParams {
@@ -79,6 +79,11 @@ struct TransportParams {
     int hull;
     int hx0, hy0, hz0, hnx, hny, hnz;         // the box in voxel indices: [hx0, hx0 + hnx) x ...
     const float* tab_maj_out;    // [ne]
+    // secondary-electron transport (anm_options.electron_transport; reading C28): residual CSDA range above
+    // the electron cutoff, [nm][n_t] g/cm^2 on the kinetic-energy grid t_min + k dt; t_min = the cutoff
+    const float* e_range;
+    int n_t;
+    float t_min, e_dt, e_inv_dt;
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -293,6 +298,70 @@ __device__ __forceinline__ unsigned sample_source(const TransportParams& p, cons
     return voxel;
 }
 
+// ------------------------------------------------------------------------------------------------
+// Secondary electrons (electrons are followed down to a 200 keV cutoff, the rest is deposited locally;
+// DESIGN.md reading C28): continuous slowing down along a straight line.  r = R_m(T) is the residual mass range above
+// the cutoff (piecewise linear in T); a chord l through a voxel of density rho leaves r' = r - rho l and
+// T' = R_m^{-1}(r'); T - T' goes into the voxel; r' <= 0: the electron reaches the cutoff here and all of T is local.
+// Starts in voxel `vox` (the photon's collision voxel) at (x, y, z) with unit direction (ex, ey, ez).  Returns the
+// energy carried out of the grid.  No random numbers: photon histories are the same with and without it.
+__device__ __forceinline__ float e_range_of(const TransportParams& p, const float* __restrict__ R, float T, int& k) {
+    const float xq = fmaxf((T - p.t_min) * p.e_inv_dt, 0.0f);
+    k = min((int)xq, p.n_t - 2);
+    const float r0 = __ldg(R + k), r1 = __ldg(R + k + 1);
+    return fmaf(xq - (float)k, r1 - r0, r0);
+}
+
+__device__ __noinline__ float electron_walk(const TransportParams& p, float x, float y, float z, float ex, float ey, float ez,
+                                            unsigned vox, float T) {
+    const unsigned nxy = (unsigned)p.nx * (unsigned)p.ny;
+    int iz = (int)(vox / nxy);
+    const unsigned rem = vox - (unsigned)iz * nxy;
+    int iy = (int)(rem / (unsigned)p.nx), ix = (int)(rem - (unsigned)iy * (unsigned)p.nx);
+    const float inf = __int_as_float(0x7f800000);
+    // distance along the ray to the next face on each axis, and between faces
+    float tx = ex > 0.0f ? __fdividef((float)(ix + 1) * p.dx - x, ex) : (ex < 0.0f ? __fdividef((float)ix * p.dx - x, ex) : inf);
+    float ty = ey > 0.0f ? __fdividef((float)(iy + 1) * p.dy - y, ey) : (ey < 0.0f ? __fdividef((float)iy * p.dy - y, ey) : inf);
+    float tz = ez > 0.0f ? __fdividef((float)(iz + 1) * p.dz - z, ez) : (ez < 0.0f ? __fdividef((float)iz * p.dz - z, ez) : inf);
+    tx = fmaxf(tx, 0.0f); ty = fmaxf(ty, 0.0f); tz = fmaxf(tz, 0.0f);
+    const float dtx = ex != 0.0f ? fabsf(__fdividef(p.dx, ex)) : inf, dty = ey != 0.0f ? fabsf(__fdividef(p.dy, ey)) : inf,
+                dtz = ez != 0.0f ? fabsf(__fdividef(p.dz, ez)) : inf;
+    float t = 0.0f;
+    for (;;) {
+        const unsigned texel = __ldg(p.texels + vox);
+        const float rho = (float)(texel & 0xffffffu) * kDensityStep;
+        const float* R = p.e_range + (texel >> 24) * (unsigned)p.n_t;
+        const float t_next = fminf(tx, fminf(ty, tz));
+        int k;
+        const float r = e_range_of(p, R, T, k);
+        const float r_new = r - rho * (t_next - t);
+        if (!(r_new > 0.0f)) { atomicAdd(p.batch + vox, T); return 0.0f; }
+        while (k > 0 && __ldg(R + k) > r_new) --k;                 // segment with R[k] <= r_new < R[k+1]
+        const float r0 = __ldg(R + k), r1 = __ldg(R + k + 1);
+        const float T_new = fmaf((float)k + __fdividef(r_new - r0, r1 - r0), p.e_dt, p.t_min);
+        if (T > T_new) atomicAdd(p.batch + vox, T - T_new);
+        T = fminf(T, T_new);
+        t = t_next;
+        if (tx <= ty && tx <= tz) { ix += ex > 0.0f ? 1 : -1; tx += dtx; if ((unsigned)ix >= (unsigned)p.nx) return T; }
+        else if (ty <= tz) { iy += ey > 0.0f ? 1 : -1; ty += dty; if ((unsigned)iy >= (unsigned)p.ny) return T; }
+        else { iz += ez > 0.0f ? 1 : -1; tz += dtz; if ((unsigned)iz >= (unsigned)p.nz) return T; }
+        vox = (unsigned)ix + (unsigned)p.nx * ((unsigned)iy + (unsigned)p.ny * (unsigned)iz);
+    }
+}
+
+// inspection / parity hook (anm_trace_electrons): one given electron per thread, in = {x, y, z (cm), ex, ey, ez, T}
+__global__ void electron_trace_kernel(const __grid_constant__ TransportParams p, const float* __restrict__ in, unsigned n,
+                                      double* __restrict__ escaped) {
+    const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float* e = in + 7 * (size_t)i;
+    const float x = e[0], y = e[1], z = e[2];
+    const int ix = __float2int_rd(x * p.inv_dx), iy = __float2int_rd(y * p.inv_dy), iz = __float2int_rd(z * p.inv_dz);
+    const unsigned vox = (unsigned)ix + (unsigned)p.nx * ((unsigned)iy + (unsigned)p.ny * (unsigned)iz);
+    const float out = electron_walk(p, x, y, z, e[3], e[4], e[5], vox, e[6]);
+    if (out > 0.0f) atomicAdd(escaped, (double)out);
+}
+
 template <bool STATS, bool WAGG>
 __global__ void __launch_bounds__(kThreads, kMinBlocksPerSM)
 transport_kernel(const __grid_constant__ TransportParams p) {
@@ -470,7 +539,7 @@ enum : int { F_X = 0, F_Y, F_Z, F_U, F_V, F_W, F_E, F_TV /* FLY: ln-E grid coord
 enum : int { Q_F = 0, Q_C = 1, Q_S = 2, Q_R = 3, Q_NONE = 4 };
 constexpr size_t kPoolWarpBytes = (size_t)kSlotFields * kSlots * 4 + 4 * kSlots;   // slots + the four queues (bytes)
 
-template <bool STATS>
+template <bool STATS, bool ELEC>
 __global__ void __launch_bounds__(kPoolThreads, kPoolMinBlocksPerSM)
 transport_pool_kernel(const __grid_constant__ TransportParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -503,7 +572,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
     const float t_max = (float)(p.ne - 1) - 1.0f / 1024.0f;
 
     float esc = 0.0f;
-    unsigned c_pe = 0, c_co = 0, c_ra = 0, c_esc = 0, c_cut = 0;
+    unsigned c_pe = 0, c_co = 0, c_ra = 0, c_esc = 0, c_cut = 0, c_el = 0;
     FlyCounters fc = {0u, 0u};
 
     // Push every processed slot onto the ring of its next event (all 32 lanes call it; idle lanes pass Q_NONE):
@@ -595,7 +664,14 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                 SU[F_META * kSlots] = ended ? meta_end : meta_go;
                 if (coll) reinterpret_cast<unsigned*>(Bk)[F_TV * kSlots] = vox;
                 next = code == FLY_COMPTON ? Q_C : (code == FLY_RAYLEIGH ? Q_R : ((ended && !partner) ? Q_S : Q_F));
-                if (code == FLY_PE) { if (STATS) ++c_pe; atomicAdd(p.batch + vox, Bk[F_E * kSlots]); }      // all energy local
+                if (code == FLY_PE) {               // all energy to one electron: local, or transported along the photon's direction
+                    if (STATS) ++c_pe;
+                    const float Epe = Bk[F_E * kSlots];
+                    if (ELEC && Epe > p.t_min) {
+                        const float out = electron_walk(p, x, y, z, u, v, w, vox, Epe);
+                        if (STATS) { esc += out; ++c_el; }
+                    } else atomicAdd(p.batch + vox, Epe);
+                }
                 if (STATS && code == FLY_ESCAPED) { esc += Bk[F_E * kSlots]; ++c_esc; }
             }
             push_all(next, slot);
@@ -611,22 +687,36 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                 if (compton_try(E, r, eps, t)) {
                     if (STATS) ++c_co;
                     const unsigned vox = reinterpret_cast<unsigned*>(Bk)[F_TV * kSlots];
-                    float dep = E * (1.0f - eps);     // recoil electron deposited locally
+                    float dep = E * (1.0f - eps);     // recoil electron: deposited locally, or transported (ELEC)
+                    const bool walk = ELEC && dep > p.t_min;
+                    float u = 0.0f, v = 0.0f, w = 1.0f;
                     E *= eps;
-                    if (E < p.cutoff) {               // the rest is deposited locally
+                    const bool ends = E < p.cutoff;
+                    if (!ends || walk) {
+                        u = Bk[F_U * kSlots]; v = Bk[F_V * kSlots]; w = Bk[F_W * kSlots];
+                        const float u0 = u, v0 = v, w0 = w;
+                        rotate(u, v, w, 1.0f - t, kTwoPi * u01(r.w));
+                        if (walk) {                   // along the electron's momentum d - eps d' (photon momentum = E / c)
+                            float ex = fmaf(-eps, u, u0), ey = fmaf(-eps, v, v0), ez = fmaf(-eps, w, w0);
+                            const float n2 = fmaf(ex, ex, fmaf(ey, ey, ez * ez));
+                            if (n2 > 0.0f) { const float inv = rsqrtf(n2); ex *= inv; ey *= inv; ez *= inv; } else { ex = u0; ey = v0; ez = w0; }
+                            const float out = electron_walk(p, Bk[F_X * kSlots], Bk[F_Y * kSlots], Bk[F_Z * kSlots], ex, ey, ez, vox, dep);
+                            if (STATS) { esc += out; ++c_el; }
+                            dep = 0.0f;
+                        }
+                    }
+                    if (ends) {                       // the rest is deposited locally
                         dep += E;
                         if (STATS) ++c_cut;
                         photon_ends(meta);
                     } else {
-                        float u = Bk[F_U * kSlots], v = Bk[F_V * kSlots], w = Bk[F_W * kSlots];
-                        rotate(u, v, w, 1.0f - t, kTwoPi * u01(r.w));
                         Bk[F_U * kSlots] = u; Bk[F_V * kSlots] = v; Bk[F_W * kSlots] = w;
                         Bk[F_E * kSlots] = E;
                         Bk[F_TV * kSlots] = fminf(fmaxf((__logf(E) - p.lnE_min) * p.inv_dlnE, 0.0f), t_max);
                         SU[F_META * kSlots] = (meta & ~0x74u) + 256u;     // a scatter clears AWAY
                         next = Q_F;
                     }
-                    atomicAdd(p.batch + vox, dep);
+                    if (dep > 0.0f) atomicAdd(p.batch + vox, dep);
                 } else {
                     SU[F_META * kSlots] = meta + 256u;
                     next = Q_C;
@@ -690,6 +780,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
             c_ra += __shfl_xor_sync(0xffffffffu, c_ra, o);
             c_esc += __shfl_xor_sync(0xffffffffu, c_esc, o);
             c_cut += __shfl_xor_sync(0xffffffffu, c_cut, o);
+            c_el += __shfl_xor_sync(0xffffffffu, c_el, o);
         }
         if (lane == 0) {
             atomicAdd(&p.stats->escaped_MeV, (double)esc);
@@ -700,6 +791,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
             atomicAdd(&p.stats->n_rayleigh, (unsigned long long)c_ra);
             atomicAdd(&p.stats->n_escaped, (unsigned long long)c_esc);
             atomicAdd(&p.stats->n_cutoff, (unsigned long long)c_cut);
+            atomicAdd(&p.stats->n_electrons, (unsigned long long)c_el);
         }
     }
 }
