@@ -340,9 +340,33 @@ int flight_woodcock(const OrcProblem& p, const Xs& xs, double majorant, Rng& g, 
 struct Tally {
     double* batch;           // [V] energy of the current batch (MeV)
     double deposited;        // this history
+    // history-by-history scoring ("the corresponding uncertainty is evaluated using the history-by-
+    // history method (Walters et al., 2002)"), all null / unused unless requested:
+    double* hbh_sumsq;       // [V] sum over finished histories of X_h^2, X_h = energy history h left in the voxel
+    double* hbh_temp;        // [V] energy the voxel has received from the history last seen there
+    int64_t* hbh_last;       // [V] index of that history (-1: none yet)
+    int64_t history;         // the current history
 };
 
-inline void deposit(Tally& ty, int64_t v, double e) { ty.batch[v] += e; ty.deposited += e; }
+// Walters' bookkeeping: a voxel's per-history energy is accumulated in hbh_temp while the same history keeps hitting
+// it; the first hit by a NEW history closes the previous one: its square goes to hbh_sumsq.  (The sum of X_h itself
+// is the batch tally's sum.)  A final sweep closes what is still open (hbh_close).
+inline void deposit(Tally& ty, int64_t v, double e) {
+    ty.batch[v] += e;
+    ty.deposited += e;
+    if (ty.hbh_sumsq) {
+        if (ty.hbh_last[v] == ty.history) ty.hbh_temp[v] += e;
+        else {
+            ty.hbh_sumsq[v] += ty.hbh_temp[v] * ty.hbh_temp[v];
+            ty.hbh_temp[v] = e;
+            ty.hbh_last[v] = ty.history;
+        }
+    }
+}
+
+inline void hbh_close(Tally& ty, uint64_t V) {
+    for (uint64_t v = 0; v < V; ++v) { ty.hbh_sumsq[v] += ty.hbh_temp[v] * ty.hbh_temp[v]; ty.hbh_temp[v] = 0.0; }
+}
 
 struct Workspace {
     std::vector<double> rho_max;   // per material, for the Woodcock cross-check
@@ -601,8 +625,9 @@ int orc_electron_walk(const OrcProblem* p, const double* pos, const double* e, d
 //   organ_batch[B][n_organs+1] = sum over the organ's voxels of x_{b,i} / (rho_i V_vox)  (MeV/g); column 0 = unlabelled
 //   fc_dist/fc_dep[h1-h0]  first-collision distance (cm; -1 = escaped uncollided) and deposit of photon A (may be null)
 // Returns 0, or -1 on bad arguments.
+//   hbh_sumsq[V]           += sum over the histories of this call of X_{h,i}^2 (MeV^2), history-by-history (may be null)
 int orc_run(const OrcProblem* pp, uint64_t h0, uint64_t h1, double* sum, double* sumsq,
-            double* organ_batch, OrcStats* stats, double* fc_dist, double* fc_dep) {
+            double* organ_batch, OrcStats* stats, double* fc_dist, double* fc_dep, double* hbh_sumsq) {
     const OrcProblem& p = *pp;
     if (p.n_batches < 1 || p.n_total == 0 || p.n_total % (uint64_t)p.n_batches) return -1;
     const uint64_t nb = p.n_total / (uint64_t)p.n_batches;
@@ -621,7 +646,10 @@ int orc_run(const OrcProblem* pp, uint64_t h0, uint64_t h1, double* sum, double*
             ws.rho_max[p.material[v]] = std::fmax(ws.rho_max[p.material[v]], (double)p.density[v]);
 
     std::vector<double> batch(V, 0.0);
-    Tally ty{batch.data(), 0.0};
+    std::vector<double> hbh_acc, hbh_temp;
+    std::vector<int64_t> hbh_last;
+    if (hbh_sumsq) { hbh_acc.assign(V, 0.0); hbh_temp.assign(V, 0.0); hbh_last.assign(V, -1); }
+    Tally ty{batch.data(), 0.0, hbh_sumsq ? hbh_acc.data() : nullptr, hbh_temp.data(), hbh_last.data(), -1};
     OrcStats st;
     std::memset(&st, 0, sizeof st);
 
@@ -634,6 +662,7 @@ int orc_run(const OrcProblem* pp, uint64_t h0, uint64_t h1, double* sum, double*
             sample_source(p, g, pos, d, vox);
             double emitted = 0.0, escaped = 0.0;
             ty.deposited = 0.0;
+            ty.history = (int64_t)h;           // one decay (positron energy + both photons + their electrons) = one history
             if (p.positron_ke > 0.0) {   // constant positron kinetic energy deposited in the decay voxel (C10)
                 emitted += p.positron_ke;
                 deposit(ty, vox_index(p, vox), p.positron_ke);
@@ -664,6 +693,10 @@ int orc_run(const OrcProblem* pp, uint64_t h0, uint64_t h1, double* sum, double*
                 batch[v] = 0.0;
             }
         }
+    }
+    if (hbh_sumsq) {
+        hbh_close(ty, V);
+        for (uint64_t v = 0; v < V; ++v) hbh_sumsq[v] += hbh_acc[v];
     }
     if (stats) *stats = st;
     return 0;

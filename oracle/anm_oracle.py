@@ -100,7 +100,7 @@ def lib():
         L.orc_electron_walk.restype = C.c_int
         L.orc_electron_walk.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
         L.orc_run.restype = C.c_int
-        L.orc_run.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64] + [C.c_void_p] * 6
+        L.orc_run.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64] + [C.c_void_p] * 7
         _lib = L
     return _lib
 
@@ -188,8 +188,8 @@ class Oracle:
         self.tables = tables
 
     # ------------------------------------------------------------------ runs
-    def run(self, b0: int = 0, b1: int | None = None, first_collision: bool = False) -> dict:
-        """Run batches [b0, b1) in this process."""
+    def run(self, b0: int = 0, b1: int | None = None, first_collision: bool = False, hbh: bool = False) -> dict:
+        """Run batches [b0, b1) in this process.  hbh: also score sum over histories of X_h^2 per voxel (NEXT-4)."""
         b1 = self.n_batches if b1 is None else b1
         nb = self.n_decays // self.n_batches
         h0, h1 = b0 * nb, b1 * nb
@@ -200,7 +200,8 @@ class Oracle:
         fcd = np.zeros(h1 - h0, np.float64) if first_collision else None
         fce = np.zeros(h1 - h0, np.float64) if first_collision else None
         t0 = time.perf_counter()
-        rc = lib().orc_run(C.byref(self.p), h0, h1, _ptr(s), _ptr(q), _ptr(ob), C.byref(st), _ptr(fcd), _ptr(fce))
+        hq = np.zeros(self.V, np.float64) if hbh else None
+        rc = lib().orc_run(C.byref(self.p), h0, h1, _ptr(s), _ptr(q), _ptr(ob), C.byref(st), _ptr(fcd), _ptr(fce), _ptr(hq))
         dt = time.perf_counter() - t0
         if rc != 0:
             raise ValueError("orc_run: bad arguments (N %% B != 0, or range not on batch boundaries)")
@@ -208,26 +209,31 @@ class Oracle:
                "n_decays_run": h1 - h0}
         if first_collision:
             out["fc_dist"], out["fc_dep"] = fcd, fce
+        if hbh:
+            out["hbh_sumsq"] = hq
         return out
 
-    def run_parallel(self, n_procs: int | None = None) -> dict:
+    def run_parallel(self, n_procs: int | None = None, hbh: bool = False) -> dict:
         """All batches, split as whole batches over n_procs forked single-threaded processes."""
         n_procs = min(n_procs or os.cpu_count() or 1, self.n_batches)
         if n_procs <= 1:
-            r = self.run()
+            r = self.run(hbh=hbh)
             r["cores"] = 1
             return r
         ctx = mp.get_context("fork")
         V, B, no = self.V, self.n_batches, self.n_organs + 1
         sh_sum, sh_sq = ctx.RawArray("d", V), ctx.RawArray("d", V)
         sh_ob = ctx.RawArray("d", B * no)
+        sh_hq = ctx.RawArray("d", V) if hbh else None
         lock = ctx.Lock()
         qout = ctx.Queue()
         bounds = np.linspace(0, B, n_procs + 1).astype(int)
 
         def work(i):
-            r = self.run(int(bounds[i]), int(bounds[i + 1]))
+            r = self.run(int(bounds[i]), int(bounds[i + 1]), hbh=hbh)
             with lock:
+                if hbh:
+                    np.frombuffer(sh_hq, np.float64)[:] += r["hbh_sumsq"]
                 np.frombuffer(sh_sum, np.float64)[:] += r["sum"]
                 np.frombuffer(sh_sq, np.float64)[:] += r["sumsq"]
                 np.frombuffer(sh_ob, np.float64)[:] += r["organ_batch"].reshape(-1)
@@ -243,10 +249,13 @@ class Oracle:
         wall = time.perf_counter() - t0
         stats = {k: (max(r[0][k] for r in res) if k == "max_history_residual" else sum(r[0][k] for r in res))
                  for k in res[0][0]}
-        return {"sum": np.frombuffer(sh_sum, np.float64).copy(), "sumsq": np.frombuffer(sh_sq, np.float64).copy(),
-                "organ_batch": np.frombuffer(sh_ob, np.float64).reshape(B, no).copy(), "stats": stats,
-                "seconds": wall, "cpu_seconds": sum(r[1] for r in res), "cores": n_procs,
-                "n_decays_run": self.n_decays}
+        out = {"sum": np.frombuffer(sh_sum, np.float64).copy(), "sumsq": np.frombuffer(sh_sq, np.float64).copy(),
+               "organ_batch": np.frombuffer(sh_ob, np.float64).reshape(B, no).copy(), "stats": stats,
+               "seconds": wall, "cpu_seconds": sum(r[1] for r in res), "cores": n_procs,
+               "n_decays_run": self.n_decays}
+        if hbh:
+            out["hbh_sumsq"] = np.frombuffer(sh_hq, np.float64).copy()
+        return out
 
     # ------------------------------------------------------------------ electron pins
     def electron_range(self, m: int, T: float) -> float:
@@ -277,6 +286,10 @@ class Oracle:
         s_abs = np.sqrt(np.maximum(var, 0.0))                                  # standard error of ybar
         rel = np.divide(s_abs, ybar, out=np.zeros_like(S), where=ybar > 0)
         out = {"energy": S, "dose": dose, "rel_sigma": rel, "dose_sigma": dose * rel}
+        if "hbh_sumsq" in r:
+            # history-by-history (Walters et al. 2002): s^2 of the mean = (sum X^2 / N - (sum X / N)^2) / (N - 1)
+            var_h = (r["hbh_sumsq"] / N - ybar * ybar) / (N - 1.0)
+            out["rel_sigma_hbh"] = np.divide(np.sqrt(np.maximum(var_h, 0.0)), ybar, out=np.zeros_like(S), where=ybar > 0)
         if total_activity_bq is not None:
             out["dose_rate"] = dose * total_activity_bq                        # Eq. 1
         if self.labels is not None and self.n_organs > 0:
