@@ -94,7 +94,12 @@ typedef struct {
     int32_t electron_transport; /* 0: secondary electrons deposited where they are set free (north_star);
                                    1: Compton / photo-electrons above the electron cutoff are transported
                                    (needs anm_set_electron_tables; schedule 0 or 2 only)      */
-    int32_t reserved0;
+    int32_t uncertainty;        /* 0: batch method (north_star; reading C1);
+                                   1: history by history, the paper's estimator (Walters et al. 2002):
+                                      one decay = one history, X_h = the energy it leaves in a voxel,
+                                      s^2 of the mean = (sum X_h^2 / N - (sum X_h / N)^2) / (N - 1).  anm_get_uncertainty
+                                      and the organs' Eq. 3 value then use it; the organ sigma_mean stays the batch
+                                      one.  Schedule 0 or 2, without electron_transport; not mergeable (anm_merge). */
 } anm_options;
 
 /* Electron data for anm_options.electron_transport ("The cutoff energies for
@@ -127,6 +132,7 @@ typedef struct {
     double emitted_MeV, deposited_MeV, escaped_MeV;   /* escaped and the counters need collect_stats   */
     uint64_t n_decays, n_steps, n_real, n_pe, n_compton, n_rayleigh, n_escaped, n_cutoff;
     uint64_t n_electrons;                                  /* electrons transported (collect_stats)         */
+    uint64_t n_hbh_overflow;                               /* decays whose deposit list was merged early (uncertainty = 1, collect_stats; expected 0) */
     double ms_transport, ms_fold, ms_finalize, ms_setup;   /* device time of the last anm_run / last setup */
     uint64_t n_launches;                                   /* kernels launched by the last anm_run         */
     double ms_load_ct, ms_load_pet;                        /* device time of the last anm_load_ct / anm_load_pet

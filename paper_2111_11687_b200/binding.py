@@ -44,7 +44,7 @@ class anm_options(C.Structure):
                 ("zero_air_dose", C.c_int32), ("photon_cutoff_MeV", C.c_double), ("positron_ke_MeV", C.c_double),
                 ("schedule", C.c_int32), ("collect_stats", C.c_int32), ("warp_aggregate", C.c_int32),
                 ("hull_majorant", C.c_int32), ("history_offset", C.c_uint64),
-                ("electron_transport", C.c_int32), ("reserved0", C.c_int32)]
+                ("electron_transport", C.c_int32), ("uncertainty", C.c_int32)]
 
 
 class anm_electron_tables(C.Structure):
@@ -60,7 +60,7 @@ class anm_organ(C.Structure):
 
 class anm_stats(C.Structure):
     _fields_ = [("emitted_MeV", C.c_double), ("deposited_MeV", C.c_double), ("escaped_MeV", C.c_double)] + [
-        (n, C.c_uint64) for n in ("n_decays", "n_steps", "n_real", "n_pe", "n_compton", "n_rayleigh", "n_escaped", "n_cutoff", "n_electrons")] + [
+        (n, C.c_uint64) for n in ("n_decays", "n_steps", "n_real", "n_pe", "n_compton", "n_rayleigh", "n_escaped", "n_cutoff", "n_electrons", "n_hbh_overflow")] + [
         ("ms_transport", C.c_double), ("ms_fold", C.c_double), ("ms_finalize", C.c_double), ("ms_setup", C.c_double),
         ("n_launches", C.c_uint64), ("ms_load_ct", C.c_double), ("ms_load_pet", C.c_double)]
 

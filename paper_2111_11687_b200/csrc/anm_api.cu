@@ -83,6 +83,9 @@ struct anm_ctx {
     // device memory
     DevBuf<uint32_t> texels;
     DevBuf<float> batch, sum, sumsq, scratch;
+    DevBuf<float> hbh_sq;                 // [Vpad] sum over histories of X_h^2 (anm_options.uncertainty = 1)
+    DevBuf<uint2> hbh_list;               // [(kHbhCap + 1) * hbh_nslots] per-slot deposit lists
+    bool run_hbh = false;                 // the last run scored history by history
     DevBuf<uint8_t> labels;
     DevBuf<uint4> alias;
     DevBuf<unsigned> counters;
@@ -270,10 +273,12 @@ struct HostE0 { int ie; float fe, maj, inv_maj; };
 using TransportFn = void (*)(const TransportParams);
 
 // schedule 1 (history-based lanes) or 2 (warp-scope event pool), with / without counters and warp aggregation
-TransportFn pick_transport(int schedule, bool stats, bool wagg, bool elec) {
-    if (schedule == 2)
-        return elec ? (stats ? transport_pool_kernel<true, true> : transport_pool_kernel<false, true>)
-                    : (stats ? transport_pool_kernel<true, false> : transport_pool_kernel<false, false>);
+TransportFn pick_transport(int schedule, bool stats, bool wagg, bool elec, bool hbh) {
+    if (schedule == 2) {
+        if (hbh) return stats ? transport_pool_kernel<true, false, true> : transport_pool_kernel<false, false, true>;
+        return elec ? (stats ? transport_pool_kernel<true, true, false> : transport_pool_kernel<false, true, false>)
+                    : (stats ? transport_pool_kernel<true, false, false> : transport_pool_kernel<false, false, false>);
+    }
     return stats ? (wagg ? transport_kernel<true, true> : transport_kernel<true, false>)
                  : (wagg ? transport_kernel<false, true> : transport_kernel<false, false>);
 }
@@ -286,8 +291,8 @@ int finalize_and_collect(anm_ctx* c, int B, uint64_t nb, uint64_t n_decays, cons
     ANM_CUDA(c, cudaMemsetAsync(c->organ_acc.p, 0, 256 * sizeof(OrganAccum), st));
     ANM_CUDA(c, cudaMemsetAsync(c->total_energy.p, 0, 8, st));
     finalize_kernel<<<grid_blocks(c, c->V, kFoldThreads), kFoldThreads, 0, st>>>(
-        c->sum.p, c->sumsq.p, c->have_organs ? c->labels.p : nullptr, c->organ_acc.p, c->total_energy.p,
-        c->n_organs, c->V, B);
+        c->sum.p, c->run_hbh ? c->hbh_sq.p : c->sumsq.p, c->have_organs ? c->labels.p : nullptr, c->organ_acc.p,
+        c->total_energy.p, c->n_organs, c->V, c->run_hbh ? (double)n_decays : (double)B);
     ANM_CUDA(c, cudaGetLastError());
     std::vector<double> ob;
     OrganAccum acc[256];
@@ -929,6 +934,9 @@ int anm_set_options(anm_ctx* c, const anm_options* o) {
     if (o->hull_majorant < 0 || o->hull_majorant > 2) return fail(c, ANM_E_ARG, "options: hull_majorant must be 0, 1 or 2");
     if (o->schedule == 2 && o->warp_aggregate) return fail(c, ANM_E_UNSUPPORTED, "options: warp_aggregate is a schedule-1 option");
     if (o->electron_transport != 0 && o->electron_transport != 1) return fail(c, ANM_E_ARG, "options: electron_transport must be 0 or 1");
+    if (o->uncertainty != 0 && o->uncertainty != 1) return fail(c, ANM_E_ARG, "options: uncertainty must be 0 (batch) or 1 (history by history)");
+    if (o->uncertainty == 1 && o->schedule == 1) return fail(c, ANM_E_UNSUPPORTED, "options: history-by-history scoring runs in the event-pool schedule (0 or 2)");
+    if (o->uncertainty == 1 && o->electron_transport) return fail(c, ANM_E_UNSUPPORTED, "options: history-by-history scoring with electron transport is not implemented");
     if (o->electron_transport && o->schedule == 1) return fail(c, ANM_E_UNSUPPORTED, "options: electron transport runs in the event-pool schedule (0 or 2)");
     c->opt = *o;
     c->dev_tables_dirty = true;
@@ -1005,7 +1013,8 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     const size_t smem = smem_tables + (schedule == 2 ? (size_t)kPoolWarps * kPoolWarpBytes : (size_t)6 * kThreads * 4);
     const bool S = c->opt.collect_stats != 0, W = c->opt.warp_aggregate != 0;
     const bool EL = c->opt.electron_transport != 0;
-    const TransportFn kern = pick_transport(schedule, S, W, EL);
+    const bool HB = c->opt.uncertainty == 1;
+    const TransportFn kern = pick_transport(schedule, S, W, EL, HB);
     ANM_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 0;
     ANM_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem));
@@ -1015,6 +1024,15 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     const int blocks = (int)std::max<uint64_t>(1, std::min<uint64_t>((uint64_t)c->num_sms * per_sm, (nb + per_block - 1) / per_block));
     const int fold_blocks = grid_blocks(c, c->Vpad / 4, kFoldThreads);
     const float inv_vox = (float)(1.0 / (c->dx * c->dy * c->dz));
+    c->run_hbh = HB;
+    if (HB) {   // history-by-history scoring: sum of X_h^2 over the whole run + one deposit list per decay slot
+        const size_t nslots = (size_t)blocks * kPoolWarps * kSlots;
+        ANM_CUDA(c, c->hbh_sq.alloc(c->Vpad));
+        ANM_CUDA(c, c->hbh_list.alloc((size_t)(kHbhCap + 1) * nslots));
+        ANM_CUDA(c, cudaMemsetAsync(c->hbh_sq.p, 0, c->Vpad * 4, st));
+        ANM_CUDA(c, cudaMemsetAsync(c->hbh_list.p, 0, nslots * sizeof(uint2), st));     // the counts
+        p.hbh_list = c->hbh_list.p; p.hbh_sq = c->hbh_sq.p; p.hbh_nslots = (unsigned)nslots;
+    }
 
     std::vector<cudaEvent_t> ev((size_t)2 * B + 2, nullptr);
     auto free_events = [&]() { for (auto e : ev) if (e) cudaEventDestroy(e); };
@@ -1065,6 +1083,7 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     s.escaped_MeV = ds.escaped_MeV;
     s.n_steps = ds.n_steps; s.n_real = ds.n_real; s.n_pe = ds.n_pe; s.n_compton = ds.n_compton;
     s.n_rayleigh = ds.n_rayleigh; s.n_escaped = ds.n_escaped; s.n_cutoff = ds.n_cutoff; s.n_electrons = ds.n_electrons;
+    s.n_hbh_overflow = ds.n_hbh_overflow;
     s.ms_transport = ms_t; s.ms_fold = ms_f; s.ms_finalize = ms_fin; s.ms_setup = c->ms_setup;
     s.ms_load_ct = c->ms_load_ct; s.ms_load_pet = c->ms_load_pet;
     s.n_launches = (uint64_t)2 * B + 1;
@@ -1084,7 +1103,8 @@ static int readout(anm_ctx* c, float* out, size_t n, int on_device, int mode, do
     if (!on_device) { ANM_CUDA(c, c->scratch.alloc(c->Vpad)); dst = c->scratch.p; }
     const double factor = kGyPerMeVPerGram * scale / ((double)c->run_decays * c->dx * c->dy * c->dz);
     readout_kernel<<<grid_blocks(c, c->V, kFoldThreads), kFoldThreads, 0, c->stream>>>(
-        c->sum.p, c->sumsq.p, c->texels.p, dst, c->V, mode, factor, c->run_batches, c->opt.zero_air_dose);
+        c->sum.p, c->run_hbh ? c->hbh_sq.p : c->sumsq.p, c->texels.p, dst, c->V, mode, factor,
+        c->run_hbh ? (double)c->run_decays : (double)c->run_batches, c->opt.zero_air_dose);
     ANM_CUDA(c, cudaGetLastError());
     if (!on_device) ANM_CUDA(c, cudaMemcpyAsync(out, dst, c->V * 4, cudaMemcpyDeviceToHost, c->stream));
     ANM_CUDA(c, cudaStreamSynchronize(c->stream));
@@ -1134,6 +1154,7 @@ int anm_get_tally_buffers(anm_ctx* c, float** d_sum, float** d_sumsq, size_t* n_
 int anm_merge(anm_ctx* c, uint64_t total_decays, int total_batches, const double* organ_rows_all, const anm_stats* summed) {
     if (!c) return ANM_E_ARG;
     if (!c->have_results) return fail(c, ANM_E_STATE, "merge: no completed run");
+    if (c->run_hbh) return fail(c, ANM_E_UNSUPPORTED, "merge: history-by-history runs are not merged (use the batch estimator across GPUs)");
     if (total_batches < c->run_batches || total_batches < 2 || total_decays == 0 || total_decays % (uint64_t)total_batches)
         return fail(c, ANM_E_ARG, "merge: total_decays must be a positive multiple of total_batches >= this run's batches");
     const uint64_t nb = c->run_decays / (uint64_t)c->run_batches;
@@ -1146,7 +1167,7 @@ int anm_merge(anm_ctx* c, uint64_t total_decays, int total_batches, const double
     if (rc != ANM_OK) { c->have_results = false; return rc; }
     anm_stats& s = c->stats;
     const double dep = s.deposited_MeV;
-    if (summed) s = *summed; else { s = mine; s.escaped_MeV = 0; s.n_steps = s.n_real = s.n_pe = s.n_compton = s.n_rayleigh = s.n_escaped = s.n_cutoff = s.n_electrons = 0; }
+    if (summed) s = *summed; else { s = mine; s.escaped_MeV = 0; s.n_steps = s.n_real = s.n_pe = s.n_compton = s.n_rayleigh = s.n_escaped = s.n_cutoff = s.n_electrons = s.n_hbh_overflow = 0; }
     s.n_launches += 1;     // the finalize launch of the merge
     s.n_decays = total_decays;
     s.emitted_MeV = (double)total_decays * ((double)kE0 * c->opt.photons_per_decay + c->opt.positron_ke_MeV);

@@ -45,7 +45,7 @@ enum : int { ST_NEED = 0, ST_SOURCE = 1, ST_FLY = 2, ST_COMPTON = 3, ST_RAYLEIGH
 
 struct DeviceStats {   // accumulated with atomics at kernel exit (collect_stats only)
     double escaped_MeV;
-    unsigned long long n_steps, n_real, n_pe, n_compton, n_rayleigh, n_escaped, n_cutoff, n_electrons;
+    unsigned long long n_steps, n_real, n_pe, n_compton, n_rayleigh, n_escaped, n_cutoff, n_electrons, n_hbh_overflow;
 };
 
 struct TransportParams {
@@ -84,6 +84,12 @@ struct TransportParams {
     const float* e_range;
     int n_t;
     float t_min, e_dt, e_inv_dt;
+    // history-by-history scoring (anm_options.uncertainty = 1, Walters et al. 2002): per decay slot a
+    // list of the decay's deposits {voxel, energy} in global scratch, hbh_list[i * hbh_nslots + slot], entry 0 =
+    // {count, -}; merged per voxel when the decay is complete: batch[v] += X, hbh_sq[v] += X^2
+    uint2* hbh_list;
+    float* hbh_sq;               // [V] sum over histories of X_h^2 (MeV^2), whole run
+    unsigned hbh_nslots;
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -512,6 +518,41 @@ transport_kernel(const __grid_constant__ TransportParams p) {
 }
 
 // ------------------------------------------------------------------------------------------------
+// History-by-history scoring.  X_h = the energy ONE decay (positron energy,
+// both photons) leaves in a voxel; the estimator needs sum_h X_h^2, so the deposits of a decay cannot go to the tally
+// one by one.  They are appended to the decay slot's list; when the decay is complete its list is merged per voxel
+// and each distinct voxel gets one RED into the batch tally (X) and one into hbh_sq (X^2).  A decay with more than
+// kHbhCap deposits is merged early (its X is then split in two; counted in n_hbh_overflow, expected 0).
+constexpr unsigned kHbhCap = 63;
+
+__device__ __forceinline__ void hbh_flush(const TransportParams& p, unsigned gslot) {
+    uint2* L = p.hbh_list + gslot;
+    const unsigned n = L[0].x;
+    for (unsigned i = 1; i <= n; ++i) {
+        const uint2 a = L[(size_t)i * p.hbh_nslots];
+        bool seen = false;
+        for (unsigned j = 1; j < i; ++j) seen = seen || (L[(size_t)j * p.hbh_nslots].x == a.x);
+        if (seen) continue;
+        float X = __uint_as_float(a.y);
+        for (unsigned j = i + 1; j <= n; ++j) {
+            const uint2 b = L[(size_t)j * p.hbh_nslots];
+            if (b.x == a.x) X += __uint_as_float(b.y);
+        }
+        atomicAdd(p.batch + a.x, X);
+        atomicAdd(p.hbh_sq + a.x, X * X);
+    }
+    L[0].x = 0u;
+}
+
+__device__ __forceinline__ void hbh_push(const TransportParams& p, unsigned gslot, unsigned vox, float e, unsigned& overflow) {
+    uint2* L = p.hbh_list + gslot;
+    unsigned n = L[0].x;
+    if (n == kHbhCap) { hbh_flush(p, gslot); ++overflow; n = 0u; }
+    L[(size_t)(n + 1u) * p.hbh_nslots] = make_uint2(vox, __float_as_uint(e));
+    L[0].x = n + 1u;
+}
+
+// ------------------------------------------------------------------------------------------------
 // Schedule 2: event-based at warp scope.  Each warp owns kSlots decay slots in shared memory (SoA, one word per
 // field per slot; two banks of photon state, bank 0 = photon A, bank 1 = photon B, both written at the decay) and
 // four ring queues of slot numbers, one per event type (FLY, COMPTON, SOURCE = free, RAYLEIGH).  A trip: pick the
@@ -539,7 +580,7 @@ enum : int { F_X = 0, F_Y, F_Z, F_U, F_V, F_W, F_E, F_TV /* FLY: ln-E grid coord
 enum : int { Q_F = 0, Q_C = 1, Q_S = 2, Q_R = 3, Q_NONE = 4 };
 constexpr size_t kPoolWarpBytes = (size_t)kSlotFields * kSlots * 4 + 4 * kSlots;   // slots + the four queues (bytes)
 
-template <bool STATS, bool ELEC>
+template <bool STATS, bool ELEC, bool HBH>
 __global__ void __launch_bounds__(kPoolThreads, kPoolMinBlocksPerSM)
 transport_pool_kernel(const __grid_constant__ TransportParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -572,8 +613,9 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
     const float t_max = (float)(p.ne - 1) - 1.0f / 1024.0f;
 
     float esc = 0.0f;
-    unsigned c_pe = 0, c_co = 0, c_ra = 0, c_esc = 0, c_cut = 0, c_el = 0;
+    unsigned c_pe = 0, c_co = 0, c_ra = 0, c_esc = 0, c_cut = 0, c_el = 0, c_ovf = 0;
     FlyCounters fc = {0u, 0u};
+    const unsigned gslot0 = (blockIdx.x * (unsigned)kPoolWarps + (threadIdx.x >> 5)) * (unsigned)kSlots;   // HBH: this warp's lists
 
     // Push every processed slot onto the ring of its next event (all 32 lanes call it; idle lanes pass Q_NONE):
     // one match groups the lanes by destination, the rank inside the group is the ring offset, one packed warp
@@ -670,10 +712,12 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                     if (ELEC && Epe > p.t_min) {
                         const float out = electron_walk(p, x, y, z, u, v, w, vox, Epe);
                         if (STATS) { esc += out; ++c_el; }
-                    } else atomicAdd(p.batch + vox, Epe);
+                    } else if (HBH) hbh_push(p, gslot0 + slot, vox, Epe, c_ovf);
+                    else atomicAdd(p.batch + vox, Epe);
                 }
                 if (STATS && code == FLY_ESCAPED) { esc += Bk[F_E * kSlots]; ++c_esc; }
             }
+            if (HBH && next == Q_S) hbh_flush(p, gslot0 + slot);      // the decay is complete: merge its deposits per voxel
             push_all(next, slot);
         } else if (X == Q_C) {
             if (active) {
@@ -716,12 +760,13 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                         SU[F_META * kSlots] = (meta & ~0x74u) + 256u;     // a scatter clears AWAY
                         next = Q_F;
                     }
-                    if (dep > 0.0f) atomicAdd(p.batch + vox, dep);
+                    if (dep > 0.0f) { if (HBH) hbh_push(p, gslot0 + slot, vox, dep, c_ovf); else atomicAdd(p.batch + vox, dep); }
                 } else {
                     SU[F_META * kSlots] = meta + 256u;
                     next = Q_C;
                 }
             }
+            if (HBH && next == Q_S) hbh_flush(p, gslot0 + slot);      // the decay is complete: merge its deposits per voxel
             push_all(next, slot);
         } else if (X == Q_S) {
             if (active) {
@@ -738,7 +783,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                 B1[F_E * kSlots] = kE0; B1[F_TV * kSlots] = t0;
                 SU[F_HL * kSlots] = hl_new;
                 SU[F_META * kSlots] = in_box ? (2u | 8u) : 0u;
-                if (p.positron_ke > 0.0f) atomicAdd(p.batch + voxel, p.positron_ke);
+                if (p.positron_ke > 0.0f) { if (HBH) hbh_push(p, gslot0 + slot, voxel, p.positron_ke, c_ovf); else atomicAdd(p.batch + voxel, p.positron_ke); }
                 q[Q_F * kSlots + ((heads + cnts + lane) & (kSlots - 1))] = (unsigned char)slot;
             }
             cnts += n;
@@ -781,6 +826,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
             c_esc += __shfl_xor_sync(0xffffffffu, c_esc, o);
             c_cut += __shfl_xor_sync(0xffffffffu, c_cut, o);
             c_el += __shfl_xor_sync(0xffffffffu, c_el, o);
+            c_ovf += __shfl_xor_sync(0xffffffffu, c_ovf, o);
         }
         if (lane == 0) {
             atomicAdd(&p.stats->escaped_MeV, (double)esc);
@@ -792,6 +838,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
             atomicAdd(&p.stats->n_escaped, (unsigned long long)c_esc);
             atomicAdd(&p.stats->n_cutoff, (unsigned long long)c_cut);
             atomicAdd(&p.stats->n_electrons, (unsigned long long)c_el);
+            atomicAdd(&p.stats->n_hbh_overflow, (unsigned long long)c_ovf);
         }
     }
 }
@@ -844,15 +891,17 @@ fold_kernel(float4* __restrict__ batch, float4* __restrict__ sum, float4* __rest
 // energy;  total deposited energy.  rel^2 = (B Q / S^2 - 1) / (B - 1)  (batch standard error of the mean / mean).
 struct OrganAccum { double rel2, n_nonzero, energy; };
 
-__device__ __forceinline__ float rel_sigma(float S, float Q, int B) {
+// (B, Q) = (batches, sum of squared batch sums), or for history-by-history scoring (histories, sum of X_h^2): the same
+// formula, PAPER.md:L67 / Walters et al. 2002.
+__device__ __forceinline__ float rel_sigma(float S, float Q, double B) {
     if (!(S > 0.0f)) return 0.0f;
-    const double r2 = ((double)B * (double)Q / ((double)S * (double)S) - 1.0) / (double)(B - 1);
+    const double r2 = (B * (double)Q / ((double)S * (double)S) - 1.0) / (B - 1.0);
     return r2 > 0.0 ? (float)sqrt(r2) : 0.0f;
 }
 
 __global__ void __launch_bounds__(kFoldThreads)
 finalize_kernel(const float* __restrict__ sum, const float* __restrict__ sumsq, const uint8_t* __restrict__ labels,
-                OrganAccum* __restrict__ organ, double* __restrict__ total_energy, int n_organs, size_t V, int B) {
+                OrganAccum* __restrict__ organ, double* __restrict__ total_energy, int n_organs, size_t V, double B) {
     __shared__ double s_rel2[256], s_nz[256], s_en[256];
     __shared__ double s_tot;
     s_rel2[threadIdx.x] = 0.0; s_nz[threadIdx.x] = 0.0; s_en[threadIdx.x] = 0.0;
@@ -907,7 +956,7 @@ organ_mass_kernel(const uint8_t* __restrict__ labels, const uint32_t* __restrict
 // read-out: mode 0 energy (MeV), 1 dose = S k / (N rho V) * scale (scale = 1 or A(t_s), Eq. 1), 2 relative sigma
 __global__ void __launch_bounds__(kFoldThreads)
 readout_kernel(const float* __restrict__ sum, const float* __restrict__ sumsq, const uint32_t* __restrict__ texels,
-               float* __restrict__ out, size_t V, int mode, double dose_factor /* k*scale/(N V_vox) */, int B, int zero_air) {
+               float* __restrict__ out, size_t V, int mode, double dose_factor /* k*scale/(N V_vox) */, double B, int zero_air) {
     for (size_t i = (size_t)blockIdx.x * kFoldThreads + threadIdx.x; i < V; i += (size_t)gridDim.x * kFoldThreads) {
         const float S = sum[i];
         float o;
