@@ -119,6 +119,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-frontend", action="store_true", help="skip the image front-end timing (anm_load_ct / anm_load_pet)")
+    ap.add_argument("--no-variants", action="store_true", help="skip the electron-transport / history-by-history runs")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -237,24 +238,28 @@ def main():
         hm, hr = torch.from_numpy(cfg["material"]).pin_memory(), torch.from_numpy(cfg["density"]).pin_memory()
         ha, hl = torch.from_numpy(cfg["activity"]).pin_memory(), torch.from_numpy(cfg["labels"]).pin_memory()
         out_d, out_u = torch.empty(V, dtype=torch.float32).pin_memory(), torch.empty(V, dtype=torch.float32).pin_memory()
+        def e2e_step():
+            with Simulation(local_rank) as s2:
+                s2.set_grid(cfg["shape"], cfg["spacing_mm"])
+                s2.load_phantom(hm, hr)
+                s2.load_activity(ha)
+                s2.load_organs(hl, cfg["n_organs"])
+                s2.set_physics_tables(tables)
+                s2.set_options(**opts)
+                step(s2)
+                s2.get_dose(out_d)
+                s2.get_uncertainty(out_u)
+                return s2.get_organ_doses(), s2.get_stats()
+
+        e2e_step()                                   # untimed: first-touch of the pinned buffers, allocator warm-up
         if dist:
             dist.barrier()
         torch.cuda.synchronize(dev)
         t0 = time.perf_counter()
-        with Simulation(local_rank) as s2:
-            s2.set_grid(cfg["shape"], cfg["spacing_mm"])
-            s2.load_phantom(hm, hr)
-            s2.load_activity(ha)
-            s2.load_organs(hl, cfg["n_organs"])
-            s2.set_physics_tables(tables)
-            s2.set_options(**opts)
-            step(s2)
-            s2.get_dose(out_d)
-            s2.get_uncertainty(out_u)
-            organs = s2.get_organ_doses()
-            st2 = s2.get_stats()
+        for _ in range(args.steps):                  # every step: full set-up from host buffers, run, read-back
+            organs, st2 = e2e_step()
         torch.cuda.synchronize(dev)
-        dt = time.perf_counter() - t0
+        dt = (time.perf_counter() - t0) / args.steps
         if dist:
             t = torch.tensor([dt], device=dev)
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -294,6 +299,22 @@ def main():
                     "load_pet_frac": b_pet / (min(ms_pet[1:]) * 1e-3) / 1e9 / hbm}
         del hu_d, pet_d
 
+    # ---- the widened rows on the same workload: 1e8 decays each, device time of anm_run ----
+    variants = None
+    if not args.no_variants and world == 1:
+        variants = {}
+        nv = min(D, 100_000_000)
+        with torch.cuda.stream(stream):
+            sim.set_electron_tables(anm_inputs.make_electron_tables())
+            for name, kw in (("default_same_size", {}), ("electron_transport", {"electron_transport": 1}), ("uncertainty_hbh", {"uncertainty": 1})):
+                sim.set_options(collect_stats=0, **opts, **kw)
+                sim.run(nv, cfg["seed"])                      # warm-up (first launch of this kernel variant)
+                sim.run(nv, cfg["seed"])
+                stv = sim.get_stats()
+                ms = stv["ms_transport"] + stv["ms_fold"] + stv["ms_finalize"]
+                variants[name] = {"decays": nv, "ms": ms, "value": nv / (ms * 1e-3), "unit": "decays/s"}
+            sim.set_options(collect_stats=0, **opts)
+
     if rank != 0:
         if dist:
             dist.destroy_process_group()
@@ -321,7 +342,7 @@ def main():
                    "multi_gpu": "one logical run of N*D decays: whole-batch shards via history_offset, NCCL sum-all-reduce of the tallies + merged finalize at the end of every step" if world > 1 else "single GPU"},
         "clocks": clk, "e2e": e2e, "gpu_launches": int(launches),
         "phase_ms_per_step": {"transport": ms_t / args.steps, "fold": ms_f / args.steps, "finalize": ms_fin / args.steps},
-        "roofline": roofline, "cpu_baseline": cpu, "frontend": frontend,
+        "roofline": roofline, "cpu_baseline": cpu, "frontend": frontend, "variants": variants,
         "paper_context": "ARCHER-NM on a Titan V: 1e9 decays in <0.5 min (>=3.3e7 decays/s), GATE 376 min (PAPER.md:L117); other hardware, other phantom, electron transport on",
     }))
     if dist:

@@ -318,7 +318,7 @@ __device__ __forceinline__ float e_range_of(const TransportParams& p, const floa
     return fmaf(xq - (float)k, r1 - r0, r0);
 }
 
-__device__ __noinline__ float electron_walk(const TransportParams& p, float x, float y, float z, float ex, float ey, float ez,
+__device__ __forceinline__ float electron_walk(const TransportParams& p, float x, float y, float z, float ex, float ey, float ez,
                                             unsigned vox, float T) {
     const unsigned nxy = (unsigned)p.nx * (unsigned)p.ny;
     int iz = (int)(vox / nxy);
