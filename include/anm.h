@@ -100,6 +100,12 @@ typedef struct {
                                       s^2 of the mean = (sum X_h^2 / N - (sum X_h / N)^2) / (N - 1).  anm_get_uncertainty
                                       and the organs' Eq. 3 value then use it; the organ sigma_mean stays the batch
                                       one.  Schedule 0 or 2, without electron_transport; not mergeable (anm_merge). */
+    int32_t batch_pipeline;     /* launch pipeline over batches: 0 auto (3), 1 serial (one launch at a time on the ctx
+                                   stream; per-launch ms_transport / ms_fold), 2 | 3: that many batch tallies and
+                                   internal streams, so that the CTAs of batch b+1 take over the SMs as those of batch
+                                   b drain; the same histories and tallies; then ms_transport covers the whole
+                                   pipeline (folds inside it) and ms_fold is 0.  Forced to 1 with uncertainty = 1.   */
+    int32_t reserved1;
 } anm_options;
 
 /* Electron data for anm_options.electron_transport ("The cutoff energies for

@@ -44,7 +44,8 @@ class anm_options(C.Structure):
                 ("zero_air_dose", C.c_int32), ("photon_cutoff_MeV", C.c_double), ("positron_ke_MeV", C.c_double),
                 ("schedule", C.c_int32), ("collect_stats", C.c_int32), ("warp_aggregate", C.c_int32),
                 ("hull_majorant", C.c_int32), ("history_offset", C.c_uint64),
-                ("electron_transport", C.c_int32), ("uncertainty", C.c_int32)]
+                ("electron_transport", C.c_int32), ("uncertainty", C.c_int32),
+                ("batch_pipeline", C.c_int32), ("reserved1", C.c_int32)]
 
 
 class anm_electron_tables(C.Structure):

@@ -83,6 +83,8 @@ struct anm_ctx {
     // device memory
     DevBuf<uint32_t> texels;
     DevBuf<float> batch, sum, sumsq, scratch;
+    DevBuf<float> batch2, batch3;         // extra batch tallies of the launch pipeline (anm_options.batch_pipeline)
+    cudaStream_t pipe[3] = {nullptr, nullptr, nullptr};   // internal streams of the pipeline, created on first use
     DevBuf<float> hbh_sq;                 // [Vpad] sum over histories of X_h^2 (anm_options.uncertainty = 1)
     DevBuf<uint2> hbh_list;               // [(kHbhCap + 1) * hbh_nslots] per-slot deposit lists
     bool run_hbh = false;                 // the last run scored history by history
@@ -376,7 +378,9 @@ int anm_destroy(anm_ctx* c) {
     c->labels.release(); c->alias.release(); c->counters.release(); c->dstats.release();
     c->organ_batch.release(); c->organ_acc.release(); c->organ_mass.release(); c->organ_count.release();
     c->total_energy.release(); c->d_tot.release(); c->d_maj.release(); c->d_majo.release(); c->d_x2.release(); c->d_cum.release();
-    c->d_pec.release(); c->d_flags.release();
+    c->d_pec.release(); c->d_flags.release(); c->d_erange.release(); c->hbh_sq.release(); c->hbh_list.release();
+    c->batch2.release(); c->batch3.release();
+    for (auto& ps : c->pipe) if (ps) { cudaStreamDestroy(ps); ps = nullptr; }
     delete c;
     return ANM_OK;
 }
@@ -934,6 +938,7 @@ int anm_set_options(anm_ctx* c, const anm_options* o) {
     if (o->hull_majorant < 0 || o->hull_majorant > 2) return fail(c, ANM_E_ARG, "options: hull_majorant must be 0, 1 or 2");
     if (o->schedule == 2 && o->warp_aggregate) return fail(c, ANM_E_UNSUPPORTED, "options: warp_aggregate is a schedule-1 option");
     if (o->electron_transport != 0 && o->electron_transport != 1) return fail(c, ANM_E_ARG, "options: electron_transport must be 0 or 1");
+    if (o->batch_pipeline < 0 || o->batch_pipeline > 3) return fail(c, ANM_E_ARG, "options: batch_pipeline must be 0 (auto), 1, 2 or 3");
     if (o->uncertainty != 0 && o->uncertainty != 1) return fail(c, ANM_E_ARG, "options: uncertainty must be 0 (batch) or 1 (history by history)");
     if (o->uncertainty == 1 && o->schedule == 1) return fail(c, ANM_E_UNSUPPORTED, "options: history-by-history scoring runs in the event-pool schedule (0 or 2)");
     if (o->uncertainty == 1 && o->electron_transport) return fail(c, ANM_E_UNSUPPORTED, "options: history-by-history scoring with electron transport is not implemented");
@@ -1034,25 +1039,53 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
         p.hbh_list = c->hbh_list.p; p.hbh_sq = c->hbh_sq.p; p.hbh_nslots = (unsigned)nslots;
     }
 
-    std::vector<cudaEvent_t> ev((size_t)2 * B + 2, nullptr);
+    std::vector<cudaEvent_t> ev((size_t)2 * B + 3, nullptr);   // [0] start, [2b+1] / [2b+2] before / after fold b, [2B+1] end, [2B+2] pipeline join
     auto free_events = [&]() { for (auto e : ev) if (e) cudaEventDestroy(e); };
     for (auto& e : ev) if (cudaEventCreate(&e) != cudaSuccess) { free_events(); return fail(c, ANM_E_CUDA, "cudaEventCreate failed"); }
 #define ANM_CUDA_EV(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { cudaGetLastError(); free_events(); \
         return fail(c, ANM_E_CUDA, "%s: %s", #call, cudaGetErrorString(e_)); } } while (0)
 
+    // Launch pipeline (anm_options.batch_pipeline): a transport launch is one resident wave of persistent CTAs, so its
+    // tail (the last decays draining, ~0.2 ms) leaves SMs idle.  With `depth` batch tallies the launches of
+    // consecutive batches go to `depth` internal streams: the CTAs of batch b+1 take over each SM as the CTAs of batch
+    // b exit, the fold of batch b runs in the gaps.  The folds are serialised among themselves (they all update sum /
+    // sumsq); batch b+depth reuses the tally of batch b after its fold (same stream).  Same histories, same tallies.
+    const int depth = HB ? 1 : std::max(1, std::min(c->opt.batch_pipeline == 0 ? 3 : c->opt.batch_pipeline, B));
+    float* bufs[3] = {c->batch.p, nullptr, nullptr};
+    if (depth > 1) {
+        ANM_CUDA_EV(c->batch2.alloc(c->Vpad));
+        ANM_CUDA_EV(cudaMemsetAsync(c->batch2.p, 0, c->Vpad * 4, st));
+        bufs[1] = c->batch2.p;
+        if (depth > 2) {
+            ANM_CUDA_EV(c->batch3.alloc(c->Vpad));
+            ANM_CUDA_EV(cudaMemsetAsync(c->batch3.p, 0, c->Vpad * 4, st));
+            bufs[2] = c->batch3.p;
+        }
+        for (int k = 0; k < depth; ++k)
+            if (!c->pipe[k]) ANM_CUDA_EV(cudaStreamCreateWithFlags(&c->pipe[k], cudaStreamNonBlocking));
+    }
     ANM_CUDA_EV(cudaEventRecord(ev[0], st));
+    if (depth > 1) for (int k = 0; k < depth; ++k) ANM_CUDA_EV(cudaStreamWaitEvent(c->pipe[k], ev[0], 0));
     for (int b = 0; b < B; ++b) {
+        cudaStream_t sb = depth > 1 ? c->pipe[b % depth] : st;
+        p.batch = bufs[b % depth];
         p.counter = c->counters.p + b;
         p.hist_base = c->opt.history_offset + (unsigned long long)b * nb;
-        kern<<<blocks, threads, smem, st>>>(p);
+        kern<<<blocks, threads, smem, sb>>>(p);
         ANM_CUDA_EV(cudaGetLastError());
-        ANM_CUDA_EV(cudaEventRecord(ev[2 * b + 1], st));
-        fold_kernel<<<fold_blocks, kFoldThreads, 0, st>>>(
-            (float4*)c->batch.p, (float4*)c->sum.p, (float4*)c->sumsq.p,
+        if (depth > 1 && b > 0) ANM_CUDA_EV(cudaStreamWaitEvent(sb, ev[2 * (b - 1) + 2], 0));    // after the previous fold
+        ANM_CUDA_EV(cudaEventRecord(ev[2 * b + 1], sb));
+        fold_kernel<<<fold_blocks, kFoldThreads, 0, sb>>>(
+            (float4*)p.batch, (float4*)c->sum.p, (float4*)c->sumsq.p,
             c->have_organs ? (const uint32_t*)c->labels.p : nullptr, (const uint4*)c->texels.p,
             c->organ_batch.p + (size_t)b * 256, c->n_organs, c->Vpad / 4, inv_vox);
         ANM_CUDA_EV(cudaGetLastError());
-        ANM_CUDA_EV(cudaEventRecord(ev[2 * b + 2], st));
+        ANM_CUDA_EV(cudaEventRecord(ev[2 * b + 2], sb));
+    }
+    if (depth > 1) {    // join: the caller's stream continues after the last fold (which follows every other launch)
+        ANM_CUDA_EV(cudaStreamWaitEvent(st, ev[2 * (B - 1) + 2], 0));
+        for (int b = std::max(0, B - depth); b < B - 1; ++b) ANM_CUDA_EV(cudaStreamWaitEvent(st, ev[2 * b + 2], 0));
+        ANM_CUDA_EV(cudaEventRecord(ev[2 * B + 2], st));
     }
     {
         const int rc = finalize_and_collect(c, B, nb, n_decays, nullptr);
@@ -1064,13 +1097,19 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     ANM_CUDA_EV(cudaStreamSynchronize(st));
 
     double ms_t = 0, ms_f = 0, ms_fin = 0;
-    for (int b = 0; b < B; ++b) {
+    if (depth > 1) {
+        // overlapped launches have no separate durations: the whole pipeline (transport with the folds inside it) is
+        // reported as transport time, conservatively; ms_fold = 0
+        float a = 0;
+        cudaEventElapsedTime(&a, ev[0], ev[2 * B + 2]);
+        ms_t = a;
+    } else for (int b = 0; b < B; ++b) {
         float a = 0, f = 0;
         cudaEventElapsedTime(&a, ev[2 * b], ev[2 * b + 1]);
         cudaEventElapsedTime(&f, ev[2 * b + 1], ev[2 * b + 2]);
         ms_t += a; ms_f += f;
     }
-    { float f = 0; cudaEventElapsedTime(&f, ev[2 * B], ev[2 * B + 1]); ms_fin = f; }
+    { float f = 0; cudaEventElapsedTime(&f, ev[depth > 1 ? 2 * B + 2 : 2 * B], ev[2 * B + 1]); ms_fin = f; }
     free_events();
 #undef ANM_CUDA_EV
 

@@ -34,7 +34,10 @@ namespace anm {
 
 constexpr int kThreads = 256;
 constexpr int kMinBlocksPerSM = 4;
-constexpr unsigned kChunk = 128;            // histories a warp takes per atomic
+#ifndef ANM_CHUNK
+#define ANM_CHUNK 128
+#endif
+constexpr unsigned kChunk = ANM_CHUNK;      // histories a warp takes per atomic (32 was measured slower: the refill atomic's latency shows)
 constexpr float kE0 = 0.51099895f;          // MeV, "0.511 MeV"
 constexpr float kInvE0 = 1.0f / 0.51099895f;
 constexpr float kTwoPi = 6.283185307179586f;
