@@ -31,7 +31,7 @@ def needs_build() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or needs_build():
         tmp = LIB + ".tmp.%d" % os.getpid()
-        extra = os.environ.get("ANM_NVCC_EXTRA", "").split()      # e.g. -DANM_SLOTS=128 -DANM_POOL_THREADS=512 (tuning experiments)
+        extra = os.environ.get("ANM_NVCC_EXTRA", "").split()      # e.g. -DANM_POOL_THREADS=768 -DANM_CHUNK=64 (tuning experiments)
         cmd = [nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
         subprocess.check_call(cmd)
         os.replace(tmp, LIB)
