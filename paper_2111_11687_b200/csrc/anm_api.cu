@@ -856,7 +856,7 @@ int anm_set_physics_tables(anm_ctx* c, const anm_tables* t) {
 // electron part of the kernel parameters (zeros when no tables are set)
 static void fill_electron_params(const anm_ctx* c, TransportParams& p) {
     p.e_range = c->have_etables ? c->d_erange.p : nullptr;
-    p.n_t = c->e_nt;
+    p.n_t = c->e_nt; p.e_nm = c->e_nm;
     p.t_min = (float)c->e_tmin; p.e_dt = (float)c->e_dt; p.e_inv_dt = c->e_dt > 0 ? (float)(1.0 / c->e_dt) : 0.0f;
 }
 
@@ -1015,7 +1015,8 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     const int schedule = c->opt.schedule == 0 ? kAutoSchedule : c->opt.schedule;
     const size_t smem_tables = (size_t)c->nm * c->ne * 12 + (size_t)c->ne * 8 + (size_t)c->n_x2 * 4 + (size_t)c->nm * c->n_x2 * 4;
     const int threads = schedule == 2 ? kPoolThreads : kThreads;
-    const size_t smem = smem_tables + (schedule == 2 ? (size_t)kPoolWarps * kPoolWarpBytes : (size_t)6 * kThreads * 4);
+    const size_t smem_el = (c->opt.electron_transport && schedule == 2) ? (size_t)c->e_nm * c->e_nt * 4 : 0;   // range tables
+    const size_t smem = smem_tables + smem_el + (schedule == 2 ? (size_t)kPoolWarps * kPoolWarpBytes : (size_t)6 * kThreads * 4);
     const bool S = c->opt.collect_stats != 0, W = c->opt.warp_aggregate != 0;
     const bool EL = c->opt.electron_transport != 0;
     const bool HB = c->opt.uncertainty == 1;

@@ -85,7 +85,7 @@ struct TransportParams {
     // secondary-electron transport (anm_options.electron_transport; reading C28): residual CSDA range above
     // the electron cutoff, [nm][n_t] g/cm^2 on the kinetic-energy grid t_min + k dt; t_min = the cutoff
     const float* e_range;
-    int n_t;
+    int n_t, e_nm;               // e_nm materials in the electron tables
     float t_min, e_dt, e_inv_dt;
     // history-by-history scoring (anm_options.uncertainty = 1, Walters et al. 2002): per decay slot a
     // list of the decay's deposits {voxel, energy} in global scratch, hbh_list[i * hbh_nslots + slot], entry 0 =
@@ -317,12 +317,13 @@ __device__ __forceinline__ unsigned sample_source(const TransportParams& p, cons
 __device__ __forceinline__ float e_range_of(const TransportParams& p, const float* __restrict__ R, float T, int& k) {
     const float xq = fmaxf((T - p.t_min) * p.e_inv_dt, 0.0f);
     k = min((int)xq, p.n_t - 2);
-    const float r0 = __ldg(R + k), r1 = __ldg(R + k + 1);
+    const float r0 = R[k], r1 = R[k + 1];
     return fmaf(xq - (float)k, r1 - r0, r0);
 }
 
-__device__ __forceinline__ float electron_walk(const TransportParams& p, float x, float y, float z, float ex, float ey, float ez,
-                                            unsigned vox, float T) {
+// `er` = the range tables [nm][n_t] (the transport kernel's shared-memory copy, or p.e_range).
+__device__ __forceinline__ float electron_walk(const TransportParams& p, const float* __restrict__ er, float x, float y, float z,
+                                            float ex, float ey, float ez, unsigned vox, float T) {
     const unsigned nxy = (unsigned)p.nx * (unsigned)p.ny;
     int iz = (int)(vox / nxy);
     const unsigned rem = vox - (unsigned)iz * nxy;
@@ -339,14 +340,14 @@ __device__ __forceinline__ float electron_walk(const TransportParams& p, float x
     for (;;) {
         const unsigned texel = __ldg(p.texels + vox);
         const float rho = (float)(texel & 0xffffffu) * kDensityStep;
-        const float* R = p.e_range + (texel >> 24) * (unsigned)p.n_t;
+        const float* R = er + (texel >> 24) * (unsigned)p.n_t;
         const float t_next = fminf(tx, fminf(ty, tz));
         int k;
         const float r = e_range_of(p, R, T, k);
         const float r_new = r - rho * (t_next - t);
         if (!(r_new > 0.0f)) { atomicAdd(p.batch + vox, T); return 0.0f; }
-        while (k > 0 && __ldg(R + k) > r_new) --k;                 // segment with R[k] <= r_new < R[k+1]
-        const float r0 = __ldg(R + k), r1 = __ldg(R + k + 1);
+        while (k > 0 && R[k] > r_new) --k;                         // segment with R[k] <= r_new < R[k+1]
+        const float r0 = R[k], r1 = R[k + 1];
         const float T_new = fmaf((float)k + __fdividef(r_new - r0, r1 - r0), p.e_dt, p.t_min);
         if (T > T_new) atomicAdd(p.batch + vox, T - T_new);
         T = fminf(T, T_new);
@@ -367,7 +368,7 @@ __global__ void electron_trace_kernel(const __grid_constant__ TransportParams p,
     const float x = e[0], y = e[1], z = e[2];
     const int ix = __float2int_rd(x * p.inv_dx), iy = __float2int_rd(y * p.inv_dy), iz = __float2int_rd(z * p.inv_dz);
     const unsigned vox = (unsigned)ix + (unsigned)p.nx * ((unsigned)iy + (unsigned)p.ny * (unsigned)iz);
-    const float out = electron_walk(p, x, y, z, e[3], e[4], e[5], vox, e[6]);
+    const float out = electron_walk(p, p.e_range, x, y, z, e[3], e[4], e[5], vox, e[6]);
     if (out > 0.0f) atomicAdd(escaped, (double)out);
 }
 
@@ -593,7 +594,9 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
     float* s_majo = s_maj + p.ne;                                   // [ne]
     float* s_x2 = s_majo + p.ne;                                    // [n_x2]
     float* s_cum = s_x2 + p.n_x2;                                   // [nm*n_x2]
-    unsigned char* s_pool = reinterpret_cast<unsigned char*>(s_cum + p.nm * p.n_x2);
+    float* s_er = s_cum + p.nm * p.n_x2;                            // [nm*n_t] electron range tables (ELEC only)
+    unsigned char* s_pool = reinterpret_cast<unsigned char*>(s_er + (ELEC ? p.e_nm * p.n_t : 0));
+    if (ELEC) for (int i = threadIdx.x; i < p.e_nm * p.n_t; i += kPoolThreads) s_er[i] = p.e_range[i];
     for (int i = threadIdx.x; i < p.nm * p.ne; i += kPoolThreads) { s_pec[i] = p.tab_pec[i]; s_tot[i] = p.tab_tot[i]; }
     for (int i = threadIdx.x; i < p.ne; i += kPoolThreads) { s_maj[i] = p.tab_maj[i]; s_majo[i] = p.tab_maj_out[i]; }
     for (int i = threadIdx.x; i < p.n_x2; i += kPoolThreads) s_x2[i] = p.ray_x2[i];
@@ -713,7 +716,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                     if (STATS) ++c_pe;
                     const float Epe = Bk[F_E * kSlots];
                     if (ELEC && Epe > p.t_min) {
-                        const float out = electron_walk(p, x, y, z, u, v, w, vox, Epe);
+                        const float out = electron_walk(p, s_er, x, y, z, u, v, w, vox, Epe);
                         if (STATS) { esc += out; ++c_el; }
                     } else if (HBH) hbh_push(p, gslot0 + slot, vox, Epe, c_ovf);
                     else atomicAdd(p.batch + vox, Epe);
@@ -747,7 +750,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                             float ex = fmaf(-eps, u, u0), ey = fmaf(-eps, v, v0), ez = fmaf(-eps, w, w0);
                             const float n2 = fmaf(ex, ex, fmaf(ey, ey, ez * ez));
                             if (n2 > 0.0f) { const float inv = rsqrtf(n2); ex *= inv; ey *= inv; ez *= inv; } else { ex = u0; ey = v0; ez = w0; }
-                            const float out = electron_walk(p, Bk[F_X * kSlots], Bk[F_Y * kSlots], Bk[F_Z * kSlots], ex, ey, ez, vox, dep);
+                            const float out = electron_walk(p, s_er, Bk[F_X * kSlots], Bk[F_Y * kSlots], Bk[F_Z * kSlots], ex, ey, ez, vox, dep);
                             if (STATS) { esc += out; ++c_el; }
                             dep = 0.0f;
                         }
