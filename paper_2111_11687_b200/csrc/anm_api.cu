@@ -1034,9 +1034,9 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     if (HB) {   // history-by-history scoring: sum of X_h^2 over the whole run + one deposit list per decay slot
         const size_t nslots = (size_t)blocks * kPoolWarps * kSlots;
         ANM_CUDA(c, c->hbh_sq.alloc(c->Vpad));
-        ANM_CUDA(c, c->hbh_list.alloc((size_t)(kHbhCap + 1) * nslots));
+        if (nb > (uint64_t)kHbhHistMask) return fail(c, ANM_E_UNSUPPORTED, "run: history-by-history scoring holds at most 2^26 decays per batch");
+        ANM_CUDA(c, c->hbh_list.alloc((size_t)kHbhCap * nslots));
         ANM_CUDA(c, cudaMemsetAsync(c->hbh_sq.p, 0, c->Vpad * 4, st));
-        ANM_CUDA(c, cudaMemsetAsync(c->hbh_list.p, 0, nslots * sizeof(uint2), st));     // the counts
         p.hbh_list = c->hbh_list.p; p.hbh_sq = c->hbh_sq.p; p.hbh_nslots = (unsigned)nslots;
     }
 

@@ -88,8 +88,8 @@ struct TransportParams {
     int n_t, e_nm;               // e_nm materials in the electron tables
     float t_min, e_dt, e_inv_dt;
     // history-by-history scoring (anm_options.uncertainty = 1, Walters et al. 2002): per decay slot a
-    // list of the decay's deposits {voxel, energy} in global scratch, hbh_list[i * hbh_nslots + slot], entry 0 =
-    // {count, -}; merged per voxel when the decay is complete: batch[v] += X, hbh_sq[v] += X^2
+    // list of the decay's deposits {voxel, energy} in global scratch, hbh_list[i * hbh_nslots + slot] (its length in the
+    // slot's shared-memory history word); merged per voxel when the slot is re-used: batch[v] += X, hbh_sq[v] += X^2
     uint2* hbh_list;
     float* hbh_sq;               // [V] sum over histories of X_h^2 (MeV^2), whole run
     unsigned hbh_nslots;
@@ -524,36 +524,38 @@ transport_kernel(const __grid_constant__ TransportParams p) {
 // ------------------------------------------------------------------------------------------------
 // History-by-history scoring.  X_h = the energy ONE decay (positron energy,
 // both photons) leaves in a voxel; the estimator needs sum_h X_h^2, so the deposits of a decay cannot go to the tally
-// one by one.  They are appended to the decay slot's list; when the decay is complete its list is merged per voxel
-// and each distinct voxel gets one RED into the batch tally (X) and one into hbh_sq (X^2).  A decay with more than
+// one by one.  They are appended to the decay slot's list; the list is merged per voxel -- each distinct voxel gets one
+// RED into the batch tally (X) and one into hbh_sq (X^2) -- when the freed slot is handed its next history (the SOURCE
+// event, up to 32 slots at once) or, for the last decays of a launch, in a sweep at the end.  A decay with more than
 // kHbhCap deposits is merged early (its X is then split in two; counted in n_hbh_overflow, expected 0).
 constexpr unsigned kHbhCap = 63;
+constexpr unsigned kHbhShift = 26;          // the list length lives in bits 26-31 of the slot's history word (shared memory)
+constexpr unsigned kHbhHistMask = (1u << kHbhShift) - 1u;   // so a launch may hold at most 2^26 histories in this mode
 
-__device__ __forceinline__ void hbh_flush(const TransportParams& p, unsigned gslot) {
-    uint2* L = p.hbh_list + gslot;
-    const unsigned n = L[0].x;
-    for (unsigned i = 1; i <= n; ++i) {
+// hl = the slot's history word in shared memory: history index of the launch | list length << 26
+__device__ __forceinline__ void hbh_flush(const TransportParams& p, unsigned gslot, unsigned& hl) {
+    const uint2* L = p.hbh_list + gslot;
+    const unsigned n = hl >> kHbhShift;
+    for (unsigned i = 0; i < n; ++i) {
         const uint2 a = L[(size_t)i * p.hbh_nslots];
         bool seen = false;
-        for (unsigned j = 1; j < i; ++j) seen = seen || (L[(size_t)j * p.hbh_nslots].x == a.x);
+        for (unsigned j = 0; j < i; ++j) seen = seen || (L[(size_t)j * p.hbh_nslots].x == a.x);
         if (seen) continue;
         float X = __uint_as_float(a.y);
-        for (unsigned j = i + 1; j <= n; ++j) {
+        for (unsigned j = i + 1; j < n; ++j) {
             const uint2 b = L[(size_t)j * p.hbh_nslots];
             if (b.x == a.x) X += __uint_as_float(b.y);
         }
         atomicAdd(p.batch + a.x, X);
         atomicAdd(p.hbh_sq + a.x, X * X);
     }
-    L[0].x = 0u;
+    hl &= kHbhHistMask;
 }
 
-__device__ __forceinline__ void hbh_push(const TransportParams& p, unsigned gslot, unsigned vox, float e, unsigned& overflow) {
-    uint2* L = p.hbh_list + gslot;
-    unsigned n = L[0].x;
-    if (n == kHbhCap) { hbh_flush(p, gslot); ++overflow; n = 0u; }
-    L[(size_t)(n + 1u) * p.hbh_nslots] = make_uint2(vox, __float_as_uint(e));
-    L[0].x = n + 1u;
+__device__ __forceinline__ void hbh_push(const TransportParams& p, unsigned gslot, unsigned& hl, unsigned vox, float e, unsigned& overflow) {
+    if ((hl >> kHbhShift) == kHbhCap) { hbh_flush(p, gslot, hl); ++overflow; }
+    p.hbh_list[gslot + (size_t)(hl >> kHbhShift) * p.hbh_nslots] = make_uint2(vox, __float_as_uint(e));
+    hl += 1u << kHbhShift;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -609,6 +611,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
     unsigned char* q = reinterpret_cast<unsigned char*>(slots + kSlotFields * kSlots);   // [4][kSlots]
 #pragma unroll
     for (int k = 0; k < kSlots / 32; ++k) q[Q_S * kSlots + lane + 32 * k] = (unsigned char)(lane + 32 * k);   // all free
+    if (HBH) for (int k = 0; k < kSlots / 32; ++k) slots_u[F_HL * kSlots + lane + 32 * k] = 0u;                  // empty deposit lists
     __syncthreads();
 
     // ring heads and lengths, one byte per event type (byte Q_F .. Q_R), warp-uniform; all slots start free (Q_S)
@@ -684,7 +687,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
             if (active) {
                 const unsigned meta = SU[F_META * kSlots];
                 const unsigned ph = meta & 1u;
-                const unsigned long long h = p.hist_base + SU[F_HL * kSlots];
+                const unsigned long long h = p.hist_base + (HBH ? SU[F_HL * kSlots] & kHbhHistMask : SU[F_HL * kSlots]);
                 const uint4 r = philox4x32_10(make_uint4((unsigned)h, (unsigned)(h >> 32), meta >> 8, 1u + ph), p);
                 float* Bk = S + ph * (kBankFields * kSlots);
                 float x = Bk[F_X * kSlots], y = Bk[F_Y * kSlots], z = Bk[F_Z * kSlots];
@@ -718,18 +721,17 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                     if (ELEC && Epe > p.t_min) {
                         const float out = electron_walk(p, s_er, x, y, z, u, v, w, vox, Epe);
                         if (STATS) { esc += out; ++c_el; }
-                    } else if (HBH) hbh_push(p, gslot0 + slot, vox, Epe, c_ovf);
+                    } else if (HBH) hbh_push(p, gslot0 + slot, SU[F_HL * kSlots], vox, Epe, c_ovf);
                     else atomicAdd(p.batch + vox, Epe);
                 }
                 if (STATS && code == FLY_ESCAPED) { esc += Bk[F_E * kSlots]; ++c_esc; }
             }
-            if (HBH && next == Q_S) hbh_flush(p, gslot0 + slot);      // the decay is complete: merge its deposits per voxel
             push_all(next, slot);
         } else if (X == Q_C) {
             if (active) {
                 const unsigned meta = SU[F_META * kSlots];
                 const unsigned ph = meta & 1u;
-                const unsigned long long h = p.hist_base + SU[F_HL * kSlots];
+                const unsigned long long h = p.hist_base + (HBH ? SU[F_HL * kSlots] & kHbhHistMask : SU[F_HL * kSlots]);
                 const uint4 r = philox4x32_10(make_uint4((unsigned)h, (unsigned)(h >> 32), meta >> 8, 1u + ph), p);
                 float* Bk = S + ph * (kBankFields * kSlots);
                 float E = Bk[F_E * kSlots];
@@ -766,16 +768,18 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                         SU[F_META * kSlots] = (meta & ~0x74u) + 256u;     // a scatter clears AWAY
                         next = Q_F;
                     }
-                    if (dep > 0.0f) { if (HBH) hbh_push(p, gslot0 + slot, vox, dep, c_ovf); else atomicAdd(p.batch + vox, dep); }
+                    if (dep > 0.0f) { if (HBH) hbh_push(p, gslot0 + slot, SU[F_HL * kSlots], vox, dep, c_ovf); else atomicAdd(p.batch + vox, dep); }
                 } else {
                     SU[F_META * kSlots] = meta + 256u;
                     next = Q_C;
                 }
             }
-            if (HBH && next == Q_S) hbh_flush(p, gslot0 + slot);      // the decay is complete: merge its deposits per voxel
             push_all(next, slot);
         } else if (X == Q_S) {
             if (active) {
+                // HBH: the slot's previous decay is complete; its deposits are merged per voxel HERE, where up to 32 freed
+                // slots are handled by 32 lanes at once, not at the photon's end, where one or two lanes of a trip would do it
+                if (HBH) hbh_flush(p, gslot0 + slot, SU[F_HL * kSlots]);
                 const unsigned long long h = p.hist_base + hl_new;
                 float x, y, z, u, v, w;
                 bool in_box;
@@ -789,7 +793,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                 B1[F_E * kSlots] = kE0; B1[F_TV * kSlots] = t0;
                 SU[F_HL * kSlots] = hl_new;
                 SU[F_META * kSlots] = in_box ? (2u | 8u) : 0u;
-                if (p.positron_ke > 0.0f) { if (HBH) hbh_push(p, gslot0 + slot, voxel, p.positron_ke, c_ovf); else atomicAdd(p.batch + voxel, p.positron_ke); }
+                if (p.positron_ke > 0.0f) { if (HBH) hbh_push(p, gslot0 + slot, SU[F_HL * kSlots], voxel, p.positron_ke, c_ovf); else atomicAdd(p.batch + voxel, p.positron_ke); }
                 q[Q_F * kSlots + ((heads + cnts + lane) & (kSlots - 1))] = (unsigned char)slot;
             }
             cnts += n;
@@ -797,7 +801,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
             if (active) {
                 const unsigned meta = SU[F_META * kSlots];
                 const unsigned ph = meta & 1u;
-                const unsigned long long h = p.hist_base + SU[F_HL * kSlots];
+                const unsigned long long h = p.hist_base + (HBH ? SU[F_HL * kSlots] & kHbhHistMask : SU[F_HL * kSlots]);
                 const uint4 r = philox4x32_10(make_uint4((unsigned)h, (unsigned)(h >> 32), meta >> 8, 1u + ph), p);
                 float* Bk = S + ph * (kBankFields * kSlots);
                 const float E = Bk[F_E * kSlots];
@@ -819,6 +823,11 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
         }
     }
 
+    if (HBH) {      // the decays that completed after the last SOURCE trip
+        __syncwarp();
+#pragma unroll 1
+        for (int k = 0; k < kSlots / 32; ++k) hbh_flush(p, gslot0 + lane + 32u * (unsigned)k, slots_u[F_HL * kSlots + lane + 32 * k]);
+    }
     if (STATS) {
         unsigned c_steps = fc.steps, c_real = fc.real;
 #pragma unroll
