@@ -85,6 +85,7 @@ struct anm_ctx {
     DevBuf<float> batch, sum, sumsq, scratch;
     DevBuf<float> batch2, batch3;         // extra batch tallies of the launch pipeline (anm_options.batch_pipeline)
     cudaStream_t pipe[3] = {nullptr, nullptr, nullptr};   // internal streams of the pipeline, created on first use
+    DevBuf<float> e_ring;                 // waiting electrons of the event pool (electron_transport)
     DevBuf<float> hbh_sq;                 // [Vpad] sum over histories of X_h^2 (anm_options.uncertainty = 1)
     DevBuf<uint2> hbh_list;               // [(kHbhCap + 1) * hbh_nslots] per-slot deposit lists
     bool run_hbh = false;                 // the last run scored history by history
@@ -378,7 +379,7 @@ int anm_destroy(anm_ctx* c) {
     c->labels.release(); c->alias.release(); c->counters.release(); c->dstats.release();
     c->organ_batch.release(); c->organ_acc.release(); c->organ_mass.release(); c->organ_count.release();
     c->total_energy.release(); c->d_tot.release(); c->d_maj.release(); c->d_majo.release(); c->d_x2.release(); c->d_cum.release();
-    c->d_pec.release(); c->d_flags.release(); c->d_erange.release(); c->hbh_sq.release(); c->hbh_list.release();
+    c->d_pec.release(); c->d_flags.release(); c->d_erange.release(); c->e_ring.release(); c->hbh_sq.release(); c->hbh_list.release();
     c->batch2.release(); c->batch3.release();
     for (auto& ps : c->pipe) if (ps) { cudaStreamDestroy(ps); ps = nullptr; }
     delete c;
@@ -1031,6 +1032,10 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     const int fold_blocks = grid_blocks(c, c->Vpad / 4, kFoldThreads);
     const float inv_vox = (float)(1.0 / (c->dx * c->dy * c->dz));
     c->run_hbh = HB;
+    if (EL) {   // per-warp arrays of electrons waiting for their walk
+        ANM_CUDA(c, c->e_ring.alloc((size_t)3 * blocks * kPoolWarps * 8 * kPend));     // one per launch in flight
+        p.e_ring = c->e_ring.p;
+    }
     if (HB) {   // history-by-history scoring: sum of X_h^2 over the whole run + one deposit list per decay slot
         const size_t nslots = (size_t)blocks * kPoolWarps * kSlots;
         ANM_CUDA(c, c->hbh_sq.alloc(c->Vpad));
@@ -1070,6 +1075,7 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     for (int b = 0; b < B; ++b) {
         cudaStream_t sb = depth > 1 ? c->pipe[b % depth] : st;
         p.batch = bufs[b % depth];
+        if (EL) p.e_ring = c->e_ring.p + (size_t)(b % depth) * blocks * kPoolWarps * 8 * kPend;
         p.counter = c->counters.p + b;
         p.hist_base = c->opt.history_offset + (unsigned long long)b * nb;
         kern<<<blocks, threads, smem, sb>>>(p);

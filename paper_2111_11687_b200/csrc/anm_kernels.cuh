@@ -86,6 +86,7 @@ struct TransportParams {
     // the electron cutoff, [nm][n_t] g/cm^2 on the kinetic-energy grid t_min + k dt; t_min = the cutoff
     const float* e_range;
     int n_t, e_nm;               // e_nm materials in the electron tables
+    float* e_ring;               // [warps of the launch][8][kPend] electrons waiting for their walk (event pool)
     float t_min, e_dt, e_inv_dt;
     // history-by-history scoring (anm_options.uncertainty = 1, Walters et al. 2002): per decay slot a
     // list of the decay's deposits {voxel, energy} in global scratch, hbh_list[i * hbh_nslots + slot] (its length in the
@@ -577,6 +578,7 @@ constexpr int kPoolThreads = ANM_POOL_THREADS;
 constexpr int kPoolWarps = kPoolThreads / 32;
 constexpr int kPoolMinBlocksPerSM = ANM_POOL_MIN_BLOCKS;
 constexpr int kSlots = 64;                  // per warp (a power of two: the queues are rings)
+constexpr unsigned kPend = 64;              // capacity of a warp's array of waiting electrons (ELEC)
 constexpr int kRayleighBatch = 8;           // run the (rare) Rayleigh event once this many slots wait for it
 // photon bank fields (bank b at word offset b * kBankFields * kSlots)
 enum : int { F_X = 0, F_Y, F_Z, F_U, F_V, F_W, F_E, F_TV /* FLY: ln-E grid coordinate; COMPTON/RAYLEIGH: voxel */,
@@ -636,6 +638,42 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
         if (next != Q_NONE)
             q[next * kSlots + ((((heads + cnts) >> sh) + rank) & (kSlots - 1))] = (unsigned char)slot;
         cnts += __reduce_add_sync(0xffffffffu, next != Q_NONE ? 1u << sh : 0u);
+    };
+
+    // ELEC: electrons set free by this warp's photons wait in a per-warp array (global scratch, [field][kPend]) and are
+    // walked 32 at a time by all lanes -- inside the COMPTON event only the quarter of the lanes whose recoil electron
+    // exceeds the cutoff would walk while the others wait.  pend < 32 between trips, so an event adds at most 32 more.
+    unsigned pend = 0;                      // warp-uniform
+    float* ering = ELEC ? p.e_ring + (size_t)(gslot0 / (unsigned)kSlots) * (8u * kPend) : nullptr;
+    bool e_want = false;
+    float e_x = 0, e_y = 0, e_z = 0, e_ex = 0, e_ey = 0, e_ez = 1, e_T = 0;
+    unsigned e_vox = 0;
+    auto e_append = [&]() {                 // all 32 lanes call it
+        const unsigned b = __ballot_sync(0xffffffffu, e_want);
+        if (b) {
+            if (e_want) {
+                float* E = ering + pend + __popc(b & lanemask_lt);
+                E[0 * kPend] = e_x; E[1 * kPend] = e_y; E[2 * kPend] = e_z;
+                E[3 * kPend] = e_ex; E[4 * kPend] = e_ey; E[5 * kPend] = e_ez;
+                E[6 * kPend] = e_T; E[7 * kPend] = __uint_as_float(e_vox);
+            }
+            pend += __popc(b);
+            e_want = false;
+        }
+    };
+    auto e_drain = [&](const unsigned min_fill) {
+        while (pend >= min_fill && pend > 0u) {
+            __syncwarp();
+            const unsigned n = min(pend, 32u);
+            pend -= n;
+            if (lane < n) {
+                const float* E = ering + pend + lane;
+                const float out = electron_walk(p, s_er, E[0 * kPend], E[1 * kPend], E[2 * kPend], E[3 * kPend], E[4 * kPend],
+                                                E[5 * kPend], __float_as_uint(E[7 * kPend]), E[6 * kPend]);
+                if (STATS) { esc += out; ++c_el; }
+            }
+            __syncwarp();
+        }
     };
 
     for (;;) {
@@ -718,7 +756,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                 if (code == FLY_PE) {               // all energy to one electron: local, or transported along the photon's direction
                     if (STATS) ++c_pe;
                     const float Epe = Bk[F_E * kSlots];
-                    if (ELEC && Epe > p.t_min) {
+                    if (ELEC && Epe > p.t_min) {          // rare (0.002 per decay): walked on the spot, not queued
                         const float out = electron_walk(p, s_er, x, y, z, u, v, w, vox, Epe);
                         if (STATS) { esc += out; ++c_el; }
                     } else if (HBH) hbh_push(p, gslot0 + slot, SU[F_HL * kSlots], vox, Epe, c_ovf);
@@ -752,8 +790,8 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                             float ex = fmaf(-eps, u, u0), ey = fmaf(-eps, v, v0), ez = fmaf(-eps, w, w0);
                             const float n2 = fmaf(ex, ex, fmaf(ey, ey, ez * ez));
                             if (n2 > 0.0f) { const float inv = rsqrtf(n2); ex *= inv; ey *= inv; ez *= inv; } else { ex = u0; ey = v0; ez = w0; }
-                            const float out = electron_walk(p, s_er, Bk[F_X * kSlots], Bk[F_Y * kSlots], Bk[F_Z * kSlots], ex, ey, ez, vox, dep);
-                            if (STATS) { esc += out; ++c_el; }
+                            e_want = true; e_x = Bk[F_X * kSlots]; e_y = Bk[F_Y * kSlots]; e_z = Bk[F_Z * kSlots];
+                            e_ex = ex; e_ey = ey; e_ez = ez; e_T = dep; e_vox = vox;
                             dep = 0.0f;
                         }
                     }
@@ -774,6 +812,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                     next = Q_C;
                 }
             }
+            if (ELEC) { e_append(); e_drain(32u); }
             push_all(next, slot);
         } else if (X == Q_S) {
             if (active) {
@@ -823,6 +862,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
         }
     }
 
+    if (ELEC) e_drain(1u);                  // the electrons still waiting
     if (HBH) {      // the decays that completed after the last SOURCE trip
         __syncwarp();
 #pragma unroll 1
