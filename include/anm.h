@@ -232,6 +232,12 @@ int anm_get_stats(anm_ctx* c, anm_stats* out);    /* before a completed run: zer
  * activity map (point-source mode has no table). */
 int anm_get_alias_table(anm_ctx* c, uint32_t* out, size_t capacity_entries, size_t* n_entries);
 
+/* Parity hook of the random number generator (north_star (d): Philox4x32 keyed by history index; 10 rounds, DESIGN.md
+ * reading C23): out[i] = Philox4x32-10(counter = counters[4i .. 4i+3], key = (seed low 32 bits, seed high 32 bits)),
+ * computed on the device by the very function the transport kernels call (round keys in the kernel parameters).
+ * counters and out are HOST arrays of 4 n uint32.  Needs only a ctx. */
+int anm_philox_blocks(anm_ctx* c, uint64_t seed, const uint32_t* counters, size_t n, uint32_t* out);
+
 /* Parity hook of the electron walk: the n given electrons {x, y, z (mm), ex, ey, ez (unit vector), T (MeV)} (HOST
  * array of 7 n floats, T above the cutoff, start points inside the grid) are walked by the same device function the
  * transport kernel calls; out_MeV (HOST, nx*ny*nz floats) receives the energy each voxel got, *escaped_MeV the

@@ -21,7 +21,7 @@ ANM_SYMBOLS = [
     "anm_default_options", "anm_run", "anm_get_energy", "anm_get_dose", "anm_get_dose_rate", "anm_get_uncertainty",
     "anm_get_organ_doses", "anm_get_stats", "anm_get_tally_buffers", "anm_merge", "anm_get_alias_table",
     "anm_default_hu_ramp", "anm_load_ct", "anm_get_phantom", "anm_load_pet",
-    "anm_set_electron_tables", "anm_trace_electrons",
+    "anm_set_electron_tables", "anm_trace_electrons", "anm_philox_blocks",
 ]
 
 STATUS = {0: "ANM_OK", -1: "ANM_E_ARG", -2: "ANM_E_STATE", -3: "ANM_E_CUDA", -4: "ANM_E_NOMEM", -5: "ANM_E_UNSUPPORTED"}
@@ -134,6 +134,7 @@ def load(build_if_missing: bool = True):
         "anm_get_alias_table": (i32, [vp, vp, sz, C.POINTER(sz)]),
         "anm_set_electron_tables": (i32, [vp, C.POINTER(anm_electron_tables)]),
         "anm_trace_electrons": (i32, [vp, vp, sz, vp, sz, C.POINTER(dbl)]),
+        "anm_philox_blocks": (i32, [vp, u64, vp, sz, vp]),
         "anm_default_hu_ramp": (i32, [C.POINTER(anm_hu_ramp)]),
         "anm_load_ct": (i32, [vp, vp, i32, i32, i32, dbl, dbl, dbl, dbl, dbl, dbl, C.POINTER(anm_hu_ramp), i32]),
         "anm_get_phantom": (i32, [vp, vp, vp, sz, i32]),
@@ -309,6 +310,13 @@ class Simulation:
         esc = C.c_double(0.0)
         self._ck(self._L.anm_trace_electrons(self._ctx, e.ctypes.data, e.shape[0], out.ctypes.data, self.V, C.byref(esc)))
         return out.reshape(nz, ny, nx), float(esc.value)
+
+    def philox_blocks(self, seed: int, counters) -> np.ndarray:
+        """Device Philox4x32-10 blocks for counters [n][4] (uint32) under key = seed: [n][4] uint32."""
+        ctr = np.ascontiguousarray(counters, np.uint32).reshape(-1, 4)
+        out = np.zeros_like(ctr)
+        self._ck(self._L.anm_philox_blocks(self._ctx, int(seed), ctr.ctypes.data, ctr.shape[0], out.ctypes.data))
+        return out
 
     def default_options(self) -> anm_options:
         o = anm_options()

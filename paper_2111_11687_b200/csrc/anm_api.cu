@@ -886,6 +886,28 @@ int anm_set_electron_tables(anm_ctx* c, const anm_electron_tables* t) {
     return ANM_OK;
 }
 
+int anm_philox_blocks(anm_ctx* c, uint64_t seed, const uint32_t* counters, size_t n, uint32_t* out) {
+    if (!c) return ANM_E_ARG;
+    if (!counters || !out || n == 0 || n > (1u << 24)) return fail(c, ANM_E_ARG, "philox: null pointer or bad count");
+    ANM_CUDA(c, cudaSetDevice(c->device));
+    DevBuf<uint4> d_in, d_out;
+    struct Rel { DevBuf<uint4>&a, &b; ~Rel() { a.release(); b.release(); } } rel{d_in, d_out};
+    ANM_CUDA(c, d_in.alloc(n));
+    ANM_CUDA(c, d_out.alloc(n));
+    ANM_CUDA(c, cudaMemcpyAsync(d_in.p, counters, n * 16, cudaMemcpyHostToDevice, c->stream));
+    TransportParams p;
+    std::memset(&p, 0, sizeof p);
+    for (int r = 0; r < 10; ++r) {      // the same round keys anm_run sets
+        p.rk[2 * r] = (unsigned)seed + (unsigned)r * 0x9E3779B9u;
+        p.rk[2 * r + 1] = (unsigned)(seed >> 32) + (unsigned)r * 0xBB67AE85u;
+    }
+    philox_probe_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(p, d_in.p, d_out.p, (unsigned)n);
+    ANM_CUDA(c, cudaGetLastError());
+    ANM_CUDA(c, cudaMemcpyAsync(out, d_out.p, n * 16, cudaMemcpyDeviceToHost, c->stream));
+    ANM_CUDA(c, cudaStreamSynchronize(c->stream));
+    return ANM_OK;
+}
+
 int anm_trace_electrons(anm_ctx* c, const float* electrons, size_t n, float* out_MeV, size_t n_voxels, double* escaped_MeV) {
     if (!c) return ANM_E_ARG;
     if (!electrons || !out_MeV || !escaped_MeV || n == 0 || n > 0x7fffffffu) return fail(c, ANM_E_ARG, "trace: null pointer or bad count");

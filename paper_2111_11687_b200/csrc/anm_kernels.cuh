@@ -110,6 +110,12 @@ __device__ __forceinline__ uint4 philox4x32_10(uint4 c, const TransportParams& p
     return c;
 }
 
+// inspection / parity hook (anm_philox_blocks): the generator exactly as the transport kernels call it
+__global__ void philox_probe_kernel(const __grid_constant__ TransportParams p, const uint4* __restrict__ ctr, uint4* __restrict__ out, unsigned n) {
+    const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = philox4x32_10(ctr[i], p);
+}
+
 // uniform on (0,1): ((r >> 8) + 0.5) 2^-24
 __device__ __forceinline__ float u01(unsigned r) {
     return fmaf(__uint2float_rn(r >> 8), 5.9604644775390625e-08f, 2.98023223876953125e-08f);
