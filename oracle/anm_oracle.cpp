@@ -14,6 +14,10 @@
 //   Klein-Nishina : plain rejection from the uniform envelope on epsilon         (CUDA: Kahn-style)
 //   arithmetic    : fp64 throughout, fp64 tallies                                (CUDA: fp32)
 //
+// A second, LOCKSTEP mode (tracking = 2 / 3, namespace lockstep below) restates the CUDA path's documented algorithm
+// and draw schedule in fp64 so that the two can be compared history by history; it is pinned against
+// the exact transport above (tests/test_oracle_lockstep.py).
+//
 // Parity pins (tests/test_oracle_*.py, -m "not gpu"): P1 Philox known answers; P3 KN sampler vs
 // closed-form CDF and mean energy transfer; P4 flight vs brute-force line integrals of mu and
 // exp(-mu x); P5 energy conservation; P6 infinite medium; P7 first-collision kerma; P8 source
@@ -618,6 +622,252 @@ int orc_electron_walk(const OrcProblem* p, const double* pos, const double* e, d
     return n;
 }
 
+// ---------------------------------------------------------------------------------------------
+// LOCKSTEP mode (OrcProblem.tracking = 2; "a --lockstep mode re-implements Woodcock with the GPU's draw
+// schedule for per-history debugging").  NOT the oracle's own route: it restates, in fp64 and from DESIGN.md alone
+// (readings C13, C14, C19, C23 and §5.1), the algorithm the CUDA path documents -- Woodcock delta tracking against the
+// global majorant (hull majorant off), Kahn-style Klein-Nishina composition-rejection, the form-factor Rayleigh try,
+// and the draw schedule: counter = (history lo, hi, block, stream), stream 0 = source, 1 + k = photon k, one block per
+// event trip (FLY: two sub-steps {path, accept / channel} x 2; COMPTON: {branch, eps, accept, phi}; RAYLEIGH:
+// {x^2, accept, phi}), uniforms u = ((r >> 8) + 0.5) 2^-24.  With the same seed it follows the SAME histories as the
+// CUDA path up to fp32 rounding, so the two can be compared history by history (tests/test_gpu_lockstep.py).
+// Point-source mode only (the decay-voxel pick of the CUDA path is an alias table the oracle does not rebuild).
+// ---------------------------------------------------------------------------------------------
+namespace lockstep {
+
+inline double u24(uint32_t r) { return ((double)(r >> 8) + 0.5) * (1.0 / 16777216.0); }
+
+struct Tables {
+    std::vector<float> maj_f;       // [ne] majorant at the grid nodes, 1/cm (fp32 like the cross-section tables)
+    double t_max, t0;
+    // hull majorant (reading C24; tracking = 3): the box of voxel indices [lo, hi) that encloses every voxel
+    // denser than 1/20 of the densest one, and the majorant of the voxels OUTSIDE it
+    bool hull = false;
+    int lo[3] = {0, 0, 0}, hi[3] = {0, 0, 0};
+    std::vector<float> majo_f;
+    bool in_box(const int v[3]) const { return v[0] >= lo[0] && v[0] < hi[0] && v[1] >= lo[1] && v[1] < hi[1] && v[2] >= lo[2] && v[2] < hi[2]; }
+};
+
+inline void block(const OrcProblem& p, uint64_t h, uint32_t blk, uint32_t stream, uint32_t out[4]) {
+    const uint32_t key[2] = {(uint32_t)p.seed, (uint32_t)(p.seed >> 32)};
+    const uint32_t ctr[4] = {(uint32_t)h, (uint32_t)(h >> 32), blk, stream};
+    philox4x32_10(ctr, key, out);
+}
+
+// value of a [n_energy] float table at grid coordinate t (linear in the coordinate = linear in ln E, reading C19)
+inline double lerp_t(const float* row, double t) {
+    const int i = (int)t;
+    const double f = t - (double)i;
+    return (double)row[i] + f * ((double)row[i + 1] - (double)row[i]);
+}
+
+inline double energy_coordinate(const OrcProblem& p, const Tables& T, double E) {
+    const double t = (std::log(E) - p.t.lnE_min) / p.t.dlnE;
+    return std::fmin(std::fmax(t, 0.0), T.t_max);
+}
+
+Tables make_tables(const OrcProblem& p) {
+    Tables T;
+    const int ne = p.t.n_energy, nm = p.t.n_materials;
+    const uint64_t V = (uint64_t)p.nx * p.ny * p.nz;
+    std::vector<double> rho_max(nm, 0.0);
+    for (uint64_t v = 0; v < V; ++v) rho_max[p.material[v]] = std::fmax(rho_max[p.material[v]], (double)p.density[v]);
+    T.maj_f.assign(ne, 0.0f);
+    for (int k = 0; k < ne; ++k) {
+        double mx = 0.0;
+        for (int m = 0; m < nm; ++m) {
+            const size_t i = (size_t)m * ne + k;
+            const double tot = (double)p.t.mu_pe[i] + (double)p.t.mu_compton[i] + (p.rayleigh_on ? (double)p.t.mu_rayleigh[i] : 0.0);
+            mx = std::fmax(mx, rho_max[m] * tot);
+        }
+        T.maj_f[k] = (float)(mx * 1.000001 + 1e-30);   // DESIGN.md C19: x (1 + 1e-6), stored in fp32
+    }
+    T.t_max = (double)(ne - 1) - 1.0 / 1024.0;
+    T.t0 = energy_coordinate(p, T, kElectronMassMeV);
+    T.majo_f = T.maj_f;
+    if (p.tracking == 3) {
+        // densities sit on the 2^-20 g/cm^3 grid (C18): compare in counts, threshold = floor(max count / 20)
+        uint64_t cmax = 0;
+        for (uint64_t v = 0; v < V; ++v) cmax = std::max<uint64_t>(cmax, (uint64_t)std::llround((double)p.density[v] * 1048576.0));
+        const uint64_t thr = cmax / 20;
+        int lo[3] = {p.nx, p.ny, p.nz}, hi[3] = {0, 0, 0};
+        for (int iz = 0; iz < p.nz; ++iz) for (int iy = 0; iy < p.ny; ++iy) for (int ix = 0; ix < p.nx; ++ix) {
+            const int64_t v = (int64_t)ix + (int64_t)p.nx * ((int64_t)iy + (int64_t)p.ny * iz);
+            if ((uint64_t)std::llround((double)p.density[v] * 1048576.0) > thr) {
+                const int q[3] = {ix, iy, iz};
+                for (int a = 0; a < 3; ++a) { lo[a] = std::min(lo[a], q[a]); hi[a] = std::max(hi[a], q[a] + 1); }
+            }
+        }
+        const bool ok = hi[0] > lo[0] && hi[1] > lo[1] && hi[2] > lo[2] &&
+                        (double)(hi[0] - lo[0]) * (hi[1] - lo[1]) * (hi[2] - lo[2]) <= 0.9 * (double)V;
+        if (ok) {
+            T.hull = true;
+            for (int a = 0; a < 3; ++a) { T.lo[a] = lo[a]; T.hi[a] = hi[a]; }
+            std::vector<double> rho_out(nm, 0.0);
+            for (int iz = 0; iz < p.nz; ++iz) for (int iy = 0; iy < p.ny; ++iy) for (int ix = 0; ix < p.nx; ++ix) {
+                const int q[3] = {ix, iy, iz};
+                if (T.in_box(q)) continue;
+                const int64_t v = (int64_t)ix + (int64_t)p.nx * ((int64_t)iy + (int64_t)p.ny * iz);
+                rho_out[p.material[v]] = std::fmax(rho_out[p.material[v]], (double)p.density[v]);
+            }
+            for (int k = 0; k < ne; ++k) {
+                double mo = 0.0;
+                for (int m = 0; m < nm; ++m) {
+                    const size_t i = (size_t)m * ne + k;
+                    const double tot = (double)p.t.mu_pe[i] + (double)p.t.mu_compton[i] + (p.rayleigh_on ? (double)p.t.mu_rayleigh[i] : 0.0);
+                    mo = std::fmax(mo, rho_out[m] * tot);
+                }
+                T.majo_f[k] = (float)(mo * 1.000001 + 1e-30);
+            }
+        }
+    }
+    return T;
+}
+
+// rotate d by polar angle (cos_t) and azimuth phi, in the CUDA path's convention (DESIGN.md §5.1 "rotate")
+inline void rotate_ls(double d[3], double cos_t, double phi) {
+    const double sin_t = std::sqrt(std::fmax(0.0, 1.0 - cos_t * cos_t));
+    const double sp = std::sin(phi), cp = std::cos(phi);
+    const double u = d[0], v = d[1], w = d[2];
+    double a, b, c;
+    if (std::fabs(w) < 0.99999) {
+        const double s = std::sqrt(1.0 - w * w);
+        const double k = sin_t / s;
+        a = k * (u * w * cp - v * sp) + u * cos_t;
+        b = k * (v * w * cp + u * sp) + v * cos_t;
+        c = -(sin_t * s) * cp + w * cos_t;
+    } else {
+        a = sin_t * cp; b = sin_t * sp; c = std::copysign(cos_t, w);
+    }
+    const double n = 1.0 / std::sqrt(a * a + b * b + c * c);
+    d[0] = a * n; d[1] = b * n; d[2] = c * n;
+}
+
+// One photon, stream = 1 + k, from (pos, d) at E0.  Returns nothing; tallies into ty, escaped energy into *escaped.
+// Hull state of a photon (C24): IN = its last landing point (or its start) was inside the box; AWAY = it is outside the
+// box and has flown straight since a point inside it -- a straight ray that has left a convex box never re-enters it,
+// so an AWAY photon flies against the majorant of the voxels outside the box.  A scatter clears AWAY.
+void photon(const OrcProblem& p, const Tables& T, uint64_t h, uint32_t stream, double pos[3], double d[3], Tally& ty,
+            OrcStats& st, double* escaped, bool start_in_box) {
+    bool hull_in = start_in_box, hull_away = false;
+    const double hvox[3] = {p.dx, p.dy, p.dz};
+    const int n[3] = {p.nx, p.ny, p.nz};
+    const int ne = p.t.n_energy;
+    double E = kElectronMassMeV, t = T.t0;
+    uint32_t blk = 0;
+    ++st.n_photons;
+    for (;;) {
+        // ---- FLY: sub-steps until a real collision or escape, two per block
+        int channel = -1;          // 0 photoelectric, 1 Compton, 2 Rayleigh
+        int64_t v = -1;
+        int m = 0;
+        while (channel < 0) {
+            uint32_t r[4];
+            block(p, h, blk++, stream, r);
+            for (int sub = 0; sub < 2 && channel < 0; ++sub) {
+                const double maj = lerp_t(hull_away ? T.majo_f.data() : T.maj_f.data(), t);
+                const double s = -std::log(u24(r[2 * sub])) / maj;
+                int vox[3];
+                bool inside = true;
+                for (int a = 0; a < 3; ++a) {
+                    pos[a] += s * d[a];
+                    vox[a] = (int)std::floor(pos[a] / hvox[a]);
+                    inside = inside && vox[a] >= 0 && vox[a] < n[a];
+                }
+                ++st.n_virtual;                                   // counts every sub-step here
+                if (!inside) { *escaped += E; ++st.n_escaped; return; }
+                if (T.hull) {
+                    if (T.in_box(vox)) { hull_in = true; hull_away = false; }
+                    else { hull_away = hull_in || hull_away; hull_in = false; }
+                }
+                v = vox_index(p, vox);
+                m = p.material[v];
+                const double rho = (double)p.density[v];
+                const size_t row = (size_t)m * ne;
+                const double pe = lerp_t(p.t.mu_pe + row, t), co = lerp_t(p.t.mu_compton + row, t);
+                const double ra = p.rayleigh_on ? lerp_t(p.t.mu_rayleigh + row, t) : 0.0;
+                const double rr = u24(r[2 * sub + 1]) * maj;
+                if (rr < rho * (pe + co + ra)) {                  // real; the same draw picks the channel
+                    ++st.n_collisions;
+                    channel = rr < rho * pe ? 0 : ((rr < rho * (pe + co) || !p.rayleigh_on) ? 1 : 2);
+                }
+            }
+        }
+        if (channel == 0) { ++st.n_pe; deposit(ty, v, E); return; }
+        if (channel == 1) {
+            // ---- COMPTON: one Kahn-style composition-rejection try per block
+            for (;;) {
+                uint32_t r[4];
+                block(p, h, blk++, stream, r);
+                const double alpha = E / kElectronMassMeV;
+                const double eps0 = 1.0 / (1.0 + 2.0 * alpha), eps0sq = eps0 * eps0;
+                const double a1 = -std::log(eps0), a2 = a1 + 0.5 * (1.0 - eps0sq);
+                const double u2 = u24(r[1]);
+                double eps, epssq;
+                if (a1 > a2 * u24(r[0])) { eps = std::exp(-a1 * u2); epssq = eps * eps; }
+                else { epssq = eps0sq + (1.0 - eps0sq) * u2; eps = std::sqrt(epssq); }
+                const double tt = (1.0 - eps) / (alpha * eps);                 // 1 - cos(theta)
+                const double sint2 = std::fmax(0.0, tt * (2.0 - tt));
+                const double g = 1.0 - eps * sint2 / (1.0 + epssq);
+                if (!(g >= u24(r[2]))) continue;
+                ++st.n_compton;
+                double dep = E * (1.0 - eps);
+                E *= eps;
+                if (E < p.photon_cutoff) { dep += E; ++st.n_cutoff; deposit(ty, v, dep); return; }
+                rotate_ls(d, 1.0 - tt, kTwoPi * u24(r[3]));
+                hull_away = false;
+                t = energy_coordinate(p, T, E);
+                deposit(ty, v, dep);
+                break;
+            }
+        } else {
+            // ---- RAYLEIGH: one form-factor try per block
+            for (;;) {
+                uint32_t r[4];
+                block(p, h, blk++, stream, r);
+                const float* x2 = p.t.ray_x2;
+                const float* cum = p.t.ray_cum + (size_t)m * p.t.n_x2;
+                const double xm = E * (1000.0 / 12.398419843), TT = xm * xm;
+                const double A_T = interp_grid(x2, cum, p.t.n_x2, TT);
+                const double target = u24(r[0]) * A_T;
+                int lo = 0, hi = p.t.n_x2 - 1;
+                while (hi - lo > 1) { const int mid = (lo + hi) / 2; if ((double)cum[mid] <= target) lo = mid; else hi = mid; }
+                double xx = (double)x2[lo];
+                const double dc = (double)cum[hi] - (double)cum[lo];
+                if (dc > 0.0) xx += (target - (double)cum[lo]) / dc * ((double)x2[hi] - (double)x2[lo]);
+                xx = std::fmin(xx, TT);
+                const double c = 1.0 - 2.0 * xx / TT;
+                if (!(2.0 * u24(r[1]) <= 1.0 + c * c)) continue;
+                ++st.n_rayleigh;
+                rotate_ls(d, c, kTwoPi * u24(r[2]));
+                hull_away = false;
+                break;
+            }
+        }
+    }
+}
+
+// One decay in point-source mode: stream 0 block 1 words 2, 3 give cos(theta) and phi of photon A; photon B = -A.
+void history(const OrcProblem& p, const Tables& T, uint64_t h, Tally& ty, OrcStats& st, double* escaped, double* emitted) {
+    const double hvox[3] = {p.dx, p.dy, p.dz};
+    uint32_t r2[4];
+    block(p, h, 1, 0, r2);
+    const double ct = 2.0 * u24(r2[2]) - 1.0, sn = std::sqrt(std::fmax(0.0, 1.0 - ct * ct)), phi = kTwoPi * u24(r2[3]);
+    const double d0[3] = {sn * std::cos(phi), sn * std::sin(phi), ct};
+    int vox[3];
+    const double src[3] = {p.px, p.py, p.pz};
+    for (int a = 0; a < 3; ++a) vox[a] = (int)std::floor(src[a] / hvox[a]);
+    if (p.positron_ke > 0.0) { *emitted += p.positron_ke; deposit(ty, vox_index(p, vox), p.positron_ke); }
+    for (int k = 0; k < p.photons_per_decay; ++k) {
+        double pos[3] = {src[0], src[1], src[2]};
+        double d[3] = {k == 0 ? d0[0] : -d0[0], k == 0 ? d0[1] : -d0[1], k == 0 ? d0[2] : -d0[2]};
+        *emitted += kElectronMassMeV;
+        photon(p, T, h, 1u + (uint32_t)k, pos, d, ty, st, escaped, T.hull && T.in_box(vox));
+    }
+}
+
+}  // namespace lockstep
+
 // ----------------------------------------------------------------- the run
 // Histories [h0, h1) of a run of n_total decays in n_batches batches; h0 and h1 must be batch
 // boundaries (batch b = h / (n_total / n_batches); reading C15: n_total % n_batches == 0).
@@ -645,6 +895,9 @@ int orc_run(const OrcProblem* pp, uint64_t h0, uint64_t h1, double* sum, double*
         for (uint64_t v = 0; v < V; ++v)
             ws.rho_max[p.material[v]] = std::fmax(ws.rho_max[p.material[v]], (double)p.density[v]);
 
+    if (p.tracking >= 2 && (!p.use_point_source || p.electron_on)) return -1;
+    lockstep::Tables ls_tables;
+    if (p.tracking >= 2) ls_tables = lockstep::make_tables(p);
     std::vector<double> batch(V, 0.0);
     std::vector<double> hbh_acc, hbh_temp;
     std::vector<int64_t> hbh_last;
@@ -655,6 +908,17 @@ int orc_run(const OrcProblem* pp, uint64_t h0, uint64_t h1, double* sum, double*
 
     for (uint64_t b = h0 / nb; b < h1 / nb; ++b) {
         for (uint64_t h = b * nb; h < (b + 1) * nb; ++h) {
+            if (p.tracking >= 2) {              // lockstep with the CUDA path's draw schedule (point source only)
+                double emitted = 0.0, escaped = 0.0;
+                ty.deposited = 0.0;
+                ty.history = (int64_t)h;
+                lockstep::history(p, ls_tables, h, ty, st, &escaped, &emitted);
+                st.emitted += emitted; st.deposited += ty.deposited; st.escaped += escaped;
+                const double res = std::fabs(ty.deposited + escaped - emitted);
+                if (res > st.max_history_residual) st.max_history_residual = res;
+                ++st.n_histories;
+                continue;
+            }
             Rng g;
             g.start(p.seed, h);
             double pos[3], d[3];

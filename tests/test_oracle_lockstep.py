@@ -1,0 +1,57 @@
+"""Pins of the oracle's LOCKSTEP mode (tracking = 2 / 3: Woodcock tracking with the CUDA path's documented draw schedule,
+without / with the hull majorant; SURVEY.md §8(c) "lockstep", pin P6 "Woodcock vs exact DDA") against the oracle's own
+exact voxel-boundary transport: different algorithms, same distribution.  What lockstep is FOR -- following the CUDA
+path history by history -- is tested on the GPU (tests/test_gpu_lockstep.py); here it must first be right."""
+import numpy as np
+import pytest
+
+import anm_inputs
+from oracle import anm_oracle as O
+
+
+@pytest.fixture(scope="module")
+def tables():
+    return anm_inputs.make_tables()
+
+
+def _point_cfg(scale=8, src=(271.0, 231.0, 1130.0), **kw):
+    base = anm_inputs.make_config(3, scale)
+    return dict(base, activity=None, point_source_mm=src, **kw)
+
+
+@pytest.mark.parametrize("tracking", [2, 3])
+def test_lockstep_agrees_with_exact_tracking(tables, tracking):
+    cfg = _point_cfg()
+    n, B = 200_000, 20
+    a = O.Oracle(cfg, tables, n_decays=n, n_batches=B, seed=11)
+    ra = a.run_parallel(8); fa = a.finalize(ra)
+    b = O.Oracle(cfg, tables, n_decays=n, n_batches=B, seed=12, tracking=tracking)
+    rb = b.run_parallel(8); fb = b.finalize(rb)
+    sa, sb = ra["stats"], rb["stats"]
+    assert sb["max_history_residual"] < 2e-9 and sa["max_history_residual"] < 2e-9       # energy conservation per history
+    # total deposited energy: per-decay spread <= 0.6 MeV
+    assert abs(sa["deposited"] - sb["deposited"]) / n < 4.0 * np.sqrt(2.0) * 0.6 / np.sqrt(n)
+    for k in ("n_compton", "n_pe", "n_rayleigh", "n_escaped"):
+        assert sa[k] == pytest.approx(sb[k], rel=4.0 / np.sqrt(min(sa[k], sb[k])) + 1e-3), k
+    big = fa["organs"]["n_voxels"] >= 4
+    d = np.abs(fa["organs"]["mean"][big] - fb["organs"]["mean"][big])
+    s = np.sqrt(fa["organs"]["sigma_mean"][big] ** 2 + fb["organs"]["sigma_mean"][big] ** 2)
+    assert np.all(d <= 4.5 * s + 1e-3 * fa["organs"]["mean"][big])
+
+
+def test_hull_majorant_changes_the_steps_not_the_physics(tables):
+    """Source in the skin: many photons leave the body at once.  With the hull majorant they take fewer sub-steps in the
+    air margin; the deposits follow the same distribution."""
+    cfg = _point_cfg(src=(256.0, 150.0, 640.0))
+    n, B = 100_000, 10
+    r2 = O.Oracle(cfg, tables, n_decays=n, n_batches=B, seed=3, tracking=2).run_parallel(8)
+    r3 = O.Oracle(cfg, tables, n_decays=n, n_batches=B, seed=3, tracking=3).run_parallel(8)
+    assert r3["stats"]["n_virtual"] < 0.8 * r2["stats"]["n_virtual"]          # sub-steps (every one is counted there)
+    assert abs(r2["stats"]["deposited"] - r3["stats"]["deposited"]) / n < 4.0 * np.sqrt(2.0) * 0.6 / np.sqrt(n)
+    assert r2["stats"]["n_compton"] == pytest.approx(r3["stats"]["n_compton"], rel=0.01)
+
+
+def test_lockstep_needs_a_point_source(tables):
+    cfg = anm_inputs.make_config(3, 16)
+    with pytest.raises(ValueError):
+        O.Oracle(cfg, tables, n_decays=100, n_batches=2, tracking=2).run()
