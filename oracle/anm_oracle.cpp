@@ -761,6 +761,7 @@ void photon(const OrcProblem& p, const Tables& T, uint64_t h, uint32_t stream, d
         int channel = -1;          // 0 photoelectric, 1 Compton, 2 Rayleigh
         int64_t v = -1;
         int m = 0;
+        int cvox[3] = {0, 0, 0};   // the collision voxel
         while (channel < 0) {
             uint32_t r[4];
             block(p, h, blk++, stream, r);
@@ -781,6 +782,7 @@ void photon(const OrcProblem& p, const Tables& T, uint64_t h, uint32_t stream, d
                     else { hull_away = hull_in || hull_away; hull_in = false; }
                 }
                 v = vox_index(p, vox);
+                cvox[0] = vox[0]; cvox[1] = vox[1]; cvox[2] = vox[2];
                 m = p.material[v];
                 const double rho = (double)p.density[v];
                 const size_t row = (size_t)m * ne;
@@ -793,7 +795,7 @@ void photon(const OrcProblem& p, const Tables& T, uint64_t h, uint32_t stream, d
                 }
             }
         }
-        if (channel == 0) { ++st.n_pe; deposit(ty, v, E); return; }
+        if (channel == 0) { ++st.n_pe; release_electron(p, pos, d, cvox, E, ty, st, escaped); return; }   // electron along the photon
         if (channel == 1) {
             // ---- COMPTON: one Kahn-style composition-rejection try per block
             for (;;) {
@@ -811,13 +813,23 @@ void photon(const OrcProblem& p, const Tables& T, uint64_t h, uint32_t stream, d
                 const double g = 1.0 - eps * sint2 / (1.0 + epssq);
                 if (!(g >= u24(r[2]))) continue;
                 ++st.n_compton;
-                double dep = E * (1.0 - eps);
+                const double Te = E * (1.0 - eps);                      // recoil electron
+                const double E_old = E;
                 E *= eps;
-                if (E < p.photon_cutoff) { dep += E; ++st.n_cutoff; deposit(ty, v, dep); return; }
-                rotate_ls(d, 1.0 - tt, kTwoPi * u24(r[3]));
+                const bool ends = E < p.photon_cutoff;
+                const bool walk = p.electron_on && Te > p.electron_cutoff;
+                const double d_old[3] = {d[0], d[1], d[2]};
+                if (!ends || walk) rotate_ls(d, 1.0 - tt, kTwoPi * u24(r[3]));
+                if (walk) {
+                    double pe[3];
+                    compton_electron_direction(E_old, eps, d_old, d, pe);
+                    release_electron(p, pos, pe, cvox, Te, ty, st, escaped);
+                } else {
+                    deposit(ty, v, Te);
+                }
+                if (ends) { ++st.n_cutoff; deposit(ty, v, E); return; }
                 hull_away = false;
                 t = energy_coordinate(p, T, E);
-                deposit(ty, v, dep);
                 break;
             }
         } else {
@@ -895,7 +907,7 @@ int orc_run(const OrcProblem* pp, uint64_t h0, uint64_t h1, double* sum, double*
         for (uint64_t v = 0; v < V; ++v)
             ws.rho_max[p.material[v]] = std::fmax(ws.rho_max[p.material[v]], (double)p.density[v]);
 
-    if (p.tracking >= 2 && (!p.use_point_source || p.electron_on)) return -1;
+    if (p.tracking >= 2 && !p.use_point_source) return -1;
     lockstep::Tables ls_tables;
     if (p.tracking >= 2) ls_tables = lockstep::make_tables(p);
     std::vector<double> batch(V, 0.0);
