@@ -126,6 +126,7 @@ struct OrcProblem {
     double electron_cutoff;                // MeV; must equal t_min (the range table is "range above the cutoff")
     double t_min, dt;
     const float* e_range;                  // [n_materials][n_t] residual CSDA range above the cutoff, g/cm^2
+    const float* activity;                 // [V] the activity map itself (lockstep mode rebuilds the alias table from it)
 };
 
 struct OrcStats {
@@ -645,6 +646,9 @@ struct Tables {
     bool hull = false;
     int lo[3] = {0, 0, 0}, hi[3] = {0, 0, 0};
     std::vector<float> majo_f;
+    // decay-voxel sampler of the CUDA path (DESIGN.md §5.1a SOURCE; anm.h anm_get_alias_table): alias table over the
+    // active voxels, built by the ordered sweep described in build_alias below
+    std::vector<uint32_t> a_thr, a_own, a_alias;
     bool in_box(const int v[3]) const { return v[0] >= lo[0] && v[0] < hi[0] && v[1] >= lo[1] && v[1] < hi[1] && v[2] >= lo[2] && v[2] < hi[2]; }
 };
 
@@ -666,6 +670,49 @@ inline double energy_coordinate(const OrcProblem& p, const Tables& T, double E) 
     return std::fmin(std::fmax(t, 0.0), T.t_max);
 }
 
+// Walker / Vose alias table by the ORDERED sweep (DESIGN.md §2 "alias"): the M active voxels, weights w = a M / sum(a)
+// (mean 1), are split in index order into light (w <= 1) and heavy (w > 1) ones.  Buckets are filled one by one: the
+// current light voxel owns a bucket with probability w and the current heavy voxel tops it up; the heavy voxel's
+// residual r shrinks by 1 - w each time, and once r < 1 the heavy voxel itself owns the next bucket with probability r,
+// topped up by the next heavy voxel (whose residual absorbs the difference).  With L, H the exclusive prefix sums of the
+// light / heavy weights, after i light and j heavy voxels are done the residual of heavy voxel j is
+// r = L[i] + H[j+1] - (i + j).  threshold = floor(P(own) 2^32), saturated.
+void build_alias(const OrcProblem& p, Tables& T) {
+    const uint64_t V = (uint64_t)p.nx * p.ny * p.nz;
+    double total = 0.0;
+    uint64_t M = 0;
+    for (uint64_t v = 0; v < V; ++v) if (p.activity[v] > 0.0f) { total += (double)p.activity[v]; ++M; }
+    const double scale = (double)M / total;
+    std::vector<uint32_t> light, heavy;
+    for (uint64_t v = 0; v < V; ++v) {
+        const float a = p.activity[v];
+        if (a > 0.0f) ((double)a * scale <= 1.0 ? light : heavy).push_back((uint32_t)v);
+    }
+    const size_t nl = light.size(), nh = heavy.size();
+    std::vector<double> L(nl + 1, 0.0), H(nh + 1, 0.0);
+    for (size_t i = 0; i < nl; ++i) L[i + 1] = L[i] + (double)p.activity[light[i]] * scale;
+    for (size_t j = 0; j < nh; ++j) H[j + 1] = H[j] + (double)p.activity[heavy[j]] * scale;
+    auto thr = [](double prob) -> uint32_t {
+        const double t = std::floor(std::fmin(std::fmax(prob, 0.0), 1.0) * 4294967296.0);
+        return t >= 4294967295.0 ? 0xffffffffu : (uint32_t)t;
+    };
+    T.a_thr.resize(M); T.a_own.resize(M); T.a_alias.resize(M);
+    size_t i = 0, j = 0;
+    for (uint64_t k = 0; k < M; ++k) {
+        if (nh == 0) { T.a_thr[k] = 0xffffffffu; T.a_own[k] = T.a_alias[k] = light[k]; continue; }
+        const double r = L[i] + (j + 1 <= nh ? H[j + 1] : H[nh]) - (double)k;       // residual of heavy voxel j
+        if (i < nl && (r >= 1.0 || j >= nh)) {
+            const uint32_t v = light[i];
+            T.a_thr[k] = thr((double)p.activity[v] * scale); T.a_own[k] = v; T.a_alias[k] = heavy[std::min(j, nh - 1)];
+            ++i;
+        } else {
+            const uint32_t v = heavy[j];
+            T.a_thr[k] = thr(r); T.a_own[k] = v; T.a_alias[k] = j + 1 < nh ? heavy[j + 1] : v;
+            ++j;
+        }
+    }
+}
+
 Tables make_tables(const OrcProblem& p) {
     Tables T;
     const int ne = p.t.n_energy, nm = p.t.n_materials;
@@ -685,6 +732,7 @@ Tables make_tables(const OrcProblem& p) {
     T.t_max = (double)(ne - 1) - 1.0 / 1024.0;
     T.t0 = energy_coordinate(p, T, kElectronMassMeV);
     T.majo_f = T.maj_f;
+    if (!p.use_point_source) build_alias(p, T);
     if (p.tracking == 3) {
         // densities sit on the 2^-20 g/cm^3 grid (C18): compare in counts, threshold = floor(max count / 20)
         uint64_t cmax = 0;
@@ -862,13 +910,25 @@ void photon(const OrcProblem& p, const Tables& T, uint64_t h, uint32_t stream, d
 // One decay in point-source mode: stream 0 block 1 words 2, 3 give cos(theta) and phi of photon A; photon B = -A.
 void history(const OrcProblem& p, const Tables& T, uint64_t h, Tally& ty, OrcStats& st, double* escaped, double* emitted) {
     const double hvox[3] = {p.dx, p.dy, p.dz};
-    uint32_t r2[4];
+    uint32_t r1[4], r2[4];
+    block(p, h, 0, 0, r1);
     block(p, h, 1, 0, r2);
     const double ct = 2.0 * u24(r2[2]) - 1.0, sn = std::sqrt(std::fmax(0.0, 1.0 - ct * ct)), phi = kTwoPi * u24(r2[3]);
     const double d0[3] = {sn * std::cos(phi), sn * std::sin(phi), ct};
     int vox[3];
-    const double src[3] = {p.px, p.py, p.pz};
-    for (int a = 0; a < 3; ++a) vox[a] = (int)std::floor(src[a] / hvox[a]);
+    double src[3] = {p.px, p.py, p.pz};
+    if (p.use_point_source) {
+        for (int a = 0; a < 3; ++a) vox[a] = (int)std::floor(src[a] / hvox[a]);
+    } else {
+        // bucket = floor(r64 M / 2^64) from 64 random bits; own voxel iff w2 < threshold, else the alias voxel;
+        // uniform point inside the voxel from w3 and the first two words of block 1
+        const unsigned __int128 r64 = ((unsigned __int128)r1[0] << 32) | r1[1];
+        const uint64_t k = (uint64_t)((r64 * (unsigned __int128)T.a_thr.size()) >> 64);
+        const uint32_t v = r1[2] < T.a_thr[k] ? T.a_own[k] : T.a_alias[k];
+        vox[0] = (int)(v % (uint32_t)p.nx); vox[1] = (int)((v / (uint32_t)p.nx) % (uint32_t)p.ny); vox[2] = (int)(v / ((uint32_t)p.nx * (uint32_t)p.ny));
+        const double off[3] = {u24(r1[3]), u24(r2[0]), u24(r2[1])};
+        for (int a = 0; a < 3; ++a) src[a] = ((double)vox[a] + off[a]) * hvox[a];
+    }
     if (p.positron_ke > 0.0) { *emitted += p.positron_ke; deposit(ty, vox_index(p, vox), p.positron_ke); }
     for (int k = 0; k < p.photons_per_decay; ++k) {
         double pos[3] = {src[0], src[1], src[2]};
@@ -907,7 +967,7 @@ int orc_run(const OrcProblem* pp, uint64_t h0, uint64_t h1, double* sum, double*
         for (uint64_t v = 0; v < V; ++v)
             ws.rho_max[p.material[v]] = std::fmax(ws.rho_max[p.material[v]], (double)p.density[v]);
 
-    if (p.tracking >= 2 && !p.use_point_source) return -1;
+    if (p.tracking >= 2 && !p.use_point_source && !p.activity) return -1;
     lockstep::Tables ls_tables;
     if (p.tracking >= 2) ls_tables = lockstep::make_tables(p);
     std::vector<double> batch(V, 0.0);

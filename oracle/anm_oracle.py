@@ -57,7 +57,7 @@ class OrcProblem(C.Structure):
                 ("n_total", C.c_uint64), ("n_batches", C.c_int32), ("pad2_", C.c_int32),
                 ("seed", C.c_uint64), ("t", OrcTables),
                 ("electron_on", C.c_int32), ("n_t", C.c_int32), ("electron_cutoff", C.c_double),
-                ("t_min", C.c_double), ("dt", C.c_double), ("e_range", C.c_void_p)]
+                ("t_min", C.c_double), ("dt", C.c_double), ("e_range", C.c_void_p), ("activity", C.c_void_p)]
 
 
 class OrcStats(C.Structure):
@@ -165,6 +165,8 @@ class Oracle:
         else:
             act = np.ascontiguousarray(cfg["activity"], np.float32).reshape(-1)
             assert act.size == self.V and float(act.min()) >= 0.0 and float(act.max()) > 0.0
+            self.activity = act
+            p.activity = _ptr(act)
             self.cdf = np.zeros(self.V, np.float64)
             lib().orc_build_cdf(_ptr(act), self.V, _ptr(self.cdf))
             p.cdf = _ptr(self.cdf)

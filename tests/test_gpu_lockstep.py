@@ -98,3 +98,33 @@ def test_histories_match_with_electron_transport(case):
     assert st["n_electrons"] == pytest.approx(r["stats"]["n_electrons"], rel=2e-3)
     if case == "fine_water":
         assert r["stats"]["n_electron_crossings"] > 0.5 * r["stats"]["n_electrons"]
+
+
+def test_histories_match_from_the_activity_map():
+    """The bench workload's shape: decays drawn from the patient's activity map through the alias table (which the oracle
+    rebuilds by the ordered sweep from the same activity volume), uniform point in the voxel, pairs, positron energy,
+    Rayleigh, hull majorant.  Every step of SURVEY.md §8(a) A1-A9 is then followed history by history."""
+    import paper_2111_11687_b200 as pkg
+    tables = anm_inputs.make_tables()
+    base = anm_inputs.make_config(3, 4)
+    nx, ny, nz = base["shape"]
+    iz, iy, ix = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    labels = (1 + (ix + 7 * iy + 13 * iz) % 255).astype(np.uint8)
+    cfg = dict(base, labels=labels, n_organs=255)
+    n, seed = 30_000, 42
+    with pkg.Simulation(0) as sim:
+        sim.load_config(cfg, tables, n_batches=n, collect_stats=1)
+        alias_g = sim.get_alias_table()
+        sim.run(n, seed)
+        st = sim.get_stats()
+        rows_g = sim.get_tally_buffers()[2].cpu().numpy()[:, 1:256].copy()
+    o = O.Oracle(cfg, tables, n_decays=n, n_batches=n, seed=seed, tracking=3)
+    r = o.run_parallel(8)
+    rows_o = r["organ_batch"][:, 1:256]
+    scale = rows_o.max()
+    same = np.all(np.abs(rows_g - rows_o) <= 2e-4 * np.abs(rows_o) + 1e-7 * scale, axis=1)
+    print("activity source: histories identical %.4f (%d of %d differ)" % (same.mean(), int((~same).sum()), n))
+    assert same.mean() > 0.998
+    assert st["n_steps"] == pytest.approx(r["stats"]["n_virtual"], rel=2e-3)
+    assert st["deposited_MeV"] == pytest.approx(r["stats"]["deposited"], rel=1e-3)
+    assert alias_g.shape[0] == int((base["activity"] > 0).sum())
