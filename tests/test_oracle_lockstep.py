@@ -51,7 +51,24 @@ def test_hull_majorant_changes_the_steps_not_the_physics(tables):
     assert r2["stats"]["n_compton"] == pytest.approx(r3["stats"]["n_compton"], rel=0.01)
 
 
-def test_lockstep_needs_a_point_source(tables):
+def test_lockstep_source_follows_the_activity_pdf(tables):
+    """The lockstep source (alias table rebuilt by the ordered sweep, bucket from 64 random bits) must draw decay voxels
+    with probability a_v / sum(a) like the oracle's own inverse-CDF pick (P8).  Near-vacuum phantom: the photons leave
+    without interacting, the 1 MeV 'positron energy' stays in the decay voxel, so the energy map counts the decays."""
     cfg = anm_inputs.make_config(3, 16)
-    with pytest.raises(ValueError):
-        O.Oracle(cfg, tables, n_decays=100, n_batches=2, tracking=2).run()
+    cfg = dict(cfg, density=np.full_like(cfg["density"], 1e-4), material=np.zeros_like(cfg["material"]),
+               positron_ke_mev=1.0, photons_per_decay=1)
+    n = 400_000
+    r = O.Oracle(cfg, tables, n_decays=n, n_batches=4, seed=9, tracking=2).run_parallel(4)
+    assert r["stats"]["n_collisions"] < 400
+    counts = r["sum"]
+    a = cfg["activity"].astype(np.float64).reshape(-1)
+    expect = n * a / a.sum()
+    assert counts[a == 0].sum() < 400 * 0.6            # nothing where there is no activity (a stray collision aside)
+    sel = expect > 5
+    chi2 = ((counts[sel] - expect[sel]) ** 2 / expect[sel]).sum()
+    dof = sel.sum() - 1
+    assert abs(chi2 - dof) < 5.0 * np.sqrt(2.0 * dof), (chi2, dof)
+    # the hottest voxels individually
+    top = np.argsort(expect)[-20:]
+    assert np.all(np.abs(counts[top] - expect[top]) < 5.0 * np.sqrt(expect[top]))
