@@ -128,3 +128,63 @@ def test_histories_match_from_the_activity_map():
     assert st["n_steps"] == pytest.approx(r["stats"]["n_virtual"], rel=2e-3)
     assert st["deposited_MeV"] == pytest.approx(r["stats"]["deposited"], rel=1e-3)
     assert alias_g.shape[0] == int((base["activity"] > 0).sum())
+
+
+def test_energy_and_hbh_sigma_maps_voxel_by_voxel():
+    """With the histories in step the tallies themselves can be compared element by element: the energy map and the
+    history-by-history sigma map (NEXT-4) of a 200 000-decay run, voxel by voxel, against the lockstep oracle's."""
+    import paper_2111_11687_b200 as pkg
+    tables = anm_inputs.make_tables()
+    cfg = anm_inputs.make_config(3, 4)
+    n, B, seed = 200_000, 10, 42
+    with pkg.Simulation(0) as sim:
+        sim.load_config(cfg, tables, n_batches=B, collect_stats=1, uncertainty=1)
+        sim.run(n, seed)
+        e_g = sim.get_energy().astype(np.float64)
+        rel_g = sim.get_uncertainty().astype(np.float64)
+        organs = sim.get_organ_doses()
+    o = O.Oracle(cfg, tables, n_decays=n, n_batches=B, seed=seed, tracking=3)
+    r = o.run_parallel(10, hbh=True)
+    f = o.finalize(r)
+    e_o, rel_o = f["energy"], f["rel_sigma_hbh"]
+    hit = (e_o > 0) | (e_g > 0)
+    ok = np.abs(e_g - e_o) <= 1e-4 * e_o + 1e-9
+    print("voxels with energy %d, energy identical in %.5f, sum ratio %.7f" % (int(hit.sum()), ok[hit].mean(), e_g.sum() / e_o.sum()))
+    assert ok[hit].mean() > 0.999                      # a history that parts ways touches a handful of voxels
+    assert e_g.sum() == pytest.approx(e_o.sum(), rel=2e-5)
+    both = ok & (e_o > 0)
+    assert np.allclose(rel_g[both], rel_o[both], rtol=2e-3, atol=1e-6)
+    # organ doses (Eq. 2) and their batch sigma from the same histories: equal, not merely compatible
+    big = f["organs"]["n_voxels"] >= 20
+    assert np.allclose(organs["mean_Gy_per_decay"][big], f["organs"]["mean"][big], rtol=2e-4)
+    assert np.allclose(organs["sigma_mean"][big], f["organs"]["sigma_mean"][big], rtol=5e-3)
+
+
+def test_full_size_patient_in_the_bench_configuration():
+    """BASELINE.json cfg3 at full size (256 x 256 x 400 voxels) in the configuration bench.py times -- 100 batches, the
+    default event-pool kernel, hull majorant, launch pipeline, positron energy -- on 1e6 of its decays: the lockstep
+    oracle follows the same histories, so the energy map is compared voxel by voxel and the 27 organ doses number by number."""
+    import paper_2111_11687_b200 as pkg
+    tables = anm_inputs.make_tables()
+    cfg = anm_inputs.make_config(3)
+    n, B, seed = 1_000_000, 100, cfg["seed"]
+    with pkg.Simulation(0) as sim:
+        sim.load_config(cfg, tables, n_batches=B)
+        sim.run(n, seed)
+        e_g = sim.get_energy().astype(np.float64)
+        organs = sim.get_organ_doses()
+    o = O.Oracle(cfg, tables, n_decays=n, n_batches=B, seed=seed, tracking=3)
+    r = o.run_parallel(10)
+    f = o.finalize(r)
+    e_o = f["energy"]
+    hit = (e_o > 0) | (e_g > 0)
+    ok = np.abs(e_g - e_o) <= 1e-4 * e_o + 1e-9
+    print("full size: voxels with energy %d, identical %.5f, sum ratio %.7f" % (int(hit.sum()), ok[hit].mean(), e_g.sum() / e_o.sum()))
+    assert hit.sum() > 1_000_000
+    assert ok[hit].mean() > 0.999
+    assert e_g.sum() == pytest.approx(e_o.sum(), rel=2e-5)
+    nz_ = f["organs"]["n_voxels"] > 0
+    assert np.array_equal(organs["n_voxels"][nz_].astype(np.int64), f["organs"]["n_voxels"][nz_].astype(np.int64))
+    assert np.allclose(organs["mean_Gy_per_decay"][nz_], f["organs"]["mean"][nz_], rtol=1e-3, atol=1e-4 * f["organs"]["mean"].max())
+    big = f["organs"]["n_voxels"] >= 1000
+    assert np.allclose(organs["mean_Gy_per_decay"][big], f["organs"]["mean"][big], rtol=2e-4)
