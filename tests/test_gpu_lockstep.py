@@ -188,3 +188,28 @@ def test_full_size_patient_in_the_bench_configuration():
     assert np.allclose(organs["mean_Gy_per_decay"][nz_], f["organs"]["mean"][nz_], rtol=1e-3, atol=1e-4 * f["organs"]["mean"].max())
     big = f["organs"]["n_voxels"] >= 1000
     assert np.allclose(organs["mean_Gy_per_decay"][big], f["organs"]["mean"][big], rtol=2e-4)
+
+
+@pytest.mark.parametrize("k,scale", [(0, 1), (1, 2), (2, 2)])
+def test_other_configs_voxel_by_voxel(k, scale):
+    """cfg0 (point source, full size), cfg1 (single active voxel, one photon per history) and cfg2 (water / lung / bone
+    slabs, activity box, pairs) at half resolution: energy map voxel by voxel against the lockstep oracle."""
+    import paper_2111_11687_b200 as pkg
+    tables = anm_inputs.make_tables()
+    cfg = anm_inputs.make_config(k, scale)
+    n, B, seed = 200_000, 10, cfg["seed"]
+    with pkg.Simulation(0) as sim:
+        sim.load_config(cfg, tables, n_batches=B, collect_stats=1)
+        sim.run(n, seed)
+        e_g = sim.get_energy().astype(np.float64)
+        st = sim.get_stats()
+    o = O.Oracle(cfg, tables, n_decays=n, n_batches=B, seed=seed, tracking=3)
+    r = o.run_parallel(10)
+    e_o = r["sum"]
+    hit = (e_o > 0) | (e_g > 0)
+    ok = np.abs(e_g - e_o) <= 1e-4 * e_o + 1e-9
+    print("cfg%d: voxels with energy %d, identical %.5f, sum ratio %.7f" % (k, int(hit.sum()), ok[hit].mean(), e_g.sum() / e_o.sum()))
+    assert ok[hit].mean() > 0.998
+    assert e_g.sum() == pytest.approx(e_o.sum(), rel=5e-5)
+    assert st["escaped_MeV"] == pytest.approx(r["stats"]["escaped"], rel=5e-5)
+    assert st["n_compton"] == pytest.approx(r["stats"]["n_compton"], rel=1e-3)
