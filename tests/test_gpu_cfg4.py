@@ -78,3 +78,24 @@ def test_cfg4_full_size_properties(anm, tables):
     assert big.sum() >= 8
     assert np.allclose(organs["mean_Gy_per_decay"][big], oh["mean_Gy_per_decay"][big], rtol=0.05)
     print("cfg4 full size: %.3e decays/s (schedule 2), steps/decay %.2f" % (n / ((a["ms_transport"] + a["ms_fold"]) * 1e-3), a["n_steps"] / n))
+
+
+def test_cfg4_full_size_voxel_by_voxel(anm, tables):
+    """The full 157 M-voxel grid against the lockstep oracle (same histories): energy map voxel by voxel on
+    2e5 of its decays, 100 batches."""
+    cfg = anm_inputs.make_config(4)
+    n, B, seed = 200_000, 100, cfg["seed"]
+    with anm.Simulation(0) as sim:
+        sim.load_config(cfg, tables, n_batches=B)
+        sim.run(n, seed)
+        e_g = sim.get_energy().astype(np.float64)
+    o = O.Oracle(cfg, tables, n_decays=n, n_batches=B, seed=seed, tracking=3)
+    r = o.run_parallel(2)
+    e_o = r["sum"]
+    hit = (e_o > 0) | (e_g > 0)
+    ok = np.abs(e_g - e_o) <= 1e-4 * e_o + 1e-9
+    print("cfg4 full size: voxels with energy %d, identical %.5f, sum ratio %.7f" % (int(hit.sum()), ok[hit].mean(), e_g.sum() / e_o.sum()))
+    # 0.98 mm voxels, coordinates up to 180 cm: an fp32 position (ulp 1.5e-5 cm) lands across a voxel face more often
+    # than on the 2 mm grid (measured 99.79 %); a displaced deposit shows up in two voxels
+    assert ok[hit].mean() > 0.995
+    assert e_g.sum() == pytest.approx(e_o.sum(), rel=5e-5)
