@@ -118,6 +118,9 @@ def main():
     ap.add_argument("--cpu-baseline-decays-per-core", type=int, default=400_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--config", type=int, default=3, choices=[3, 4],
+                    help="BASELINE.json config to run: 3 = the bench workload (default); 4 = the 512x512x600 scale case, "
+                         "for profiling only (use with --no-frontend --no-variants; its line is not a bench number)")
     ap.add_argument("--no-frontend", action="store_true", help="skip the image front-end timing (anm_load_ct / anm_load_pet)")
     ap.add_argument("--no-variants", action="store_true", help="skip the electron-transport / history-by-history runs")
     args = ap.parse_args()
@@ -142,7 +145,7 @@ def main():
     dev = torch.device("cuda", local_rank)
     torch.cuda.set_device(dev)
 
-    cfg = anm_inputs.make_config(3)
+    cfg = anm_inputs.make_config(args.config)
     tables = anm_inputs.make_tables()
     D = int(args.decays)
     B = cfg["n_batches"]
@@ -271,7 +274,7 @@ def main():
 
     # ---- image front end: set-up, not part of decays/s; HBM roofline of its two kernels -------
     frontend = None
-    if not args.no_frontend and world == 1:
+    if not args.no_frontend and world == 1 and args.config == 3:
         img = anm_inputs.make_ct_pet(cfg, ct_shape=(512, 512, 400))          # 1 x 1 x 4 mm CT over the cfg3 grid
         hu_d = torch.from_numpy(img["ct_hu"]).to(dev)
         pet_d = torch.from_numpy(img["pet_bqml"]).to(dev)
@@ -337,7 +340,8 @@ def main():
         "sec_per_1e9_decays": 1e9 / value, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": WORKLOAD, "decays_per_step_per_gpu": D, "seed": cfg["seed"],
+        "config": {"workload": WORKLOAD if args.config == 3 else "cfg4_fullres 512x512x600 @0.98x0.98x3mm (profiling only, not the bench workload)",
+                   "decays_per_step_per_gpu": D, "seed": cfg["seed"],
                    "l2": "working set (texels 105 MB + batch tally 105 MB + sum/sumsq 210 MB) exceeds the 126 MB L2; no flush needed",
                    "multi_gpu": "one logical run of N*D decays: whole-batch shards via history_offset, NCCL sum-all-reduce of the tallies + merged finalize at the end of every step" if world > 1 else "single GPU"},
         "clocks": clk, "e2e": e2e, "gpu_launches": int(launches),
