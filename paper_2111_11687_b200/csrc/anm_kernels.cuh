@@ -4,7 +4,12 @@
 //   transport_kernel : source sampling + Woodcock photon transport + fp32 RED tally
 //   fold_kernel      : per-batch fold  sum += x, sumsq += x^2, x = 0, organ partial sums   (A10)
 //   finalize_kernel  : organ Eq. 3 accumulators, organ energy / mass / counts, total energy (A11)
-//   get_*_kernel     : dose / dose rate / relative sigma read-out                           (A11)
+//   readout_kernel   : dose / dose rate / relative sigma read-out                           (A11)
+//   pack_texels / rho_max / hull_box / organ_mass kernels : set-up (A0); the alias table is in anm_alias.cuh,
+//                      the image front end in anm_frontend.cuh
+//   electron_walk (device function) + electron_trace_kernel : secondary electrons
+//   hbh_push / hbh_flush (device functions)                 : history-by-history scoring (NEXT-4)
+//   philox_probe_kernel                                     : parity hook of the generator (anm_philox_blocks)
 //
 // Two schedules of the same per-event code (anm_options.schedule):
 //   1  transport_kernel       history-based: every lane owns one photon and runs a per-lane state machine;
