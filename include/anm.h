@@ -99,7 +99,8 @@ typedef struct {
                                       one decay = one history, X_h = the energy it leaves in a voxel,
                                       s^2 of the mean = (sum X_h^2 / N - (sum X_h / N)^2) / (N - 1).  anm_get_uncertainty
                                       and the organs' Eq. 3 value then use it; the organ sigma_mean stays the batch
-                                      one.  Schedule 0 or 2, without electron_transport; not mergeable (anm_merge). */
+                                      one.  Schedule 0 or 2; not mergeable (anm_merge).  With electron_transport the
+                                      electrons are walked inside the events (their deposits belong to the decay). */
     int32_t batch_pipeline;     /* launch pipeline over batches: 0 auto (3), 1 serial (one launch at a time on the ctx
                                    stream; per-launch ms_transport / ms_fold), 2 | 3: that many batch tallies and
                                    internal streams, so that the CTAs of batch b+1 take over the SMs as those of batch

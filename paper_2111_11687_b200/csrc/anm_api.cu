@@ -278,7 +278,8 @@ using TransportFn = void (*)(const TransportParams);
 // schedule 1 (history-based lanes) or 2 (warp-scope event pool), with / without counters and warp aggregation
 TransportFn pick_transport(int schedule, bool stats, bool wagg, bool elec, bool hbh) {
     if (schedule == 2) {
-        if (hbh) return stats ? transport_pool_kernel<true, false, true> : transport_pool_kernel<false, false, true>;
+        if (hbh) return elec ? (stats ? transport_pool_kernel<true, true, true> : transport_pool_kernel<false, true, true>)
+                             : (stats ? transport_pool_kernel<true, false, true> : transport_pool_kernel<false, false, true>);
         return elec ? (stats ? transport_pool_kernel<true, true, false> : transport_pool_kernel<false, true, false>)
                     : (stats ? transport_pool_kernel<true, false, false> : transport_pool_kernel<false, false, false>);
     }
@@ -964,7 +965,6 @@ int anm_set_options(anm_ctx* c, const anm_options* o) {
     if (o->batch_pipeline < 0 || o->batch_pipeline > 3) return fail(c, ANM_E_ARG, "options: batch_pipeline must be 0 (auto), 1, 2 or 3");
     if (o->uncertainty != 0 && o->uncertainty != 1) return fail(c, ANM_E_ARG, "options: uncertainty must be 0 (batch) or 1 (history by history)");
     if (o->uncertainty == 1 && o->schedule == 1) return fail(c, ANM_E_UNSUPPORTED, "options: history-by-history scoring runs in the event-pool schedule (0 or 2)");
-    if (o->uncertainty == 1 && o->electron_transport) return fail(c, ANM_E_UNSUPPORTED, "options: history-by-history scoring with electron transport is not implemented");
     if (o->electron_transport && o->schedule == 1) return fail(c, ANM_E_UNSUPPORTED, "options: electron transport runs in the event-pool schedule (0 or 2)");
     c->opt = *o;
     c->dev_tables_dirty = true;

@@ -334,8 +334,10 @@ __device__ __forceinline__ float e_range_of(const TransportParams& p, const floa
 }
 
 // `er` = the range tables [nm][n_t] (the transport kernel's shared-memory copy, or p.e_range).
-__device__ __forceinline__ float electron_walk(const TransportParams& p, const float* __restrict__ er, float x, float y, float z,
-                                            float ex, float ey, float ez, unsigned vox, float T) {
+// dep(voxel, energy) receives the deposits: a RED into the batch tally, or an append to the decay's list (HBH).
+template <class Dep>
+__device__ __forceinline__ float electron_walk_to(const TransportParams& p, const float* __restrict__ er, float x, float y, float z,
+                                               float ex, float ey, float ez, unsigned vox, float T, Dep dep) {
     const unsigned nxy = (unsigned)p.nx * (unsigned)p.ny;
     int iz = (int)(vox / nxy);
     const unsigned rem = vox - (unsigned)iz * nxy;
@@ -357,11 +359,11 @@ __device__ __forceinline__ float electron_walk(const TransportParams& p, const f
         int k;
         const float r = e_range_of(p, R, T, k);
         const float r_new = r - rho * (t_next - t);
-        if (!(r_new > 0.0f)) { atomicAdd(p.batch + vox, T); return 0.0f; }
+        if (!(r_new > 0.0f)) { dep(vox, T); return 0.0f; }
         while (k > 0 && R[k] > r_new) --k;                         // segment with R[k] <= r_new < R[k+1]
         const float r0 = R[k], r1 = R[k + 1];
         const float T_new = fmaf((float)k + __fdividef(r_new - r0, r1 - r0), p.e_dt, p.t_min);
-        if (T > T_new) atomicAdd(p.batch + vox, T - T_new);
+        if (T > T_new) dep(vox, T - T_new);
         T = fminf(T, T_new);
         t = t_next;
         if (tx <= ty && tx <= tz) { ix += ex > 0.0f ? 1 : -1; tx += dtx; if ((unsigned)ix >= (unsigned)p.nx) return T; }
@@ -369,6 +371,11 @@ __device__ __forceinline__ float electron_walk(const TransportParams& p, const f
         else { iz += ez > 0.0f ? 1 : -1; tz += dtz; if ((unsigned)iz >= (unsigned)p.nz) return T; }
         vox = (unsigned)ix + (unsigned)p.nx * ((unsigned)iy + (unsigned)p.ny * (unsigned)iz);
     }
+}
+
+__device__ __forceinline__ float electron_walk(const TransportParams& p, const float* __restrict__ er, float x, float y, float z,
+                                            float ex, float ey, float ez, unsigned vox, float T) {
+    return electron_walk_to(p, er, x, y, z, ex, ey, ez, vox, T, [&](unsigned v, float e) { atomicAdd(p.batch + v, e); });
 }
 
 // inspection / parity hook (anm_trace_electrons): one given electron per thread, in = {x, y, z (cm), ex, ey, ez, T}
@@ -768,7 +775,9 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                     if (STATS) ++c_pe;
                     const float Epe = Bk[F_E * kSlots];
                     if (ELEC && Epe > p.t_min) {          // rare (0.002 per decay): walked on the spot, not queued
-                        const float out = electron_walk(p, s_er, x, y, z, u, v, w, vox, Epe);
+                        const float out = HBH ? electron_walk_to(p, s_er, x, y, z, u, v, w, vox, Epe, [&](unsigned vv, float ee) {
+                                                    hbh_push(p, gslot0 + slot, SU[F_HL * kSlots], vv, ee, c_ovf); })
+                                              : electron_walk(p, s_er, x, y, z, u, v, w, vox, Epe);
                         if (STATS) { esc += out; ++c_el; }
                     } else if (HBH) hbh_push(p, gslot0 + slot, SU[F_HL * kSlots], vox, Epe, c_ovf);
                     else atomicAdd(p.batch + vox, Epe);
@@ -801,8 +810,15 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                             float ex = fmaf(-eps, u, u0), ey = fmaf(-eps, v, v0), ez = fmaf(-eps, w, w0);
                             const float n2 = fmaf(ex, ex, fmaf(ey, ey, ez * ez));
                             if (n2 > 0.0f) { const float inv = rsqrtf(n2); ex *= inv; ey *= inv; ez *= inv; } else { ex = u0; ey = v0; ez = w0; }
-                            e_want = true; e_x = Bk[F_X * kSlots]; e_y = Bk[F_Y * kSlots]; e_z = Bk[F_Z * kSlots];
-                            e_ex = ex; e_ey = ey; e_ez = ez; e_T = dep; e_vox = vox;
+                            if (HBH) {            // the deposits belong to this decay's list: walked on the spot
+                                const float out = electron_walk_to(p, s_er, Bk[F_X * kSlots], Bk[F_Y * kSlots], Bk[F_Z * kSlots], ex, ey, ez,
+                                                                   vox, dep, [&](unsigned vv, float ee) {
+                                                                       hbh_push(p, gslot0 + slot, SU[F_HL * kSlots], vv, ee, c_ovf); });
+                                if (STATS) { esc += out; ++c_el; }
+                            } else {
+                                e_want = true; e_x = Bk[F_X * kSlots]; e_y = Bk[F_Y * kSlots]; e_z = Bk[F_Z * kSlots];
+                                e_ex = ex; e_ey = ey; e_ez = ez; e_T = dep; e_vox = vox;
+                            }
                             dep = 0.0f;
                         }
                     }
@@ -823,7 +839,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                     next = Q_C;
                 }
             }
-            if (ELEC) { e_append(); e_drain(32u); }
+            if (ELEC && !HBH) { e_append(); e_drain(32u); }
             push_all(next, slot);
         } else if (X == Q_S) {
             if (active) {
@@ -873,7 +889,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
         }
     }
 
-    if (ELEC) e_drain(1u);                  // the electrons still waiting
+    if (ELEC && !HBH) e_drain(1u);          // the electrons still waiting
     if (HBH) {      // the decays that completed after the last SOURCE trip
         __syncwarp();
 #pragma unroll 1

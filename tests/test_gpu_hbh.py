@@ -124,9 +124,6 @@ def test_hbh_error_codes(anm, tables):
         with pytest.raises(anm.AnmError) as e:
             sim.set_options(n_batches=4, uncertainty=1, schedule=1)
         assert e.value.code == -5
-        with pytest.raises(anm.AnmError) as e:
-            sim.set_options(n_batches=4, uncertainty=1, electron_transport=1)
-        assert e.value.code == -5
         sim.set_options(n_batches=4, uncertainty=1)
         sim.run(4000, 1)
         with pytest.raises(anm.AnmError) as e:

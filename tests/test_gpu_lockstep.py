@@ -213,3 +213,38 @@ def test_other_configs_voxel_by_voxel(k, scale):
     assert e_g.sum() == pytest.approx(e_o.sum(), rel=5e-5)
     assert st["escaped_MeV"] == pytest.approx(r["stats"]["escaped"], rel=5e-5)
     assert st["n_compton"] == pytest.approx(r["stats"]["n_compton"], rel=1e-3)
+
+
+def test_the_papers_configuration_electrons_and_history_by_history():
+    """PAPER.md:L67 as a whole: secondary electrons followed down to 200 keV AND the history-by-history uncertainty.
+    0.5 mm water voxels (the paper's water test, L79), point source; energy map and sigma map voxel by voxel."""
+    import paper_2111_11687_b200 as pkg
+    tables = anm_inputs.make_tables()
+    et = anm_inputs.make_electron_tables()
+    nv = 64
+    cfg = dict(anm_inputs.make_config(0, 1), shape=(nv,) * 3, spacing_mm=(0.5,) * 3, material=np.full((nv,) * 3, 2, np.uint8),
+               density=anm_inputs.phantoms.quantize_density(np.full((nv,) * 3, 1.0)), point_source_mm=(16.2, 15.9, 16.1),
+               labels=None, n_organs=0, photons_per_decay=2, positron_ke_mev=0.0)
+    n, B, seed = 2_000_000, 10, 3
+    with pkg.Simulation(0) as sim:
+        sim.load_config(cfg, tables, n_batches=B)
+        sim.set_electron_tables(et)
+        sim.set_options(n_batches=B, collect_stats=1, electron_transport=1, uncertainty=1, photons_per_decay=2, rayleigh_on=1,
+                        photon_cutoff_MeV=0.010, positron_ke_MeV=0.0)
+        sim.run(n, seed)
+        e_g = sim.get_energy().astype(np.float64)
+        rel_g = sim.get_uncertainty().astype(np.float64)
+        st = sim.get_stats()
+    o = O.Oracle(cfg, tables, n_decays=n, n_batches=B, seed=seed, tracking=3, electron_tables=et)
+    r = o.run_parallel(10, hbh=True)
+    f = o.finalize(r)
+    e_o, rel_o = f["energy"], f["rel_sigma_hbh"]
+    assert st["n_hbh_overflow"] == 0 and st["n_electrons"] == pytest.approx(r["stats"]["n_electrons"], rel=1e-3)
+    hit = (e_o > 0) | (e_g > 0)
+    ok = np.abs(e_g - e_o) <= 2e-4 * e_o + 2e-5
+    print("electrons + HbH: voxels with energy %d, identical %.5f, sum ratio %.7f" % (int(hit.sum()), ok[hit].mean(), e_g.sum() / e_o.sum()))
+    assert ok[hit].mean() > 0.995
+    assert e_g.sum() == pytest.approx(e_o.sum(), rel=5e-5)
+    both = ok & (e_o > 0.5)                       # voxels hit by several histories
+    assert both.sum() > 1000
+    assert np.allclose(rel_g[both], rel_o[both], rtol=5e-3, atol=1e-6)
