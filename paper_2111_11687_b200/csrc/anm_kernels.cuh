@@ -597,7 +597,10 @@ constexpr int kPoolWarps = kPoolThreads / 32;
 constexpr int kPoolMinBlocksPerSM = ANM_POOL_MIN_BLOCKS;
 constexpr int kSlots = 64;                  // per warp (a power of two: the queues are rings)
 constexpr unsigned kPend = 64;              // capacity of a warp's array of waiting electrons (ELEC)
-constexpr int kRayleighBatch = 8;           // run the (rare) Rayleigh event once this many slots wait for it
+#ifndef ANM_RAYBATCH
+#define ANM_RAYBATCH 8
+#endif
+constexpr int kRayleighBatch = ANM_RAYBATCH;           // run the (rare) Rayleigh event once this many slots wait for it
 // photon bank fields (bank b at word offset b * kBankFields * kSlots)
 enum : int { F_X = 0, F_Y, F_Z, F_U, F_V, F_W, F_E, F_TV /* FLY: ln-E grid coordinate; COMPTON/RAYLEIGH: voxel */,
              kBankFields, F_HL = 2 * kBankFields, F_META, kSlotFields };
