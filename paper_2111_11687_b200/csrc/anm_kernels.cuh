@@ -954,12 +954,22 @@ fold_kernel(float4* __restrict__ batch, float4* __restrict__ sum, float4* __rest
                 const uint4 t = texels4[i];
                 const float xs[4] = {xv.x, xv.y, xv.z, xv.w};
                 const unsigned ts[4] = {t.x, t.y, t.z, t.w};
+                // x / (rho V) in fp32 (1e-7 relative), accumulated in fp64.  The four voxels of a thread usually carry one
+                // label: one shared-memory atomic per thread instead of four (neighbouring lanes hit the same organ bin).
+                const unsigned l0 = l4 & 0xffu;
+                if (l4 == l0 * 0x01010101u) {
+                    double acc = 0.0;
 #pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    const unsigned l = (l4 >> (8 * k)) & 0xffu;
-                    if (l && xs[k] != 0.0f)
-                        atomicAdd(&s_org[l], (double)xs[k] * (double)inv_vox_cm3 /
-                                                 ((double)(ts[k] & 0xffffffu) * (double)kDensityStep));
+                    for (int k = 0; k < 4; ++k)
+                        if (xs[k] != 0.0f) acc += (double)__fdividef(xs[k] * inv_vox_cm3, (float)(ts[k] & 0xffffffu) * kDensityStep);
+                    if (acc != 0.0) atomicAdd(&s_org[l0], acc);
+                } else {
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        const unsigned l = (l4 >> (8 * k)) & 0xffu;
+                        if (l && xs[k] != 0.0f)
+                            atomicAdd(&s_org[l], (double)__fdividef(xs[k] * inv_vox_cm3, (float)(ts[k] & 0xffffffu) * kDensityStep));
+                    }
                 }
             }
         }
