@@ -105,7 +105,7 @@ typedef struct {
                                    stream; per-launch ms_transport / ms_fold), 2 | 3: that many batch tallies and
                                    internal streams, so that the CTAs of batch b+1 take over the SMs as those of batch
                                    b drain; the same histories and tallies; then ms_transport covers the whole
-                                   pipeline (folds inside it) and ms_fold is 0.  Forced to 1 with uncertainty = 1.   */
+                                   pipeline (folds inside it) and ms_fold is 0.                                    */
     int32_t reserved1;
 } anm_options;
 

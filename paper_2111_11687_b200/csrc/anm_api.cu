@@ -1062,7 +1062,7 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
         const size_t nslots = (size_t)blocks * kPoolWarps * kSlots;
         ANM_CUDA(c, c->hbh_sq.alloc(c->Vpad));
         if (nb > (uint64_t)kHbhHistMask) return fail(c, ANM_E_UNSUPPORTED, "run: history-by-history scoring holds at most 2^26 decays per batch");
-        ANM_CUDA(c, c->hbh_list.alloc((size_t)kHbhCap * nslots));
+        ANM_CUDA(c, c->hbh_list.alloc((size_t)3 * kHbhCap * nslots));      // one set of lists per launch in flight
         ANM_CUDA(c, cudaMemsetAsync(c->hbh_sq.p, 0, c->Vpad * 4, st));
         p.hbh_list = c->hbh_list.p; p.hbh_sq = c->hbh_sq.p; p.hbh_nslots = (unsigned)nslots;
     }
@@ -1078,7 +1078,7 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     // consecutive batches go to `depth` internal streams: the CTAs of batch b+1 take over each SM as the CTAs of batch
     // b exit, the fold of batch b runs in the gaps.  The folds are serialised among themselves (they all update sum /
     // sumsq); batch b+depth reuses the tally of batch b after its fold (same stream).  Same histories, same tallies.
-    const int depth = HB ? 1 : std::max(1, std::min(c->opt.batch_pipeline == 0 ? 3 : c->opt.batch_pipeline, B));
+    const int depth = std::max(1, std::min(c->opt.batch_pipeline == 0 ? 3 : c->opt.batch_pipeline, B));
     float* bufs[3] = {c->batch.p, nullptr, nullptr};
     if (depth > 1) {
         ANM_CUDA_EV(c->batch2.alloc(c->Vpad));
@@ -1098,6 +1098,7 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
         cudaStream_t sb = depth > 1 ? c->pipe[b % depth] : st;
         p.batch = bufs[b % depth];
         if (EL) p.e_ring = c->e_ring.p + (size_t)(b % depth) * blocks * kPoolWarps * 8 * kPend;
+        if (HB) p.hbh_list = c->hbh_list.p + (size_t)(b % depth) * kHbhCap * p.hbh_nslots;
         p.counter = c->counters.p + b;
         p.hist_base = c->opt.history_offset + (unsigned long long)b * nb;
         kern<<<blocks, threads, smem, sb>>>(p);
