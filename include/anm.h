@@ -99,7 +99,7 @@ typedef struct {
                                       one decay = one history, X_h = the energy it leaves in a voxel,
                                       s^2 of the mean = (sum X_h^2 / N - (sum X_h / N)^2) / (N - 1).  anm_get_uncertainty
                                       and the organs' Eq. 3 value then use it; the organ sigma_mean stays the batch
-                                      one.  Schedule 0 or 2; not mergeable (anm_merge).  With electron_transport the
+                                      one.  Schedule 0 or 2.  With electron_transport the
                                       electrons are walked inside the events (their deposits belong to the decay). */
     int32_t batch_pipeline;     /* launch pipeline over batches: 0 auto (3), 1 serial (one launch at a time on the ctx
                                    stream; per-launch ms_transport / ms_fold), 2 | 3: that many batch tallies and
@@ -251,7 +251,7 @@ int anm_trace_electrons(anm_ctx* c, const float* electrons, size_t n, float* out
  * batch count, and calls anm_run on its N/B * n_batches decays.  The one exchange step is the merge of the tallies:
  *
  *   anm_get_tally_buffers  returns the ctx-owned DEVICE pointers of the last run's per-voxel sum and sum of squares
- *                          over batches (n_floats = nx*ny*nz rounded up to a multiple of 4, fp32, MeV and MeV^2)
+ *                          over batches (over histories when uncertainty = 1: sum of X_h^2, additive as well) (n_floats = nx*ny*nz rounded up to a multiple of 4, fp32, MeV and MeV^2)
  *                          and of its organ rows (n_rows = this run's n_batches rows of 256 fp64: row[b][label] =
  *                          sum over the organ's voxels of x / (rho V_vox) in batch b).  The caller sum-all-reduces
  *                          d_sum and d_sumsq IN PLACE across ranks (NCCL over NVLink) and gathers the organ rows of

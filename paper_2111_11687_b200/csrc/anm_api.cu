@@ -1215,7 +1215,9 @@ int anm_get_tally_buffers(anm_ctx* c, float** d_sum, float** d_sumsq, size_t* n_
     if (!c) return ANM_E_ARG;
     if (!d_sum || !d_sumsq || !n_floats || !d_organ_rows || !n_rows) return fail(c, ANM_E_ARG, "tally buffers: null pointer");
     if (!c->have_results) return fail(c, ANM_E_STATE, "tally buffers: no completed run");
-    *d_sum = c->sum.p; *d_sumsq = c->sumsq.p; *n_floats = c->Vpad;
+    // the sum-of-squares volume of the run's estimator: over batches, or over histories (uncertainty = 1) -- both add up
+    // across shards
+    *d_sum = c->sum.p; *d_sumsq = c->run_hbh ? c->hbh_sq.p : c->sumsq.p; *n_floats = c->Vpad;
     *d_organ_rows = c->organ_batch.p; *n_rows = c->run_batches;
     return ANM_OK;
 }
@@ -1223,7 +1225,6 @@ int anm_get_tally_buffers(anm_ctx* c, float** d_sum, float** d_sumsq, size_t* n_
 int anm_merge(anm_ctx* c, uint64_t total_decays, int total_batches, const double* organ_rows_all, const anm_stats* summed) {
     if (!c) return ANM_E_ARG;
     if (!c->have_results) return fail(c, ANM_E_STATE, "merge: no completed run");
-    if (c->run_hbh) return fail(c, ANM_E_UNSUPPORTED, "merge: history-by-history runs are not merged (use the batch estimator across GPUs)");
     if (total_batches < c->run_batches || total_batches < 2 || total_decays == 0 || total_decays % (uint64_t)total_batches)
         return fail(c, ANM_E_ARG, "merge: total_decays must be a positive multiple of total_batches >= this run's batches");
     const uint64_t nb = c->run_decays / (uint64_t)c->run_batches;

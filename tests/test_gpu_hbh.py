@@ -126,9 +126,6 @@ def test_hbh_error_codes(anm, tables):
         assert e.value.code == -5
         sim.set_options(n_batches=4, uncertainty=1)
         sim.run(4000, 1)
-        with pytest.raises(anm.AnmError) as e:
-            sim.merge(8000, 8, np.zeros((8, 256)))
-        assert e.value.code == -5
         # back to the batch estimator on the same ctx
         sim.set_options(n_batches=4, uncertainty=0)
         sim.run(4000, 1)

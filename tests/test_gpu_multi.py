@@ -19,14 +19,15 @@ def _load(sim, cfg, tables, **opts):
     sim.load_config(cfg, tables, **opts)
 
 
-def test_two_emulated_ranks_merge_to_the_undivided_run(tables):
+@pytest.mark.parametrize("uncertainty", [0, 1])
+def test_two_emulated_ranks_merge_to_the_undivided_run(tables, uncertainty):
     import torch
     from paper_2111_11687_b200 import Simulation
     from paper_2111_11687_b200.multi_gpu import STAT_SUM_KEYS, plan_shards
     cfg = anm_inputs.make_config(3, 4)
     n, B = 500_000, 10
     with Simulation(0) as one:
-        _load(one, cfg, tables, n_batches=B, collect_stats=1)
+        _load(one, cfg, tables, n_batches=B, collect_stats=1, uncertainty=uncertainty)
         one.run(n, cfg["seed"])
         ref = {"energy": one.get_energy().astype(np.float64), "rel": one.get_uncertainty().astype(np.float64),
                "dose": one.get_dose().astype(np.float64), "organs": one.get_organ_doses(), "stats": one.get_stats()}
@@ -35,7 +36,7 @@ def test_two_emulated_ranks_merge_to_the_undivided_run(tables):
     try:
         bufs, stats = [], []
         for sh, sim in zip(shards, sims):
-            _load(sim, cfg, tables, n_batches=sh.n_batches, history_offset=sh.history_offset, collect_stats=1)
+            _load(sim, cfg, tables, n_batches=sh.n_batches, history_offset=sh.history_offset, collect_stats=1, uncertainty=uncertainty)
             sim.run(sh.n_decays, cfg["seed"])
             bufs.append(sim.get_tally_buffers())
             stats.append(sim.get_stats())
