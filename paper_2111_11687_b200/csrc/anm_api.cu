@@ -26,6 +26,10 @@ namespace {
 constexpr double kGyPerMeVPerGram = 1.602176634e-10;
 constexpr int kAutoSchedule = 2;   // anm_options.schedule = 0: the warp event pool (1.4x schedule 1 on cfg3, profiles/)
 
+// Device buffers come from the device's default stream-ordered memory pool (its release threshold is raised in
+// anm_create, so freed blocks stay cached in the process): creating and destroying contexts then costs microseconds
+// instead of driver allocations of hundreds of MB.  alloc / release keep cudaMalloc / cudaFree semantics: the pointer
+// is usable on any stream on return, and a release waits for the device like cudaFree does.
 template <typename T>
 struct DevBuf {
     T* p = nullptr;
@@ -34,11 +38,15 @@ struct DevBuf {
         if (count == n && p) return cudaSuccess;
         release();
         if (count == 0) return cudaSuccess;
-        cudaError_t e = cudaMalloc(&p, count * sizeof(T));
+        cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&p), count * sizeof(T), (cudaStream_t)0);
+        if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)0);
         if (e == cudaSuccess) n = count; else p = nullptr;
         return e;
     }
-    void release() { if (p) cudaFree(p); p = nullptr; n = 0; }
+    void release() {
+        if (p) { cudaDeviceSynchronize(); cudaFreeAsync(p, (cudaStream_t)0); }
+        p = nullptr; n = 0;
+    }
 };
 
 }  // namespace
@@ -369,6 +377,14 @@ int anm_create(anm_ctx** out, int cuda_device) {
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, cuda_device) != cudaSuccess) { delete c; return ANM_E_CUDA; }
     c->num_sms = prop.multiProcessorCount;
+    {   // keep freed device memory cached in the default pool (see DevBuf)
+        cudaMemPool_t pool;
+        if (cudaDeviceGetDefaultMemPool(&pool, cuda_device) == cudaSuccess) {
+            unsigned long long keep = ~0ull;
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        }
+        cudaGetLastError();
+    }
     *out = c;
     return ANM_OK;
 }
