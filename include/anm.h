@@ -26,7 +26,9 @@
  *   - `on_device` = 0: the pointer is host memory (borrowed for the duration of the call, copied);
  *     `on_device` = 1: it is a CUDA device pointer on the ctx's device (e.g. torch.Tensor.data_ptr()),
  *     read / written on the ctx stream.  The caller owns every buffer it passes in or receives into.
- *   - The ctx owns all device memory it allocates and frees it in anm_destroy.  A ctx is not thread-safe;
+ *   - The ctx owns all device memory it allocates and frees it in anm_destroy (the blocks come from the device's
+ *     default stream-ordered memory pool, whose release threshold anm_create raises so that they stay cached in the
+ *     process -- the one process-wide setting the library touches).  A ctx is not thread-safe;
  *     separate ctxs are independent.  There is no global state, no CPU fallback and no other backend:
  *     every call that needs the GPU fails with ANM_E_CUDA when there is none.
  *   - Units: mm at this interface for lengths, MeV for energies, g/cm^3, cm^2/g, Gy, Bq.
@@ -87,8 +89,9 @@ typedef struct {
                                    (regenerate in place, compact by event type); same histories either way */
     int32_t collect_stats;      /* 1: fill the counters and escaped energy of anm_stats (slower)         */
     int32_t warp_aggregate;     /* 1: merge same-voxel deposits within a warp before the atomic (schedule 1) */
-    int32_t hull_majorant;      /* 0 auto / 1 on: flights outside the bounding box of the dense voxels use the
-                                   low-density margin's own majorant and stop on the box surface; 2 off     */
+    int32_t hull_majorant;      /* 0 auto / 1 on: a photon that has left the bounding box of the dense voxels on a
+                                   straight line (it cannot re-enter a convex box) flies against the majorant of
+                                   the low-density margin outside the box until it scatters; 2 off            */
     uint64_t history_offset;    /* index of the first history: anm_run simulates offset .. offset+n_decays-1
                                    (multi-GPU sharding of one logical run by whole batches); default 0      */
     int32_t electron_transport; /* 0: secondary electrons deposited where they are set free (north_star);
