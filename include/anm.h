@@ -88,7 +88,11 @@ typedef struct {
     int32_t schedule;           /* 0 auto, 1 history-based persistent lanes, 2 event-based warp pool
                                    (regenerate in place, compact by event type); same histories either way */
     int32_t collect_stats;      /* 1: fill the counters and escaped energy of anm_stats (slower)         */
-    int32_t warp_aggregate;     /* 1: merge same-voxel deposits within a warp before the atomic (schedule 1) */
+    int32_t warp_aggregate;     /* deposits of the lanes of a warp that hit the same voxel in one trip are merged
+                                   (__match_any_sync) into one atomic.  Pays only where deposits pile onto few voxels
+                                   (DESIGN.md §5.1 has the measurement): 0 auto = on iff positron energy is deposited and
+                                   the source is a point or fewer than 1024 active voxels; 1 on; 2 off.  Same tallies up
+                                   to fp32 atomic order.  1 with electron_transport or uncertainty = 1: ANM_E_UNSUPPORTED */
     int32_t hull_majorant;      /* 0 auto / 1 on: a photon that has left the bounding box of the dense voxels on a
                                    straight line (it cannot re-enter a convex box) flies against the majorant of
                                    the low-density margin outside the box until it scatters; 2 off            */
@@ -247,6 +251,29 @@ int anm_philox_blocks(anm_ctx* c, uint64_t seed, const uint32_t* counters, size_
  * transport kernel calls; out_MeV (HOST, nx*ny*nz floats) receives the energy each voxel got, *escaped_MeV the
  * energy carried out of the grid.  Needs grid, phantom and electron tables; leaves the run state untouched. */
 int anm_trace_electrons(anm_ctx* c, const float* electrons, size_t n, float* out_MeV, size_t n_voxels, double* escaped_MeV);
+
+/* --- roofline microbenchmarks (BASELINE.json metric "% of L2/atomic roofline") ----------
+ * What this device sustains for the three things the transport kernel does, measured with hand-written kernels of the
+ * same access shape (csrc/anm_peaks.cuh), best of 3 timed launches after a warm-up, CUDA events on the ctx stream:
+ *   issue_gtis      1e9 thread-instructions/s of a dependency-free FFMA + LOP3 stream at full occupancy (the
+ *                   denominator of the ALU / issue roofline; the loop's own overhead is not counted: a lower bound)
+ *   philox_gblocks  1e9 Philox4x32-10 blocks/s, back to back (the generator the kernels call)
+ *   gather_gps[k]   1e9 random 4-byte ld.global.nc per second over an array of bytes[k] (the texel fetch)
+ *   red_gps[k]      1e9 random fp32 RED.ADD per second over an array of bytes[k] (the tally)
+ * k = 0: small_bytes (choose a size that fits the L2, e.g. cfg3's 105 MB volume), k = 1: large_bytes (one that does not,
+ * e.g. cfg4's 630 MB).  Sizes are rounded down to a multiple of 4, must be >= 4096 and < 16 GiB.  Scratch memory is
+ * allocated for the call and released.  Needs only a ctx.  ANM_E_ARG for bad sizes, ANM_E_NOMEM / ANM_E_CUDA. */
+typedef struct {
+    double issue_gtis;
+    double issue_sm_mhz;      /* SM clock held during the issue stream (clock64 over the launch / its duration): a pure
+                                 FFMA + LOP3 stream on every SM is power-limited, so the clock drops below clocks.max.sm;
+                                 issue_gtis / (SMs x 128 lanes x issue_sm_mhz) = the fraction of issue slots filled */
+    double philox_gblocks;
+    double gather_gps[2];
+    double red_gps[2];
+    uint64_t bytes[2];
+} anm_peaks;
+int anm_measure_peaks(anm_ctx* c, uint64_t small_bytes, uint64_t large_bytes, anm_peaks* out);
 
 /* --- one logical run over several GPUs ---------------------------------------
  * Histories are independent and keyed by index (Philox counter = history index), so a run of N decays in B batches

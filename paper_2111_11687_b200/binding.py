@@ -21,7 +21,7 @@ ANM_SYMBOLS = [
     "anm_default_options", "anm_run", "anm_get_energy", "anm_get_dose", "anm_get_dose_rate", "anm_get_uncertainty",
     "anm_get_organ_doses", "anm_get_stats", "anm_get_tally_buffers", "anm_merge", "anm_get_alias_table",
     "anm_default_hu_ramp", "anm_load_ct", "anm_get_phantom", "anm_load_pet",
-    "anm_set_electron_tables", "anm_trace_electrons", "anm_philox_blocks",
+    "anm_set_electron_tables", "anm_trace_electrons", "anm_philox_blocks", "anm_measure_peaks",
 ]
 
 STATUS = {0: "ANM_OK", -1: "ANM_E_ARG", -2: "ANM_E_STATE", -3: "ANM_E_CUDA", -4: "ANM_E_NOMEM", -5: "ANM_E_UNSUPPORTED"}
@@ -67,6 +67,11 @@ class anm_stats(C.Structure):
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
+
+
+class anm_peaks(C.Structure):
+    _fields_ = [("issue_gtis", C.c_double), ("issue_sm_mhz", C.c_double), ("philox_gblocks", C.c_double), ("gather_gps", C.c_double * 2),
+                ("red_gps", C.c_double * 2), ("bytes", C.c_uint64 * 2)]
 
 
 ANM_MAX_RAMP_NODES = 16
@@ -135,6 +140,7 @@ def load(build_if_missing: bool = True):
         "anm_set_electron_tables": (i32, [vp, C.POINTER(anm_electron_tables)]),
         "anm_trace_electrons": (i32, [vp, vp, sz, vp, sz, C.POINTER(dbl)]),
         "anm_philox_blocks": (i32, [vp, u64, vp, sz, vp]),
+        "anm_measure_peaks": (i32, [vp, u64, u64, C.POINTER(anm_peaks)]),
         "anm_default_hu_ramp": (i32, [C.POINTER(anm_hu_ramp)]),
         "anm_load_ct": (i32, [vp, vp, i32, i32, i32, dbl, dbl, dbl, dbl, dbl, dbl, C.POINTER(anm_hu_ramp), i32]),
         "anm_get_phantom": (i32, [vp, vp, vp, sz, i32]),
@@ -379,6 +385,14 @@ class Simulation:
         s = anm_stats()
         self._ck(self._L.anm_get_stats(self._ctx, C.byref(s)))
         return s.as_dict()
+
+    def measure_peaks(self, small_bytes: int = 104_857_600, large_bytes: int = 629_145_600) -> dict:
+        """Roofline microbenchmarks of this device (include/anm.h anm_measure_peaks)."""
+        pk = anm_peaks()
+        self._ck(self._L.anm_measure_peaks(self._ctx, int(small_bytes), int(large_bytes), C.byref(pk)))
+        return {"issue_gtis": pk.issue_gtis, "issue_sm_mhz": pk.issue_sm_mhz, "philox_gblocks": pk.philox_gblocks,
+                "gather_gps": [pk.gather_gps[0], pk.gather_gps[1]], "red_gps": [pk.red_gps[0], pk.red_gps[1]],
+                "bytes": [int(pk.bytes[0]), int(pk.bytes[1])]}
 
     def get_alias_table(self) -> np.ndarray:
         """uint32 [n_entries][4] = {threshold, own voxel, alias voxel, 0} of the loaded activity map."""

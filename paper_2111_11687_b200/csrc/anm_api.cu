@@ -13,6 +13,7 @@
 #include "anm_kernels.cuh"
 #include "anm_alias.cuh"
 #include "anm_frontend.cuh"
+#include "anm_peaks.cuh"
 
 #include <cub/device/device_scan.cuh>
 #include <cub/device/device_select.cuh>
@@ -288,8 +289,9 @@ TransportFn pick_transport(int schedule, bool stats, bool wagg, bool elec, bool 
     if (schedule == 2) {
         if (hbh) return elec ? (stats ? transport_pool_kernel<true, true, true> : transport_pool_kernel<false, true, true>)
                              : (stats ? transport_pool_kernel<true, false, true> : transport_pool_kernel<false, false, true>);
-        return elec ? (stats ? transport_pool_kernel<true, true, false> : transport_pool_kernel<false, true, false>)
-                    : (stats ? transport_pool_kernel<true, false, false> : transport_pool_kernel<false, false, false>);
+        if (elec) return stats ? transport_pool_kernel<true, true, false> : transport_pool_kernel<false, true, false>;
+        if (wagg) return stats ? transport_pool_kernel<true, false, false, true> : transport_pool_kernel<false, false, false, true>;
+        return stats ? transport_pool_kernel<true, false, false> : transport_pool_kernel<false, false, false>;
     }
     return stats ? (wagg ? transport_kernel<true, true> : transport_kernel<true, false>)
                  : (wagg ? transport_kernel<false, true> : transport_kernel<false, false>);
@@ -976,7 +978,9 @@ int anm_set_options(anm_ctx* c, const anm_options* o) {
     if (!(o->positron_ke_MeV >= 0) || !std::isfinite(o->positron_ke_MeV)) return fail(c, ANM_E_ARG, "options: positron energy must be >= 0");
     if (o->schedule < 0 || o->schedule > 2) return fail(c, ANM_E_ARG, "options: schedule must be 0, 1 or 2");
     if (o->hull_majorant < 0 || o->hull_majorant > 2) return fail(c, ANM_E_ARG, "options: hull_majorant must be 0, 1 or 2");
-    if (o->schedule == 2 && o->warp_aggregate) return fail(c, ANM_E_UNSUPPORTED, "options: warp_aggregate is a schedule-1 option");
+    if (o->warp_aggregate < 0 || o->warp_aggregate > 2) return fail(c, ANM_E_ARG, "options: warp_aggregate must be 0 (auto), 1 (on) or 2 (off)");
+    if (o->warp_aggregate == 1 && (o->electron_transport || o->uncertainty == 1))
+        return fail(c, ANM_E_UNSUPPORTED, "options: warp_aggregate merges direct tally atomics; electron_transport / history-by-history scoring do not use them");
     if (o->electron_transport != 0 && o->electron_transport != 1) return fail(c, ANM_E_ARG, "options: electron_transport must be 0 or 1");
     if (o->batch_pipeline < 0 || o->batch_pipeline > 3) return fail(c, ANM_E_ARG, "options: batch_pipeline must be 0 (auto), 1, 2 or 3");
     if (o->uncertainty != 0 && o->uncertainty != 1) return fail(c, ANM_E_ARG, "options: uncertainty must be 0 (batch) or 1 (history by history)");
@@ -1056,9 +1060,13 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     const int threads = schedule == 2 ? kPoolThreads : kThreads;
     const size_t smem_el = (c->opt.electron_transport && schedule == 2) ? (size_t)c->e_nm * c->e_nt * 4 : 0;   // range tables
     const size_t smem = smem_tables + smem_el + (schedule == 2 ? (size_t)kPoolWarps * kPoolWarpBytes : (size_t)6 * kThreads * 4);
-    const bool S = c->opt.collect_stats != 0, W = c->opt.warp_aggregate != 0;
     const bool EL = c->opt.electron_transport != 0;
     const bool HB = c->opt.uncertainty == 1;
+    // warp-aggregated tally atomics: on request, or (auto) where every decay's positron energy lands in one or a few
+    // voxels -- a point source or a handful of active voxels -- and 32 same-address atomics per SOURCE trip would
+    // serialise at the L2 (measured: 160 ms -> 18 ms per 1e8 histories on cfg1 with positron energy)
+    const bool hot_source = c->opt.positron_ke_MeV > 0 && (c->point_source || c->n_alias < 1024u);
+    const bool S = c->opt.collect_stats != 0, W = c->opt.warp_aggregate == 1 || (c->opt.warp_aggregate == 0 && hot_source && !EL && !HB);
     const TransportFn kern = pick_transport(schedule, S, W, EL, HB);
     ANM_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 0;
@@ -1260,6 +1268,81 @@ int anm_merge(anm_ctx* c, uint64_t total_decays, int total_batches, const double
     s.deposited_MeV = dep;
     c->run_decays = total_decays;
     c->run_batches = total_batches;
+    return ANM_OK;
+}
+
+// ---- roofline microbenchmarks (anm_peaks.cuh) -------------------------------------------------------------------
+int anm_measure_peaks(anm_ctx* c, uint64_t small_bytes, uint64_t large_bytes, anm_peaks* out) {
+    if (!c) return ANM_E_ARG;
+    if (!out) return fail(c, ANM_E_ARG, "peaks: null pointer");
+    const uint64_t sizes[2] = {small_bytes / 4 * 4, large_bytes / 4 * 4};
+    for (uint64_t b : sizes)
+        if (b < 4096 || b >= (16ull << 30)) return fail(c, ANM_E_ARG, "peaks: array sizes must be in [4096, 16 GiB)");
+    ANM_CUDA(c, cudaSetDevice(c->device));
+    std::memset(out, 0, sizeof *out);
+    cudaStream_t st = c->stream;
+    cudaEvent_t e0, e1;
+    ANM_CUDA(c, cudaEventCreate(&e0));
+    ANM_CUDA(c, cudaEventCreate(&e1));
+    DevBuf<float> arr, sink;
+    struct Cleanup { DevBuf<float>&a, &b; cudaEvent_t &e0, &e1; ~Cleanup() { a.release(); b.release(); cudaEventDestroy(e0); cudaEventDestroy(e1); } } cleanup{arr, sink, e0, e1};
+    ANM_CUDA(c, sink.alloc(4));
+    const int blocks = c->num_sms * 2;            // 64 resident warps per SM
+    const double threads = (double)blocks * kPeakThreads;
+    // best of 3 timed launches after one warm-up; returns seconds
+    auto timed = [&](auto&& launch, double* sec) -> int {
+        double best = 1e30;
+        for (int rep = 0; rep < 4; ++rep) {
+            ANM_CUDA(c, cudaEventRecord(e0, st));
+            launch();
+            ANM_CUDA(c, cudaGetLastError());
+            ANM_CUDA(c, cudaEventRecord(e1, st));
+            ANM_CUDA(c, cudaEventSynchronize(e1));
+            float ms = 0;
+            ANM_CUDA(c, cudaEventElapsedTime(&ms, e0, e1));
+            if (rep > 0) best = std::min(best, (double)ms * 1e-3);
+        }
+        *sec = best;
+        return ANM_OK;
+    };
+    double sec = 0;
+    int rc;
+    {
+        const int iters = 4096;
+        DevBuf<long long> cyc;
+        ANM_CUDA(c, cyc.alloc(1));
+        rc = timed([&] { issue_kernel<<<blocks, kPeakThreads, 0, st>>>(sink.p, cyc.p, iters, 1.0000001f, 1e-9f, 0x5bd1e995u); }, &sec);
+        long long cycles = 0;
+        if (rc == ANM_OK && cudaMemcpy(&cycles, cyc.p, 8, cudaMemcpyDeviceToHost) != cudaSuccess) rc = fail(c, ANM_E_CUDA, "peaks: copy failed");
+        cyc.release();
+        if (rc != ANM_OK) return rc;
+        out->issue_gtis = threads * iters * kIssueUnroll * kIssuePerIter / sec * 1e-9;
+        // two CTAs share an SM and run the whole launch side by side, so the first warp's loop spans the launch
+        out->issue_sm_mhz = (double)cycles / sec * 1e-6;
+    }
+    {
+        TransportParams p;
+        std::memset(&p, 0, sizeof p);
+        for (int r = 0; r < 10; ++r) { p.rk[2 * r] = 42u + (unsigned)r * 0x9E3779B9u; p.rk[2 * r + 1] = (unsigned)r * 0xBB67AE85u; }
+        const int nb = 2048;
+        rc = timed([&] { philox_chain_kernel<<<blocks, kPeakThreads, 0, st>>>(p, (unsigned*)sink.p, nb); }, &sec);
+        if (rc != ANM_OK) return rc;
+        out->philox_gblocks = threads * nb / sec * 1e-9;
+    }
+    for (int k = 0; k < 2; ++k) {
+        const size_t n = (size_t)(sizes[k] / 4);
+        out->bytes[k] = sizes[k];
+        ANM_CUDA(c, arr.alloc(n));
+        ANM_CUDA(c, cudaMemsetAsync(arr.p, 0, n * 4, st));
+        const unsigned n32 = (unsigned)std::min<size_t>(n, 0xffffffffu);
+        const int trips = 256;
+        rc = timed([&] { gather_kernel<<<blocks, kPeakThreads, 0, st>>>((const uint32_t*)arr.p, n32, trips, (unsigned*)sink.p); }, &sec);
+        if (rc != ANM_OK) return rc;
+        out->gather_gps[k] = threads * trips * kGatherInFlight / sec * 1e-9;
+        rc = timed([&] { red_kernel<<<blocks, kPeakThreads, 0, st>>>(arr.p, n32, trips / 4); }, &sec);
+        if (rc != ANM_OK) return rc;
+        out->red_gps[k] = threads * (trips / 4) * kGatherInFlight / sec * 1e-9;
+    }
     return ANM_OK;
 }
 

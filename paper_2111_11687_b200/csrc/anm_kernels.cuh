@@ -42,7 +42,11 @@ constexpr int kMinBlocksPerSM = 4;
 #ifndef ANM_CHUNK
 #define ANM_CHUNK 128
 #endif
-constexpr unsigned kChunk = ANM_CHUNK;      // histories a warp takes per atomic (32 was measured slower: the refill atomic's latency shows)
+constexpr unsigned kChunk = ANM_CHUNK;      // histories a warp takes per atomic
+#ifndef ANM_CHUNK_TAIL
+#define ANM_CHUNK_TAIL 32
+#endif
+constexpr unsigned kChunkTail = ANM_CHUNK_TAIL;   // ... near the end of a launch (event pool: guided chunk sizes)
 constexpr float kE0 = 0.51099895f;          // MeV, "0.511 MeV"
 constexpr float kInvE0 = 1.0f / 0.51099895f;
 constexpr float kTwoPi = 6.283185307179586f;
@@ -589,6 +593,7 @@ __device__ __forceinline__ void hbh_push(const TransportParams& p, unsigned gslo
 #ifndef ANM_POOL_THREADS
 #define ANM_POOL_THREADS 1024
 #endif
+
 #ifndef ANM_POOL_MIN_BLOCKS
 #define ANM_POOL_MIN_BLOCKS 1
 #endif
@@ -609,7 +614,7 @@ enum : int { F_X = 0, F_Y, F_Z, F_U, F_V, F_W, F_E, F_TV /* FLY: ln-E grid coord
 enum : int { Q_F = 0, Q_C = 1, Q_S = 2, Q_R = 3, Q_NONE = 4 };
 constexpr size_t kPoolWarpBytes = (size_t)kSlotFields * kSlots * 4 + 4 * kSlots;   // slots + the four queues (bytes)
 
-template <bool STATS, bool ELEC, bool HBH>
+template <bool STATS, bool ELEC, bool HBH, bool WAGG = false>
 __global__ void __launch_bounds__(kPoolThreads, kPoolMinBlocksPerSM)
 transport_pool_kernel(const __grid_constant__ TransportParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -641,6 +646,14 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
     unsigned heads = 0u, cnts = (unsigned)kSlots << (8 * Q_S);
     unsigned pool_next = 0, pool_end = 0;   // warp-uniform
     bool exhausted = false;                 // warp-uniform
+    // History indices are taken from the launch's counter in chunks, one atomic per chunk, asked for before the warp runs
+    // out (the reply is read a few trips later, so its latency never shows).  Guided sizes: kChunk while much of the
+    // launch is left, kChunkTail once fewer than two full chunks per warp of the grid remain -- the warps then finish
+    // within a few decays of each other instead of up to kChunk decays apart (the drain at the end of a launch).
+    unsigned pend_base = 0, pend_take = 0;  // pend_base: lane 0
+    bool pend_valid = false;                // warp-uniform
+    const unsigned tail_zone = gridDim.x * (unsigned)kPoolWarps * kChunk * 2u;
+    auto chunk_size = [&](const unsigned seen) { return (p.n_hist - min(seen, p.n_hist) > tail_zone) ? kChunk : kChunkTail; };
     const float t0 = (float)p.ie0 + p.fe0;  // ln-E grid coordinate of E0
     const float t_max = (float)(p.ne - 1) - 1.0f / 1024.0f;
 
@@ -711,16 +724,22 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
         unsigned hl_new = 0;
         if (X == Q_S) {                     // hand out history indices (warp-uniform bookkeeping)
             if (pool_next == pool_end) {
-                unsigned base = 0;
-                if (lane == 0) base = atomicAdd(p.counter, kChunk);
-                base = __shfl_sync(0xffffffffu, base, 0);
+                // the chunk asked for at the end of an earlier SOURCE trip (its atomic has been in flight since), else now
+                if (!pend_valid) { pend_take = chunk_size(pool_end); if (lane == 0) pend_base = atomicAdd(p.counter, pend_take); }
+                const unsigned base = __shfl_sync(0xffffffffu, pend_base, 0);
+                pend_valid = false;
                 pool_next = min(base, p.n_hist);
-                pool_end = min(base + kChunk, p.n_hist);
+                pool_end = min(base + pend_take, p.n_hist);
                 if (pool_next == pool_end) { exhausted = true; continue; }
             }
             n = min(n, pool_end - pool_next);
             hl_new = pool_next + lane;
             pool_next += n;
+            if (pool_end - pool_next < 32u && !pend_valid) {      // ask for the next chunk now, use it a few trips later
+                pend_take = chunk_size(pool_end);
+                if (lane == 0) pend_base = atomicAdd(p.counter, pend_take);
+                pend_valid = true;
+            }
         }
         const unsigned shX = 8u * (unsigned)X;
         const unsigned head = heads >> shX;
@@ -783,7 +802,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                                               : electron_walk(p, s_er, x, y, z, u, v, w, vox, Epe);
                         if (STATS) { esc += out; ++c_el; }
                     } else if (HBH) hbh_push(p, gslot0 + slot, SU[F_HL * kSlots], vox, Epe, c_ovf);
-                    else atomicAdd(p.batch + vox, Epe);
+                    else deposit<WAGG>(p.batch, vox, Epe);
                 }
                 if (STATS && code == FLY_ESCAPED) { esc += Bk[F_E * kSlots]; ++c_esc; }
             }
@@ -836,7 +855,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                         SU[F_META * kSlots] = (meta & ~0x74u) + 256u;     // a scatter clears AWAY
                         next = Q_F;
                     }
-                    if (dep > 0.0f) { if (HBH) hbh_push(p, gslot0 + slot, SU[F_HL * kSlots], vox, dep, c_ovf); else atomicAdd(p.batch + vox, dep); }
+                    if (dep > 0.0f) { if (HBH) hbh_push(p, gslot0 + slot, SU[F_HL * kSlots], vox, dep, c_ovf); else deposit<WAGG>(p.batch, vox, dep); }
                 } else {
                     SU[F_META * kSlots] = meta + 256u;
                     next = Q_C;
@@ -862,7 +881,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                 B1[F_E * kSlots] = kE0; B1[F_TV * kSlots] = t0;
                 SU[F_HL * kSlots] = hl_new;
                 SU[F_META * kSlots] = in_box ? (2u | 8u) : 0u;
-                if (p.positron_ke > 0.0f) { if (HBH) hbh_push(p, gslot0 + slot, SU[F_HL * kSlots], voxel, p.positron_ke, c_ovf); else atomicAdd(p.batch + voxel, p.positron_ke); }
+                if (p.positron_ke > 0.0f) { if (HBH) hbh_push(p, gslot0 + slot, SU[F_HL * kSlots], voxel, p.positron_ke, c_ovf); else deposit<WAGG>(p.batch, voxel, p.positron_ke); }
                 q[Q_F * kSlots + ((heads + cnts + lane) & (kSlots - 1))] = (unsigned char)slot;
             }
             cnts += n;

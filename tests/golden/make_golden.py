@@ -1,6 +1,7 @@
 """Writes the stored oracle results under tests/golden/ -- calls ONLY oracle/ and anm_inputs/.
 
     python tests/golden/make_golden.py --cfg 3 --decays 100000000 --procs 8
+    python tests/golden/make_golden.py --cfg 3 --decays 1000000000 --procs 6 --tag _1e9     (the north-star target size)
 
 For config k at full size this runs the CPU oracle (oracle/anm_oracle.cpp) on N decays in 100 batches
 with seed 1000 + (the config's seed) -- deliberately NOT the seed the CUDA run uses, so the two
@@ -37,6 +38,7 @@ def main():
     ap.add_argument("--decays", type=float, default=1e8)
     ap.add_argument("--procs", type=int, default=os.cpu_count())
     ap.add_argument("--sample", type=int, default=20000)
+    ap.add_argument("--tag", default="", help="file-name suffix, e.g. _1e9 -> cfg3_1e9_oracle_*.{json,csv} (keeps the 1e8 files)")
     a = ap.parse_args()
     cfg = anm_inputs.make_config(a.cfg)
     tables = anm_inputs.make_tables()
@@ -45,7 +47,7 @@ def main():
     o = O.Oracle(cfg, tables, n_decays=n, n_batches=100, seed=seed)
     r = o.run_parallel(a.procs)
     f = o.finalize(r)
-    tag = os.path.join(HERE, "cfg%d_oracle" % a.cfg)
+    tag = os.path.join(HERE, "cfg%d%s_oracle" % (a.cfg, a.tag))
     meta = {"config": cfg["name"], "shape": cfg["shape"], "spacing_mm": cfg["spacing_mm"], "n_decays": n,
             "n_batches": 100, "seed": seed, "cores": r["cores"], "wall_seconds": r["seconds"],
             "stats": r["stats"], "max_dose_gy_per_decay_non_air": float(np.where(o.material != 0, f["dose"], 0.0).max()),

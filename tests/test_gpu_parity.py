@@ -224,8 +224,9 @@ def test_determinism_and_history_keying(anm, tables):
     assert np.allclose(a["energy"], h1["energy"] + h2["energy"], rtol=1e-4, atol=1e-3)
     c = gpu_run(anm, cfg, tables, n, n_batches=B, seed=cfg["seed"] + 7)
     assert not np.allclose(a["energy"], c["energy"], rtol=1e-4, atol=1e-3)
-    w = gpu_run(anm, cfg, tables, n, n_batches=B, warp_aggregate=1)
-    assert np.allclose(a["energy"], w["energy"], rtol=1e-4, atol=1e-3)
+    for sched in (1, 2):                                             # warp-aggregated atomics: same tallies
+        w = gpu_run(anm, cfg, tables, n, n_batches=B, warp_aggregate=1, schedule=sched)
+        assert np.allclose(a["energy"], w["energy"], rtol=1e-4, atol=1e-3)
 
 
 @pytest.mark.parametrize("k,scale,n,B", [(3, 4, 400_000, 10), (0, 2, 200_000, 10), (2, 4, 200_000, 10)])
@@ -376,8 +377,9 @@ def test_error_codes(anm, tables):
                 sim.set_options(**kw)
             assert ei.value.code == -1
         with pytest.raises(E) as ei:
-            sim.set_options(schedule=2, warp_aggregate=1)
+            sim.set_options(warp_aggregate=1, uncertainty=1)         # the deposit lists of that mode use no direct atomics
         assert ei.value.code == -5                                   # ANM_E_UNSUPPORTED
+        sim.set_options(schedule=2, warp_aggregate=1)                # both schedules merge same-voxel deposits on request
         sim.set_options(n_batches=10, photons_per_decay=1)
         with pytest.raises(E) as ei:
             sim.run(1005, 1)                                         # N % B != 0 (reading C15)
