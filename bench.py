@@ -31,8 +31,11 @@ sys.path.insert(0, ROOT)
 
 WORKLOAD = "cfg3_patient 256x256x400 @2x2x4mm, 27 organs, pairs+positron KE, 100 batches"
 
-# algorithmic thread-instructions per event (what the method's arithmetic needs, counted from the
-# definitions: Philox4x32-10 = 100 integer ops per 4 words, ...), multiplied by the measured events per decay.
+# DESIGN.md §5.1 / §6: algorithmic thread-instructions per event = the SASS instructions the per-event device functions
+# execute per lane (Philox4x32-10 + uniforms, fly_land / fly_two, compton_try + rotate + energy coordinate, rayleigh_try,
+# sample_source), counted from the ncu source page of the transport kernel (profiles/r2_event_instr.md has the command and
+# the table); the event pool's scheduling instructions (ring push / pick / pop, slot load / store, meta word) are NOT in
+# them.  Multiplied by the events per decay measured by a counted run.
 INSTR_SUBSTEP = 84.0     # half a Philox block, log, 3 FMA, voxel index, texel fetch + unpack, table lerp, accept test
 INSTR_COMPTON_TRY = 210.0
 INSTR_RAYLEIGH_TRY = 180.0
@@ -114,13 +117,16 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--decays", type=float, default=1e9, help="decays per step per GPU")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--ref-decays-per-core", type=int, default=100_000)
+    ap.add_argument("--ref-decays-per-core", type=int, default=400_000)
     ap.add_argument("--cpu-baseline-decays-per-core", type=int, default=400_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--config", type=int, default=3, choices=[3, 4],
                     help="BASELINE.json config to run: 3 = the bench workload (default); 4 = the 512x512x600 scale case, "
-                         "for profiling only (use with --no-frontend --no-variants; its line is not a bench number)")
+                         "for profiling only (use with --no-frontend --no-variants; its line is not a bench number; the "
+                         "default run reports cfg4 under variants.cfg4_fullres)")
+    ap.add_argument("--no-peaks", action="store_true", help="skip the roofline microbenchmarks (anm_measure_peaks)")
+    ap.add_argument("--no-cfg4", action="store_true", help="skip the cfg4 scale case in variants")
     ap.add_argument("--no-frontend", action="store_true", help="skip the image front-end timing (anm_load_ct / anm_load_pet)")
     ap.add_argument("--no-variants", action="store_true", help="skip the electron-transport / history-by-history runs")
     args = ap.parse_args()
@@ -168,8 +174,13 @@ def main():
     act = torch.from_numpy(cfg["activity"]).to(dev)
     lab = torch.from_numpy(cfg["labels"]).to(dev)
     sim = Simulation(local_rank)
+    peaks_dev = None
     with torch.cuda.stream(stream):
         sim.set_stream(stream)
+        if not args.no_peaks:
+            # roofline microbenchmarks of THIS device: before the warm-up steps, so that the clock
+            # the power-limited issue stream pulls down has recovered when the timed region starts
+            peaks_dev = sim.measure_peaks(104_857_600, 629_145_600)
         sim.set_grid(cfg["shape"], cfg["spacing_mm"])
         sim.load_phantom(mat, rho)
         sim.load_activity(act)
@@ -210,30 +221,70 @@ def main():
         ms_total = float(t.item())
     value = world * D * args.steps / (ms_total * 1e-3)
 
-    # ---- roofline of the dominant kernel (transport): ALU / issue bound, DESIGN.md §6 ------------------------
+    # ---- roofline of the dominant kernel (transport), DESIGN.md §5.1 / §6 ------------------------------------------
+    # Four resources, each with its algorithmic demand per decay and a MEASURED denominator:
+    #   alu        thread-instructions of the method's arithmetic  vs  the issue rate of a dependency-free FFMA + LOP3
+    #              stream (anm_measure_peaks), per clock, at the SM clock this run held
+    #   l2_gather  one random 4-byte texel read per Woodcock sub-step  vs  random ld.global.nc over a 105 MB array
+    #   red        one fp32 RED per deposit (Compton, photoelectric, positron)  vs  random RED.ADD over a 105 MB array
+    #   hbm        algorithmic bytes (4 B texel, 8 B tally RMW, 16 B alias entry)  vs  MEASURED_PEAKS.json hbm_gbs
+    # (cfg4 uses the 630 MB figures.)  The binding one is named by ncu (issue-slot utilisation vs L2 / DRAM throughput,
+    # profiles/): the ALU / issue side on cfg3; `bound`, `achieved`, `peak`, `frac` repeat that entry.
     compton_tries = per_decay["n_compton"] * 1.15
     instr_per_decay = (per_decay["n_steps"] * INSTR_SUBSTEP + compton_tries * INSTR_COMPTON_TRY +
                        per_decay["n_rayleigh"] * INSTR_RAYLEIGH_TRY * 1.4 + per_decay["n_pe"] * INSTR_PE + INSTR_SOURCE)
     launches_transport = B * args.steps
     sec_per_launch = ms_t * 1e-3 / launches_transport
-    achieved = instr_per_decay * (D / B) / sec_per_launch / 1e9                     # G thread-instr / s
+    decays_per_s_kernel = (D / B) / sec_per_launch
+    achieved = instr_per_decay * decays_per_s_kernel / 1e9                          # G thread-instr / s
     sm_max = clk.get("sm_max_mhz") or 1965.0
-    peak = N_SM * LANES_PER_SM_PER_CLK * sm_max * 1e6 / 1e9
-    traffic = None          # dram__bytes_read.sum + dram__bytes_write.sum per launch, from the committed ncu capture
+    sm_run = clk.get("sm_mhz") or sm_max
+    nominal = N_SM * LANES_PER_SM_PER_CLK * sm_max * 1e6 / 1e9
+    file_peaks = {}
+    try:
+        file_peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm_peak = float(file_peaks.get("hbm_gbs", 6500.0))
+    big = args.config == 4
+    deposits = per_decay["n_compton"] + per_decay["n_pe"] + (1.0 if cfg["positron_ke_mev"] > 0 else 0.0)
+    alg_bytes = 4.0 * per_decay["n_steps"] + 8.0 * deposits + 16.0
+    if peaks_dev:
+        slots_per_clk = peaks_dev["issue_gtis"] * 1e9 / (N_SM * LANES_PER_SM_PER_CLK * peaks_dev["issue_sm_mhz"] * 1e6)
+        peak = slots_per_clk * N_SM * LANES_PER_SM_PER_CLK * sm_run * 1e6 / 1e9
+        peak_source = ("anm_measure_peaks: %.1f Gthread-instr/s at %.0f MHz (power-limited) = %.3f of the issue slots per clock, "
+                       "x 148 SM x 128 lanes x %.0f MHz held during the timed region" % (peaks_dev["issue_gtis"], peaks_dev["issue_sm_mhz"], slots_per_clk, sm_run))
+        g_peak, r_peak = peaks_dev["gather_gps"][1 if big else 0], peaks_dev["red_gps"][1 if big else 0]
+    else:
+        peak, peak_source = nominal, "nominal 148 SM x 4 SMSP x 32 lanes x %.0f MHz (clocks.max.sm); --no-peaks" % sm_max
+        g_peak = r_peak = None
+    g_ach = per_decay["n_steps"] * decays_per_s_kernel / 1e9
+    r_ach = deposits * decays_per_s_kernel / 1e9
+    h_ach = alg_bytes * decays_per_s_kernel / 1e9
+    traffic, traffic_source = None, None   # dram__bytes_read.sum + dram__bytes_write.sum per launch, from the committed ncu capture
     tdir = os.path.join(ROOT, "profiles")
     for name in sorted(os.listdir(tdir) if os.path.isdir(tdir) else [], reverse=True):
         if name.endswith("_transport_traffic.csv"):
             import csv
             rows = list(csv.DictReader(open(os.path.join(tdir, name))))
-            if rows and int(rows[-1]["decays_per_launch"]) == D // B:
+            if rows and int(rows[-1]["decays_per_launch"]) == D // B and args.config == 3:
                 traffic = int(rows[-1]["dram_bytes_read"]) + int(rows[-1]["dram_bytes_write"])
+                traffic_source = "profiles/%s (ncu --set full capture of this kernel and launch size; not measured in this run)" % name
             break
     roofline = {"bound": "alu", "kernel": "transport_pool_kernel", "achieved": achieved, "peak": peak, "unit": "Gthread-instr/s",
-                "frac": achieved / peak, "traffic": traffic,
-                "peak_source": "148 SM x 4 SMSP x 32 lanes x %.0f MHz (clocks.max.sm), DESIGN.md §6" % sm_max,
+                "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_source, "peak_source": peak_source,
+                "alu": {"achieved": achieved, "peak": peak, "frac": achieved / peak, "unit": "Gthread-instr/s",
+                        "peak_nominal": nominal, "peak_power_limited": peaks_dev["issue_gtis"] if peaks_dev else None},
+                "l2_gather": {"achieved": g_ach, "peak": g_peak, "frac": g_ach / g_peak if g_peak else None, "unit": "G loads/s",
+                              "array_bytes": peaks_dev["bytes"][1 if big else 0] if peaks_dev else None},
+                "red": {"achieved": r_ach, "peak": r_peak, "frac": r_ach / r_peak if r_peak else None, "unit": "G atomics/s"},
+                "hbm": {"achieved": h_ach, "peak": hbm_peak, "frac": h_ach / hbm_peak, "unit": "GB/s",
+                        "peak_source": "MEASURED_PEAKS.json hbm_gbs" if file_peaks else "fallback 6500 GB/s"},
+                "peaks_measured": peaks_dev,
                 "instr_per_decay_algorithmic": instr_per_decay, "events_per_decay": per_decay,
                 "avg_launch_ms": sec_per_launch * 1e3, "share_of_step": ms_t / max(ms_t + ms_f + ms_fin, 1e-9),
-                "texel_bytes_per_decay": 4.0 * per_decay["n_steps"], "tally_bytes_per_decay": 8.0 * (per_decay["n_real"] - per_decay["n_rayleigh"] + 1)}
+                "texel_bytes_per_decay": 4.0 * per_decay["n_steps"], "tally_bytes_per_decay": 8.0 * deposits,
+                "algorithmic_bytes_per_decay": alg_bytes}
 
     # ---- end to end through the C ABI from host buffers ----------------------------------------------------
     e2e = None
@@ -241,20 +292,33 @@ def main():
         hm, hr = torch.from_numpy(cfg["material"]).pin_memory(), torch.from_numpy(cfg["density"]).pin_memory()
         ha, hl = torch.from_numpy(cfg["activity"]).pin_memory(), torch.from_numpy(cfg["labels"]).pin_memory()
         out_d, out_u = torch.empty(V, dtype=torch.float32).pin_memory(), torch.empty(V, dtype=torch.float32).pin_memory()
+        phases = {}
+
         def e2e_step():
+            tp = time.perf_counter()
+
+            def lap(name):
+                nonlocal tp
+                t = time.perf_counter()
+                phases[name] = phases.get(name, 0.0) + (t - tp) * 1e3
+                tp = t
+
             with Simulation(local_rank) as s2:
-                s2.set_grid(cfg["shape"], cfg["spacing_mm"])
-                s2.load_phantom(hm, hr)
-                s2.load_activity(ha)
-                s2.load_organs(hl, cfg["n_organs"])
+                s2.set_grid(cfg["shape"], cfg["spacing_mm"]); lap("create+set_grid")
+                s2.load_phantom(hm, hr); lap("load_phantom (131 MB H2D + pack + hull)")
+                s2.load_activity(ha); lap("load_activity (105 MB H2D + alias table)")
+                s2.load_organs(hl, cfg["n_organs"]); lap("load_organs (26 MB H2D + masses)")
                 s2.set_physics_tables(tables)
-                s2.set_options(**opts)
-                step(s2)
-                s2.get_dose(out_d)
-                s2.get_uncertainty(out_u)
-                return s2.get_organ_doses(), s2.get_stats()
+                s2.set_options(**opts); lap("tables+options")
+                step(s2); lap("run")
+                s2.get_dose(out_d); lap("get_dose (kernel + 105 MB D2H)")
+                s2.get_uncertainty(out_u); lap("get_uncertainty (kernel + 105 MB D2H)")
+                r = s2.get_organ_doses(), s2.get_stats()
+            lap("organs+stats+destroy")
+            return r
 
         e2e_step()                                   # untimed: first-touch of the pinned buffers, allocator warm-up
+        phases.clear()
         if dist:
             dist.barrier()
         torch.cuda.synchronize(dev)
@@ -270,6 +334,7 @@ def main():
         assert float(out_d.sum()) > 0 and organs["mean_Gy_per_decay"].max() > 0
         e2e = {"value": world * D / dt, "unit": "decays/s", "h2d_bytes_per_step": V * (1 + 4 + 4 + 1),
                "d2h_bytes_per_step": V * 8 + 27 * 56, "seconds": dt, "ms_setup_device": st2["ms_setup"],
+               "phases_ms": {k: v / args.steps for k, v in phases.items()},
                "what": "anm_set_grid + load_phantom/activity/organs (host) + tables + anm_run + get_dose + get_uncertainty + get_organ_doses (host)"}
 
     # ---- image front end: set-up, not part of decays/s; HBM roofline of its two kernels -------
@@ -317,6 +382,34 @@ def main():
                 ms = stv["ms_transport"] + stv["ms_fold"] + stv["ms_finalize"]
                 variants[name] = {"decays": nv, "ms": ms, "value": nv / (ms * 1e-3), "unit": "decays/s"}
             sim.set_options(collect_stats=0, **opts)
+        # BASELINE.json configs[4], the full-resolution scale case (tally 630 MB > L2: the HBM-atomic regime), 1e9 of its
+        # decays, device time of anm_run; its own context (4.5 GB), released afterwards
+        if not args.no_cfg4 and args.config == 3:
+            del mat, rho, act, lab
+            cfg4 = anm_inputs.make_config(4)
+            with torch.cuda.stream(stream), Simulation(local_rank) as s4:
+                s4.set_stream(stream)
+                s4.load_config(cfg4, tables, n_batches=100, collect_stats=1)
+                s4.run(10_000_000, cfg4["seed"])
+                c4 = s4.get_stats()
+                s4.set_options(n_batches=100, positron_ke_MeV=cfg4["positron_ke_mev"])
+                n4 = min(D, 1_000_000_000)
+                s4.run(n4, cfg4["seed"])
+                s4.run(n4, cfg4["seed"])
+                st4 = s4.get_stats()
+                ms4 = st4["ms_transport"] + st4["ms_fold"] + st4["ms_finalize"]
+                dps4 = n4 / (ms4 * 1e-3)
+                steps4, dep4 = c4["n_steps"] / 1e7, (c4["n_compton"] + c4["n_pe"]) / 1e7 + 1.0
+                v4 = {"workload": "cfg4_fullres 512x512x600 @0.98x0.98x3mm, 27 organs, pairs+positron KE, 100 batches",
+                      "decays": n4, "ms": ms4, "value": dps4, "unit": "decays/s",
+                      "events_per_decay": {"n_steps": steps4, "deposits": dep4}}
+                if peaks_dev:      # the memory side binds here: random DRAM gathers + REDs over 630 MB volumes
+                    t_model = steps4 / (peaks_dev["gather_gps"][1] * 1e9) + dep4 / (peaks_dev["red_gps"][1] * 1e9)
+                    v4["roofline"] = {"bound": "hbm random access", "gather_frac": steps4 * dps4 / 1e9 / peaks_dev["gather_gps"][1],
+                                      "red_frac": dep4 * dps4 / 1e9 / peaks_dev["red_gps"][1],
+                                      "decays_per_s_if_gathers_and_reds_were_serial_at_peak": 1.0 / t_model}
+            variants["cfg4_fullres"] = v4
+            del cfg4
 
     if rank != 0:
         if dist:

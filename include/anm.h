@@ -113,7 +113,21 @@ typedef struct {
                                    internal streams, so that the CTAs of batch b+1 take over the SMs as those of batch
                                    b drain; the same histories and tallies; then ms_transport covers the whole
                                    pipeline (folds inside it) and ms_fold is 0.                                    */
-    int32_t reserved1;
+    int32_t tally;              /* how deposits reach the per-batch tally: 1 = one fp32 atomic (RED) per
+                                   deposit into the batch volume; 2 = tile-binned: a deposit is appended as an 8-byte record
+                                   {voxel, energy} to the list of the voxel's tile (2^14 consecutive voxels; position from
+                                   one atomic on the tile's counter, shared by the lanes of a warp that hit the same
+                                   tile) and the per-batch fold sums each tile's list in shared memory -- streaming HBM
+                                   traffic instead of random read-modify-writes once the volume no longer fits the L2.
+                                   The first batch of a run counts the deposits per tile (it runs with direct atomics)
+                                   and sizes the lists; a deposit that finds its list full takes the direct path
+                                   (anm_stats.n_tally_overflow), so the result never depends on the sizing.  0 auto = 1:
+                                   measured on one B200 the binned path gains 3 % on BASELINE.json cfg4 (630 MB volumes)
+                                   and loses on cfg3 (the tile counters' same-address atomics bound it).
+                                   2 needs the event-pool schedule, the batch estimator, local electrons and no warp
+                                   aggregation (else ANM_E_UNSUPPORTED).  Same tallies up to fp32 summation order.
+                                   Test hook: the environment variable ANM_TALLY_CAPACITY=<n> fixes every list at n
+                                   records (forces the overflow path).                                              */
 } anm_options;
 
 /* Electron data for anm_options.electron_transport ("The cutoff energies for
@@ -151,6 +165,9 @@ typedef struct {
     uint64_t n_launches;                                   /* kernels launched by the last anm_run         */
     double ms_load_ct, ms_load_pet;                        /* device time of the last anm_load_ct / anm_load_pet
                                                               resample kernels (also counted in ms_setup)   */
+    uint64_t tally_binned;                                 /* 1: the last run used the tile-binned tally (anm_options.tally) */
+    uint64_t n_tally_overflow;                             /* deposits that found their tile's list full and took the
+                                                              direct path; the counting batch is not included        */
 } anm_stats;
 
 /* HU -> (material, density) conversion curve ("Hounsfield unit (HU)-to-density conversion curve";

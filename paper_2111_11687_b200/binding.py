@@ -45,7 +45,7 @@ class anm_options(C.Structure):
                 ("schedule", C.c_int32), ("collect_stats", C.c_int32), ("warp_aggregate", C.c_int32),
                 ("hull_majorant", C.c_int32), ("history_offset", C.c_uint64),
                 ("electron_transport", C.c_int32), ("uncertainty", C.c_int32),
-                ("batch_pipeline", C.c_int32), ("reserved1", C.c_int32)]
+                ("batch_pipeline", C.c_int32), ("tally", C.c_int32)]
 
 
 class anm_electron_tables(C.Structure):
@@ -63,7 +63,8 @@ class anm_stats(C.Structure):
     _fields_ = [("emitted_MeV", C.c_double), ("deposited_MeV", C.c_double), ("escaped_MeV", C.c_double)] + [
         (n, C.c_uint64) for n in ("n_decays", "n_steps", "n_real", "n_pe", "n_compton", "n_rayleigh", "n_escaped", "n_cutoff", "n_electrons", "n_hbh_overflow")] + [
         ("ms_transport", C.c_double), ("ms_fold", C.c_double), ("ms_finalize", C.c_double), ("ms_setup", C.c_double),
-        ("n_launches", C.c_uint64), ("ms_load_ct", C.c_double), ("ms_load_pet", C.c_double)]
+        ("n_launches", C.c_uint64), ("ms_load_ct", C.c_double), ("ms_load_pet", C.c_double),
+        ("tally_binned", C.c_uint64), ("n_tally_overflow", C.c_uint64)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}

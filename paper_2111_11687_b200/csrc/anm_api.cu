@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -97,6 +98,11 @@ struct anm_ctx {
     DevBuf<float> e_ring;                 // waiting electrons of the event pool (electron_transport)
     DevBuf<float> hbh_sq;                 // [Vpad] sum over histories of X_h^2 (anm_options.uncertainty = 1)
     DevBuf<uint2> hbh_list;               // [(kHbhCap + 1) * hbh_nslots] per-slot deposit lists
+    // tile-binned tally (anm_options.tally): per launch in flight the tiles' counters and deposit records; one table of
+    // {offset, capacity} per tile; the device counter of deposits that overflowed their segment
+    DevBuf<unsigned> bin_cnt;
+    DevBuf<uint2> bin_seg, bin_seg0, bin_rec;
+    DevBuf<unsigned long long> bin_ovf;
     bool run_hbh = false;                 // the last run scored history by history
     DevBuf<uint8_t> labels;
     DevBuf<uint4> alias;
@@ -284,17 +290,18 @@ struct HostE0 { int ie; float fe, maj, inv_maj; };
 
 using TransportFn = void (*)(const TransportParams);
 
-// schedule 1 (history-based lanes) or 2 (warp-scope event pool), with / without counters and warp aggregation
-TransportFn pick_transport(int schedule, bool stats, bool wagg, bool elec, bool hbh) {
+// schedule 1 (history-based lanes) or 2 (warp-scope event pool), with / without counters; tally = TALLY_RED / _WAGG / _BINNED
+TransportFn pick_transport(int schedule, bool stats, int tally, bool elec, bool hbh) {
     if (schedule == 2) {
         if (hbh) return elec ? (stats ? transport_pool_kernel<true, true, true> : transport_pool_kernel<false, true, true>)
                              : (stats ? transport_pool_kernel<true, false, true> : transport_pool_kernel<false, false, true>);
         if (elec) return stats ? transport_pool_kernel<true, true, false> : transport_pool_kernel<false, true, false>;
-        if (wagg) return stats ? transport_pool_kernel<true, false, false, true> : transport_pool_kernel<false, false, false, true>;
+        if (tally == TALLY_WAGG) return stats ? transport_pool_kernel<true, false, false, TALLY_WAGG> : transport_pool_kernel<false, false, false, TALLY_WAGG>;
+        if (tally == TALLY_BINNED) return stats ? transport_pool_kernel<true, false, false, TALLY_BINNED> : transport_pool_kernel<false, false, false, TALLY_BINNED>;
         return stats ? transport_pool_kernel<true, false, false> : transport_pool_kernel<false, false, false>;
     }
-    return stats ? (wagg ? transport_kernel<true, true> : transport_kernel<true, false>)
-                 : (wagg ? transport_kernel<false, true> : transport_kernel<false, false>);
+    return stats ? (tally == TALLY_WAGG ? transport_kernel<true, TALLY_WAGG> : transport_kernel<true, TALLY_RED>)
+                 : (tally == TALLY_WAGG ? transport_kernel<false, TALLY_WAGG> : transport_kernel<false, TALLY_RED>);
 }
 
 // A11 on the current sum / sumsq volumes: finalize_kernel, then the organ arithmetic of SURVEY.md §8(c) step 7 on the
@@ -399,7 +406,7 @@ int anm_destroy(anm_ctx* c) {
     c->organ_batch.release(); c->organ_acc.release(); c->organ_mass.release(); c->organ_count.release();
     c->total_energy.release(); c->d_tot.release(); c->d_maj.release(); c->d_majo.release(); c->d_x2.release(); c->d_cum.release();
     c->d_pec.release(); c->d_flags.release(); c->d_erange.release(); c->e_ring.release(); c->hbh_sq.release(); c->hbh_list.release();
-    c->batch2.release(); c->batch3.release();
+    c->batch2.release(); c->batch3.release(); c->bin_cnt.release(); c->bin_seg.release(); c->bin_seg0.release(); c->bin_rec.release(); c->bin_ovf.release();
     for (auto& ps : c->pipe) if (ps) { cudaStreamDestroy(ps); ps = nullptr; }
     delete c;
     return ANM_OK;
@@ -984,6 +991,9 @@ int anm_set_options(anm_ctx* c, const anm_options* o) {
     if (o->electron_transport != 0 && o->electron_transport != 1) return fail(c, ANM_E_ARG, "options: electron_transport must be 0 or 1");
     if (o->batch_pipeline < 0 || o->batch_pipeline > 3) return fail(c, ANM_E_ARG, "options: batch_pipeline must be 0 (auto), 1, 2 or 3");
     if (o->uncertainty != 0 && o->uncertainty != 1) return fail(c, ANM_E_ARG, "options: uncertainty must be 0 (batch) or 1 (history by history)");
+    if (o->tally < 0 || o->tally > 2) return fail(c, ANM_E_ARG, "options: tally must be 0 (auto), 1 (direct atomics) or 2 (tile-binned)");
+    if (o->tally == 2 && (o->schedule == 1 || o->electron_transport || o->uncertainty == 1 || o->warp_aggregate == 1))
+        return fail(c, ANM_E_UNSUPPORTED, "options: the tile-binned tally runs in the event-pool schedule with the batch estimator, local electrons and no warp aggregation");
     if (o->uncertainty == 1 && o->schedule == 1) return fail(c, ANM_E_UNSUPPORTED, "options: history-by-history scoring runs in the event-pool schedule (0 or 2)");
     if (o->electron_transport && o->schedule == 1) return fail(c, ANM_E_UNSUPPORTED, "options: electron transport runs in the event-pool schedule (0 or 2)");
     c->opt = *o;
@@ -1067,7 +1077,11 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     // serialise at the L2 (measured: 160 ms -> 18 ms per 1e8 histories on cfg1 with positron energy)
     const bool hot_source = c->opt.positron_ke_MeV > 0 && (c->point_source || c->n_alias < 1024u);
     const bool S = c->opt.collect_stats != 0, W = c->opt.warp_aggregate == 1 || (c->opt.warp_aggregate == 0 && hot_source && !EL && !HB);
-    const TransportFn kern = pick_transport(schedule, S, W, EL, HB);
+    // tile-binned tally: on request only -- measured +3 % on cfg4 (630 MB volumes) and 0.43x on cfg3, the
+    // tile counters' same-address atomics bound it; needs the event pool, the batch estimator and local electrons
+    const bool can_bin = schedule == 2 && !EL && !HB && !W;
+    const bool BIN = can_bin && c->opt.tally == 2;
+    const TransportFn kern = pick_transport(schedule, S, BIN ? TALLY_BINNED : (W ? TALLY_WAGG : TALLY_RED), EL, HB);
     ANM_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 0;
     ANM_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem));
@@ -1116,23 +1130,73 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
         for (int k = 0; k < depth; ++k)
             if (!c->pipe[k]) ANM_CUDA_EV(cudaStreamCreateWithFlags(&c->pipe[k], cudaStreamNonBlocking));
     }
+    // tile-binned tally: counters per launch in flight, one {offset, capacity} table; the capacities come from batch 0,
+    // which runs with empty segments (every deposit takes the direct-RED path and is counted per tile)
+    const unsigned n_tiles = (unsigned)((c->Vpad + kTileVoxels - 1) >> kTileShift);
+    const unsigned n_lists = n_tiles * kTileSub;
+    size_t bin_total = 0;                 // records per launch in flight
+    if (BIN) {
+        ANM_CUDA_EV(c->bin_cnt.alloc((size_t)depth * n_lists));
+        ANM_CUDA_EV(c->bin_seg.alloc(n_lists));
+        ANM_CUDA_EV(c->bin_seg0.alloc(n_lists));
+        ANM_CUDA_EV(cudaMemsetAsync(c->bin_seg0.p, 0, (size_t)n_lists * 8, st));
+        ANM_CUDA_EV(c->bin_ovf.alloc(2));      // [0] the run's overflow count, [1] the counting batch's (discarded)
+        ANM_CUDA_EV(cudaMemsetAsync(c->bin_cnt.p, 0, (size_t)depth * n_lists * 4, st));
+        ANM_CUDA_EV(cudaMemsetAsync(c->bin_seg.p, 0, (size_t)n_lists * 8, st));
+        ANM_CUDA_EV(cudaMemsetAsync(c->bin_ovf.p, 0, 16, st));
+        ANM_CUDA_EV(cudaFuncSetAttribute(bin_fold_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kTileVoxels * 4)));
+        p.bin_seg = c->bin_seg.p;
+    }
     ANM_CUDA_EV(cudaEventRecord(ev[0], st));
     if (depth > 1) for (int k = 0; k < depth; ++k) ANM_CUDA_EV(cudaStreamWaitEvent(c->pipe[k], ev[0], 0));
     for (int b = 0; b < B; ++b) {
         cudaStream_t sb = depth > 1 ? c->pipe[b % depth] : st;
         p.batch = bufs[b % depth];
+        if (BIN) {
+            p.bin_cnt = c->bin_cnt.p + (size_t)(b % depth) * n_lists;
+            p.bin_rec = c->bin_rec.p ? c->bin_rec.p + (size_t)(b % depth) * bin_total : nullptr;
+        }
         if (EL) p.e_ring = c->e_ring.p + (size_t)(b % depth) * blocks * kPoolWarps * 8 * kPend;
         if (HB) p.hbh_list = c->hbh_list.p + (size_t)(b % depth) * kHbhCap * p.hbh_nslots;
         p.counter = c->counters.p + b;
         p.hist_base = c->opt.history_offset + (unsigned long long)b * nb;
         kern<<<blocks, threads, smem, sb>>>(p);
         ANM_CUDA_EV(cudaGetLastError());
+        if (BIN && b == 0) {
+            // the counting batch has run: size every tile's segment for the batches to come -- its count plus six
+            // standard deviations of a Poisson count plus 32 (a tile that still overflows loses nothing: the surplus
+            // takes the direct-RED path into the batch volume, bin_fold_kernel adds both)
+            std::vector<unsigned> cnt(n_lists);
+            ANM_CUDA_EV(cudaMemcpyAsync(cnt.data(), p.bin_cnt, (size_t)n_lists * 4, cudaMemcpyDeviceToHost, sb));
+            ANM_CUDA_EV(cudaStreamSynchronize(sb));
+            std::vector<uint2> seg(n_lists);
+            const char* cap_env = std::getenv("ANM_TALLY_CAPACITY");      // test hook (anm.h): a fixed capacity per tile
+            const long cap_test = cap_env ? std::atol(cap_env) : 0;
+            for (unsigned t = 0; t < n_lists; ++t) {
+                const double want = (double)cnt[t] + 6.0 * std::sqrt((double)cnt[t]) + 32.0;
+                const unsigned cap = cap_test > 0 ? (unsigned)cap_test : (unsigned)std::min(want, 4.0e9 - 1.0);
+                if (bin_total + cap > 0xfffffff0ull) { free_events(); return fail(c, ANM_E_UNSUPPORTED, "run: more than 2^32 deposit records per batch; use more batches or tally = 1"); }
+                seg[t] = make_uint2((unsigned)bin_total, cap);
+                bin_total += cap;
+            }
+            ANM_CUDA_EV(c->bin_rec.alloc((size_t)depth * bin_total));
+            ANM_CUDA_EV(cudaMemcpyAsync(c->bin_seg.p, seg.data(), (size_t)n_lists * 8, cudaMemcpyHostToDevice, sb));
+            ANM_CUDA_EV(cudaStreamSynchronize(sb));     // seg is a host temporary; every later launch (any stream) sees the table
+        }
         if (depth > 1 && b > 0) ANM_CUDA_EV(cudaStreamWaitEvent(sb, ev[2 * (b - 1) + 2], 0));    // after the previous fold
         ANM_CUDA_EV(cudaEventRecord(ev[2 * b + 1], sb));
-        fold_kernel<<<fold_blocks, kFoldThreads, 0, sb>>>(
-            (float4*)p.batch, (float4*)c->sum.p, (float4*)c->sumsq.p,
-            c->have_organs ? (const uint32_t*)c->labels.p : nullptr, (const uint4*)c->texels.p,
-            c->organ_batch.p + (size_t)b * 256, c->n_organs, c->Vpad / 4, inv_vox);
+        if (BIN) {
+            // batch 0 counted against empty segments; its fold must see them empty too (the table is already final)
+            bin_fold_kernel<<<std::min<unsigned>(n_tiles, (unsigned)c->num_sms * 3u), kBinFoldThreads, kTileVoxels * 4, sb>>>(
+                p.bin_cnt, b == 0 ? c->bin_seg0.p : c->bin_seg.p, p.bin_rec, (float4*)p.batch, (float4*)c->sum.p, (float4*)c->sumsq.p,
+                c->have_organs ? (const uint32_t*)c->labels.p : nullptr, (const uint4*)c->texels.p,
+                c->organ_batch.p + (size_t)b * 256, c->n_organs, c->Vpad / 4, n_tiles, inv_vox, c->bin_ovf.p + (b == 0 ? 1 : 0));
+        } else {
+            fold_kernel<<<fold_blocks, kFoldThreads, 0, sb>>>(
+                (float4*)p.batch, (float4*)c->sum.p, (float4*)c->sumsq.p,
+                c->have_organs ? (const uint32_t*)c->labels.p : nullptr, (const uint4*)c->texels.p,
+                c->organ_batch.p + (size_t)b * 256, c->n_organs, c->Vpad / 4, inv_vox);
+        }
         ANM_CUDA_EV(cudaGetLastError());
         ANM_CUDA_EV(cudaEventRecord(ev[2 * b + 2], sb));
     }
@@ -1147,6 +1211,8 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     }
     ANM_CUDA_EV(cudaEventRecord(ev[2 * B + 1], st));
     DeviceStats ds;
+    unsigned long long bin_overflow = 0;
+    if (BIN) ANM_CUDA_EV(cudaMemcpyAsync(&bin_overflow, c->bin_ovf.p, 8, cudaMemcpyDeviceToHost, st));
     ANM_CUDA_EV(cudaMemcpyAsync(&ds, c->dstats.p, sizeof ds, cudaMemcpyDeviceToHost, st));
     ANM_CUDA_EV(cudaStreamSynchronize(st));
 
@@ -1180,6 +1246,8 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     s.ms_transport = ms_t; s.ms_fold = ms_f; s.ms_finalize = ms_fin; s.ms_setup = c->ms_setup;
     s.ms_load_ct = c->ms_load_ct; s.ms_load_pet = c->ms_load_pet;
     s.n_launches = (uint64_t)2 * B + 1;
+    s.tally_binned = BIN ? 1 : 0;
+    s.n_tally_overflow = bin_overflow;
     c->run_decays = n_decays;
     c->run_batches = B;
     c->have_results = true;

@@ -103,6 +103,13 @@ struct TransportParams {
     uint2* hbh_list;
     float* hbh_sq;               // [V] sum over histories of X_h^2 (MeV^2), whole run
     unsigned hbh_nslots;
+    // tile-binned tally (anm_options.tally): when the tally volume does not fit the L2, a deposit is not a
+    // random RED into HBM but a record {voxel, energy} appended to the list of the voxel's tile (kTileVoxels consecutive
+    // voxels): bin_cnt[tile] hands out positions, bin_seg[tile] = {offset, capacity} of the tile's segment of bin_rec;
+    // a deposit beyond the capacity goes to the batch volume as before.  bin_fold_kernel sums the lists in shared memory.
+    unsigned* bin_cnt;
+    const uint2* bin_seg;
+    uint2* bin_rec;
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -150,17 +157,41 @@ __device__ __forceinline__ void rotate(float& u, float& v, float& w, float cos_t
     u = a * n; v = b * n; w = c * n;
 }
 
-template <bool WAGG>
-__device__ __forceinline__ void deposit(float* __restrict__ batch, unsigned vox, float e) {
-    if (WAGG) {
+// How a deposit reaches the tally (template parameter of the transport kernels)
+enum : int { TALLY_RED = 0, TALLY_WAGG = 1, TALLY_BINNED = 2 };
+constexpr int kTileShift = 14;                       // tile = 2^14 consecutive voxels = 64 KB of fp32 in shared memory
+constexpr unsigned kTileVoxels = 1u << kTileShift;
+#ifndef ANM_TILE_SUBLISTS
+#define ANM_TILE_SUBLISTS 1
+#endif
+constexpr unsigned kTileSub = ANM_TILE_SUBLISTS;     // lists per tile (a CTA appends to list blockIdx % kTileSub).  Same-address atomics serialise at the L2:
+                                                     // 8 lists per tile took cfg3 from 559 to 348 ms per 1e9 decays, but cfg4 from 505 to 534 ms (more open
+                                                     // write streams); neither beats direct atomics on cfg3 (238 ms), cfg4 gains 3 % at 1
+
+template <int TALLY>
+__device__ __forceinline__ void deposit(const TransportParams& p, unsigned vox, float e) {
+    if (TALLY == TALLY_WAGG) {
         // merge the deposits of lanes that hit the same voxel in this trip: one RED per distinct voxel
         const unsigned act = __activemask();
         const unsigned peers = __match_any_sync(act, vox);
         float total = 0.0f;
         for (unsigned rem = peers; rem; rem &= rem - 1) total += __shfl_sync(peers, e, __ffs(rem) - 1);
-        if ((threadIdx.x & 31) == (unsigned)(__ffs(peers) - 1)) atomicAdd(batch + vox, total);
+        if ((threadIdx.x & 31) == (unsigned)(__ffs(peers) - 1)) atomicAdd(p.batch + vox, total);
+    } else if (TALLY == TALLY_BINNED) {
+        // append {voxel, energy} to the tile's list; the lanes of this trip that hit the same tile share one atomic
+        const unsigned tile = (vox >> kTileShift) * kTileSub + (blockIdx.x & (kTileSub - 1u));
+        const unsigned act = __activemask();
+        const unsigned peers = __match_any_sync(act, tile);
+        const int leader = __ffs(peers) - 1;
+        unsigned base = 0;
+        if ((int)(threadIdx.x & 31) == leader) base = atomicAdd(p.bin_cnt + tile, (unsigned)__popc(peers));
+        base = __shfl_sync(peers, base, leader);
+        const unsigned pos = base + __popc(peers & ((1u << (threadIdx.x & 31)) - 1u));
+        const uint2 seg = __ldg(p.bin_seg + tile);
+        if (pos < seg.y) __stcs(p.bin_rec + (size_t)seg.x + pos, make_uint2(vox, __float_as_uint(e)));
+        else atomicAdd(p.batch + vox, e);            // the segment is full (or this is the counting batch): direct RED
     } else {
-        atomicAdd(batch + vox, e);
+        atomicAdd(p.batch + vox, e);
     }
 }
 
@@ -395,7 +426,7 @@ __global__ void electron_trace_kernel(const __grid_constant__ TransportParams p,
     if (out > 0.0f) atomicAdd(escaped, (double)out);
 }
 
-template <bool STATS, bool WAGG>
+template <bool STATS, int TALLY>
 __global__ void __launch_bounds__(kThreads, kMinBlocksPerSM)
 transport_kernel(const __grid_constant__ TransportParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -468,7 +499,7 @@ transport_kernel(const __grid_constant__ TransportParams p) {
             const unsigned voxel = sample_source(p, h, x, y, z, u, v, w, in_box);
             stash[0 * kThreads] = x; stash[1 * kThreads] = y; stash[2 * kThreads] = z;
             stash[3 * kThreads] = u; stash[4 * kThreads] = v; stash[5 * kThreads] = w;
-            if (p.positron_ke > 0.0f) deposit<WAGG>(p.batch, voxel, p.positron_ke);
+            if (p.positron_ke > 0.0f) deposit<TALLY>(p, voxel, p.positron_ke);
             E = kE0; set_t(t0);
             hb_src = in_box ? 1u : 0u; hb = hb_src;
             photon = 0; blk = 0; state = ST_FLY;
@@ -482,7 +513,7 @@ transport_kernel(const __grid_constant__ TransportParams p) {
             const int code = fly_two<STATS>(p, s_tot, s_pec, x, y, z, u, v, w, ie, fe, maj, inv_maj, majo, inv_majo, r, hb, vox, mat, fc);
             ANM_TR("S1 h=%llu ph=%d blk=%u FLY code=%d E=%.9g t=%d+%.9g pos=%.9g %.9g %.9g vox=%u hb=%u\n", h, photon, blk - 1, code, E, ie, fe, x, y, z, vox, hb);
             if (code == FLY_ESCAPED) { if (STATS) { esc += E; ++c_esc; } dead = true; }
-            else if (code == FLY_PE) { if (STATS) ++c_pe; deposit<WAGG>(p.batch, vox, E); dead = true; }   // all energy local
+            else if (code == FLY_PE) { if (STATS) ++c_pe; deposit<TALLY>(p, vox, E); dead = true; }   // all energy local
             else if (code == FLY_COMPTON) state = ST_COMPTON;
             else if (code == FLY_RAYLEIGH) state = ST_RAYLEIGH;
         } else if (state == ST_COMPTON) {
@@ -493,7 +524,7 @@ transport_kernel(const __grid_constant__ TransportParams p) {
                 E *= eps;
                 if (E < p.cutoff) { dep += E; dead = true; if (STATS) ++c_cut; }
                 else { rotate(u, v, w, 1.0f - t, kTwoPi * u01(r.w)); set_energy(E); hb &= 1u; state = ST_FLY; }
-                deposit<WAGG>(p.batch, vox, dep);
+                deposit<TALLY>(p, vox, dep);
             }
         } else {   // ST_RAYLEIGH
             float c;
@@ -614,7 +645,7 @@ enum : int { F_X = 0, F_Y, F_Z, F_U, F_V, F_W, F_E, F_TV /* FLY: ln-E grid coord
 enum : int { Q_F = 0, Q_C = 1, Q_S = 2, Q_R = 3, Q_NONE = 4 };
 constexpr size_t kPoolWarpBytes = (size_t)kSlotFields * kSlots * 4 + 4 * kSlots;   // slots + the four queues (bytes)
 
-template <bool STATS, bool ELEC, bool HBH, bool WAGG = false>
+template <bool STATS, bool ELEC, bool HBH, int TALLY = TALLY_RED>
 __global__ void __launch_bounds__(kPoolThreads, kPoolMinBlocksPerSM)
 transport_pool_kernel(const __grid_constant__ TransportParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -802,7 +833,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                                               : electron_walk(p, s_er, x, y, z, u, v, w, vox, Epe);
                         if (STATS) { esc += out; ++c_el; }
                     } else if (HBH) hbh_push(p, gslot0 + slot, SU[F_HL * kSlots], vox, Epe, c_ovf);
-                    else deposit<WAGG>(p.batch, vox, Epe);
+                    else deposit<TALLY>(p, vox, Epe);
                 }
                 if (STATS && code == FLY_ESCAPED) { esc += Bk[F_E * kSlots]; ++c_esc; }
             }
@@ -855,7 +886,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                         SU[F_META * kSlots] = (meta & ~0x74u) + 256u;     // a scatter clears AWAY
                         next = Q_F;
                     }
-                    if (dep > 0.0f) { if (HBH) hbh_push(p, gslot0 + slot, SU[F_HL * kSlots], vox, dep, c_ovf); else deposit<WAGG>(p.batch, vox, dep); }
+                    if (dep > 0.0f) { if (HBH) hbh_push(p, gslot0 + slot, SU[F_HL * kSlots], vox, dep, c_ovf); else deposit<TALLY>(p, vox, dep); }
                 } else {
                     SU[F_META * kSlots] = meta + 256u;
                     next = Q_C;
@@ -881,7 +912,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                 B1[F_E * kSlots] = kE0; B1[F_TV * kSlots] = t0;
                 SU[F_HL * kSlots] = hl_new;
                 SU[F_META * kSlots] = in_box ? (2u | 8u) : 0u;
-                if (p.positron_ke > 0.0f) { if (HBH) hbh_push(p, gslot0 + slot, SU[F_HL * kSlots], voxel, p.positron_ke, c_ovf); else deposit<WAGG>(p.batch, voxel, p.positron_ke); }
+                if (p.positron_ke > 0.0f) { if (HBH) hbh_push(p, gslot0 + slot, SU[F_HL * kSlots], voxel, p.positron_ke, c_ovf); else deposit<TALLY>(p, voxel, p.positron_ke); }
                 q[Q_F * kSlots + ((heads + cnts + lane) & (kSlots - 1))] = (unsigned char)slot;
             }
             cnts += n;
@@ -952,6 +983,41 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
 // Streaming; most voxels of a patient volume are untouched air (x == 0) and cost one 16-byte read per 4.
 constexpr int kFoldThreads = 256;
 
+// one group of four voxels: sum += x, sumsq += x^2, organ bins += x / (rho V)
+__device__ __forceinline__ void fold_group(const float4 xv, const size_t i, float4* __restrict__ sum, float4* __restrict__ sumsq,
+                                           const uint32_t* __restrict__ labels4, const uint4* __restrict__ texels4,
+                                           double* s_org, const float inv_vox_cm3) {
+    float4 s = sum[i], q = sumsq[i];
+    s.x += xv.x; s.y += xv.y; s.z += xv.z; s.w += xv.w;
+    q.x = fmaf(xv.x, xv.x, q.x); q.y = fmaf(xv.y, xv.y, q.y); q.z = fmaf(xv.z, xv.z, q.z); q.w = fmaf(xv.w, xv.w, q.w);
+    sum[i] = s; sumsq[i] = q;
+    if (labels4 != nullptr) {
+        const uint32_t l4 = labels4[i];
+        if (l4) {
+            const uint4 t = texels4[i];
+            const float xs[4] = {xv.x, xv.y, xv.z, xv.w};
+            const unsigned ts[4] = {t.x, t.y, t.z, t.w};
+            // x / (rho V) in fp32 (1e-7 relative), accumulated in fp64.  The four voxels of a thread usually carry one
+            // label: one shared-memory atomic per thread instead of four (neighbouring lanes hit the same organ bin).
+            const unsigned l0 = l4 & 0xffu;
+            if (l4 == l0 * 0x01010101u) {
+                double acc = 0.0;
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    if (xs[k] != 0.0f) acc += (double)__fdividef(xs[k] * inv_vox_cm3, (float)(ts[k] & 0xffffffu) * kDensityStep);
+                if (acc != 0.0) atomicAdd(&s_org[l0], acc);
+            } else {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const unsigned l = (l4 >> (8 * k)) & 0xffu;
+                    if (l && xs[k] != 0.0f)
+                        atomicAdd(&s_org[l], (double)__fdividef(xs[k] * inv_vox_cm3, (float)(ts[k] & 0xffffffu) * kDensityStep));
+                }
+            }
+        }
+    }
+}
+
 __global__ void __launch_bounds__(kFoldThreads)
 fold_kernel(float4* __restrict__ batch, float4* __restrict__ sum, float4* __restrict__ sumsq,
             const uint32_t* __restrict__ labels4, const uint4* __restrict__ texels4, double* __restrict__ organ_row,
@@ -962,40 +1028,70 @@ fold_kernel(float4* __restrict__ batch, float4* __restrict__ sum, float4* __rest
     for (size_t i = (size_t)blockIdx.x * kFoldThreads + threadIdx.x; i < n4; i += (size_t)gridDim.x * kFoldThreads) {
         const float4 xv = batch[i];
         if (xv.x == 0.0f && xv.y == 0.0f && xv.z == 0.0f && xv.w == 0.0f) continue;
-        float4 s = sum[i], q = sumsq[i];
-        s.x += xv.x; s.y += xv.y; s.z += xv.z; s.w += xv.w;
-        q.x = fmaf(xv.x, xv.x, q.x); q.y = fmaf(xv.y, xv.y, q.y); q.z = fmaf(xv.z, xv.z, q.z); q.w = fmaf(xv.w, xv.w, q.w);
-        sum[i] = s; sumsq[i] = q;
         batch[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (organs) {
-            const uint32_t l4 = labels4[i];
-            if (l4) {
-                const uint4 t = texels4[i];
-                const float xs[4] = {xv.x, xv.y, xv.z, xv.w};
-                const unsigned ts[4] = {t.x, t.y, t.z, t.w};
-                // x / (rho V) in fp32 (1e-7 relative), accumulated in fp64.  The four voxels of a thread usually carry one
-                // label: one shared-memory atomic per thread instead of four (neighbouring lanes hit the same organ bin).
-                const unsigned l0 = l4 & 0xffu;
-                if (l4 == l0 * 0x01010101u) {
-                    double acc = 0.0;
-#pragma unroll
-                    for (int k = 0; k < 4; ++k)
-                        if (xs[k] != 0.0f) acc += (double)__fdividef(xs[k] * inv_vox_cm3, (float)(ts[k] & 0xffffffu) * kDensityStep);
-                    if (acc != 0.0) atomicAdd(&s_org[l0], acc);
-                } else {
-#pragma unroll
-                    for (int k = 0; k < 4; ++k) {
-                        const unsigned l = (l4 >> (8 * k)) & 0xffu;
-                        if (l && xs[k] != 0.0f)
-                            atomicAdd(&s_org[l], (double)__fdividef(xs[k] * inv_vox_cm3, (float)(ts[k] & 0xffffffu) * kDensityStep));
-                    }
-                }
-            }
-        }
+        fold_group(xv, i, sum, sumsq, labels4, texels4, s_org, inv_vox_cm3);
     }
     if (organs) {
         __syncthreads();
         if ((int)threadIdx.x <= n_organs && threadIdx.x > 0 && s_org[threadIdx.x] != 0.0)
+            atomicAdd(organ_row + threadIdx.x, s_org[threadIdx.x]);
+    }
+}
+
+// A10 for the tile-binned tally: a CTA takes one tile at a time, sums the tile's deposit list into a
+// 64 KB shared-memory image of the tile (fp32 shared-memory atomics), adds what overflowed into the batch volume (only
+// if the tile's counter exceeded its capacity), folds the image like fold_kernel and resets the counter.  Tiles that
+// received nothing cost one 4-byte read.  overflow[0] += deposits that did not fit their segment (diagnostic).
+constexpr int kBinFoldThreads = 512;
+__global__ void __launch_bounds__(kBinFoldThreads)
+bin_fold_kernel(unsigned* __restrict__ bin_cnt, const uint2* __restrict__ bin_seg, const uint2* __restrict__ bin_rec,
+                float4* __restrict__ batch, float4* __restrict__ sum, float4* __restrict__ sumsq,
+                const uint32_t* __restrict__ labels4, const uint4* __restrict__ texels4, double* __restrict__ organ_row,
+                int n_organs, size_t n4, unsigned n_tiles, float inv_vox_cm3, unsigned long long* __restrict__ overflow) {
+    extern __shared__ __align__(16) float s_tile[];        // [kTileVoxels]
+    __shared__ double s_org[256];
+    const bool organs = (labels4 != nullptr);
+    if (threadIdx.x < 256) s_org[threadIdx.x] = 0.0;
+    for (unsigned tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        unsigned cnt[kTileSub], any = 0u;
+#pragma unroll
+        for (unsigned k = 0; k < kTileSub; ++k) { cnt[k] = bin_cnt[tile * kTileSub + k]; any |= cnt[k]; }
+        if (any == 0u) continue;                           // block-uniform
+        bool ovf = false;
+        __syncthreads();                                   // everyone has read the counters; the previous tile's image is done with
+        for (unsigned j = threadIdx.x; j < kTileVoxels / 4; j += kBinFoldThreads) reinterpret_cast<float4*>(s_tile)[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+        __syncthreads();
+#pragma unroll 1
+        for (unsigned k = 0; k < kTileSub; ++k) {
+            if (cnt[k] == 0u) continue;
+            const uint2 seg = bin_seg[tile * kTileSub + k];
+            const unsigned n = min(cnt[k], seg.y);
+            if (cnt[k] > seg.y) { ovf = true; if (threadIdx.x == 0) atomicAdd(overflow, (unsigned long long)(cnt[k] - seg.y)); }
+            if (threadIdx.x == 0) bin_cnt[tile * kTileSub + k] = 0u;
+            const uint2* rec = bin_rec + (size_t)seg.x;
+            for (unsigned i = threadIdx.x; i < n; i += kBinFoldThreads) {
+                const uint2 r = __ldcs(rec + i);
+                atomicAdd(&s_tile[r.x & (kTileVoxels - 1u)], __uint_as_float(r.y));
+            }
+        }
+        __syncthreads();
+        const size_t g0 = (size_t)tile * (kTileVoxels / 4);
+        for (unsigned j = threadIdx.x; j < kTileVoxels / 4 && g0 + j < n4; j += kBinFoldThreads) {
+            float4 xv = reinterpret_cast<const float4*>(s_tile)[j];
+            if (ovf) {
+                const float4 o = batch[g0 + j];
+                if (o.x != 0.0f || o.y != 0.0f || o.z != 0.0f || o.w != 0.0f) {
+                    xv.x += o.x; xv.y += o.y; xv.z += o.z; xv.w += o.w;
+                    batch[g0 + j] = make_float4(0.f, 0.f, 0.f, 0.f);
+                }
+            }
+            if (xv.x == 0.0f && xv.y == 0.0f && xv.z == 0.0f && xv.w == 0.0f) continue;
+            fold_group(xv, g0 + j, sum, sumsq, labels4, texels4, s_org, inv_vox_cm3);
+        }
+    }
+    if (organs) {
+        __syncthreads();
+        if ((int)threadIdx.x <= n_organs && threadIdx.x > 0 && threadIdx.x < 256 && s_org[threadIdx.x] != 0.0)
             atomicAdd(organ_row + threadIdx.x, s_org[threadIdx.x]);
     }
 }

@@ -1,0 +1,77 @@
+"""Tile-binned tally (anm_options.tally = 2) against the direct-atomic tally: the same histories, the
+same tallies up to fp32 summation order -- whatever the list capacities are (the overflow path is exact too)."""
+import os
+
+import numpy as np
+import pytest
+
+import anm_inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def anm():
+    import paper_2111_11687_b200 as pkg
+    return pkg
+
+
+@pytest.fixture(scope="module")
+def tables():
+    return anm_inputs.make_tables()
+
+
+def run(anm, cfg, tables, n, **opt):
+    with anm.Simulation(0) as sim:
+        sim.load_config(cfg, tables, **opt)
+        sim.run(n, cfg["seed"])
+        return dict(energy=sim.get_energy(), sigma=sim.get_uncertainty(), organs=sim.get_organ_doses() if cfg["n_organs"] else None,
+                    stats=sim.get_stats())
+
+
+@pytest.mark.parametrize("k,scale,n,B", [(3, 4, 400_000, 10), (2, 4, 200_000, 10), (0, 1, 200_000, 10)])
+def test_binned_equals_direct(anm, tables, k, scale, n, B):
+    cfg = anm_inputs.make_config(k, scale)
+    a = run(anm, cfg, tables, n, n_batches=B, collect_stats=1, tally=1)
+    b = run(anm, cfg, tables, n, n_batches=B, collect_stats=1, tally=2)
+    assert a["stats"]["tally_binned"] == 0 and b["stats"]["tally_binned"] == 1
+    for key in ("n_steps", "n_real", "n_pe", "n_compton", "n_rayleigh", "n_escaped", "n_cutoff"):
+        assert a["stats"][key] == b["stats"][key], key
+    assert np.allclose(a["energy"], b["energy"], rtol=1e-4, atol=1e-3)
+    assert abs(b["stats"]["deposited_MeV"] / a["stats"]["deposited_MeV"] - 1) < 1e-6
+    st = b["stats"]
+    assert abs(st["deposited_MeV"] + st["escaped_MeV"] - st["emitted_MeV"]) < 2e-5 * st["emitted_MeV"]
+    big = a["sigma"] > 0
+    assert np.allclose(a["sigma"][big], b["sigma"][big], rtol=2e-3, atol=1e-5)
+    if a["organs"] is not None:
+        assert np.allclose(a["organs"]["mean_Gy_per_decay"], b["organs"]["mean_Gy_per_decay"], rtol=1e-5)
+        assert np.allclose(a["organs"]["sigma_mean"], b["organs"]["sigma_mean"], rtol=1e-3, atol=1e-30)
+
+
+def test_binned_overflow_path_is_exact(anm, tables):
+    """Lists of 64 records per tile overflow at once: most deposits take the direct path, the sums do not change."""
+    cfg = anm_inputs.make_config(3, 4)
+    n, B = 400_000, 10
+    a = run(anm, cfg, tables, n, n_batches=B, tally=1)
+    os.environ["ANM_TALLY_CAPACITY"] = "64"
+    try:
+        b = run(anm, cfg, tables, n, n_batches=B, tally=2)
+    finally:
+        del os.environ["ANM_TALLY_CAPACITY"]
+    assert b["stats"]["tally_binned"] == 1 and b["stats"]["n_tally_overflow"] > 0
+    assert np.allclose(a["energy"], b["energy"], rtol=1e-4, atol=1e-3)
+    c = run(anm, cfg, tables, n, n_batches=B, tally=2)
+    assert c["stats"]["n_tally_overflow"] < 1e-3 * 6 * n          # sized from the counting batch: overflow is the exception
+
+
+def test_binned_is_refused_where_it_cannot_run(anm, tables):
+    cfg = anm_inputs.make_config(0, 2)
+    with anm.Simulation(0) as sim:
+        sim.load_config(cfg, tables)
+        for kw in (dict(tally=2, schedule=1), dict(tally=2, uncertainty=1), dict(tally=2, warp_aggregate=1)):
+            with pytest.raises(anm.AnmError) as ei:
+                sim.set_options(**kw)
+            assert ei.value.code == -5
+        with pytest.raises(anm.AnmError) as ei:
+            sim.set_options(tally=3)
+        assert ei.value.code == -1
