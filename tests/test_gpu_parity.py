@@ -79,7 +79,9 @@ def check_voxels_z(dose_g, sig_g, dose_o, sig_o, material, frac=1e-3):
 
 def check_balance(st, tol=2e-5):
     assert abs(st["deposited_MeV"] + st["escaped_MeV"] - st["emitted_MeV"]) < tol * st["emitted_MeV"], st
-    assert st["n_real"] == st["n_pe"] + st["n_compton"] + st["n_rayleigh"] + 0 or st["n_real"] >= st["n_pe"] + st["n_compton"]
+    # every real collision ends in exactly one channel; n_compton counts ACCEPTED Klein-Nishina samples and n_rayleigh
+    # accepted form-factor samples, one per collision of that kind
+    assert st["n_real"] == st["n_pe"] + st["n_compton"] + st["n_rayleigh"], st
 
 
 def check_total(st_g, st_o, n, rel_floor=1e-3):
@@ -160,22 +162,24 @@ def test_high_cutoff_vs_oracle(anm, tables):
 
 
 # ------------------------------------------------------------------------------------------------- full size vs golden
-def _golden(k):
-    tag = os.path.join(HERE, "golden", "cfg%d_oracle" % k)
+def _golden(k, tag=""):
+    tag = os.path.join(HERE, "golden", "cfg%d%s_oracle" % (k, tag))
     meta = json.load(open(tag + "_meta.json"))
     org = list(csv.DictReader(open(tag + "_organs.csv")))
     vox = np.loadtxt(tag + "_voxels.csv", delimiter=",", skiprows=1, ndmin=2)
     return meta, org, vox
 
 
-@pytest.mark.parametrize("k", [1, 2, 3])
-def test_full_size_vs_golden(anm, tables, k):
-    """cfg1/cfg2/cfg3 at full size, 1e8 decays, 100 batches, the config's own seed, in the launch configuration
-    bench.py times (collect_stats off); oracle side from tests/golden/ (1e8 decays, seed + 1000)."""
-    meta, org, vox = _golden(k)
+@pytest.mark.parametrize("k,tag", [(1, ""), (2, ""), (3, ""), (3, "_1e9"), (4, "")])
+def test_full_size_vs_golden(anm, tables, k, tag):
+    """cfg1 / cfg2 / cfg3 / cfg4 at full size, 100 batches, the config's own seed, in the launch configuration bench.py
+    times (collect_stats off); oracle side from tests/golden/ (same number of decays, seed + 1000).  cfg1-4 at 1e8
+    decays (north_star: ">= 1e8"); cfg3 also at the north-star target size of 1e9 decays (golden tag _1e9), where the
+    statistical errors are 3.2 times smaller; cfg4 is the full-resolution 512 x 512 x 600 scale case."""
+    meta, org, vox = _golden(k, tag)
     cfg = anm_inputs.make_config(k)
-    assert list(meta["shape"]) == list(cfg["shape"]) and meta["n_decays"] == 100_000_000
-    n, B = 100_000_000, 100
+    n, B = int(meta["n_decays"]), 100
+    assert list(meta["shape"]) == list(cfg["shape"]) and n == (1_000_000_000 if tag == "_1e9" else 100_000_000)
     with anm.Simulation(0) as sim:
         sim.load_config(cfg, tables)
         sim.run(n, cfg["seed"])
@@ -196,15 +200,23 @@ def test_full_size_vs_golden(anm, tables, k):
     S_o, Q_o = vox[:, 1], vox[:, 2]
     nb = n / B
     vox_g = cfg["density"].reshape(-1)[idx].astype(np.float64) * float(np.prod(cfg["spacing_mm"])) * 1e-3
-    dose_mean = 0.5 * (energy[idx].astype(np.float64) + S_o) / n * 1.602176634e-10 / vox_g
-    keep = dose_mean > 0.1 * meta["max_dose_gy_per_decay_non_air"]
-    assert keep.sum() >= min(10, keep.size)
-    idx, S_o, Q_o = idx[keep], S_o[keep], Q_o[keep]
+    k_gy = 1.602176634e-10
     var_o = np.maximum((Q_o / (nb * nb) / B - (S_o / n) ** 2) / (B - 1), 0.0)       # of the per-decay mean energy
     y_g = energy[idx].astype(np.float64) / n
     s_g = y_g * rel[idx].astype(np.float64)
     den = np.sqrt(var_o + s_g ** 2)
-    z = (y_g - S_o / n) / np.where(den > 0, den, 1.0)
+    z_all = (y_g - S_o / n) / np.where(den > 0, den, 1.0)
+    dose_mean = 0.5 * (energy[idx].astype(np.float64) + S_o) / n * k_gy / vox_g
+    keep = dose_mean > 0.1 * meta["max_dose_gy_per_decay_non_air"]
+    assert keep.sum() >= min(10, keep.size)
+    z = z_all[keep]
+    # north_star's literal population beside it (reported, not asserted: the cut on the oracle's own noisy dose selects
+    # its upward fluctuations, reading C25): sampled non-air voxels whose ORACLE dose exceeds 10 % of the oracle's maximum
+    lit = S_o / n * k_gy / vox_g > 0.1 * meta["max_dose_gy_per_decay_non_air"]
+    print("\ncfg%d%s n=%.0e: |z|>4 in %d of %d voxels (C25 population, mean z %.3f, std %.3f); literal oracle-side cut: %d of %d "
+          "(mean z %.3f, std %.3f)" % (k, tag, n, int((np.abs(z) > 4).sum()), z.size, z.mean(), z.std(),
+                                       int((np.abs(z_all[lit]) > 4).sum()), int(lit.sum()), z_all[lit].mean() if lit.any() else 0.0,
+                                       z_all[lit].std() if lit.any() else 0.0))
     assert (np.abs(z) > 4).sum() <= max(1, int(1e-3 * z.size)), ((np.abs(z) > 4).sum(), z.size)
     if z.size > 1000:
         assert abs(z.mean()) < 0.1 and 0.85 < z.std() < 1.2, (z.mean(), z.std())
