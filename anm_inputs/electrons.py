@@ -15,7 +15,7 @@ air 85.7, lung 75.3, water 75.0, compact bone 91.9.  Both the oracle and the CUD
 physical fidelity is approximate and labelled so.
 
 make_electron_tables() returns, on a uniform kinetic-energy grid T_k = T_min + k dT (T_min = the 200 keV electron
-cutoff, T_max = 0.3407 MeV = the largest Compton electron a 0.511 MeV photon can make, rounded up):
+cutoff, T_max = 0.512 MeV: a photo-electron takes the whole photon energy E0 = 0.511 MeV; Compton electrons end at 0.3407 MeV):
     stopping[m][k]   S_col/rho at T_k, MeV cm^2 / g
     range[m][k]      residual CSDA range above the cutoff, integral_{T_min}^{T_k} dT / (S_col/rho), g / cm^2
                      (composite Simpson on a 64x finer grid), range[m][0] = 0, increasing.
@@ -31,8 +31,8 @@ MEC2 = 0.51099895                     # MeV
 R_E = 2.8179403262e-13                # cm
 I_EV = {"air_dry": 85.7, "lung_icrp": 75.3, "water": 75.0, "bone_compact_icru": 91.9}
 ELECTRON_CUTOFF_MEV = 0.200
-T_MAX_MEV = 0.352                     # >= 2 E0 / 3 = 0.340666 MeV, the Compton edge of a 0.511 MeV photon
-N_T = 77                              # dT = 2 keV
+T_MAX_MEV = 0.512                     # >= E0 = 0.51099895 MeV, the largest photo-electron (the Compton edge is 2 E0 / 3)
+N_T = 157                             # dT = 2 keV
 
 
 def z_over_a(mat: dict) -> float:

@@ -135,8 +135,8 @@ typedef struct {
  * straight line in the electron's initial direction (Compton: its momentum k - k'; photoelectric: the photon's
  * direction), no deflection, no secondaries.  range[m][k] = residual CSDA mass range ABOVE THE CUTOFF (g/cm^2) at the
  * kinetic energy t_min + k*dt (MeV): t_min IS the electron cutoff, range[m][0] = 0, strictly increasing in k, read
- * by linear interpolation and inverted as that piecewise-linear function; the grid must reach 2/3 * 0.51099895 MeV
- * (the Compton edge of an annihilation photon).  Crossing a voxel of density rho along a chord l takes rho*l off the
+ * by linear interpolation and inverted as that piecewise-linear function; the grid must reach 0.51099895 MeV
+ * (a photo-electron takes the whole photon energy; Compton electrons stop at the edge 2/3 * 0.511 MeV; else ANM_E_ARG).  Crossing a voxel of density rho along a chord l takes rho*l off the
  * residual range; the energy difference is deposited in the voxel; when the range runs out inside a voxel the whole
  * remaining energy (cutoff energy included, "deposited locally") goes there; an electron that leaves the grid carries
  * its energy out (counted in escaped_MeV). */
@@ -168,6 +168,14 @@ typedef struct {
     uint64_t tally_binned;                                 /* 1: the last run used the tile-binned tally (anm_options.tally) */
     uint64_t n_tally_overflow;                             /* deposits that found their tile's list full and took the
                                                               direct path; the counting batch is not included        */
+    /* Run-level "statistical uncertainty" ("0.47 %", L117 "1.19 %": quoted per run, definition not given;
+     * DESIGN.md reading C17): RMS of the voxels' relative sigma over the NON-AIR voxels (material id != 0; PAPER.md:L119
+     * sets the dose in air to zero) whose dose exceeds 10 % / 50 % of the largest non-air voxel dose, and how many voxels
+     * that is.  Uses the run's estimator (batch, or history by history with uncertainty = 1); after anm_merge: of the
+     * merged run. */
+    double rms_rel_sigma_gt10, rms_rel_sigma_gt50;
+    uint64_t n_voxels_gt10, n_voxels_gt50;
+    double max_dose_Gy_per_decay;                          /* the largest non-air voxel dose                          */
 } anm_stats;
 
 /* HU -> (material, density) conversion curve ("Hounsfield unit (HU)-to-density conversion curve";

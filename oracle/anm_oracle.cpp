@@ -114,7 +114,8 @@ struct OrcProblem {
     int32_t n_organs;
     int32_t photons_per_decay;             // 1 | 2
     int32_t rayleigh_on;
-    int32_t tracking;                      // 0 exact DDA (the oracle); 1 Woodcock (cross-check only)
+    int32_t tracking;                      // 0 exact DDA (the oracle); 1 Woodcock (cross-check only);
+                                           // 2 | 3 lockstep with the CUDA path's documented schedule (global | hull majorant)
     double photon_cutoff;                  // MeV, 0.010
     double positron_ke;                    // MeV, 0 or 0.2498
     uint64_t n_total;                      // N decays of the whole run
@@ -132,7 +133,8 @@ struct OrcProblem {
 struct OrcStats {
     double emitted, deposited, escaped, max_history_residual;
     uint64_t n_histories, n_photons, n_crossings, n_collisions, n_pe, n_compton, n_rayleigh,
-        n_escaped, n_cutoff, n_virtual, n_electrons, n_electron_crossings;
+        n_escaped, n_cutoff, n_virtual, n_electrons, n_electron_crossings,
+        n_substeps;   // lockstep mode (tracking 2 | 3): every Woodcock sub-step, real or virtual (the CUDA path's n_steps)
 };
 
 // ------------------------------------------------------------------ P1
@@ -394,7 +396,7 @@ double e_range_of(const OrcProblem& p, int m, double T) {          // R_m(T)
     double x = (T - p.t_min) / p.dt;
     if (x <= 0.0) return 0.0;
     int k = (int)std::floor(x);
-    if (k > p.n_t - 2) k = p.n_t - 2;                              // (set-up checks that the grid covers T)
+    if (k > p.n_t - 2) k = p.n_t - 2;                              // (orc_run requires the grid to reach E0, the largest electron)
     return (double)R[k] + (x - (double)k) * ((double)R[k + 1] - (double)R[k]);
 }
 
@@ -632,7 +634,8 @@ int orc_electron_walk(const OrcProblem* p, const double* pos, const double* e, d
 // event trip (FLY: two sub-steps {path, accept / channel} x 2; COMPTON: {branch, eps, accept, phi}; RAYLEIGH:
 // {x^2, accept, phi}), uniforms u = ((r >> 8) + 0.5) 2^-24.  With the same seed it follows the SAME histories as the
 // CUDA path up to fp32 rounding, so the two can be compared history by history (tests/test_gpu_lockstep.py).
-// Point-source mode only (the decay-voxel pick of the CUDA path is an alias table the oracle does not rebuild).
+// Decay sites: the given point, or from the activity map through an alias table rebuilt here by the ordered Walker /
+// Vose sweep the CUDA set-up is defined by (build_alias below).
 // ---------------------------------------------------------------------------------------------
 namespace lockstep {
 
@@ -823,7 +826,7 @@ void photon(const OrcProblem& p, const Tables& T, uint64_t h, uint32_t stream, d
                     vox[a] = (int)std::floor(pos[a] / hvox[a]);
                     inside = inside && vox[a] >= 0 && vox[a] < n[a];
                 }
-                ++st.n_virtual;                                   // counts every sub-step here
+                ++st.n_substeps;
                 if (!inside) { *escaped += E; ++st.n_escaped; return; }
                 if (T.hull) {
                     if (T.in_box(vox)) { hull_in = true; hull_away = false; }
@@ -957,7 +960,7 @@ int orc_run(const OrcProblem* pp, uint64_t h0, uint64_t h1, double* sum, double*
     if (!p.use_point_source && !p.cdf) return -1;
     if (p.photons_per_decay != 1 && p.photons_per_decay != 2) return -1;
     if (p.electron_on && (!p.e_range || p.n_t < 2 || !(p.dt > 0.0) || p.electron_cutoff != p.t_min ||
-                          p.t_min + p.dt * (p.n_t - 1) < 2.0 * kElectronMassMeV / 3.0)) return -1;
+                          p.t_min + p.dt * (p.n_t - 1) < kElectronMassMeV)) return -1;   // photo-electrons carry the whole photon energy (<= E0)
     const uint64_t V = (uint64_t)p.nx * p.ny * p.nz;
     const double vox_cm3 = p.dx * p.dy * p.dz;
 

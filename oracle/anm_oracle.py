@@ -65,7 +65,7 @@ class OrcStats(C.Structure):
                 ("max_history_residual", C.c_double)] + [
         (n, C.c_uint64) for n in ("n_histories", "n_photons", "n_crossings", "n_collisions", "n_pe",
                                   "n_compton", "n_rayleigh", "n_escaped", "n_cutoff", "n_virtual",
-                                  "n_electrons", "n_electron_crossings")]
+                                  "n_electrons", "n_electron_crossings", "n_substeps")]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
@@ -292,6 +292,16 @@ class Oracle:
             # history-by-history (Walters et al. 2002): s^2 of the mean = (sum X^2 / N - (sum X / N)^2) / (N - 1)
             var_h = (r["hbh_sumsq"] / N - ybar * ybar) / (N - 1.0)
             out["rel_sigma_hbh"] = np.divide(np.sqrt(np.maximum(var_h, 0.0)), ybar, out=np.zeros_like(S), where=ybar > 0)
+        # run-level "statistical uncertainty" (PAPER.md:L109, L117 quote one figure per run without defining it; reading
+        # C17): RMS of the relative sigma over the non-air voxels (material id 0 = air) whose dose exceeds
+        # 10 % / 50 % of the largest non-air voxel dose
+        body = self.material != 0
+        dmax = float(dose[body].max()) if body.any() else 0.0
+        out["max_dose"] = dmax
+        for name, frac in (("gt10", 0.1), ("gt50", 0.5)):
+            sel = body & (dose > frac * dmax)
+            out["n_voxels_" + name] = int(sel.sum())
+            out["rms_rel_sigma_" + name] = float(np.sqrt(np.mean(rel[sel] ** 2))) if sel.any() else 0.0
         if total_activity_bq is not None:
             out["dose_rate"] = dose * total_activity_bq                        # Eq. 1
         if self.labels is not None and self.n_organs > 0:

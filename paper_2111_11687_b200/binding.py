@@ -64,7 +64,9 @@ class anm_stats(C.Structure):
         (n, C.c_uint64) for n in ("n_decays", "n_steps", "n_real", "n_pe", "n_compton", "n_rayleigh", "n_escaped", "n_cutoff", "n_electrons", "n_hbh_overflow")] + [
         ("ms_transport", C.c_double), ("ms_fold", C.c_double), ("ms_finalize", C.c_double), ("ms_setup", C.c_double),
         ("n_launches", C.c_uint64), ("ms_load_ct", C.c_double), ("ms_load_pet", C.c_double),
-        ("tally_binned", C.c_uint64), ("n_tally_overflow", C.c_uint64)]
+        ("tally_binned", C.c_uint64), ("n_tally_overflow", C.c_uint64),
+        ("rms_rel_sigma_gt10", C.c_double), ("rms_rel_sigma_gt50", C.c_double), ("n_voxels_gt10", C.c_uint64),
+        ("n_voxels_gt50", C.c_uint64), ("max_dose_Gy_per_decay", C.c_double)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}

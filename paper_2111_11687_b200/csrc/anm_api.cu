@@ -112,7 +112,7 @@ struct anm_ctx {
     DevBuf<OrganAccum> organ_acc;         // [256]
     DevBuf<double> organ_mass;            // [256]
     DevBuf<unsigned long long> organ_count;   // [256]
-    DevBuf<double> total_energy;          // [1]
+    DevBuf<double> total_energy;          // [1] total energy, [1..4] run-level sigma accumulators, [5] maximum of S / rho (bits)
     DevBuf<float> d_tot, d_maj, d_majo, d_x2, d_cum, d_erange;
     DevBuf<float2> d_pec;
     DevBuf<unsigned> d_flags;             // [2 + ANM_MAX_MATERIALS] + [6 + ANM_MAX_MATERIALS] for the hull pass
@@ -124,6 +124,7 @@ struct anm_ctx {
     int run_batches = 0;
     std::vector<anm_organ> organs;
     anm_stats stats;
+    double run_sigma[5] = {0, 0, 0, 0, 0};   // rms > 10 %, n > 10 %, rms > 50 %, n > 50 %, max S / rho (last finalize)
     double ms_setup = 0, ms_load_ct = 0, ms_load_pet = 0;
 
     anm_ctx() { std::memset(&stats, 0, sizeof stats); anm_default_options(&opt); }
@@ -286,7 +287,11 @@ int upload_tables(anm_ctx* c) {
     return ANM_OK;
 }
 
-struct HostE0 { int ie; float fe, maj, inv_maj; };
+void fill_run_sigma(const anm_ctx* c, anm_stats& s) {
+    s.rms_rel_sigma_gt10 = c->run_sigma[0]; s.n_voxels_gt10 = (uint64_t)(c->run_sigma[1] + 0.5);
+    s.rms_rel_sigma_gt50 = c->run_sigma[2]; s.n_voxels_gt50 = (uint64_t)(c->run_sigma[3] + 0.5);
+    s.max_dose_Gy_per_decay = c->run_sigma[4];
+}
 
 using TransportFn = void (*)(const TransportParams);
 
@@ -310,17 +315,25 @@ TransportFn pick_transport(int schedule, bool stats, int tally, bool elec, bool 
 int finalize_and_collect(anm_ctx* c, int B, uint64_t nb, uint64_t n_decays, const double* rows_host) {
     cudaStream_t st = c->stream;
     ANM_CUDA(c, cudaMemsetAsync(c->organ_acc.p, 0, 256 * sizeof(OrganAccum), st));
-    ANM_CUDA(c, cudaMemsetAsync(c->total_energy.p, 0, 8, st));
+    ANM_CUDA(c, cudaMemsetAsync(c->total_energy.p, 0, 6 * 8, st));
     finalize_kernel<<<grid_blocks(c, c->V, kFoldThreads), kFoldThreads, 0, st>>>(
         c->sum.p, c->run_hbh ? c->hbh_sq.p : c->sumsq.p, c->have_organs ? c->labels.p : nullptr, c->organ_acc.p,
         c->total_energy.p, c->n_organs, c->V, c->run_hbh ? (double)n_decays : (double)B);
+    ANM_CUDA(c, cudaGetLastError());
+    // run-level figure (reading C17): RMS relative sigma over the non-air voxels above 10 % / 50 % of the maximum dose
+    dose_max_kernel<<<grid_blocks(c, c->V, kFoldThreads), kFoldThreads, 0, st>>>(
+        c->sum.p, c->texels.p, c->V, reinterpret_cast<unsigned*>(c->total_energy.p + 5));
+    ANM_CUDA(c, cudaGetLastError());
+    run_sigma_kernel<<<grid_blocks(c, c->V, kFoldThreads), kFoldThreads, 0, st>>>(
+        c->sum.p, c->run_hbh ? c->hbh_sq.p : c->sumsq.p, c->texels.p, c->V, c->run_hbh ? (double)n_decays : (double)B,
+        reinterpret_cast<const unsigned*>(c->total_energy.p + 5), c->total_energy.p + 1);
     ANM_CUDA(c, cudaGetLastError());
     std::vector<double> ob;
     OrganAccum acc[256];
     double mass[256];
     unsigned long long cnt[256];
-    double tot_e = 0;
-    ANM_CUDA(c, cudaMemcpyAsync(&tot_e, c->total_energy.p, 8, cudaMemcpyDeviceToHost, st));
+    double tot6[6] = {0, 0, 0, 0, 0, 0};
+    ANM_CUDA(c, cudaMemcpyAsync(tot6, c->total_energy.p, sizeof tot6, cudaMemcpyDeviceToHost, st));
     if (c->have_organs) {
         if (!rows_host) {
             ob.resize((size_t)B * 256);
@@ -352,7 +365,14 @@ int finalize_and_collect(anm_ctx* c, int B, uint64_t nb, uint64_t n_decays, cons
             r.mass_weighted_Gy_per_decay = mass[o] > 0 ? acc[o].energy * kGyPerMeVPerGram / ((double)n_decays * mass[o]) : 0.0;
         }
     }
-    c->stats.deposited_MeV = tot_e;
+    c->stats.deposited_MeV = tot6[0];
+    {
+        unsigned bits; std::memcpy(&bits, &tot6[5], 4);
+        float smax; std::memcpy(&smax, &bits, 4);
+        c->run_sigma[0] = tot6[2] > 0 ? std::sqrt(tot6[1] / tot6[2]) : 0.0; c->run_sigma[1] = tot6[2];
+        c->run_sigma[2] = tot6[4] > 0 ? std::sqrt(tot6[3] / tot6[4]) : 0.0; c->run_sigma[3] = tot6[4];
+        c->run_sigma[4] = (double)smax * kGyPerMeVPerGram / ((double)n_decays * c->dx * c->dy * c->dz);
+    }
     return ANM_OK;
 }
 
@@ -435,8 +455,11 @@ int anm_set_grid(anm_ctx* c, int nx, int ny, int nz, double dx_mm, double dy_mm,
     c->Vpad = (c->V + 3) / 4 * 4;
     c->have_grid = true;
     c->have_phantom = c->have_organs = c->have_results = false;
-    c->have_source = c->point_source && c->have_source;
-    if (!c->point_source) c->have_source = false;
+    // a point source set for the previous grid stays only if it lies inside the new extents (else the decay voxel
+    // would index past the volumes); an activity map never survives a grid change
+    c->have_source = c->point_source && c->have_source && c->px >= 0 && c->px < nx * c->dx && c->py >= 0 &&
+                     c->py < ny * c->dy && c->pz >= 0 && c->pz < nz * c->dz;
+    if (!c->have_source) c->point_source = false;
     ANM_CUDA(c, c->texels.alloc(c->Vpad));
     ANM_CUDA(c, c->batch.alloc(c->Vpad));
     ANM_CUDA(c, c->sum.alloc(c->Vpad));
@@ -445,7 +468,7 @@ int anm_set_grid(anm_ctx* c, int nx, int ny, int nz, double dx_mm, double dy_mm,
     ANM_CUDA(c, cudaMemsetAsync(c->batch.p, 0, c->Vpad * 4, c->stream));
     ANM_CUDA(c, c->d_flags.alloc(2 + ANM_MAX_MATERIALS + 6 + ANM_MAX_MATERIALS));
     ANM_CUDA(c, c->dstats.alloc(1));
-    ANM_CUDA(c, c->total_energy.alloc(1));
+    ANM_CUDA(c, c->total_energy.alloc(6));
     ANM_CUDA(c, c->organ_acc.alloc(256));
     ANM_CUDA(c, c->organ_mass.alloc(256));
     ANM_CUDA(c, c->organ_count.alloc(256));
@@ -893,7 +916,8 @@ int anm_set_electron_tables(anm_ctx* c, const anm_electron_tables* t) {
     if (t->n_materials < 1 || t->n_materials > ANM_MAX_MATERIALS || t->n_t < 2 || t->n_t > 1024 || !(t->dt > 0) ||
         !(t->t_min > 0) || !std::isfinite(t->t_min) || !std::isfinite(t->dt))
         return fail(c, ANM_E_ARG, "electron tables: sizes out of range");
-    if (t->t_min + t->dt * (t->n_t - 1) < 2.0 * 0.51099895 / 3.0) return fail(c, ANM_E_ARG, "electron tables: the grid must reach the Compton edge 0.3407 MeV");
+    // photo-electrons take the whole photon energy (reading C28), so the grid must cover E0, not only the Compton edge
+    if (t->t_min + t->dt * (t->n_t - 1) < 0.51099895) return fail(c, ANM_E_ARG, "electron tables: the grid must reach the photon energy 0.51099895 MeV (photo-electrons)");
     for (int m = 0; m < t->n_materials; ++m) {
         const float* R = t->range + (size_t)m * t->n_t;
         if (R[0] != 0.0f) return fail(c, ANM_E_ARG, "electron tables: range[m][0] must be 0 (t_min is the cutoff)");
@@ -1147,6 +1171,25 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
         ANM_CUDA_EV(cudaFuncSetAttribute(bin_fold_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kTileVoxels * 4)));
         p.bin_seg = c->bin_seg.p;
     }
+    {   // EXPERIMENT knobs (env): L2 fetch granularity and a persisting window on the texels
+        if (const char* g = std::getenv("ANM_L2_FETCH")) cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, (size_t)std::atol(g));
+        if (const char* h = std::getenv("ANM_L2_PERSIST")) {
+            const double ratio = std::atof(h);
+            cudaDeviceProp prop; cudaGetDeviceProperties(&prop, c->device);
+            const char* wb = std::getenv("ANM_L2_PERSIST_MB");
+            const size_t want = wb ? (size_t)std::atol(wb) << 20 : (size_t)prop.persistingL2CacheMaxSize;
+            cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, std::min(want, (size_t)prop.persistingL2CacheMaxSize));
+            cudaStreamAttrValue av; std::memset(&av, 0, sizeof av);
+            av.accessPolicyWindow.base_ptr = (void*)c->texels.p;
+            av.accessPolicyWindow.num_bytes = std::min((size_t)c->Vpad * 4, (size_t)prop.accessPolicyMaxWindowSize);
+            av.accessPolicyWindow.hitRatio = (float)ratio;
+            av.accessPolicyWindow.hitProp = ratio > 0 ? cudaAccessPropertyPersisting : cudaAccessPropertyNormal;
+            av.accessPolicyWindow.missProp = std::getenv("ANM_L2_MISS_NORMAL") ? cudaAccessPropertyNormal : cudaAccessPropertyStreaming;
+            if (std::getenv("ANM_L2_VERBOSE")) fprintf(stderr, "L2: persist max %d B, window max %d B, window %zu B ratio %.2f\n", prop.persistingL2CacheMaxSize, prop.accessPolicyMaxWindowSize, av.accessPolicyWindow.num_bytes, ratio);
+            for (int k = 0; k < depth; ++k) { cudaStream_t s_ = depth > 1 ? c->pipe[k] : st; cudaStreamSetAttribute(s_, cudaStreamAttributeAccessPolicyWindow, &av); }
+            cudaGetLastError();
+        }
+    }
     ANM_CUDA_EV(cudaEventRecord(ev[0], st));
     if (depth > 1) for (int k = 0; k < depth; ++k) ANM_CUDA_EV(cudaStreamWaitEvent(c->pipe[k], ev[0], 0));
     for (int b = 0; b < B; ++b) {
@@ -1248,6 +1291,8 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     s.n_launches = (uint64_t)2 * B + 1;
     s.tally_binned = BIN ? 1 : 0;
     s.n_tally_overflow = bin_overflow;
+    s.n_launches += 2;     // dose_max + run_sigma of the finalize
+    fill_run_sigma(c, s);
     c->run_decays = n_decays;
     c->run_batches = B;
     c->have_results = true;
@@ -1330,7 +1375,8 @@ int anm_merge(anm_ctx* c, uint64_t total_decays, int total_batches, const double
     anm_stats& s = c->stats;
     const double dep = s.deposited_MeV;
     if (summed) s = *summed; else { s = mine; s.escaped_MeV = 0; s.n_steps = s.n_real = s.n_pe = s.n_compton = s.n_rayleigh = s.n_escaped = s.n_cutoff = s.n_electrons = s.n_hbh_overflow = 0; }
-    s.n_launches += 1;     // the finalize launch of the merge
+    s.n_launches += 3;     // the finalize launches of the merge
+    fill_run_sigma(c, s);
     s.n_decays = total_decays;
     s.emitted_MeV = (double)total_decays * ((double)kE0 * c->opt.photons_per_decay + c->opt.positron_ke_MeV);
     s.deposited_MeV = dep;

@@ -5,6 +5,7 @@
 //   fold_kernel      : per-batch fold  sum += x, sumsq += x^2, x = 0, organ partial sums   (A10)
 //   finalize_kernel  : organ Eq. 3 accumulators, organ energy / mass / counts, total energy (A11)
 //   readout_kernel   : dose / dose rate / relative sigma read-out                           (A11)
+//   dose_max_kernel, run_sigma_kernel : run-level RMS relative sigma above 10 % / 50 % of the maximum dose (A11)
 //   pack_texels / rho_max / hull_box / organ_mass kernels : set-up (A0); the alias table is in anm_alias.cuh,
 //                      the image front end in anm_frontend.cuh
 //   electron_walk (device function) + electron_trace_kernel : secondary electrons
@@ -1141,6 +1142,55 @@ finalize_kernel(const float* __restrict__ sum, const float* __restrict__ sumsq, 
         atomicAdd(&organ[threadIdx.x].rel2, s_rel2[threadIdx.x]);
         atomicAdd(&organ[threadIdx.x].n_nonzero, s_nz[threadIdx.x]);
         atomicAdd(&organ[threadIdx.x].energy, s_en[threadIdx.x]);
+    }
+}
+
+// A11, the run-level "statistical uncertainty" figure ("0.47 %", L117 "1.19 %"; reading C17): the
+// RMS of the voxels' relative sigma over the non-air voxels whose dose exceeds 10 % / 50 % of the maximum dose.  Dose is
+// proportional to S / rho (voxel volume and decay count are constants), so both passes work on that ratio.
+// Pass 1: maximum of S / rho over the non-air voxels (material id != 0), as the bits of a positive float.
+__global__ void __launch_bounds__(kFoldThreads)
+dose_max_kernel(const float* __restrict__ sum, const uint32_t* __restrict__ texels, size_t V, unsigned* __restrict__ max_bits) {
+    float m = 0.0f;
+    for (size_t i = (size_t)blockIdx.x * kFoldThreads + threadIdx.x; i < V; i += (size_t)gridDim.x * kFoldThreads) {
+        const float S = sum[i];
+        if (!(S > 0.0f)) continue;
+        const unsigned t = texels[i];
+        const float rho = (float)(t & 0xffffffu) * kDensityStep;
+        if ((t >> 24) != 0u && rho > 0.0f) m = fmaxf(m, S / rho);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0 && m > 0.0f) atomicMax(max_bits, __float_as_uint(m));
+}
+
+// Pass 2: acc[0] += rel^2, acc[1] += 1 over the voxels above 10 % of the maximum; acc[2], acc[3] the same above 50 %.
+__global__ void __launch_bounds__(kFoldThreads)
+run_sigma_kernel(const float* __restrict__ sum, const float* __restrict__ sumsq, const uint32_t* __restrict__ texels, size_t V,
+                 double B, const unsigned* __restrict__ max_bits, double* __restrict__ acc) {
+    const float dmax = __uint_as_float(*max_bits);
+    double a[4] = {0.0, 0.0, 0.0, 0.0};
+    for (size_t i = (size_t)blockIdx.x * kFoldThreads + threadIdx.x; i < V; i += (size_t)gridDim.x * kFoldThreads) {
+        const float S = sum[i];
+        if (!(S > 0.0f)) continue;
+        const unsigned t = texels[i];
+        const float rho = (float)(t & 0xffffffu) * kDensityStep;
+        if ((t >> 24) == 0u || !(rho > 0.0f)) continue;
+        const float d = S / rho;
+        if (d > 0.1f * dmax) {
+            const double r = (double)rel_sigma(S, sumsq[i], B);
+            a[0] += r * r; a[1] += 1.0;
+            if (d > 0.5f * dmax) { a[2] += r * r; a[3] += 1.0; }
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) a[k] += __shfl_xor_sync(0xffffffffu, a[k], o);
+    }
+    if ((threadIdx.x & 31) == 0 && a[1] != 0.0) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) atomicAdd(acc + k, a[k]);
     }
 }
 

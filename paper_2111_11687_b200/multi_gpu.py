@@ -9,7 +9,10 @@ from __future__ import annotations
 
 from dataclasses import dataclass
 
-STAT_SUM_KEYS = ("escaped_MeV", "n_steps", "n_real", "n_pe", "n_compton", "n_rayleigh", "n_escaped", "n_cutoff", "n_launches")
+# every additive field of anm_stats (tests/test_multi_gpu_host.py checks that no uint64 counter of the struct is left out;
+# n_decays is set by anm_merge from the logical run, tally_binned is a flag)
+STAT_SUM_KEYS = ("escaped_MeV", "n_steps", "n_real", "n_pe", "n_compton", "n_rayleigh", "n_escaped", "n_cutoff", "n_launches",
+                 "n_electrons", "n_hbh_overflow", "n_tally_overflow")
 STAT_MAX_KEYS = ("ms_transport", "ms_fold", "ms_finalize", "ms_setup")
 
 
@@ -59,7 +62,7 @@ def merge_stats(stats: dict, device, group=None) -> dict:
     """Counters and escaped energy summed over ranks, phase times as the max over ranks."""
     import torch
     import torch.distributed as dist
-    s = torch.tensor([float(stats[k]) for k in STAT_SUM_KEYS], dtype=torch.float64, device=device)
+    s = torch.tensor([float(stats.get(k, 0)) for k in STAT_SUM_KEYS], dtype=torch.float64, device=device)
     m = torch.tensor([float(stats[k]) for k in STAT_MAX_KEYS], dtype=torch.float64, device=device)
     dist.all_reduce(s, op=dist.ReduceOp.SUM, group=group)
     dist.all_reduce(m, op=dist.ReduceOp.MAX, group=group)
@@ -84,5 +87,10 @@ def run_sharded(sim, n_decays: int, seed: int, n_batches: int, options: dict, gr
     s, q, rows = sim.get_tally_buffers()
     rows_all = merge_tallies(s, q, rows, shard, n_batches, group)
     stats = merge_stats(sim.get_stats(), s.device, group)
+    if s.is_cuda:
+        # the all-reduces ran on torch's current stream, anm_merge launches on the ctx stream: order them explicitly
+        # (they are the same stream in bench.py; a ctx on another non-blocking stream would otherwise race)
+        import torch
+        torch.cuda.current_stream(s.device).synchronize()
     sim.merge(n_decays, n_batches, rows_all.cpu().numpy() if sim.n_organs else None, stats)
     return shard

@@ -33,7 +33,7 @@ def etab():
     return anm_inputs.make_electron_tables()
 
 
-def _random_electrons(cfg, n, seed, t_lo=0.2005, t_hi=0.3406):
+def _random_electrons(cfg, n, seed, t_lo=0.2005, t_hi=0.51099):      # up to a photo-electron's E0 (reading C28)
     rng = np.random.default_rng(seed)
     ext = np.array(cfg["shape"], np.float64) * np.array(cfg["spacing_mm"], np.float64)
     pos = rng.uniform(0.02, 0.98, size=(n, 3)) * ext
@@ -184,7 +184,7 @@ def test_electron_error_codes(anm, tables, etab):
         short = dict(etab, n_t=10, range=etab["range"][:, :10].copy())
         with pytest.raises(anm.AnmError) as e:
             sim.set_electron_tables(short)
-        assert e.value.code == -1                        # does not reach the Compton edge
+        assert e.value.code == -1                        # does not reach E0 (photo-electrons)
         with pytest.raises(anm.AnmError) as e:
             sim.trace_electrons(np.array([[1.0, 1.0, 1.0, 1.0, 0.0, 0.0, 0.3]]))
         assert e.value.code == -2                        # no tables yet

@@ -45,7 +45,7 @@ def test_histories_match_one_by_one(photons, rayleigh, positron, hull, scale, sr
     print("histories identical: %.4f (%d of %d differ); largest relative deviation among them %.1e" % (frac, int((~same).sum()), n, rel.max()))
     assert frac > 0.998
     # totals: the same algorithm on the same random numbers -> the event counts agree far inside the statistical noise
-    assert st["n_steps"] == pytest.approx(so["n_virtual"], rel=2e-3)
+    assert st["n_steps"] == pytest.approx(so["n_substeps"], rel=2e-3)
     assert st["n_compton"] == pytest.approx(so["n_compton"], rel=2e-3)
     assert st["n_pe"] == pytest.approx(so["n_pe"], rel=0.02)
     assert st["deposited_MeV"] == pytest.approx(so["deposited"], rel=1e-3)
@@ -125,7 +125,7 @@ def test_histories_match_from_the_activity_map():
     same = np.all(np.abs(rows_g - rows_o) <= 2e-4 * np.abs(rows_o) + 1e-7 * scale, axis=1)
     print("activity source: histories identical %.4f (%d of %d differ)" % (same.mean(), int((~same).sum()), n))
     assert same.mean() > 0.998
-    assert st["n_steps"] == pytest.approx(r["stats"]["n_virtual"], rel=2e-3)
+    assert st["n_steps"] == pytest.approx(r["stats"]["n_substeps"], rel=2e-3)
     assert st["deposited_MeV"] == pytest.approx(r["stats"]["deposited"], rel=1e-3)
     assert alias_g.shape[0] == int((base["activity"] > 0).sum())
 

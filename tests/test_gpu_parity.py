@@ -38,6 +38,7 @@ def gpu_run(anm, cfg, tables, n, seed=None, **opts):
         sim.run(n, cfg["seed"] if seed is None else seed)
         out = {"energy": sim.get_energy().astype(np.float64), "dose": sim.get_dose().astype(np.float64),
                "rel": sim.get_uncertainty().astype(np.float64), "stats": sim.get_stats()}
+        out["sumsq"] = sim.get_tally_buffers()[1].cpu().numpy()[: out["energy"].size].astype(np.float64)
         if cfg.get("n_organs"):
             out["organs"] = sim.get_organ_doses()
     return out
@@ -136,6 +137,20 @@ def test_small_configs_vs_live_oracle(anm, tables, k, scale, n, B):
         mw = g["organs"]["mass_weighted_Gy_per_decay"][big] / f["organs"]["mass_weighted"][big]
         assert np.all(np.abs(mw - 1) < 0.05)
         assert np.allclose(g["organs"]["mass_g"][big], f["organs"]["mass_g"][big], rtol=1e-6)
+    # run-level statistical uncertainty (reading C17): RMS relative sigma over the non-air voxels
+    # above 10 % / 50 % of the maximum dose.  (a) the reduction itself, exactly: the oracle's finalize applied to the
+    # CUDA path's own sum / sum-of-squares volumes must give the figure anm_stats reports; (b) against the oracle's own
+    # run, statistically (the population is selected on a noisy maximum, so it is compared loosely).
+    st = g["stats"]
+    o = O.Oracle(cfg, tables, n_decays=n, n_batches=B, seed=cfg["seed"])
+    fg = o.finalize({"sum": g["energy"], "sumsq": g["sumsq"], "organ_batch": np.zeros((B, cfg["n_organs"] + 1))})
+    assert st["max_dose_Gy_per_decay"] == pytest.approx(fg["max_dose"], rel=1e-5)
+    for name in ("gt10", "gt50"):
+        assert abs(int(st["n_voxels_" + name]) - fg["n_voxels_" + name]) <= max(2, 1e-4 * fg["n_voxels_" + name]), name
+        assert st["rms_rel_sigma_" + name] == pytest.approx(fg["rms_rel_sigma_" + name], rel=2e-3), name
+        assert fg["n_voxels_" + name] > 0 and 0.0 < st["rms_rel_sigma_" + name] < 1.0
+    if k == 3:      # an extended source: hundreds of voxels above the cut, the two runs' figures agree
+        assert st["rms_rel_sigma_gt10"] == pytest.approx(f["rms_rel_sigma_gt10"], rel=0.15)
 
 
 def test_no_rayleigh_single_photon_vs_oracle(anm, tables):
@@ -416,6 +431,22 @@ def test_error_codes(anm, tables):
         assert sim.get_energy().sum() > 0
         with pytest.raises(ValueError):
             sim.get_energy(np.empty(7, np.float32))
+        # a point source set for one grid does not survive a smaller grid that no longer contains it (its decay voxel
+        # would index past the volumes): the run is refused until a source is set again; one that still fits is kept
+        nx, ny, nz = cfg["shape"]
+        sim.set_grid((nx // 4, ny // 4, nz // 4), cfg["spacing_mm"])          # the centre of the old grid is now outside
+        small = (nz // 4, ny // 4, nx // 4)
+        sim.load_phantom(np.full(small, 2, np.uint8), np.ones(small, np.float32))
+        with pytest.raises(E) as ei:
+            sim.run(1000, 1)
+        assert ei.value.code == -2
+        sim.set_point_source((1.0, 1.0, 1.0))
+        sim.set_grid(cfg["shape"], cfg["spacing_mm"])                         # still inside: kept
+        sim.load_phantom(cfg["material"], cfg["density"])
+        sim.set_options(n_batches=10, photons_per_decay=1, positron_ke_MeV=0.2498)
+        sim.run(1000, 1)
+        e = sim.get_energy()
+        assert e[0] >= 1000 * 0.2498 * (1 - 1e-5)                              # the positron energy lands in voxel (0, 0, 0)
 
 
 # ------------------------------------------------------------------------------------------------- A0: alias table

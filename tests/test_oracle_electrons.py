@@ -47,7 +47,7 @@ def test_bethe_table_against_published_water_values(etab):
     k300 = int(round((0.3 - etab["t_min"]) / etab["dt"]))
     assert etab["t_min"] + k300 * etab["dt"] == pytest.approx(0.3, abs=1e-12)
     assert float(etab["range"][WATER, k300]) == pytest.approx(0.08421 - 0.04488, rel=1e-2)
-    assert etab["t_min"] == 0.2 and etab["t_min"] + etab["dt"] * (etab["n_t"] - 1) >= 2 * 0.51099895 / 3
+    assert etab["t_min"] == 0.2 and etab["t_min"] + etab["dt"] * (etab["n_t"] - 1) >= 0.51099895     # photo-electrons: all of E0
     assert np.all(np.diff(etab["range"], axis=1) > 0) and np.all(etab["range"][:, 0] == 0)
     # the table is the integral of 1/S: check one entry per material by adaptive quadrature
     for m, mat in enumerate(anm_inputs.MATERIALS):
@@ -101,6 +101,38 @@ def test_walk_in_water_matches_direct_integration(tables, etab):
     q, _ = integrate.quad(lambda t: 1.0 / el.bethe_collision_stopping(t, w), 0.2, T0)
     assert len(dep) == int(np.floor((0.005 + q) / 0.01)) + 1
     assert 0.05 < q < 0.06
+
+
+def test_photo_electron_walk_matches_direct_integration(tables, etab):
+    """A photo-electron takes the whole photon energy (reading C28): up to E0 = 0.511 MeV, beyond the Compton edge.
+    0.1 mm voxels of water, electron of 0.51099895 MeV along +x: every voxel's deposit equals T(entry) - T(exit) from
+    integrating the Bethe formula directly (no table), the walk ends where the energy reaches the 0.2 MeV cutoff; the
+    CSDA path 0.511 -> 0.2 MeV is the difference of the published water ranges (ESTAR: 0.5 MeV 0.1766, 0.2 MeV 0.04488
+    g/cm^2, so a little over 1.3 mm).  The range table must therefore cover E0 (orc_run refuses one that does not)."""
+    o = _slab_problem(tables, etab)
+    T0 = 0.51099895
+    dep, esc = o.electron_walk((0.005, 1.5, 1.5), (1.0, 0.0, 0.0), T0)
+    assert esc == 0.0 and sum(e for _, e in dep) == pytest.approx(T0, abs=1e-12)
+    w = anm_inputs.MATERIALS[WATER]
+    T = T0
+    edges = [0.005] + [0.01 * (i + 1) for i in range(40)]
+    for i, (v, e) in enumerate(dep):
+        assert v == 40 * (1 + 3 * 1) + i
+        T_next = _csda_energy_after(w, T, edges[i + 1] - edges[i])
+        if i < len(dep) - 1:
+            assert e == pytest.approx(T - T_next, abs=3e-6), i
+            T = T_next
+        else:
+            assert T_next < 0.2 + 3e-6 and e == pytest.approx(T, abs=1e-5)
+    q, _ = integrate.quad(lambda t: 1.0 / el.bethe_collision_stopping(t, w), 0.2, T0)
+    assert len(dep) == int(np.floor((0.005 + q) / 0.01)) + 1
+    assert q == pytest.approx(0.1766 + (0.51099895 - 0.5) / 2.034 - 0.04488, rel=1.5e-2)       # published ranges
+    # a table that stops at the Compton edge is refused: the walk would extrapolate its last segment
+    short = dict(etab, n_t=77, range=etab["range"][:, :77].copy())
+    assert short["t_min"] + short["dt"] * 76 > 2 * 0.51099895 / 3
+    bad = _slab_problem(tables, short)
+    with pytest.raises(Exception):
+        bad.run()
 
 
 def test_walk_across_materials_and_out_of_the_grid(tables, etab):

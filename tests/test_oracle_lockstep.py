@@ -46,7 +46,7 @@ def test_hull_majorant_changes_the_steps_not_the_physics(tables):
     n, B = 100_000, 10
     r2 = O.Oracle(cfg, tables, n_decays=n, n_batches=B, seed=3, tracking=2).run_parallel(8)
     r3 = O.Oracle(cfg, tables, n_decays=n, n_batches=B, seed=3, tracking=3).run_parallel(8)
-    assert r3["stats"]["n_virtual"] < 0.8 * r2["stats"]["n_virtual"]          # sub-steps (every one is counted there)
+    assert r3["stats"]["n_substeps"] < 0.8 * r2["stats"]["n_substeps"]          # every Woodcock sub-step, real or virtual
     assert abs(r2["stats"]["deposited"] - r3["stats"]["deposited"]) / n < 4.0 * np.sqrt(2.0) * 0.6 / np.sqrt(n)
     assert r2["stats"]["n_compton"] == pytest.approx(r3["stats"]["n_compton"], rel=0.01)
 
