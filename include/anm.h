@@ -128,6 +128,14 @@ typedef struct {
                                    aggregation (else ANM_E_UNSUPPORTED).  Same tallies up to fp32 summation order.
                                    Test hook: the environment variable ANM_TALLY_CAPACITY=<n> fixes every list at n
                                    records (forces the overflow path).                                              */
+    int32_t batches_per_launch; /* batch groups: one transport launch covers this many consecutive batches, each with its own
+                                   tally volume (deposits are batch-tagged), followed by their folds -- the fixed cost of a
+                                   launch (its last decays draining, ~0.25 ms) is paid n_batches / G times instead of
+                                   n_batches times.  0 auto: as many as keep the tallies in flight within 4 GiB (at most
+                                   256, and below 2^32 histories per launch); 1..256: at most that many.  Always 1 with
+                                   schedule 1, electron_transport or tally = 2.  Same histories, same per-batch tallies.
+                                   The ctx then owns pipeline depth x G tally volumes (anm_stats.batches_per_launch = G). */
+    int32_t reserved1;
 } anm_options;
 
 /* Electron data for anm_options.electron_transport ("The cutoff energies for
@@ -176,6 +184,10 @@ typedef struct {
     double rms_rel_sigma_gt10, rms_rel_sigma_gt50;
     uint64_t n_voxels_gt10, n_voxels_gt50;
     double max_dose_Gy_per_decay;                          /* the largest non-air voxel dose                          */
+    uint64_t batches_per_launch;                           /* G of the last run (anm_options.batches_per_launch)      */
+    uint64_t n_check_violations;                           /* library built with -DANM_BOUNDS_CHECK: indices the transport
+                                                              kernels found out of range (counted, not trapped); 0 in a
+                                                              normal build, and expected 0 in a checking one               */
 } anm_stats;
 
 /* HU -> (material, density) conversion curve ("Hounsfield unit (HU)-to-density conversion curve";

@@ -92,8 +92,8 @@ struct anm_ctx {
 
     // device memory
     DevBuf<uint32_t> texels;
-    DevBuf<float> batch, sum, sumsq, scratch;
-    DevBuf<float> batch2, batch3;         // extra batch tallies of the launch pipeline (anm_options.batch_pipeline)
+    DevBuf<float> batch, sum, sumsq, scratch;   // batch: [pipeline depth][batches per launch][Vpad] per-batch tallies
+    bool batch_clean = false;             // `batch` holds zeros (the folds of a completed run leave it so)
     cudaStream_t pipe[3] = {nullptr, nullptr, nullptr};   // internal streams of the pipeline, created on first use
     DevBuf<float> e_ring;                 // waiting electrons of the event pool (electron_transport)
     DevBuf<float> hbh_sq;                 // [Vpad] sum over histories of X_h^2 (anm_options.uncertainty = 1)
@@ -426,7 +426,7 @@ int anm_destroy(anm_ctx* c) {
     c->organ_batch.release(); c->organ_acc.release(); c->organ_mass.release(); c->organ_count.release();
     c->total_energy.release(); c->d_tot.release(); c->d_maj.release(); c->d_majo.release(); c->d_x2.release(); c->d_cum.release();
     c->d_pec.release(); c->d_flags.release(); c->d_erange.release(); c->e_ring.release(); c->hbh_sq.release(); c->hbh_list.release();
-    c->batch2.release(); c->batch3.release(); c->bin_cnt.release(); c->bin_seg.release(); c->bin_seg0.release(); c->bin_rec.release(); c->bin_ovf.release();
+    c->bin_cnt.release(); c->bin_seg.release(); c->bin_seg0.release(); c->bin_rec.release(); c->bin_ovf.release();
     for (auto& ps : c->pipe) if (ps) { cudaStreamDestroy(ps); ps = nullptr; }
     delete c;
     return ANM_OK;
@@ -461,11 +461,10 @@ int anm_set_grid(anm_ctx* c, int nx, int ny, int nz, double dx_mm, double dy_mm,
                      c->py < ny * c->dy && c->pz >= 0 && c->pz < nz * c->dz;
     if (!c->have_source) c->point_source = false;
     ANM_CUDA(c, c->texels.alloc(c->Vpad));
-    ANM_CUDA(c, c->batch.alloc(c->Vpad));
     ANM_CUDA(c, c->sum.alloc(c->Vpad));
     ANM_CUDA(c, c->sumsq.alloc(c->Vpad));
     ANM_CUDA(c, cudaMemsetAsync(c->texels.p, 0, c->Vpad * 4, c->stream));
-    ANM_CUDA(c, cudaMemsetAsync(c->batch.p, 0, c->Vpad * 4, c->stream));
+    c->batch.release(); c->batch_clean = false;     // sized by anm_run (batch groups)
     ANM_CUDA(c, c->d_flags.alloc(2 + ANM_MAX_MATERIALS + 6 + ANM_MAX_MATERIALS));
     ANM_CUDA(c, c->dstats.alloc(1));
     ANM_CUDA(c, c->total_energy.alloc(6));
@@ -987,7 +986,7 @@ int anm_trace_electrons(anm_ctx* c, const float* electrons, size_t n, float* out
     TransportParams p;
     std::memset(&p, 0, sizeof p);
     p.texels = c->texels.p; p.batch = d_vol.p;
-    p.nx = c->nx; p.ny = c->ny; p.nz = c->nz;
+    p.nx = c->nx; p.ny = c->ny; p.nz = c->nz; p.n_vox = (unsigned)c->V; p.stats = c->dstats.p;
     p.dx = (float)c->dx; p.dy = (float)c->dy; p.dz = (float)c->dz;
     p.inv_dx = (float)(1.0 / c->dx); p.inv_dy = (float)(1.0 / c->dy); p.inv_dz = (float)(1.0 / c->dz);
     fill_electron_params(c, p);
@@ -1015,6 +1014,7 @@ int anm_set_options(anm_ctx* c, const anm_options* o) {
     if (o->electron_transport != 0 && o->electron_transport != 1) return fail(c, ANM_E_ARG, "options: electron_transport must be 0 or 1");
     if (o->batch_pipeline < 0 || o->batch_pipeline > 3) return fail(c, ANM_E_ARG, "options: batch_pipeline must be 0 (auto), 1, 2 or 3");
     if (o->uncertainty != 0 && o->uncertainty != 1) return fail(c, ANM_E_ARG, "options: uncertainty must be 0 (batch) or 1 (history by history)");
+    if (o->batches_per_launch < 0 || o->batches_per_launch > 256) return fail(c, ANM_E_ARG, "options: batches_per_launch must be 0 (auto) or 1..256");
     if (o->tally < 0 || o->tally > 2) return fail(c, ANM_E_ARG, "options: tally must be 0 (auto), 1 (direct atomics) or 2 (tile-binned)");
     if (o->tally == 2 && (o->schedule == 1 || o->electron_transport || o->uncertainty == 1 || o->warp_aggregate == 1))
         return fail(c, ANM_E_UNSUPPORTED, "options: the tile-binned tally runs in the event-pool schedule with the batch estimator, local electrons and no warp aggregation");
@@ -1046,13 +1046,10 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     c->have_results = false;
     if (c->dev_tables_dirty) { const int rc = upload_tables(c); if (rc != ANM_OK) return rc; }
 
-    ANM_CUDA(c, c->counters.alloc((size_t)B));
     ANM_CUDA(c, c->organ_batch.alloc((size_t)B * 256));
     cudaStream_t st = c->stream;
     ANM_CUDA(c, cudaMemsetAsync(c->sum.p, 0, c->Vpad * 4, st));
     ANM_CUDA(c, cudaMemsetAsync(c->sumsq.p, 0, c->Vpad * 4, st));
-    ANM_CUDA(c, cudaMemsetAsync(c->batch.p, 0, c->Vpad * 4, st));
-    ANM_CUDA(c, cudaMemsetAsync(c->counters.p, 0, (size_t)B * 4, st));
     ANM_CUDA(c, cudaMemsetAsync(c->organ_batch.p, 0, (size_t)B * 256 * 8, st));
     ANM_CUDA(c, cudaMemsetAsync(c->organ_acc.p, 0, 256 * sizeof(OrganAccum), st));
     ANM_CUDA(c, cudaMemsetAsync(c->dstats.p, 0, sizeof(DeviceStats), st));
@@ -1062,7 +1059,7 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     std::memset(&p, 0, sizeof p);
     p.texels = c->texels.p; p.batch = c->batch.p; p.alias = c->alias.p; p.stats = c->dstats.p;
     p.tab_tot = c->d_tot.p; p.tab_pec = c->d_pec.p; p.tab_maj = c->d_maj.p; p.ray_x2 = c->d_x2.p; p.ray_cum = c->d_cum.p;
-    p.n_hist = (unsigned)nb; p.n_alias = c->n_alias;
+    p.n_hist = (unsigned)nb; p.n_alias = c->n_alias; p.n_vox = (unsigned)c->V;
     for (int r = 0; r < 10; ++r) {      // Philox4x32-10 round keys
         p.rk[2 * r] = (unsigned)seed + (unsigned)r * 0x9E3779B9u;
         p.rk[2 * r + 1] = (unsigned)(seed >> 32) + (unsigned)r * 0xBB67AE85u;
@@ -1110,50 +1107,70 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     int per_sm = 0;
     ANM_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem));
     if (per_sm < 1) return fail(c, ANM_E_UNSUPPORTED, "run: tables too large for shared memory (%zu bytes)", smem);
-    // persistent lanes: one resident wave; never more photon slots than histories
-    const uint64_t per_block = schedule == 2 ? (uint64_t)kPoolWarps * kSlots : (uint64_t)kThreads;
-    const int blocks = (int)std::max<uint64_t>(1, std::min<uint64_t>((uint64_t)c->num_sms * per_sm, (nb + per_block - 1) / per_block));
     const int fold_blocks = grid_blocks(c, c->Vpad / 4, kFoldThreads);
     const float inv_vox = (float)(1.0 / (c->dx * c->dy * c->dz));
     c->run_hbh = HB;
-    if (EL) {   // per-warp arrays of electrons waiting for their walk
-        ANM_CUDA(c, c->e_ring.alloc((size_t)3 * blocks * kPoolWarps * 8 * kPend));     // one per launch in flight
+    if (HB && nb > (uint64_t)kHbhHistMask) return fail(c, ANM_E_UNSUPPORTED, "run: history-by-history scoring holds at most 2^26 decays per batch");
+    // Batch groups (anm_options.batches_per_launch): one transport launch covers G consecutive batches, each with its own
+    // tally volume (batch-tagged deposits: the decay's batch within the group sits in its slot's meta word), and the G
+    // folds follow the launch.  A launch is one resident wave of persistent CTAs whose tail (the last decays draining,
+    // queues below 32 entries in every warp at the same time) costs ~0.25 ms whatever its size; with G batches per launch
+    // that cost is paid B / G times instead of B times.  Same histories, same per-batch tallies.
+    // G = 1 for the history-based schedule, electron transport and the tile-binned tally (their per-launch scratch is
+    // per batch); else the largest group that keeps depth * G tally volumes within the memory budget, at most 256
+    // (8 bits of the meta word), G * nb < 2^32 histories per launch (2^26 with history-by-history scoring).
+    int G = 1;
+    if (schedule == 2 && !EL && !BIN) {
+        const uint64_t hist_cap = HB ? (uint64_t)kHbhHistMask : 0xffffffffull;
+        uint64_t gmax = std::min<uint64_t>({(uint64_t)B, (uint64_t)kMaxGroup, std::max<uint64_t>(1, hist_cap / nb)});
+        if (c->opt.batches_per_launch > 0) gmax = std::min<uint64_t>(gmax, (uint64_t)c->opt.batches_per_launch);
+        else {
+            const uint64_t budget = 4ull << 30;                        // bytes of batch tallies in flight (auto)
+            gmax = std::min<uint64_t>(gmax, std::max<uint64_t>(1, budget / ((uint64_t)c->Vpad * 4 * 2)));
+        }
+        const int n_groups0 = (int)(((uint64_t)B + gmax - 1) / gmax);
+        G = (B + n_groups0 - 1) / n_groups0;                           // even groups
+    }
+    const int n_groups = (B + G - 1) / G;
+    if (HB && nb * (uint64_t)G > (uint64_t)kHbhHistMask) return fail(c, ANM_E_UNSUPPORTED, "run: history-by-history scoring holds at most 2^26 decays per launch");
+    // Launch pipeline (anm_options.batch_pipeline): with `depth` sets of G batch tallies the launches of consecutive
+    // groups go to `depth` internal streams: the CTAs of group g+1 take over each SM as the CTAs of group g exit, the folds
+    // of group g run in the gaps.  The folds are serialised among themselves (they all update sum / sumsq); group g+depth
+    // reuses the tallies of group g after their folds (same stream).
+    const int depth = std::max(1, std::min(c->opt.batch_pipeline == 0 ? (G > 1 ? 2 : 3) : c->opt.batch_pipeline, n_groups));
+    const size_t set_floats = (size_t)G * c->Vpad;
+    if (c->batch.n != (size_t)depth * set_floats) c->batch_clean = false;
+    ANM_CUDA(c, c->batch.alloc((size_t)depth * set_floats));
+    if (!c->batch_clean) ANM_CUDA(c, cudaMemsetAsync(c->batch.p, 0, (size_t)depth * set_floats * 4, st));   // the folds leave them zero
+    c->batch_clean = false;                                            // until this run's folds have completed
+    ANM_CUDA(c, c->counters.alloc((size_t)n_groups));
+    ANM_CUDA(c, cudaMemsetAsync(c->counters.p, 0, (size_t)n_groups * 4, st));
+    if (depth > 1)
+        for (int k = 0; k < depth; ++k)
+            if (!c->pipe[k]) ANM_CUDA(c, cudaStreamCreateWithFlags(&c->pipe[k], cudaStreamNonBlocking));
+    const uint64_t per_block = schedule == 2 ? (uint64_t)kPoolWarps * kSlots : (uint64_t)kThreads;
+    const int blocks = (int)std::max<uint64_t>(1, std::min<uint64_t>((uint64_t)c->num_sms * per_sm, (nb * (uint64_t)G + per_block - 1) / per_block));
+    if (EL) {   // per-warp arrays of electrons waiting for their walk, one per launch in flight
+        ANM_CUDA(c, c->e_ring.alloc((size_t)depth * blocks * kPoolWarps * 8 * kPend));
         p.e_ring = c->e_ring.p;
     }
     if (HB) {   // history-by-history scoring: sum of X_h^2 over the whole run + one deposit list per decay slot
         const size_t nslots = (size_t)blocks * kPoolWarps * kSlots;
         ANM_CUDA(c, c->hbh_sq.alloc(c->Vpad));
-        if (nb > (uint64_t)kHbhHistMask) return fail(c, ANM_E_UNSUPPORTED, "run: history-by-history scoring holds at most 2^26 decays per batch");
-        ANM_CUDA(c, c->hbh_list.alloc((size_t)3 * kHbhCap * nslots));      // one set of lists per launch in flight
+        ANM_CUDA(c, c->hbh_list.alloc((size_t)depth * kHbhCap * nslots));      // one set of lists per launch in flight
         ANM_CUDA(c, cudaMemsetAsync(c->hbh_sq.p, 0, c->Vpad * 4, st));
         p.hbh_list = c->hbh_list.p; p.hbh_sq = c->hbh_sq.p; p.hbh_nslots = (unsigned)nslots;
     }
+    p.n_per_batch = (unsigned)nb; p.batch_stride = c->Vpad;
 
-    std::vector<cudaEvent_t> ev((size_t)2 * B + 3, nullptr);   // [0] start, [2b+1] / [2b+2] before / after fold b, [2B+1] end, [2B+2] pipeline join
+    // events: [0] start, [1 + g] after the folds of group g, [n_groups + 1] pipeline join, [n_groups + 2] end;
+    // serial mode (depth 1) also [n_groups + 3 + g] between launch g and its folds, for per-phase times
+    std::vector<cudaEvent_t> ev((size_t)2 * n_groups + 3, nullptr);
     auto free_events = [&]() { for (auto e : ev) if (e) cudaEventDestroy(e); };
     for (auto& e : ev) if (cudaEventCreate(&e) != cudaSuccess) { free_events(); return fail(c, ANM_E_CUDA, "cudaEventCreate failed"); }
 #define ANM_CUDA_EV(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { cudaGetLastError(); free_events(); \
         return fail(c, ANM_E_CUDA, "%s: %s", #call, cudaGetErrorString(e_)); } } while (0)
 
-    // Launch pipeline (anm_options.batch_pipeline): a transport launch is one resident wave of persistent CTAs, so its
-    // tail (the last decays draining, ~0.2 ms) leaves SMs idle.  With `depth` batch tallies the launches of
-    // consecutive batches go to `depth` internal streams: the CTAs of batch b+1 take over each SM as the CTAs of batch
-    // b exit, the fold of batch b runs in the gaps.  The folds are serialised among themselves (they all update sum /
-    // sumsq); batch b+depth reuses the tally of batch b after its fold (same stream).  Same histories, same tallies.
-    const int depth = std::max(1, std::min(c->opt.batch_pipeline == 0 ? 3 : c->opt.batch_pipeline, B));
-    float* bufs[3] = {c->batch.p, nullptr, nullptr};
-    if (depth > 1) {
-        ANM_CUDA_EV(c->batch2.alloc(c->Vpad));
-        ANM_CUDA_EV(cudaMemsetAsync(c->batch2.p, 0, c->Vpad * 4, st));
-        bufs[1] = c->batch2.p;
-        if (depth > 2) {
-            ANM_CUDA_EV(c->batch3.alloc(c->Vpad));
-            ANM_CUDA_EV(cudaMemsetAsync(c->batch3.p, 0, c->Vpad * 4, st));
-            bufs[2] = c->batch3.p;
-        }
-        for (int k = 0; k < depth; ++k)
-            if (!c->pipe[k]) ANM_CUDA_EV(cudaStreamCreateWithFlags(&c->pipe[k], cudaStreamNonBlocking));
-    }
     // tile-binned tally: counters per launch in flight, one {offset, capacity} table; the capacities come from batch 0,
     // which runs with empty segments (every deposit takes the direct-RED path and is counted per tile)
     const unsigned n_tiles = (unsigned)((c->Vpad + kTileVoxels - 1) >> kTileShift);
@@ -1171,41 +1188,26 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
         ANM_CUDA_EV(cudaFuncSetAttribute(bin_fold_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kTileVoxels * 4)));
         p.bin_seg = c->bin_seg.p;
     }
-    {   // EXPERIMENT knobs (env): L2 fetch granularity and a persisting window on the texels
-        if (const char* g = std::getenv("ANM_L2_FETCH")) cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, (size_t)std::atol(g));
-        if (const char* h = std::getenv("ANM_L2_PERSIST")) {
-            const double ratio = std::atof(h);
-            cudaDeviceProp prop; cudaGetDeviceProperties(&prop, c->device);
-            const char* wb = std::getenv("ANM_L2_PERSIST_MB");
-            const size_t want = wb ? (size_t)std::atol(wb) << 20 : (size_t)prop.persistingL2CacheMaxSize;
-            cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, std::min(want, (size_t)prop.persistingL2CacheMaxSize));
-            cudaStreamAttrValue av; std::memset(&av, 0, sizeof av);
-            av.accessPolicyWindow.base_ptr = (void*)c->texels.p;
-            av.accessPolicyWindow.num_bytes = std::min((size_t)c->Vpad * 4, (size_t)prop.accessPolicyMaxWindowSize);
-            av.accessPolicyWindow.hitRatio = (float)ratio;
-            av.accessPolicyWindow.hitProp = ratio > 0 ? cudaAccessPropertyPersisting : cudaAccessPropertyNormal;
-            av.accessPolicyWindow.missProp = std::getenv("ANM_L2_MISS_NORMAL") ? cudaAccessPropertyNormal : cudaAccessPropertyStreaming;
-            if (std::getenv("ANM_L2_VERBOSE")) fprintf(stderr, "L2: persist max %d B, window max %d B, window %zu B ratio %.2f\n", prop.persistingL2CacheMaxSize, prop.accessPolicyMaxWindowSize, av.accessPolicyWindow.num_bytes, ratio);
-            for (int k = 0; k < depth; ++k) { cudaStream_t s_ = depth > 1 ? c->pipe[k] : st; cudaStreamSetAttribute(s_, cudaStreamAttributeAccessPolicyWindow, &av); }
-            cudaGetLastError();
-        }
-    }
     ANM_CUDA_EV(cudaEventRecord(ev[0], st));
     if (depth > 1) for (int k = 0; k < depth; ++k) ANM_CUDA_EV(cudaStreamWaitEvent(c->pipe[k], ev[0], 0));
-    for (int b = 0; b < B; ++b) {
-        cudaStream_t sb = depth > 1 ? c->pipe[b % depth] : st;
-        p.batch = bufs[b % depth];
+    for (int g = 0; g < n_groups; ++g) {
+        const int b0 = g * G, nbg = std::min(G, B - b0);          // batches b0 .. b0 + nbg - 1
+        const int set = g % depth;
+        cudaStream_t sb = depth > 1 ? c->pipe[set] : st;
+        p.batch = c->batch.p + (size_t)set * set_floats;
+        p.n_group = (unsigned)nbg;
+        p.n_hist = (unsigned)(nb * (uint64_t)nbg);
         if (BIN) {
-            p.bin_cnt = c->bin_cnt.p + (size_t)(b % depth) * n_lists;
-            p.bin_rec = c->bin_rec.p ? c->bin_rec.p + (size_t)(b % depth) * bin_total : nullptr;
+            p.bin_cnt = c->bin_cnt.p + (size_t)set * n_lists;
+            p.bin_rec = c->bin_rec.p ? c->bin_rec.p + (size_t)set * bin_total : nullptr;
         }
-        if (EL) p.e_ring = c->e_ring.p + (size_t)(b % depth) * blocks * kPoolWarps * 8 * kPend;
-        if (HB) p.hbh_list = c->hbh_list.p + (size_t)(b % depth) * kHbhCap * p.hbh_nslots;
-        p.counter = c->counters.p + b;
-        p.hist_base = c->opt.history_offset + (unsigned long long)b * nb;
+        if (EL) p.e_ring = c->e_ring.p + (size_t)set * blocks * kPoolWarps * 8 * kPend;
+        if (HB) p.hbh_list = c->hbh_list.p + (size_t)set * kHbhCap * p.hbh_nslots;
+        p.counter = c->counters.p + g;
+        p.hist_base = c->opt.history_offset + (unsigned long long)b0 * nb;
         kern<<<blocks, threads, smem, sb>>>(p);
         ANM_CUDA_EV(cudaGetLastError());
-        if (BIN && b == 0) {
+        if (BIN && g == 0) {
             // the counting batch has run: size every tile's segment for the batches to come -- its count plus six
             // standard deviations of a Poisson count plus 32 (a tile that still overflows loses nothing: the surplus
             // takes the direct-RED path into the batch volume, bin_fold_kernel adds both)
@@ -1226,53 +1228,58 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
             ANM_CUDA_EV(cudaMemcpyAsync(c->bin_seg.p, seg.data(), (size_t)n_lists * 8, cudaMemcpyHostToDevice, sb));
             ANM_CUDA_EV(cudaStreamSynchronize(sb));     // seg is a host temporary; every later launch (any stream) sees the table
         }
-        if (depth > 1 && b > 0) ANM_CUDA_EV(cudaStreamWaitEvent(sb, ev[2 * (b - 1) + 2], 0));    // after the previous fold
-        ANM_CUDA_EV(cudaEventRecord(ev[2 * b + 1], sb));
-        if (BIN) {
-            // batch 0 counted against empty segments; its fold must see them empty too (the table is already final)
-            bin_fold_kernel<<<std::min<unsigned>(n_tiles, (unsigned)c->num_sms * 3u), kBinFoldThreads, kTileVoxels * 4, sb>>>(
-                p.bin_cnt, b == 0 ? c->bin_seg0.p : c->bin_seg.p, p.bin_rec, (float4*)p.batch, (float4*)c->sum.p, (float4*)c->sumsq.p,
-                c->have_organs ? (const uint32_t*)c->labels.p : nullptr, (const uint4*)c->texels.p,
-                c->organ_batch.p + (size_t)b * 256, c->n_organs, c->Vpad / 4, n_tiles, inv_vox, c->bin_ovf.p + (b == 0 ? 1 : 0));
-        } else {
-            fold_kernel<<<fold_blocks, kFoldThreads, 0, sb>>>(
-                (float4*)p.batch, (float4*)c->sum.p, (float4*)c->sumsq.p,
-                c->have_organs ? (const uint32_t*)c->labels.p : nullptr, (const uint4*)c->texels.p,
-                c->organ_batch.p + (size_t)b * 256, c->n_organs, c->Vpad / 4, inv_vox);
+        if (depth > 1 && g > 0) ANM_CUDA_EV(cudaStreamWaitEvent(sb, ev[1 + (g - 1)], 0));    // after the previous group's folds
+        if (depth == 1) ANM_CUDA_EV(cudaEventRecord(ev[n_groups + 3 + g], sb));
+        for (int j = 0; j < nbg; ++j) {
+            const int b = b0 + j;
+            float* tally = p.batch + (size_t)j * c->Vpad;
+            if (BIN) {
+                // batch 0 counted against empty segments; its fold must see them empty too (the table is already final)
+                bin_fold_kernel<<<std::min<unsigned>(n_tiles, (unsigned)c->num_sms * 3u), kBinFoldThreads, kTileVoxels * 4, sb>>>(
+                    p.bin_cnt, b == 0 ? c->bin_seg0.p : c->bin_seg.p, p.bin_rec, (float4*)tally, (float4*)c->sum.p, (float4*)c->sumsq.p,
+                    c->have_organs ? (const uint32_t*)c->labels.p : nullptr, (const uint4*)c->texels.p,
+                    c->organ_batch.p + (size_t)b * 256, c->n_organs, c->Vpad / 4, n_tiles, inv_vox, c->bin_ovf.p + (b == 0 ? 1 : 0));
+            } else {
+                fold_kernel<<<fold_blocks, kFoldThreads, 0, sb>>>(
+                    (float4*)tally, (float4*)c->sum.p, (float4*)c->sumsq.p,
+                    c->have_organs ? (const uint32_t*)c->labels.p : nullptr, (const uint4*)c->texels.p,
+                    c->organ_batch.p + (size_t)b * 256, c->n_organs, c->Vpad / 4, inv_vox);
+            }
+            ANM_CUDA_EV(cudaGetLastError());
         }
-        ANM_CUDA_EV(cudaGetLastError());
-        ANM_CUDA_EV(cudaEventRecord(ev[2 * b + 2], sb));
+        ANM_CUDA_EV(cudaEventRecord(ev[1 + g], sb));
     }
-    if (depth > 1) {    // join: the caller's stream continues after the last fold (which follows every other launch)
-        ANM_CUDA_EV(cudaStreamWaitEvent(st, ev[2 * (B - 1) + 2], 0));
-        for (int b = std::max(0, B - depth); b < B - 1; ++b) ANM_CUDA_EV(cudaStreamWaitEvent(st, ev[2 * b + 2], 0));
-        ANM_CUDA_EV(cudaEventRecord(ev[2 * B + 2], st));
+    if (depth > 1) {    // join: the caller's stream continues after the last folds (which follow every other launch)
+        ANM_CUDA_EV(cudaStreamWaitEvent(st, ev[1 + (n_groups - 1)], 0));
+        for (int g = std::max(0, n_groups - depth); g < n_groups - 1; ++g) ANM_CUDA_EV(cudaStreamWaitEvent(st, ev[1 + g], 0));
     }
+    ANM_CUDA_EV(cudaEventRecord(ev[n_groups + 1], st));
     {
         const int rc = finalize_and_collect(c, B, nb, n_decays, nullptr);
         if (rc != ANM_OK) { free_events(); return rc; }
     }
-    ANM_CUDA_EV(cudaEventRecord(ev[2 * B + 1], st));
+    ANM_CUDA_EV(cudaEventRecord(ev[n_groups + 2], st));
     DeviceStats ds;
     unsigned long long bin_overflow = 0;
     if (BIN) ANM_CUDA_EV(cudaMemcpyAsync(&bin_overflow, c->bin_ovf.p, 8, cudaMemcpyDeviceToHost, st));
     ANM_CUDA_EV(cudaMemcpyAsync(&ds, c->dstats.p, sizeof ds, cudaMemcpyDeviceToHost, st));
     ANM_CUDA_EV(cudaStreamSynchronize(st));
+    c->batch_clean = true;      // every fold has run: the tallies are zero again
 
     double ms_t = 0, ms_f = 0, ms_fin = 0;
     if (depth > 1) {
         // overlapped launches have no separate durations: the whole pipeline (transport with the folds inside it) is
         // reported as transport time, conservatively; ms_fold = 0
         float a = 0;
-        cudaEventElapsedTime(&a, ev[0], ev[2 * B + 2]);
+        cudaEventElapsedTime(&a, ev[0], ev[n_groups + 1]);
         ms_t = a;
-    } else for (int b = 0; b < B; ++b) {
+    } else for (int g = 0; g < n_groups; ++g) {
         float a = 0, f = 0;
-        cudaEventElapsedTime(&a, ev[2 * b], ev[2 * b + 1]);
-        cudaEventElapsedTime(&f, ev[2 * b + 1], ev[2 * b + 2]);
+        cudaEventElapsedTime(&a, ev[g == 0 ? 0 : g], ev[n_groups + 3 + g]);       // [g] = after the folds of group g - 1
+        cudaEventElapsedTime(&f, ev[n_groups + 3 + g], ev[1 + g]);
         ms_t += a; ms_f += f;
     }
-    { float f = 0; cudaEventElapsedTime(&f, ev[depth > 1 ? 2 * B + 2 : 2 * B], ev[2 * B + 1]); ms_fin = f; }
+    { float f = 0; cudaEventElapsedTime(&f, ev[n_groups + 1], ev[n_groups + 2]); ms_fin = f; }
     free_events();
 #undef ANM_CUDA_EV
 
@@ -1286,9 +1293,15 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     s.n_steps = ds.n_steps; s.n_real = ds.n_real; s.n_pe = ds.n_pe; s.n_compton = ds.n_compton;
     s.n_rayleigh = ds.n_rayleigh; s.n_escaped = ds.n_escaped; s.n_cutoff = ds.n_cutoff; s.n_electrons = ds.n_electrons;
     s.n_hbh_overflow = ds.n_hbh_overflow;
+    s.n_check_violations = 0;
+    for (int k = 0; k < 12; ++k) {
+        s.n_check_violations += ds.n_violations[k];
+        if (ds.n_violations[k] && std::getenv("ANM_CHECK_VERBOSE")) fprintf(stderr, "anm bounds check %d: %llu violations\n", k, ds.n_violations[k]);
+    }
     s.ms_transport = ms_t; s.ms_fold = ms_f; s.ms_finalize = ms_fin; s.ms_setup = c->ms_setup;
     s.ms_load_ct = c->ms_load_ct; s.ms_load_pet = c->ms_load_pet;
-    s.n_launches = (uint64_t)2 * B + 1;
+    s.n_launches = (uint64_t)n_groups + B + 1;
+    s.batches_per_launch = (uint64_t)G;
     s.tally_binned = BIN ? 1 : 0;
     s.n_tally_overflow = bin_overflow;
     s.n_launches += 2;     // dose_max + run_sigma of the finalize

@@ -59,7 +59,18 @@ enum : int { ST_NEED = 0, ST_SOURCE = 1, ST_FLY = 2, ST_COMPTON = 3, ST_RAYLEIGH
 struct DeviceStats {   // accumulated with atomics at kernel exit (collect_stats only)
     double escaped_MeV;
     unsigned long long n_steps, n_real, n_pe, n_compton, n_rayleigh, n_escaped, n_cutoff, n_electrons, n_hbh_overflow;
+    unsigned long long n_violations[12];   // ANM_BOUNDS_CHECK builds: indices found out of range, per check (counted, never trapped)
 };
+
+// Bounds-check build (-DANM_BOUNDS_CHECK; profiles/r2_sanitizer.md): every index the transport kernels form -- voxel,
+// material, energy-grid cell, alias bucket, pool slot, ring fill, deposit-list and electron-array position -- is tested
+// against its range and a violation is COUNTED in DeviceStats::n_violations (anm_stats.n_check_violations) instead of
+// trapping, so a bad build cannot wedge the GPU.  Compiled out otherwise.
+#ifdef ANM_BOUNDS_CHECK
+#define ANM_CHK(p, id, cond) do { if (!(cond)) atomicAdd(&(p).stats->n_violations[id], 1ull); } while (0)
+#else
+#define ANM_CHK(p, id, cond) do {} while (0)
+#endif
 
 struct TransportParams {
     const uint32_t* texels;      // [V] material<<24 | density/2^-20
@@ -75,6 +86,11 @@ struct TransportParams {
     unsigned long long hist_base;   // global index of this launch's first history
     unsigned int n_hist;         // histories in this launch
     unsigned int n_alias;
+    unsigned int n_vox;          // nx * ny * nz
+    // batch group (event pool): one launch covers n_group consecutive batches of n_per_batch histories each; history hl of
+    // the launch belongs to local batch hl / n_per_batch, whose tally is batch + local batch * batch_stride
+    unsigned int n_per_batch, n_group;
+    size_t batch_stride;         // floats between the tallies of consecutive batches of the group
     unsigned int rk[20];         // Philox round keys: rk[2r] = seed_lo + r*0x9E3779B9, rk[2r+1] = seed_hi + r*0xBB67AE85
     int nx, ny, nz;
     int nm, ne, n_x2;
@@ -170,14 +186,15 @@ constexpr unsigned kTileSub = ANM_TILE_SUBLISTS;     // lists per tile (a CTA ap
                                                      // write streams); neither beats direct atomics on cfg3 (238 ms), cfg4 gains 3 % at 1
 
 template <int TALLY>
-__device__ __forceinline__ void deposit(const TransportParams& p, unsigned vox, float e) {
+__device__ __forceinline__ void deposit(const TransportParams& p, float* __restrict__ tally, unsigned vox, float e) {
+    ANM_CHK(p, 0, vox < p.n_vox && e >= 0.0f);
     if (TALLY == TALLY_WAGG) {
-        // merge the deposits of lanes that hit the same voxel in this trip: one RED per distinct voxel
+        // merge the deposits of lanes that hit the same voxel OF THE SAME BATCH in this trip: one RED per distinct word
         const unsigned act = __activemask();
-        const unsigned peers = __match_any_sync(act, vox);
+        const unsigned peers = __match_any_sync(act, reinterpret_cast<unsigned long long>(tally + vox));
         float total = 0.0f;
         for (unsigned rem = peers; rem; rem &= rem - 1) total += __shfl_sync(peers, e, __ffs(rem) - 1);
-        if ((threadIdx.x & 31) == (unsigned)(__ffs(peers) - 1)) atomicAdd(p.batch + vox, total);
+        if ((threadIdx.x & 31) == (unsigned)(__ffs(peers) - 1)) atomicAdd(tally + vox, total);
     } else if (TALLY == TALLY_BINNED) {
         // append {voxel, energy} to the tile's list; the lanes of this trip that hit the same tile share one atomic
         const unsigned tile = (vox >> kTileShift) * kTileSub + (blockIdx.x & (kTileSub - 1u));
@@ -190,9 +207,9 @@ __device__ __forceinline__ void deposit(const TransportParams& p, unsigned vox, 
         const unsigned pos = base + __popc(peers & ((1u << (threadIdx.x & 31)) - 1u));
         const uint2 seg = __ldg(p.bin_seg + tile);
         if (pos < seg.y) __stcs(p.bin_rec + (size_t)seg.x + pos, make_uint2(vox, __float_as_uint(e)));
-        else atomicAdd(p.batch + vox, e);            // the segment is full (or this is the counting batch): direct RED
+        else atomicAdd(tally + vox, e);              // the segment is full (or this is the counting batch): direct RED
     } else {
-        atomicAdd(p.batch + vox, e);
+        atomicAdd(tally + vox, e);
     }
 }
 
@@ -241,6 +258,8 @@ __device__ __forceinline__ SubStep fly_land(const TransportParams& p, const floa
     return o;
 }
 
+__device__ __forceinline__ unsigned load_texel(const TransportParams& p, unsigned vox) { return __ldg(p.texels + vox); }
+
 template <bool STATS>
 __device__ __forceinline__ int fly_two(const TransportParams& p, const float* __restrict__ s_tot,
                                        const float2* __restrict__ s_pec, float& x, float& y, float& z,
@@ -248,12 +267,13 @@ __device__ __forceinline__ int fly_two(const TransportParams& p, const float* __
                                        const float maj, const float inv_maj, const float maj_out, const float inv_maj_out,
                                        const uint4 r, unsigned& hull_bits, unsigned& vox, int& mat, FlyCounters& cnt) {
     const SubStep a = fly_land(p, x, y, z, u, v, w, maj, inv_maj, maj_out, inv_maj_out, r.x, hull_bits);
-    const unsigned ta = a.inside ? __ldg(p.texels + a.vox) : 0u;
+    const unsigned ta = a.inside ? load_texel(p, a.vox) : 0u;
     const SubStep b = fly_land(p, a.x, a.y, a.z, u, v, w, maj, inv_maj, maj_out, inv_maj_out, r.z, a.hull_bits);
     const bool b_inside = a.inside && b.inside;
-    const unsigned tb = b_inside ? __ldg(p.texels + b.vox) : 0u;
+    const unsigned tb = b_inside ? load_texel(p, b.vox) : 0u;
     // real / virtual: u' * majorant < rho * (mu/rho)_tot(E)
     const int mat_a = (int)(ta >> 24), mat_b = (int)(tb >> 24);
+    ANM_CHK(p, 1, mat_a < p.nm && mat_b < p.nm && ie >= 0 && ie <= p.ne - 2 && (!a.inside || a.vox < p.n_vox) && (!b_inside || b.vox < p.n_vox));
     const float rho_a = (float)(ta & 0xffffffu) * kDensityStep, rho_b = (float)(tb & 0xffffffu) * kDensityStep;
     const float* row_a = s_tot + mat_a * p.ne + ie;
     const float* row_b = s_tot + mat_b * p.ne + ie;
@@ -336,8 +356,10 @@ __device__ __forceinline__ unsigned sample_source(const TransportParams& p, cons
     } else {
         const unsigned long long r64 = ((unsigned long long)r.x << 32) | r.y;
         const unsigned j = (unsigned)__umul64hi(r64, (unsigned long long)p.n_alias);
+        ANM_CHK(p, 2, j < p.n_alias);
         const uint4 a = __ldcs(p.alias + j);      // one use per decay, 16 B out of ~100 MB: evict-first, keep L2 for texels + tally
         voxel = (r.z < a.x) ? a.y : a.z;
+        ANM_CHK(p, 3, voxel < p.n_vox);
         const unsigned nxy = (unsigned)p.nx * (unsigned)p.ny;
         iz = voxel / nxy;
         const unsigned rem = voxel - iz * nxy;
@@ -388,6 +410,7 @@ __device__ __forceinline__ float electron_walk_to(const TransportParams& p, cons
                 dtz = ez != 0.0f ? fabsf(__fdividef(p.dz, ez)) : inf;
     float t = 0.0f;
     for (;;) {
+        ANM_CHK(p, 4, vox < p.n_vox);
         const unsigned texel = __ldg(p.texels + vox);
         const float rho = (float)(texel & 0xffffffu) * kDensityStep;
         const float* R = er + (texel >> 24) * (unsigned)p.n_t;
@@ -500,7 +523,7 @@ transport_kernel(const __grid_constant__ TransportParams p) {
             const unsigned voxel = sample_source(p, h, x, y, z, u, v, w, in_box);
             stash[0 * kThreads] = x; stash[1 * kThreads] = y; stash[2 * kThreads] = z;
             stash[3 * kThreads] = u; stash[4 * kThreads] = v; stash[5 * kThreads] = w;
-            if (p.positron_ke > 0.0f) deposit<TALLY>(p, voxel, p.positron_ke);
+            if (p.positron_ke > 0.0f) deposit<TALLY>(p, p.batch, voxel, p.positron_ke);
             E = kE0; set_t(t0);
             hb_src = in_box ? 1u : 0u; hb = hb_src;
             photon = 0; blk = 0; state = ST_FLY;
@@ -514,7 +537,7 @@ transport_kernel(const __grid_constant__ TransportParams p) {
             const int code = fly_two<STATS>(p, s_tot, s_pec, x, y, z, u, v, w, ie, fe, maj, inv_maj, majo, inv_majo, r, hb, vox, mat, fc);
             ANM_TR("S1 h=%llu ph=%d blk=%u FLY code=%d E=%.9g t=%d+%.9g pos=%.9g %.9g %.9g vox=%u hb=%u\n", h, photon, blk - 1, code, E, ie, fe, x, y, z, vox, hb);
             if (code == FLY_ESCAPED) { if (STATS) { esc += E; ++c_esc; } dead = true; }
-            else if (code == FLY_PE) { if (STATS) ++c_pe; deposit<TALLY>(p, vox, E); dead = true; }   // all energy local
+            else if (code == FLY_PE) { if (STATS) ++c_pe; deposit<TALLY>(p, p.batch, vox, E); dead = true; }   // all energy local
             else if (code == FLY_COMPTON) state = ST_COMPTON;
             else if (code == FLY_RAYLEIGH) state = ST_RAYLEIGH;
         } else if (state == ST_COMPTON) {
@@ -525,7 +548,7 @@ transport_kernel(const __grid_constant__ TransportParams p) {
                 E *= eps;
                 if (E < p.cutoff) { dep += E; dead = true; if (STATS) ++c_cut; }
                 else { rotate(u, v, w, 1.0f - t, kTwoPi * u01(r.w)); set_energy(E); hb &= 1u; state = ST_FLY; }
-                deposit<TALLY>(p, vox, dep);
+                deposit<TALLY>(p, p.batch, vox, dep);
             }
         } else {   // ST_RAYLEIGH
             float c;
@@ -588,7 +611,7 @@ constexpr unsigned kHbhShift = 26;          // the list length lives in bits 26-
 constexpr unsigned kHbhHistMask = (1u << kHbhShift) - 1u;   // so a launch may hold at most 2^26 histories in this mode
 
 // hl = the slot's history word in shared memory: history index of the launch | list length << 26
-__device__ __forceinline__ void hbh_flush(const TransportParams& p, unsigned gslot, unsigned& hl) {
+__device__ __forceinline__ void hbh_flush(const TransportParams& p, float* __restrict__ tally, unsigned gslot, unsigned& hl) {
     const uint2* L = p.hbh_list + gslot;
     const unsigned n = hl >> kHbhShift;
     for (unsigned i = 0; i < n; ++i) {
@@ -601,14 +624,15 @@ __device__ __forceinline__ void hbh_flush(const TransportParams& p, unsigned gsl
             const uint2 b = L[(size_t)j * p.hbh_nslots];
             if (b.x == a.x) X += __uint_as_float(b.y);
         }
-        atomicAdd(p.batch + a.x, X);
+        atomicAdd(tally + a.x, X);
         atomicAdd(p.hbh_sq + a.x, X * X);
     }
     hl &= kHbhHistMask;
 }
 
-__device__ __forceinline__ void hbh_push(const TransportParams& p, unsigned gslot, unsigned& hl, unsigned vox, float e, unsigned& overflow) {
-    if ((hl >> kHbhShift) == kHbhCap) { hbh_flush(p, gslot, hl); ++overflow; }
+__device__ __forceinline__ void hbh_push(const TransportParams& p, float* __restrict__ tally, unsigned gslot, unsigned& hl, unsigned vox, float e, unsigned& overflow) {
+    if ((hl >> kHbhShift) == kHbhCap) { hbh_flush(p, tally, gslot, hl); ++overflow; }
+    ANM_CHK(p, 5, (hl >> kHbhShift) < kHbhCap && gslot < p.hbh_nslots && vox < p.n_vox);
     p.hbh_list[gslot + (size_t)(hl >> kHbhShift) * p.hbh_nslots] = make_uint2(vox, __float_as_uint(e));
     hl += 1u << kHbhShift;
 }
@@ -642,7 +666,9 @@ constexpr int kRayleighBatch = ANM_RAYBATCH;           // run the (rare) Rayleig
 enum : int { F_X = 0, F_Y, F_Z, F_U, F_V, F_W, F_E, F_TV /* FLY: ln-E grid coordinate; COMPTON/RAYLEIGH: voxel */,
              kBankFields, F_HL = 2 * kBankFields, F_META, kSlotFields };
 // meta = photon (bit 0) | hull bits IN, AWAY (bits 1-2) | decay voxel inside the hull box (bit 3) | material (bits 4-6)
-//        | Philox block counter (bits 8-31)
+//        | local batch of the decay within the launch's batch group (bits 8-15) | Philox block counter (bits 16-31)
+constexpr unsigned kBlkInc = 1u << 16;      // one more Philox block
+constexpr unsigned kMaxGroup = 256;         // batches per launch (8 bits of the meta word)
 enum : int { Q_F = 0, Q_C = 1, Q_S = 2, Q_R = 3, Q_NONE = 4 };
 constexpr size_t kPoolWarpBytes = (size_t)kSlotFields * kSlots * 4 + 4 * kSlots;   // slots + the four queues (bytes)
 
@@ -694,6 +720,9 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
     FlyCounters fc = {0u, 0u};
     const unsigned gslot0 = (blockIdx.x * (unsigned)kPoolWarps + (threadIdx.x >> 5)) * (unsigned)kSlots;   // HBH: this warp's lists
 
+    // the tally of the batch a slot's decay belongs to (meta bits 8-15 = its local batch within the launch's group)
+    auto tally_of = [&](const unsigned meta) { return p.batch + (size_t)((meta >> 8) & 0xffu) * p.batch_stride; };
+
     // Push every processed slot onto the ring of its next event (all 32 lanes call it; idle lanes pass Q_NONE):
     // one match groups the lanes by destination, the rank inside the group is the ring offset, one packed warp
     // reduction counts the four groups (head + length per byte stays below 128: no carry between the bytes).
@@ -718,6 +747,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
         const unsigned b = __ballot_sync(0xffffffffu, e_want);
         if (b) {
             if (e_want) {
+                ANM_CHK(p, 6, pend + __popc(b & lanemask_lt) < kPend);
                 float* E = ering + pend + __popc(b & lanemask_lt);
                 E[0 * kPend] = e_x; E[1 * kPend] = e_y; E[2 * kPend] = e_z;
                 E[3 * kPend] = e_ex; E[4 * kPend] = e_ey; E[5 * kPend] = e_ez;
@@ -746,6 +776,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
         __syncwarp();
         // ---- pick the event type with the longest queue ------------------------------------------------
         const unsigned nF = cnts & 255u, nC = (cnts >> 8) & 255u, nS = (cnts >> 16) & 255u, nR = cnts >> 24;
+        ANM_CHK(p, 7, nF + nC + nS + nR == (unsigned)kSlots);      // every slot waits in exactly one ring between trips
         int X = Q_F;
         unsigned best = nF;
         if (nC > best) { X = Q_C; best = nC; }
@@ -779,6 +810,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
         cnts -= n << shX;
         const unsigned slot = q[X * kSlots + ((head + lane) & (kSlots - 1))];
         const bool active = lane < n;
+        ANM_CHK(p, 8, !active || slot < (unsigned)kSlots);
         float* S = slots + slot;
         unsigned* SU = slots_u + slot;
         int next = Q_NONE;
@@ -786,7 +818,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
         // a finished photon: start the partner (bank 1, written at the decay) or free the slot
         auto photon_ends = [&](unsigned meta) {
             if (!(meta & 1u) && p.photons_per_decay == 2) {
-                SU[F_META * kSlots] = 1u | (meta & 8u) | ((meta & 8u) >> 2);   // photon B, block 0, IN = decay voxel's
+                SU[F_META * kSlots] = 1u | (meta & 0xff08u) | ((meta & 8u) >> 2);   // photon B, block 0, IN = decay voxel's, same batch
                 next = Q_F;
             } else {
                 next = Q_S;
@@ -798,7 +830,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                 const unsigned meta = SU[F_META * kSlots];
                 const unsigned ph = meta & 1u;
                 const unsigned long long h = p.hist_base + (HBH ? SU[F_HL * kSlots] & kHbhHistMask : SU[F_HL * kSlots]);
-                const uint4 r = philox4x32_10(make_uint4((unsigned)h, (unsigned)(h >> 32), meta >> 8, 1u + ph), p);
+                const uint4 r = philox4x32_10(make_uint4((unsigned)h, (unsigned)(h >> 32), meta >> 16, 1u + ph), p);
                 float* Bk = S + ph * (kBankFields * kSlots);
                 float x = Bk[F_X * kSlots], y = Bk[F_Y * kSlots], z = Bk[F_Z * kSlots];
                 const float u = Bk[F_U * kSlots], v = Bk[F_V * kSlots], w = Bk[F_W * kSlots];
@@ -812,7 +844,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                 unsigned vox = 0, hb = (meta >> 1) & 3u;
                 int mat = 0;
                 const int code = fly_two<STATS>(p, s_tot, s_pec, x, y, z, u, v, w, ie, fe, maj, inv_maj, majo, inv_majo, r, hb, vox, mat, fc);
-                ANM_TR("S2 h=%llu ph=%u blk=%u FLY code=%d t=%d+%.9g pos=%.9g %.9g %.9g vox=%u hb=%u\n", h, ph, meta >> 8, code, ie, fe, x, y, z, vox, hb);
+                ANM_TR("S2 h=%llu ph=%u blk=%u FLY code=%d t=%d+%.9g pos=%.9g %.9g %.9g vox=%u hb=%u\n", h, ph, meta >> 16, code, ie, fe, x, y, z, vox, hb);
                 Bk[F_X * kSlots] = x; Bk[F_Y * kSlots] = y; Bk[F_Z * kSlots] = z;
                 // next event and slot header, branch-free: GO -> FLY; COMPTON / RAYLEIGH -> their queues, the voxel in
                 // place of the energy coordinate; PE / ESCAPED end the photon: start the partner (bank 1, written at
@@ -820,8 +852,8 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                 const bool coll = code == FLY_COMPTON || code == FLY_RAYLEIGH;
                 const bool ended = code == FLY_PE || code == FLY_ESCAPED;
                 const bool partner = !ph && p.photons_per_decay == 2;
-                const unsigned meta_go = (((meta & ~0x76u) | (hb << 1)) + 256u) | (code == FLY_RAYLEIGH ? (unsigned)mat << 4 : 0u);
-                const unsigned meta_end = 1u | (meta & 8u) | ((meta & 8u) >> 2);   // photon B, block 0, IN = decay voxel's
+                const unsigned meta_go = (((meta & ~0x76u) | (hb << 1)) + kBlkInc) | (code == FLY_RAYLEIGH ? (unsigned)mat << 4 : 0u);
+                const unsigned meta_end = 1u | (meta & 0xff08u) | ((meta & 8u) >> 2);   // photon B, block 0, IN = decay voxel's, same batch
                 SU[F_META * kSlots] = ended ? meta_end : meta_go;
                 if (coll) reinterpret_cast<unsigned*>(Bk)[F_TV * kSlots] = vox;
                 next = code == FLY_COMPTON ? Q_C : (code == FLY_RAYLEIGH ? Q_R : ((ended && !partner) ? Q_S : Q_F));
@@ -830,11 +862,11 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                     const float Epe = Bk[F_E * kSlots];
                     if (ELEC && Epe > p.t_min) {          // rare (0.002 per decay): walked on the spot, not queued
                         const float out = HBH ? electron_walk_to(p, s_er, x, y, z, u, v, w, vox, Epe, [&](unsigned vv, float ee) {
-                                                    hbh_push(p, gslot0 + slot, SU[F_HL * kSlots], vv, ee, c_ovf); })
+                                                    hbh_push(p, tally_of(meta), gslot0 + slot, SU[F_HL * kSlots], vv, ee, c_ovf); })
                                               : electron_walk(p, s_er, x, y, z, u, v, w, vox, Epe);
                         if (STATS) { esc += out; ++c_el; }
-                    } else if (HBH) hbh_push(p, gslot0 + slot, SU[F_HL * kSlots], vox, Epe, c_ovf);
-                    else deposit<TALLY>(p, vox, Epe);
+                    } else if (HBH) hbh_push(p, tally_of(meta), gslot0 + slot, SU[F_HL * kSlots], vox, Epe, c_ovf);
+                    else deposit<TALLY>(p, tally_of(meta), vox, Epe);
                 }
                 if (STATS && code == FLY_ESCAPED) { esc += Bk[F_E * kSlots]; ++c_esc; }
             }
@@ -844,7 +876,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                 const unsigned meta = SU[F_META * kSlots];
                 const unsigned ph = meta & 1u;
                 const unsigned long long h = p.hist_base + (HBH ? SU[F_HL * kSlots] & kHbhHistMask : SU[F_HL * kSlots]);
-                const uint4 r = philox4x32_10(make_uint4((unsigned)h, (unsigned)(h >> 32), meta >> 8, 1u + ph), p);
+                const uint4 r = philox4x32_10(make_uint4((unsigned)h, (unsigned)(h >> 32), meta >> 16, 1u + ph), p);
                 float* Bk = S + ph * (kBankFields * kSlots);
                 float E = Bk[F_E * kSlots];
                 float eps, t;
@@ -867,7 +899,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                             if (HBH) {            // the deposits belong to this decay's list: walked on the spot
                                 const float out = electron_walk_to(p, s_er, Bk[F_X * kSlots], Bk[F_Y * kSlots], Bk[F_Z * kSlots], ex, ey, ez,
                                                                    vox, dep, [&](unsigned vv, float ee) {
-                                                                       hbh_push(p, gslot0 + slot, SU[F_HL * kSlots], vv, ee, c_ovf); });
+                                                                       hbh_push(p, tally_of(meta), gslot0 + slot, SU[F_HL * kSlots], vv, ee, c_ovf); });
                                 if (STATS) { esc += out; ++c_el; }
                             } else {
                                 e_want = true; e_x = Bk[F_X * kSlots]; e_y = Bk[F_Y * kSlots]; e_z = Bk[F_Z * kSlots];
@@ -884,12 +916,12 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                         Bk[F_U * kSlots] = u; Bk[F_V * kSlots] = v; Bk[F_W * kSlots] = w;
                         Bk[F_E * kSlots] = E;
                         Bk[F_TV * kSlots] = fminf(fmaxf((__logf(E) - p.lnE_min) * p.inv_dlnE, 0.0f), t_max);
-                        SU[F_META * kSlots] = (meta & ~0x74u) + 256u;     // a scatter clears AWAY
+                        SU[F_META * kSlots] = (meta & ~0x74u) + kBlkInc;     // a scatter clears AWAY
                         next = Q_F;
                     }
-                    if (dep > 0.0f) { if (HBH) hbh_push(p, gslot0 + slot, SU[F_HL * kSlots], vox, dep, c_ovf); else deposit<TALLY>(p, vox, dep); }
+                    if (dep > 0.0f) { if (HBH) hbh_push(p, tally_of(meta), gslot0 + slot, SU[F_HL * kSlots], vox, dep, c_ovf); else deposit<TALLY>(p, tally_of(meta), vox, dep); }
                 } else {
-                    SU[F_META * kSlots] = meta + 256u;
+                    SU[F_META * kSlots] = meta + kBlkInc;
                     next = Q_C;
                 }
             }
@@ -899,8 +931,10 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
             if (active) {
                 // HBH: the slot's previous decay is complete; its deposits are merged per voxel HERE, where up to 32 freed
                 // slots are handled by 32 lanes at once, not at the photon's end, where one or two lanes of a trip would do it
-                if (HBH) hbh_flush(p, gslot0 + slot, SU[F_HL * kSlots]);
+                if (HBH) hbh_flush(p, tally_of(SU[F_META * kSlots]), gslot0 + slot, SU[F_HL * kSlots]);
                 const unsigned long long h = p.hist_base + hl_new;
+                const unsigned bl = p.n_group > 1u ? hl_new / p.n_per_batch : 0u;      // the decay's batch within the group
+                ANM_CHK(p, 9, bl < p.n_group);
                 float x, y, z, u, v, w;
                 bool in_box;
                 const unsigned voxel = sample_source(p, h, x, y, z, u, v, w, in_box);
@@ -912,8 +946,8 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                 B1[F_U * kSlots] = -u; B1[F_V * kSlots] = -v; B1[F_W * kSlots] = -w;
                 B1[F_E * kSlots] = kE0; B1[F_TV * kSlots] = t0;
                 SU[F_HL * kSlots] = hl_new;
-                SU[F_META * kSlots] = in_box ? (2u | 8u) : 0u;
-                if (p.positron_ke > 0.0f) { if (HBH) hbh_push(p, gslot0 + slot, SU[F_HL * kSlots], voxel, p.positron_ke, c_ovf); else deposit<TALLY>(p, voxel, p.positron_ke); }
+                SU[F_META * kSlots] = (in_box ? (2u | 8u) : 0u) | (bl << 8);
+                if (p.positron_ke > 0.0f) { if (HBH) hbh_push(p, p.batch + (size_t)bl * p.batch_stride, gslot0 + slot, SU[F_HL * kSlots], voxel, p.positron_ke, c_ovf); else deposit<TALLY>(p, p.batch + (size_t)bl * p.batch_stride, voxel, p.positron_ke); }
                 q[Q_F * kSlots + ((heads + cnts + lane) & (kSlots - 1))] = (unsigned char)slot;
             }
             cnts += n;
@@ -922,7 +956,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                 const unsigned meta = SU[F_META * kSlots];
                 const unsigned ph = meta & 1u;
                 const unsigned long long h = p.hist_base + (HBH ? SU[F_HL * kSlots] & kHbhHistMask : SU[F_HL * kSlots]);
-                const uint4 r = philox4x32_10(make_uint4((unsigned)h, (unsigned)(h >> 32), meta >> 8, 1u + ph), p);
+                const uint4 r = philox4x32_10(make_uint4((unsigned)h, (unsigned)(h >> 32), meta >> 16, 1u + ph), p);
                 float* Bk = S + ph * (kBankFields * kSlots);
                 const float E = Bk[F_E * kSlots];
                 float c;
@@ -932,10 +966,10 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                     rotate(u, v, w, c, kTwoPi * u01(r.z));
                     Bk[F_U * kSlots] = u; Bk[F_V * kSlots] = v; Bk[F_W * kSlots] = w;
                     Bk[F_TV * kSlots] = fminf(fmaxf((__logf(E) - p.lnE_min) * p.inv_dlnE, 0.0f), t_max);
-                    SU[F_META * kSlots] = (meta & ~0x74u) + 256u;         // a scatter clears AWAY
+                    SU[F_META * kSlots] = (meta & ~0x74u) + kBlkInc;         // a scatter clears AWAY
                     next = Q_F;
                 } else {
-                    SU[F_META * kSlots] = meta + 256u;
+                    SU[F_META * kSlots] = meta + kBlkInc;
                     next = Q_R;
                 }
             }
@@ -947,7 +981,8 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
     if (HBH) {      // the decays that completed after the last SOURCE trip
         __syncwarp();
 #pragma unroll 1
-        for (int k = 0; k < kSlots / 32; ++k) hbh_flush(p, gslot0 + lane + 32u * (unsigned)k, slots_u[F_HL * kSlots + lane + 32 * k]);
+        for (int k = 0; k < kSlots / 32; ++k)
+            hbh_flush(p, tally_of(slots_u[F_META * kSlots + lane + 32 * k]), gslot0 + lane + 32u * (unsigned)k, slots_u[F_HL * kSlots + lane + 32 * k]);
     }
     if (STATS) {
         unsigned c_steps = fc.steps, c_real = fc.real;

@@ -284,6 +284,41 @@ def test_schedules_and_hull_run_the_same_histories(anm, tables, k, scale, n, B):
     assert np.allclose(hs[0]["energy"], hs[1]["energy"], rtol=1e-4, atol=1e-3)
 
 
+@pytest.mark.parametrize("case", ["patient", "point_wagg", "hbh"])
+def test_batch_groups_keep_every_batch_apart(anm, tables, case):
+    """anm_options.batches_per_launch: one launch covers G batches, every deposit tagged with its decay's batch.  The
+    histories and the per-batch tallies must not depend on G: the per-batch organ rows (a sum over the batch's own
+    tally), the energy map, the batch sum of squares and every counter agree between G = 1 (one launch per batch) and
+    grouped launches -- also with a ragged last group, with the warp-aggregated atomics of a point source (lanes of
+    DIFFERENT batches hit the same voxel in one trip) and with the history-by-history deposit lists."""
+    n, B = 240_000, 24
+    if case == "point_wagg":
+        cfg = dict(anm_inputs.make_config(0, 2), positron_ke_mev=0.2498)
+        kw = dict(warp_aggregate=1)
+    else:
+        cfg = anm_inputs.make_config(3, 4)
+        kw = dict(uncertainty=1) if case == "hbh" else {}
+    out = {}
+    for G in (1, 7, 0):
+        with anm.Simulation(0) as sim:
+            sim.load_config(cfg, tables, n_batches=B, collect_stats=1, batches_per_launch=G, **kw)
+            sim.run(n, 11)
+            st = sim.get_stats()
+            s_, q_, rows = sim.get_tally_buffers()
+            out[G] = (st, sim.get_energy().astype(np.float64), q_.cpu().numpy().astype(np.float64), rows.cpu().numpy().copy())
+    assert out[1][0]["batches_per_launch"] == 1 and out[7][0]["batches_per_launch"] == 6 and out[0][0]["batches_per_launch"] == B
+    assert out[1][0]["n_launches"] == 2 * B + 3 and out[0][0]["n_launches"] == 1 + B + 3       # (even groups: 24 = 4 x 6)
+    ref = out[1]
+    for G in (7, 0):
+        st, e, q, rows = out[G]
+        for key in ("n_steps", "n_real", "n_pe", "n_compton", "n_rayleigh", "n_escaped", "n_cutoff"):
+            assert st[key] == ref[0][key], (G, key)
+        assert np.allclose(e, ref[1], rtol=2e-5, atol=1e-4)                  # fp32 atomic order only
+        assert np.allclose(q, ref[2], rtol=1e-4, atol=1e-3)
+        assert np.allclose(rows, ref[3], rtol=1e-6, atol=1e-9)               # batch by batch, organ by organ
+    assert np.count_nonzero(ref[3].sum(1)) == B
+
+
 def test_positron_energy_lands_in_decay_voxels(anm, tables):
     n = 4
     act = np.zeros((n, n, n), np.float32)
