@@ -20,6 +20,7 @@ from .materials import AIR, LUNG, WATER, BONE
 
 GENERATOR_SEED = 2111
 DENSITY_STEP = 2.0 ** -20
+DENSITY_STEP_16 = 2.0 ** -12          # cfg4: on this grid a 16-bit texel holds every density exactly (reading C18)
 
 CONFIG_NAMES = ["cfg0_point_sanity", "cfg1_water_validation", "cfg2_slabs",
                 "cfg3_patient", "cfg4_fullres"]
@@ -60,8 +61,10 @@ _BODY_Z = 1600.0
 TOTAL_ACTIVITY_BQ = 8.0 * 3.7e7 * float(np.exp(-np.log(2.0) * 60.0 / 109.77))
 
 
-def quantize_density(rho):
-    return (np.round(np.asarray(rho, np.float64) / DENSITY_STEP) * DENSITY_STEP).astype(np.float32)
+def quantize_density(rho, step=DENSITY_STEP):
+    """Densities on the grid both sides are handed (reading C18): multiples of `step` g/cm^3 -- 2^-20, the 32-bit
+    texel's grid, or DENSITY_STEP_16 = 2^-12, on which a 16-bit texel holds the value exactly (cfg4)."""
+    return (np.round(np.asarray(rho, np.float64) / step) * step).astype(np.float32)
 
 
 def _patient_params():
@@ -132,7 +135,7 @@ def _patient_slice(x, y, z, params):
     return mat, rho, noisy, lab, act
 
 
-def _patient_volume(nx, ny, nz, dx, dy, dz, z_stretch=1.0, with_activity=True):
+def _patient_volume(nx, ny, nz, dx, dy, dz, z_stretch=1.0, with_activity=True, density_step=DENSITY_STEP):
     """Sample the analytic patient on an (nx,ny,nz) grid centred in-plane; z in mm from the grid bottom,
     divided by z_stretch to land in the cfg3 frame."""
     params = _patient_params()
@@ -148,7 +151,7 @@ def _patient_volume(nx, ny, nz, dx, dy, dz, z_stretch=1.0, with_activity=True):
         g = np.random.Generator(np.random.Philox(key=np.array([GENERATOR_SEED, iz], dtype=np.uint64)))
         noise = g.standard_normal(size=r.shape) * 0.02
         r = np.where(noisy, np.maximum(r + noise, 0.9), r)
-        mat[iz], rho[iz], lab[iz] = m, quantize_density(r), l
+        mat[iz], rho[iz], lab[iz] = m, quantize_density(r, density_step), l
         if with_activity:
             act[iz] = a
     return mat, rho, lab, act
@@ -271,7 +274,7 @@ def make_config(k: int, scale: int = 1) -> dict:
         sp = (0.98 * s, 0.98 * s, 3.0 * s)
         c = _base(CONFIG_NAMES[4], (nx, ny, nz), sp, 10_000_000_000, 42, 100, 2, positron_ke=0.2498)
         stretch = (nz * sp[2]) / _BODY_Z
-        mat, rho, lab, _ = _patient_volume(nx, ny, nz, *sp, z_stretch=stretch, with_activity=False)
+        mat, rho, lab, _ = _patient_volume(nx, ny, nz, *sp, z_stretch=stretch, with_activity=False, density_step=DENSITY_STEP_16)
         act = _trilinear_activity(nx, ny, nz, *sp, z_stretch=stretch)
         c.update(material=mat, density=rho, activity=act, labels=lab, n_organs=27,
                  organ_names=list(ORGAN_NAMES))

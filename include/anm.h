@@ -135,7 +135,14 @@ typedef struct {
                                    256, and below 2^32 histories per launch); 1..256: at most that many.  Always 1 with
                                    schedule 1, electron_transport or tally = 2.  Same histories, same per-batch tallies.
                                    The ctx then owns pipeline depth x G tally volumes (anm_stats.batches_per_launch = G). */
-    int32_t reserved1;
+    int32_t texel_bits;         /* width of the (material, density) texel the Woodcock flight reads at random: 32 =
+                                   material<<24 | density / 2^-20 g/cm^3 (every phantom); 16 = material<<13 | density / 2^-12,
+                                   used only when it holds EXACTLY the same values -- every density of the loaded phantom on
+                                   the 2^-12 grid and below 2 g/cm^3 (checked at load) -- so the histories are the same and
+                                   the random-access footprint halves (reading C18; what matters when the volume
+                                   exceeds the L2, BASELINE.json cfg4).  0 auto / 16: 16-bit when exact and the run uses the
+                                   default event-pool kernel (no electron_transport, uncertainty = 1, tally = 2), else
+                                   32-bit; 32: always 32-bit.  anm_stats.texel_bits tells which the last run read.        */
 } anm_options;
 
 /* Electron data for anm_options.electron_transport ("The cutoff energies for
@@ -185,6 +192,7 @@ typedef struct {
     uint64_t n_voxels_gt10, n_voxels_gt50;
     double max_dose_Gy_per_decay;                          /* the largest non-air voxel dose                          */
     uint64_t batches_per_launch;                           /* G of the last run (anm_options.batches_per_launch)      */
+    uint64_t texel_bits;                                   /* 16 | 32: the texels the last run read (anm_options.texel_bits) */
     uint64_t n_check_violations;                           /* library built with -DANM_BOUNDS_CHECK: indices the transport
                                                               kernels found out of range (counted, not trapped); 0 in a
                                                               normal build, and expected 0 in a checking one               */
@@ -257,7 +265,11 @@ int anm_default_options(anm_options* o);   /* 100 batches, pairs, Rayleigh on, c
 /* --- run --------------------------------------------------------------------------------------- */
 /* Simulates histories 0..n_decays-1 with Philox4x32-10 key `seed`, counter (history, block, stream), in
  * n_batches consecutive batches; replaces the previous run's tallies.  Synchronous: results are complete
- * on return.  ANM_E_STATE unless grid, phantom, tables and a source are set. */
+ * on return.  ANM_E_STATE unless grid, phantom, tables and a source are set.  ANM_E_UNSUPPORTED when the staged
+ * tables do not fit the shared memory a CTA may opt into (227 KiB on sm_100a): the event pool (schedule 0 | 2) keeps
+ * 152 KiB of photon slots beside n_materials * n_energy * 12 + n_energy * 8 + (n_materials + 1) * n_x2 * 4 bytes of
+ * tables (+ the electron range tables) -- e.g. 8 materials x 1024 energies do not fit; schedule 1 needs 6 KiB + tables.
+ * Every call leaves cuda_device current (cudaSetDevice) on the calling thread. */
 int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed);
 
 /* --- results of the last run (n must equal nx*ny*nz) -------------------------------------------- */

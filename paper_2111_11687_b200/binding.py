@@ -46,7 +46,7 @@ class anm_options(C.Structure):
                 ("hull_majorant", C.c_int32), ("history_offset", C.c_uint64),
                 ("electron_transport", C.c_int32), ("uncertainty", C.c_int32),
                 ("batch_pipeline", C.c_int32), ("tally", C.c_int32),
-                ("batches_per_launch", C.c_int32), ("reserved1", C.c_int32)]
+                ("batches_per_launch", C.c_int32), ("texel_bits", C.c_int32)]
 
 
 class anm_electron_tables(C.Structure):
@@ -68,7 +68,7 @@ class anm_stats(C.Structure):
         ("tally_binned", C.c_uint64), ("n_tally_overflow", C.c_uint64),
         ("rms_rel_sigma_gt10", C.c_double), ("rms_rel_sigma_gt50", C.c_double), ("n_voxels_gt10", C.c_uint64),
         ("n_voxels_gt50", C.c_uint64), ("max_dose_Gy_per_decay", C.c_double), ("batches_per_launch", C.c_uint64),
-        ("n_check_violations", C.c_uint64)]
+        ("texel_bits", C.c_uint64), ("n_check_violations", C.c_uint64)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}

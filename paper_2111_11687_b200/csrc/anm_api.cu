@@ -45,8 +45,8 @@ struct DevBuf {
         if (e == cudaSuccess) n = count; else p = nullptr;
         return e;
     }
-    void release() {
-        if (p) { cudaDeviceSynchronize(); cudaFreeAsync(p, (cudaStream_t)0); }
+    void release(bool synced = false) {      // synced: the caller has just synchronised the device (anm_destroy frees ~30 buffers)
+        if (p) { if (!synced) cudaDeviceSynchronize(); cudaFreeAsync(p, (cudaStream_t)0); }
         p = nullptr; n = 0;
     }
 };
@@ -92,6 +92,8 @@ struct anm_ctx {
 
     // device memory
     DevBuf<uint32_t> texels;
+    DevBuf<uint16_t> texels16;            // the same volume in 16 bits, valid iff tex16_ok (every voxel exactly representable)
+    bool tex16_ok = false;
     DevBuf<float> batch, sum, sumsq, scratch;   // batch: [pipeline depth][batches per launch][Vpad] per-batch tallies
     bool batch_clean = false;             // `batch` holds zeros (the folds of a completed run leave it so)
     cudaStream_t pipe[3] = {nullptr, nullptr, nullptr};   // internal streams of the pipeline, created on first use
@@ -296,8 +298,12 @@ void fill_run_sigma(const anm_ctx* c, anm_stats& s) {
 using TransportFn = void (*)(const TransportParams);
 
 // schedule 1 (history-based lanes) or 2 (warp-scope event pool), with / without counters; tally = TALLY_RED / _WAGG / _BINNED
-TransportFn pick_transport(int schedule, bool stats, int tally, bool elec, bool hbh) {
+TransportFn pick_transport(int schedule, bool stats, int tally, bool elec, bool hbh, bool t16) {
     if (schedule == 2) {
+        if (t16 && !elec && !hbh && tally != TALLY_BINNED) {
+            if (tally == TALLY_WAGG) return stats ? transport_pool_kernel<true, false, false, TALLY_WAGG, true> : transport_pool_kernel<false, false, false, TALLY_WAGG, true>;
+            return stats ? transport_pool_kernel<true, false, false, TALLY_RED, true> : transport_pool_kernel<false, false, false, TALLY_RED, true>;
+        }
         if (hbh) return elec ? (stats ? transport_pool_kernel<true, true, true> : transport_pool_kernel<false, true, true>)
                              : (stats ? transport_pool_kernel<true, false, true> : transport_pool_kernel<false, false, true>);
         if (elec) return stats ? transport_pool_kernel<true, true, false> : transport_pool_kernel<false, true, false>;
@@ -403,9 +409,8 @@ int anm_create(anm_ctx** out, int cuda_device) {
     anm_ctx* c = new (std::nothrow) anm_ctx();
     if (!c) return ANM_E_NOMEM;
     c->device = cuda_device;
-    cudaDeviceProp prop;
-    if (cudaGetDeviceProperties(&prop, cuda_device) != cudaSuccess) { delete c; return ANM_E_CUDA; }
-    c->num_sms = prop.multiProcessorCount;
+    // (one attribute query: cudaGetDeviceProperties fills the whole property struct and costs ~1 ms per context)
+    if (cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, cuda_device) != cudaSuccess) { delete c; return ANM_E_CUDA; }
     {   // keep freed device memory cached in the default pool (see DevBuf)
         cudaMemPool_t pool;
         if (cudaDeviceGetDefaultMemPool(&pool, cuda_device) == cudaSuccess) {
@@ -421,12 +426,13 @@ int anm_create(anm_ctx** out, int cuda_device) {
 int anm_destroy(anm_ctx* c) {
     if (!c) return ANM_OK;
     cudaSetDevice(c->device);
-    c->texels.release(); c->batch.release(); c->sum.release(); c->sumsq.release(); c->scratch.release();
-    c->labels.release(); c->alias.release(); c->counters.release(); c->dstats.release();
-    c->organ_batch.release(); c->organ_acc.release(); c->organ_mass.release(); c->organ_count.release();
-    c->total_energy.release(); c->d_tot.release(); c->d_maj.release(); c->d_majo.release(); c->d_x2.release(); c->d_cum.release();
-    c->d_pec.release(); c->d_flags.release(); c->d_erange.release(); c->e_ring.release(); c->hbh_sq.release(); c->hbh_list.release();
-    c->bin_cnt.release(); c->bin_seg.release(); c->bin_seg0.release(); c->bin_rec.release(); c->bin_ovf.release();
+    cudaDeviceSynchronize();
+    c->texels.release(true); c->texels16.release(true); c->batch.release(true); c->sum.release(true); c->sumsq.release(true); c->scratch.release(true);
+    c->labels.release(true); c->alias.release(true); c->counters.release(true); c->dstats.release(true);
+    c->organ_batch.release(true); c->organ_acc.release(true); c->organ_mass.release(true); c->organ_count.release(true);
+    c->total_energy.release(true); c->d_tot.release(true); c->d_maj.release(true); c->d_majo.release(true); c->d_x2.release(true); c->d_cum.release(true);
+    c->d_pec.release(true); c->d_flags.release(true); c->d_erange.release(true); c->e_ring.release(true); c->hbh_sq.release(true); c->hbh_list.release(true);
+    c->bin_cnt.release(true); c->bin_seg.release(true); c->bin_seg0.release(true); c->bin_rec.release(true); c->bin_ovf.release(true);
     for (auto& ps : c->pipe) if (ps) { cudaStreamDestroy(ps); ps = nullptr; }
     delete c;
     return ANM_OK;
@@ -523,8 +529,17 @@ static int phantom_setup(anm_ctx* c) {
     {
         rho_max_kernel<<<grid_blocks(c, c->V, kFoldThreads), kFoldThreads, 0, c->stream>>>(c->texels.p, c->V, c->d_flags.p + 2);
         ANM_CUDA(c, cudaGetLastError());
+        // the 16-bit copy of the texels for the transport kernels' random reads (used when it is exact)
+        unsigned not_exact = 1;
+        ANM_CUDA(c, c->texels16.alloc(c->Vpad));
+        ANM_CUDA(c, cudaMemsetAsync(c->d_flags.p, 0, 4, c->stream));
+        pack_texels16_kernel<<<grid_blocks(c, c->V, kFoldThreads), kFoldThreads, 0, c->stream>>>(c->texels.p, c->texels16.p, c->V, c->d_flags.p);
+        ANM_CUDA(c, cudaGetLastError());
         ANM_CUDA(c, cudaMemcpyAsync(c->rho_max_counts, c->d_flags.p + 2, ANM_MAX_MATERIALS * 4, cudaMemcpyDeviceToHost, c->stream));
+        ANM_CUDA(c, cudaMemcpyAsync(&not_exact, c->d_flags.p, 4, cudaMemcpyDeviceToHost, c->stream));
         ANM_CUDA(c, cudaStreamSynchronize(c->stream));
+        c->tex16_ok = (not_exact == 0);
+        if (!c->tex16_ok) c->texels16.release();
     }
     {   // hull box: bounding box of the voxels denser than 5 % of the densest voxel; outside it the majorant is
         // that of the low-density margin (air around a patient).  Used only when the box is a proper part of the grid.
@@ -1015,6 +1030,7 @@ int anm_set_options(anm_ctx* c, const anm_options* o) {
     if (o->batch_pipeline < 0 || o->batch_pipeline > 3) return fail(c, ANM_E_ARG, "options: batch_pipeline must be 0 (auto), 1, 2 or 3");
     if (o->uncertainty != 0 && o->uncertainty != 1) return fail(c, ANM_E_ARG, "options: uncertainty must be 0 (batch) or 1 (history by history)");
     if (o->batches_per_launch < 0 || o->batches_per_launch > 256) return fail(c, ANM_E_ARG, "options: batches_per_launch must be 0 (auto) or 1..256");
+    if (o->texel_bits != 0 && o->texel_bits != 16 && o->texel_bits != 32) return fail(c, ANM_E_ARG, "options: texel_bits must be 0 (auto), 16 or 32");
     if (o->tally < 0 || o->tally > 2) return fail(c, ANM_E_ARG, "options: tally must be 0 (auto), 1 (direct atomics) or 2 (tile-binned)");
     if (o->tally == 2 && (o->schedule == 1 || o->electron_transport || o->uncertainty == 1 || o->warp_aggregate == 1))
         return fail(c, ANM_E_UNSUPPORTED, "options: the tile-binned tally runs in the event-pool schedule with the batch estimator, local electrons and no warp aggregation");
@@ -1102,7 +1118,18 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     // tile counters' same-address atomics bound it; needs the event pool, the batch estimator and local electrons
     const bool can_bin = schedule == 2 && !EL && !HB && !W;
     const bool BIN = can_bin && c->opt.tally == 2;
-    const TransportFn kern = pick_transport(schedule, S, BIN ? TALLY_BINNED : (W ? TALLY_WAGG : TALLY_RED), EL, HB);
+    // 16-bit texels (anm_options.texel_bits): the default kernel of the event pool reads the exact 16-bit copy when there is one
+    const bool T16 = c->tex16_ok && c->opt.texel_bits != 32 && schedule == 2 && !EL && !HB && !BIN;
+    p.texels16 = T16 ? c->texels16.p : nullptr;
+    const TransportFn kern = pick_transport(schedule, S, BIN ? TALLY_BINNED : (W ? TALLY_WAGG : TALLY_RED), EL, HB, T16);
+    {   // the event pool needs 152 KiB of slots plus the staged tables: large tables (the header admits n_energy = 1024
+        // with 8 materials) do not fit the 227 KiB a CTA may opt into -- say so instead of failing in the attribute call
+        int optin = 0;
+        ANM_CUDA(c, cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, c->device));
+        if (smem > (size_t)optin)
+            return fail(c, ANM_E_UNSUPPORTED, "run: tables too large for shared memory (%zu bytes needed, %d available%s)", smem, optin,
+                        schedule == 2 ? "; schedule = 1 needs 146 KiB less" : "");
+    }
     ANM_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 0;
     ANM_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem));
@@ -1302,6 +1329,7 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     s.ms_load_ct = c->ms_load_ct; s.ms_load_pet = c->ms_load_pet;
     s.n_launches = (uint64_t)n_groups + B + 1;
     s.batches_per_launch = (uint64_t)G;
+    s.texel_bits = T16 ? 16 : 32;
     s.tally_binned = BIN ? 1 : 0;
     s.n_tally_overflow = bin_overflow;
     s.n_launches += 2;     // dose_max + run_sigma of the finalize

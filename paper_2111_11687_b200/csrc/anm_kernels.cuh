@@ -74,6 +74,8 @@ struct DeviceStats {   // accumulated with atomics at kernel exit (collect_stats
 
 struct TransportParams {
     const uint32_t* texels;      // [V] material<<24 | density/2^-20
+    const uint16_t* texels16;    // [V] material<<13 | density/2^-12: the same volume in 16 bits when every voxel is exactly
+                                 // representable (anm_options.texel_bits; reading C18), else null
     float* batch;                // [V] energy of the current batch (MeV)
     const uint4* alias;          // [n_alias] {threshold, own voxel, alias voxel, 0}
     unsigned int* counter;       // history counter of this launch (starts at 0)
@@ -258,19 +260,30 @@ __device__ __forceinline__ SubStep fly_land(const TransportParams& p, const floa
     return o;
 }
 
-__device__ __forceinline__ unsigned load_texel(const TransportParams& p, unsigned vox) { return __ldg(p.texels + vox); }
+// A texel read of the Woodcock flight.  T16: from the 16-bit copy, expanded to the 32-bit format (13-bit density counts
+// of 2^-12 g/cm^3 = that count << 8 in units of 2^-20): the SAME material and density values, half the bytes per
+// random read and half the footprint in the L2 -- what matters once the volume no longer fits it (cfg4).
+constexpr unsigned kT16DensityBits = 13, kT16Shift = 8;        // 2^-12 g/cm^3 steps, below 2 g/cm^3; material ids 0..7
+template <bool T16>
+__device__ __forceinline__ unsigned load_texel(const TransportParams& p, unsigned vox) {
+    if (T16) {
+        const unsigned t = __ldg(p.texels16 + vox);
+        return ((t >> kT16DensityBits) << 24) | ((t & ((1u << kT16DensityBits) - 1u)) << kT16Shift);
+    }
+    return __ldg(p.texels + vox);
+}
 
-template <bool STATS>
+template <bool STATS, bool T16 = false>
 __device__ __forceinline__ int fly_two(const TransportParams& p, const float* __restrict__ s_tot,
                                        const float2* __restrict__ s_pec, float& x, float& y, float& z,
                                        const float u, const float v, const float w, const int ie, const float fe,
                                        const float maj, const float inv_maj, const float maj_out, const float inv_maj_out,
                                        const uint4 r, unsigned& hull_bits, unsigned& vox, int& mat, FlyCounters& cnt) {
     const SubStep a = fly_land(p, x, y, z, u, v, w, maj, inv_maj, maj_out, inv_maj_out, r.x, hull_bits);
-    const unsigned ta = a.inside ? load_texel(p, a.vox) : 0u;
+    const unsigned ta = a.inside ? load_texel<T16>(p, a.vox) : 0u;
     const SubStep b = fly_land(p, a.x, a.y, a.z, u, v, w, maj, inv_maj, maj_out, inv_maj_out, r.z, a.hull_bits);
     const bool b_inside = a.inside && b.inside;
-    const unsigned tb = b_inside ? load_texel(p, b.vox) : 0u;
+    const unsigned tb = b_inside ? load_texel<T16>(p, b.vox) : 0u;
     // real / virtual: u' * majorant < rho * (mu/rho)_tot(E)
     const int mat_a = (int)(ta >> 24), mat_b = (int)(tb >> 24);
     ANM_CHK(p, 1, mat_a < p.nm && mat_b < p.nm && ie >= 0 && ie <= p.ne - 2 && (!a.inside || a.vox < p.n_vox) && (!b_inside || b.vox < p.n_vox));
@@ -672,7 +685,7 @@ constexpr unsigned kMaxGroup = 256;         // batches per launch (8 bits of the
 enum : int { Q_F = 0, Q_C = 1, Q_S = 2, Q_R = 3, Q_NONE = 4 };
 constexpr size_t kPoolWarpBytes = (size_t)kSlotFields * kSlots * 4 + 4 * kSlots;   // slots + the four queues (bytes)
 
-template <bool STATS, bool ELEC, bool HBH, int TALLY = TALLY_RED>
+template <bool STATS, bool ELEC, bool HBH, int TALLY = TALLY_RED, bool T16 = false>
 __global__ void __launch_bounds__(kPoolThreads, kPoolMinBlocksPerSM)
 transport_pool_kernel(const __grid_constant__ TransportParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -843,7 +856,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                 const float inv_majo = __fdividef(1.0f, majo);
                 unsigned vox = 0, hb = (meta >> 1) & 3u;
                 int mat = 0;
-                const int code = fly_two<STATS>(p, s_tot, s_pec, x, y, z, u, v, w, ie, fe, maj, inv_maj, majo, inv_majo, r, hb, vox, mat, fc);
+                const int code = fly_two<STATS, T16>(p, s_tot, s_pec, x, y, z, u, v, w, ie, fe, maj, inv_maj, majo, inv_majo, r, hb, vox, mat, fc);
                 ANM_TR("S2 h=%llu ph=%u blk=%u FLY code=%d t=%d+%.9g pos=%.9g %.9g %.9g vox=%u hb=%u\n", h, ph, meta >> 16, code, ie, fe, x, y, z, vox, hb);
                 Bk[F_X * kSlots] = x; Bk[F_Y * kSlots] = y; Bk[F_Z * kSlots] = z;
                 // next event and slot header, branch-free: GO -> FLY; COMPTON / RAYLEIGH -> their queues, the voxel in
@@ -1280,6 +1293,20 @@ pack_texels_kernel(const uint8_t* __restrict__ material, const float* __restrict
     }
     if (bad) atomicOr(flags, 1u);
     atomicMax(max_mat, mm);
+}
+
+// 16-bit copy of the texels (anm_options.texel_bits): material<<13 | density / 2^-12.  not_exact is set when a voxel is
+// not exactly representable (density off the 2^-12 grid or >= 2 g/cm^3; material ids always fit, < 8): the copy is then
+// not used.
+__global__ void __launch_bounds__(kFoldThreads)
+pack_texels16_kernel(const uint32_t* __restrict__ texels, uint16_t* __restrict__ texels16, size_t V, unsigned* __restrict__ not_exact) {
+    unsigned bad = 0;
+    for (size_t i = (size_t)blockIdx.x * kFoldThreads + threadIdx.x; i < V; i += (size_t)gridDim.x * kFoldThreads) {
+        const unsigned t = texels[i], m = t >> 24, r = t & 0xffffffu;
+        if ((r & ((1u << kT16Shift) - 1u)) != 0u || (r >> kT16Shift) >= (1u << kT16DensityBits) || m >= 8u) bad = 1;
+        texels16[i] = (uint16_t)((m << kT16DensityBits) | ((r >> kT16Shift) & ((1u << kT16DensityBits) - 1u)));
+    }
+    if (bad) atomicOr(not_exact, 1u);
 }
 
 // per-material maximum density (texel counts) -> majorant

@@ -319,6 +319,33 @@ def test_batch_groups_keep_every_batch_apart(anm, tables, case):
     assert np.count_nonzero(ref[3].sum(1)) == B
 
 
+def test_16_bit_texels_are_the_same_phantom(anm, tables):
+    """anm_options.texel_bits (reading C18): the Woodcock flight reads a 16-bit copy of the texels only when it
+    holds exactly the values of the 32-bit one (cfg4's generator puts every density on the 2^-12 grid), so the histories
+    are the same: every counter equal, the energy map equal up to fp32 atomic order.  A phantom with one density off the
+    grid, one above 2 g/cm^3, or a run that needs the 32-bit kernels falls back to 32 bits."""
+    cfg = anm_inputs.make_config(4, 8)
+    n, B = 200_000, 10
+    runs = {}
+    for bits in (0, 32):
+        g = gpu_run(anm, cfg, tables, n, n_batches=B, collect_stats=1, texel_bits=bits)
+        runs[bits] = g
+    assert runs[0]["stats"]["texel_bits"] == 16 and runs[32]["stats"]["texel_bits"] == 32
+    for key in ("n_steps", "n_real", "n_pe", "n_compton", "n_rayleigh", "n_escaped", "n_cutoff"):
+        assert runs[0]["stats"][key] == runs[32]["stats"][key], key
+    assert np.allclose(runs[0]["energy"], runs[32]["energy"], rtol=2e-5, atol=1e-4)
+    assert np.allclose(runs[0]["organs"]["mean_Gy_per_decay"], runs[32]["organs"]["mean_Gy_per_decay"], rtol=1e-6)
+    # not representable -> 32 bits, silently (the result is what the phantom says, never a rounded copy of it)
+    for idx, val in (((3, 4, 5), 1.0 + 2.0 ** -20), ((0, 0, 0), 2.5)):
+        rho = cfg["density"].copy(); rho[idx] = val
+        g = gpu_run(anm, dict(cfg, density=rho), tables, 20_000, n_batches=B, texel_bits=16)
+        assert g["stats"]["texel_bits"] == 32
+    assert gpu_run(anm, cfg, tables, 20_000, n_batches=B, uncertainty=1)["stats"]["texel_bits"] == 32
+    assert gpu_run(anm, anm_inputs.make_config(3, 8), tables, 20_000, n_batches=B)["stats"]["texel_bits"] == 32    # cfg3: 2^-20 grid
+    with pytest.raises(anm.AnmError):
+        gpu_run(anm, cfg, tables, 20_000, n_batches=B, texel_bits=8)
+
+
 def test_positron_energy_lands_in_decay_voxels(anm, tables):
     n = 4
     act = np.zeros((n, n, n), np.float32)
