@@ -31,16 +31,21 @@ sys.path.insert(0, ROOT)
 
 WORKLOAD = "cfg3_patient 256x256x400 @2x2x4mm, 27 organs, pairs+positron KE, 100 batches"
 
-# DESIGN.md §5.1 / §6: algorithmic thread-instructions per event = the SASS instructions the per-event device functions
-# execute per lane (Philox4x32-10 + uniforms, fly_land / fly_two, compton_try + rotate + energy coordinate, rayleigh_try,
-# sample_source), counted from the ncu source page of the transport kernel (profiles/r2_event_instr.md has the command and
-# the table); the event pool's scheduling instructions (ring push / pick / pop, slot load / store, meta word) are NOT in
-# them.  Multiplied by the events per decay measured by a counted run.
-INSTR_SUBSTEP = 84.0     # half a Philox block, log, 3 FMA, voxel index, texel fetch + unpack, table lerp, accept test
-INSTR_COMPTON_TRY = 210.0
-INSTR_RAYLEIGH_TRY = 180.0
-INSTR_SOURCE = 260.0
-INSTR_PE = 4.0
+# DESIGN.md §5.1 / §6: algorithmic thread-instructions per unit of the method = the SASS instructions the per-event device
+# functions execute per lane, counted from the ncu source page of the transport kernel (profiles/r2_event_instr.md has the
+# command, the per-region table and how each constant is put together); the event pool's scheduling (ring push / pick /
+# pop), the slot loads / stores and the speculative half of a FLY event are NOT in them.  Multiplied by the units per
+# decay a counted run of the same workload measures (anm_stats: n_steps, n_compton_tries, n_compton, ...).
+INSTR_PHILOX = 46.2          # one Philox4x32-10 block (20 IMAD.WIDE + 20 LOP3 + counter set-up)
+INSTR_U01 = 3.2              # one uniform (SHF + I2F + FFMA)
+INSTR_SUBSTEP = 101.0        # half a block (23.1) + 2 uniforms (6.4) + fly_land (38.0) + half of fly_two (30.0) + texel load (3.5)
+INSTR_COMPTON_TRY = 86.8     # block + 3 uniforms (9.6) + compton_try (31.0)
+INSTR_COMPTON_ACCEPT = 51.2  # azimuth uniform (3.2) + rotate (35.0) + energy split, cutoff test, log, grid coordinate (13)
+INSTR_RAYLEIGH_TRY = 291.0   # block + 2 uniforms + rayleigh_try (238: two bisections of the 256-point form-factor table)
+INSTR_RAYLEIGH_ACCEPT = 44.0 # azimuth uniform + rotate + grid coordinate
+INSTR_DEPOSIT = 9.7          # address of the decay's batch tally + fp32 RED (Compton, photoelectric, positron)
+INSTR_SOURCE = 208.0         # 2 blocks (92.4) + 6 uniforms (19.2) + sample_source (86.0: alias bucket, voxel -> (ix, iy, iz), position,
+                             # direction) + hull test (11.0)
 LANES_PER_SM_PER_CLK = 128.0   # 4 SMSP x 32 lanes, one instruction per SMSP per clock
 N_SM = 148
 
@@ -191,7 +196,8 @@ def main():
         n_cnt = B * 100_000
         sim.run(n_cnt, cfg["seed"])
         cnt = sim.get_stats()
-        per_decay = {k: cnt[k] / n_cnt for k in ("n_steps", "n_real", "n_pe", "n_compton", "n_rayleigh")}
+        per_decay = {k: cnt[k] / n_cnt for k in ("n_steps", "n_real", "n_pe", "n_compton", "n_rayleigh", "n_fly_trips",
+                                                 "n_compton_tries", "n_rayleigh_tries")}
         sim.set_options(collect_stats=0, **opts)
         for _ in range(args.warmup):
             step(sim)
@@ -230,12 +236,17 @@ def main():
     #   hbm        algorithmic bytes (4 B texel, 8 B tally RMW, 16 B alias entry)  vs  MEASURED_PEAKS.json hbm_gbs
     # (cfg4 uses the 630 MB figures.)  The binding one is named by ncu (issue-slot utilisation vs L2 / DRAM throughput,
     # profiles/): the ALU / issue side on cfg3; `bound`, `achieved`, `peak`, `frac` repeat that entry.
-    compton_tries = per_decay["n_compton"] * 1.15
-    instr_per_decay = (per_decay["n_steps"] * INSTR_SUBSTEP + compton_tries * INSTR_COMPTON_TRY +
-                       per_decay["n_rayleigh"] * INSTR_RAYLEIGH_TRY * 1.4 + per_decay["n_pe"] * INSTR_PE + INSTR_SOURCE)
-    launches_transport = B * args.steps
+    deposits = per_decay["n_compton"] + per_decay["n_pe"] + (1.0 if cfg["positron_ke_mev"] > 0 else 0.0)
+    instr_per_decay = (per_decay["n_steps"] * INSTR_SUBSTEP + per_decay["n_compton_tries"] * INSTR_COMPTON_TRY +
+                       per_decay["n_compton"] * INSTR_COMPTON_ACCEPT + per_decay["n_rayleigh_tries"] * INSTR_RAYLEIGH_TRY +
+                       per_decay["n_rayleigh"] * INSTR_RAYLEIGH_ACCEPT + deposits * INSTR_DEPOSIT + INSTR_SOURCE)
+    # One step = n_groups transport launches (anm_options.batches_per_launch: G batches per launch) + B folds + finalize.
+    # With the launch pipeline ms_transport is the pipeline's wall time, folds included (conservative for `achieved`).
+    G = int(st["batches_per_launch"])
+    n_groups = (B + G - 1) // G
+    launches_transport = n_groups * args.steps
     sec_per_launch = ms_t * 1e-3 / launches_transport
-    decays_per_s_kernel = (D / B) / sec_per_launch
+    decays_per_s_kernel = (D / n_groups) / sec_per_launch
     achieved = instr_per_decay * decays_per_s_kernel / 1e9                          # G thread-instr / s
     sm_max = clk.get("sm_max_mhz") or 1965.0
     sm_run = clk.get("sm_mhz") or sm_max
@@ -247,7 +258,6 @@ def main():
         pass
     hbm_peak = float(file_peaks.get("hbm_gbs", 6500.0))
     big = args.config == 4
-    deposits = per_decay["n_compton"] + per_decay["n_pe"] + (1.0 if cfg["positron_ke_mev"] > 0 else 0.0)
     alg_bytes = 4.0 * per_decay["n_steps"] + 8.0 * deposits + 16.0
     if peaks_dev:
         slots_per_clk = peaks_dev["issue_gtis"] * 1e9 / (N_SM * LANES_PER_SM_PER_CLK * peaks_dev["issue_sm_mhz"] * 1e6)
@@ -267,7 +277,7 @@ def main():
         if name.endswith("_transport_traffic.csv"):
             import csv
             rows = list(csv.DictReader(open(os.path.join(tdir, name))))
-            if rows and int(rows[-1]["decays_per_launch"]) == D // B and args.config == 3:
+            if rows and int(rows[-1]["decays_per_launch"]) == D // n_groups and args.config == 3:
                 traffic = int(rows[-1]["dram_bytes_read"]) + int(rows[-1]["dram_bytes_write"])
                 traffic_source = "profiles/%s (ncu --set full capture of this kernel and launch size; not measured in this run)" % name
             break
@@ -282,7 +292,8 @@ def main():
                         "peak_source": "MEASURED_PEAKS.json hbm_gbs" if file_peaks else "fallback 6500 GB/s"},
                 "peaks_measured": peaks_dev,
                 "instr_per_decay_algorithmic": instr_per_decay, "events_per_decay": per_decay,
-                "avg_launch_ms": sec_per_launch * 1e3, "share_of_step": ms_t / max(ms_t + ms_f + ms_fin, 1e-9),
+                "avg_launch_ms": sec_per_launch * 1e3, "batches_per_launch": G, "transport_launches_per_step": n_groups,
+                "decays_per_launch": D // n_groups, "share_of_step": ms_t / max(ms_t + ms_f + ms_fin, 1e-9),
                 "texel_bytes_per_decay": 4.0 * per_decay["n_steps"], "tally_bytes_per_decay": 8.0 * deposits,
                 "algorithmic_bytes_per_decay": alg_bytes}
 
@@ -401,8 +412,16 @@ def main():
                 dps4 = n4 / (ms4 * 1e-3)
                 steps4, dep4 = c4["n_steps"] / 1e7, (c4["n_compton"] + c4["n_pe"]) / 1e7 + 1.0
                 v4 = {"workload": "cfg4_fullres 512x512x600 @0.98x0.98x3mm, 27 organs, pairs+positron KE, 100 batches",
-                      "decays": n4, "ms": ms4, "value": dps4, "unit": "decays/s",
+                      "decays": n4, "ms": ms4, "value": dps4, "unit": "decays/s", "texel_bits": int(st4["texel_bits"]),
+                      "batches_per_launch": int(st4["batches_per_launch"]),
                       "events_per_decay": {"n_steps": steps4, "deposits": dep4}}
+                if D >= 1_000_000_000:      # the config's own size (BASELINE.json configs[4]: "Run 1e10 decays"), once
+                    s4.run(10_000_000_000, cfg4["seed"])
+                    st10 = s4.get_stats()
+                    ms10 = st10["ms_transport"] + st10["ms_fold"] + st10["ms_finalize"]
+                    v4["run_1e10"] = {"decays": 10_000_000_000, "ms": ms10, "value": 1e10 / (ms10 * 1e-3), "unit": "decays/s",
+                                      "deposited_MeV": st10["deposited_MeV"], "rms_rel_sigma_gt10": st10["rms_rel_sigma_gt10"],
+                                      "rms_rel_sigma_gt50": st10["rms_rel_sigma_gt50"]}
                 if peaks_dev:      # the memory side binds here: random DRAM gathers + REDs over 630 MB volumes
                     t_model = steps4 / (peaks_dev["gather_gps"][1] * 1e9) + dep4 / (peaks_dev["red_gps"][1] * 1e9)
                     v4["roofline"] = {"bound": "hbm random access", "gather_frac": steps4 * dps4 / 1e9 / peaks_dev["gather_gps"][1],
@@ -435,7 +454,7 @@ def main():
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": WORKLOAD if args.config == 3 else "cfg4_fullres 512x512x600 @0.98x0.98x3mm (profiling only, not the bench workload)",
                    "decays_per_step_per_gpu": D, "seed": cfg["seed"],
-                   "l2": "working set (texels 105 MB + batch tally 105 MB + sum/sumsq 210 MB) exceeds the 126 MB L2; no flush needed",
+                   "l2": "working set (texels 105 MB + per-batch tallies (one 105 MB volume per batch in flight) + sum/sumsq 210 MB + alias 94 MB) exceeds the 126 MB L2; no flush needed",
                    "multi_gpu": "one logical run of N*D decays: whole-batch shards via history_offset, NCCL sum-all-reduce of the tallies + merged finalize at the end of every step" if world > 1 else "single GPU"},
         "clocks": clk, "e2e": e2e, "gpu_launches": int(launches),
         "phase_ms_per_step": {"transport": ms_t / args.steps, "fold": ms_f / args.steps, "finalize": ms_fin / args.steps},

@@ -192,6 +192,10 @@ typedef struct {
     uint64_t n_voxels_gt10, n_voxels_gt50;
     double max_dose_Gy_per_decay;                          /* the largest non-air voxel dose                          */
     uint64_t batches_per_launch;                           /* G of the last run (anm_options.batches_per_launch)      */
+    uint64_t n_fly_trips, n_compton_tries, n_rayleigh_tries; /* event trips of the event pool (collect_stats; 0 with schedule 1):
+                                                              FLY events (each evaluates up to two Woodcock sub-steps from one
+                                                              Philox block), Klein-Nishina tries and form-factor tries (one
+                                                              block each; n_compton / n_rayleigh count the accepted ones)   */
     uint64_t texel_bits;                                   /* 16 | 32: the texels the last run read (anm_options.texel_bits) */
     uint64_t n_check_violations;                           /* library built with -DANM_BOUNDS_CHECK: indices the transport
                                                               kernels found out of range (counted, not trapped); 0 in a

@@ -68,6 +68,7 @@ class anm_stats(C.Structure):
         ("tally_binned", C.c_uint64), ("n_tally_overflow", C.c_uint64),
         ("rms_rel_sigma_gt10", C.c_double), ("rms_rel_sigma_gt50", C.c_double), ("n_voxels_gt10", C.c_uint64),
         ("n_voxels_gt50", C.c_uint64), ("max_dose_Gy_per_decay", C.c_double), ("batches_per_launch", C.c_uint64),
+        ("n_fly_trips", C.c_uint64), ("n_compton_tries", C.c_uint64), ("n_rayleigh_tries", C.c_uint64),
         ("texel_bits", C.c_uint64), ("n_check_violations", C.c_uint64)]
 
     def as_dict(self):

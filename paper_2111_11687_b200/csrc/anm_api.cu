@@ -26,6 +26,7 @@ using namespace anm;
 namespace {
 
 constexpr double kGyPerMeVPerGram = 1.602176634e-10;
+constexpr uint64_t kBatchBudget = 4ull << 30;   // bytes of per-batch tallies in flight (anm_options.batches_per_launch = 0)
 constexpr int kAutoSchedule = 2;   // anm_options.schedule = 0: the warp event pool (1.4x schedule 1 on cfg3, profiles/)
 
 // Device buffers come from the device's default stream-ordered memory pool (its release threshold is raised in
@@ -96,6 +97,7 @@ struct anm_ctx {
     bool tex16_ok = false;
     DevBuf<float> batch, sum, sumsq, scratch;   // batch: [pipeline depth][batches per launch][Vpad] per-batch tallies
     bool batch_clean = false;             // `batch` holds zeros (the folds of a completed run leave it so)
+    cudaEvent_t batch_zero_ev = nullptr;  // the memset of anm_set_grid (internal stream) has completed
     cudaStream_t pipe[3] = {nullptr, nullptr, nullptr};   // internal streams of the pipeline, created on first use
     DevBuf<float> e_ring;                 // waiting electrons of the event pool (electron_transport)
     DevBuf<float> hbh_sq;                 // [Vpad] sum over histories of X_h^2 (anm_options.uncertainty = 1)
@@ -434,6 +436,7 @@ int anm_destroy(anm_ctx* c) {
     c->d_pec.release(true); c->d_flags.release(true); c->d_erange.release(true); c->e_ring.release(true); c->hbh_sq.release(true); c->hbh_list.release(true);
     c->bin_cnt.release(true); c->bin_seg.release(true); c->bin_seg0.release(true); c->bin_rec.release(true); c->bin_ovf.release(true);
     for (auto& ps : c->pipe) if (ps) { cudaStreamDestroy(ps); ps = nullptr; }
+    if (c->batch_zero_ev) cudaEventDestroy(c->batch_zero_ev);
     delete c;
     return ANM_OK;
 }
@@ -470,7 +473,17 @@ int anm_set_grid(anm_ctx* c, int nx, int ny, int nz, double dx_mm, double dy_mm,
     ANM_CUDA(c, c->sum.alloc(c->Vpad));
     ANM_CUDA(c, c->sumsq.alloc(c->Vpad));
     ANM_CUDA(c, cudaMemsetAsync(c->texels.p, 0, c->Vpad * 4, c->stream));
-    c->batch.release(); c->batch_clean = false;     // sized by anm_run (batch groups)
+    {   // per-batch tallies of the launches in flight (anm_options.batches_per_launch): the auto size -- 2 sets of as many
+        // volumes as fit kBatchBudget -- is allocated here and zeroed on an internal stream, so that the memset overlaps
+        // the uploads that follow; anm_run re-sizes it only when the options ask for more
+        const size_t g_auto = std::max<size_t>(1, std::min<size_t>(kMaxGroup, kBatchBudget / (c->Vpad * 4 * 2)));
+        ANM_CUDA(c, c->batch.alloc(2 * g_auto * c->Vpad));
+        if (!c->pipe[0]) ANM_CUDA(c, cudaStreamCreateWithFlags(&c->pipe[0], cudaStreamNonBlocking));
+        if (!c->batch_zero_ev) ANM_CUDA(c, cudaEventCreateWithFlags(&c->batch_zero_ev, cudaEventDisableTiming));
+        ANM_CUDA(c, cudaMemsetAsync(c->batch.p, 0, c->batch.n * 4, c->pipe[0]));
+        ANM_CUDA(c, cudaEventRecord(c->batch_zero_ev, c->pipe[0]));
+        c->batch_clean = true;
+    }
     ANM_CUDA(c, c->d_flags.alloc(2 + ANM_MAX_MATERIALS + 6 + ANM_MAX_MATERIALS));
     ANM_CUDA(c, c->dstats.alloc(1));
     ANM_CUDA(c, c->total_energy.alloc(6));
@@ -1152,8 +1165,7 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
         uint64_t gmax = std::min<uint64_t>({(uint64_t)B, (uint64_t)kMaxGroup, std::max<uint64_t>(1, hist_cap / nb)});
         if (c->opt.batches_per_launch > 0) gmax = std::min<uint64_t>(gmax, (uint64_t)c->opt.batches_per_launch);
         else {
-            const uint64_t budget = 4ull << 30;                        // bytes of batch tallies in flight (auto)
-            gmax = std::min<uint64_t>(gmax, std::max<uint64_t>(1, budget / ((uint64_t)c->Vpad * 4 * 2)));
+            gmax = std::min<uint64_t>(gmax, std::max<uint64_t>(1, kBatchBudget / ((uint64_t)c->Vpad * 4 * 2)));      // auto
         }
         const int n_groups0 = (int)(((uint64_t)B + gmax - 1) / gmax);
         G = (B + n_groups0 - 1) / n_groups0;                           // even groups
@@ -1166,8 +1178,11 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     // reuses the tallies of group g after their folds (same stream).
     const int depth = std::max(1, std::min(c->opt.batch_pipeline == 0 ? (G > 1 ? 2 : 3) : c->opt.batch_pipeline, n_groups));
     const size_t set_floats = (size_t)G * c->Vpad;
-    if (c->batch.n != (size_t)depth * set_floats) c->batch_clean = false;
-    ANM_CUDA(c, c->batch.alloc((size_t)depth * set_floats));
+    if (c->batch.n < (size_t)depth * set_floats) {                     // more than anm_set_grid's auto size
+        c->batch_clean = false;
+        ANM_CUDA(c, c->batch.alloc((size_t)depth * set_floats));
+    }
+    if (c->batch_zero_ev) ANM_CUDA(c, cudaStreamWaitEvent(st, c->batch_zero_ev, 0));
     if (!c->batch_clean) ANM_CUDA(c, cudaMemsetAsync(c->batch.p, 0, (size_t)depth * set_floats * 4, st));   // the folds leave them zero
     c->batch_clean = false;                                            // until this run's folds have completed
     ANM_CUDA(c, c->counters.alloc((size_t)n_groups));
@@ -1215,6 +1230,7 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
         ANM_CUDA_EV(cudaFuncSetAttribute(bin_fold_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kTileVoxels * 4)));
         p.bin_seg = c->bin_seg.p;
     }
+    uint64_t n_fold_launches = 0;
     ANM_CUDA_EV(cudaEventRecord(ev[0], st));
     if (depth > 1) for (int k = 0; k < depth; ++k) ANM_CUDA_EV(cudaStreamWaitEvent(c->pipe[k], ev[0], 0));
     for (int g = 0; g < n_groups; ++g) {
@@ -1257,9 +1273,22 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
         }
         if (depth > 1 && g > 0) ANM_CUDA_EV(cudaStreamWaitEvent(sb, ev[1 + (g - 1)], 0));    // after the previous group's folds
         if (depth == 1) ANM_CUDA_EV(cudaEventRecord(ev[n_groups + 3 + g], sb));
-        for (int j = 0; j < nbg; ++j) {
+        // the folds of the group: one fused pass over its tallies (fold_group_kernel), in sub-groups whose per-batch
+        // organ bins fit 48 KB of shared memory; the tile-binned tally and single-batch launches fold batch by batch
+        const int fuse = (!BIN && nbg > 1) ? std::max(1, std::min(nbg, (int)(49152 / ((size_t)(c->n_organs + 1) * 8)))) : 1;
+        for (int j = 0; fuse > 1 && j < nbg; j += fuse) {
+            const int gj = std::min(fuse, nbg - j);
+            fold_group_kernel<<<fold_blocks, kFoldThreads, (size_t)gj * (c->n_organs + 1) * 8, sb>>>(
+                (float4*)(p.batch + (size_t)j * c->Vpad), c->Vpad / 4, gj, (float4*)c->sum.p, (float4*)c->sumsq.p,
+                c->have_organs ? (const uint32_t*)c->labels.p : nullptr, (const uint4*)c->texels.p,
+                c->organ_batch.p + (size_t)(b0 + j) * 256, c->n_organs, c->Vpad / 4, inv_vox);
+            ANM_CUDA_EV(cudaGetLastError());
+            n_fold_launches += 1;
+        }
+        for (int j = 0; fuse == 1 && j < nbg; ++j) {
             const int b = b0 + j;
             float* tally = p.batch + (size_t)j * c->Vpad;
+            n_fold_launches += 1;
             if (BIN) {
                 // batch 0 counted against empty segments; its fold must see them empty too (the table is already final)
                 bin_fold_kernel<<<std::min<unsigned>(n_tiles, (unsigned)c->num_sms * 3u), kBinFoldThreads, kTileVoxels * 4, sb>>>(
@@ -1320,6 +1349,7 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     s.n_steps = ds.n_steps; s.n_real = ds.n_real; s.n_pe = ds.n_pe; s.n_compton = ds.n_compton;
     s.n_rayleigh = ds.n_rayleigh; s.n_escaped = ds.n_escaped; s.n_cutoff = ds.n_cutoff; s.n_electrons = ds.n_electrons;
     s.n_hbh_overflow = ds.n_hbh_overflow;
+    s.n_fly_trips = ds.n_fly_trips; s.n_compton_tries = ds.n_compton_tries; s.n_rayleigh_tries = ds.n_rayleigh_tries;
     s.n_check_violations = 0;
     for (int k = 0; k < 12; ++k) {
         s.n_check_violations += ds.n_violations[k];
@@ -1327,7 +1357,7 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     }
     s.ms_transport = ms_t; s.ms_fold = ms_f; s.ms_finalize = ms_fin; s.ms_setup = c->ms_setup;
     s.ms_load_ct = c->ms_load_ct; s.ms_load_pet = c->ms_load_pet;
-    s.n_launches = (uint64_t)n_groups + B + 1;
+    s.n_launches = (uint64_t)n_groups + n_fold_launches + 1;
     s.batches_per_launch = (uint64_t)G;
     s.texel_bits = T16 ? 16 : 32;
     s.tally_binned = BIN ? 1 : 0;

@@ -59,6 +59,7 @@ enum : int { ST_NEED = 0, ST_SOURCE = 1, ST_FLY = 2, ST_COMPTON = 3, ST_RAYLEIGH
 struct DeviceStats {   // accumulated with atomics at kernel exit (collect_stats only)
     double escaped_MeV;
     unsigned long long n_steps, n_real, n_pe, n_compton, n_rayleigh, n_escaped, n_cutoff, n_electrons, n_hbh_overflow;
+    unsigned long long n_fly_trips, n_compton_tries, n_rayleigh_tries;   // event trips (event pool): FLY events, Klein-Nishina / form-factor tries
     unsigned long long n_violations[12];   // ANM_BOUNDS_CHECK builds: indices found out of range, per check (counted, never trapped)
 };
 
@@ -624,23 +625,52 @@ constexpr unsigned kHbhShift = 26;          // the list length lives in bits 26-
 constexpr unsigned kHbhHistMask = (1u << kHbhShift) - 1u;   // so a launch may hold at most 2^26 histories in this mode
 
 // hl = the slot's history word in shared memory: history index of the launch | list length << 26
+// The first kHbhReg entries of the list are fetched by independent loads (one exposed latency instead of a chain of
+// dependent ones) and merged per voxel in registers; a longer list (rare: a decay leaves ~7 deposits) folds its tail
+// into them where the voxel matches and handles what is left entry by entry.
+constexpr int kHbhReg = 12;
 __device__ __forceinline__ void hbh_flush(const TransportParams& p, float* __restrict__ tally, unsigned gslot, unsigned& hl) {
     const uint2* L = p.hbh_list + gslot;
     const unsigned n = hl >> kHbhShift;
-    for (unsigned i = 0; i < n; ++i) {
-        const uint2 a = L[(size_t)i * p.hbh_nslots];
-        bool seen = false;
-        for (unsigned j = 0; j < i; ++j) seen = seen || (L[(size_t)j * p.hbh_nslots].x == a.x);
-        if (seen) continue;
-        float X = __uint_as_float(a.y);
-        for (unsigned j = i + 1; j < n; ++j) {
-            const uint2 b = L[(size_t)j * p.hbh_nslots];
-            if (b.x == a.x) X += __uint_as_float(b.y);
-        }
-        atomicAdd(tally + a.x, X);
-        atomicAdd(p.hbh_sq + a.x, X * X);
-    }
     hl &= kHbhHistMask;
+    if (n == 0u) return;
+    constexpr unsigned kNone = 0xffffffffu;
+    unsigned vx[kHbhReg];
+    float ex[kHbhReg];
+#pragma unroll
+    for (int k = 0; k < kHbhReg; ++k) {
+        const uint2 a = (unsigned)k < n ? L[(size_t)k * p.hbh_nslots] : make_uint2(kNone, 0u);
+        vx[k] = a.x; ex[k] = __uint_as_float(a.y);
+    }
+    // tail (n > kHbhReg): add an entry to the register entry of the same voxel, else merge it with the later tail entries
+    // of its voxel here (an earlier tail entry of the same voxel has already taken it: skip)
+    for (unsigned j = kHbhReg; j < n; ++j) {
+        const uint2 b = L[(size_t)j * p.hbh_nslots];
+        bool taken = false;
+#pragma unroll
+        for (int k = 0; k < kHbhReg; ++k)
+            if (!taken && vx[k] == b.x) { ex[k] += __uint_as_float(b.y); taken = true; }
+        for (unsigned i = kHbhReg; i < j && !taken; ++i) taken = (L[(size_t)i * p.hbh_nslots].x == b.x);
+        if (taken) continue;
+        float X = __uint_as_float(b.y);
+        for (unsigned i = j + 1; i < n; ++i) {
+            const uint2 c = L[(size_t)i * p.hbh_nslots];
+            if (c.x == b.x) X += __uint_as_float(c.y);
+        }
+        atomicAdd(tally + b.x, X);
+        atomicAdd(p.hbh_sq + b.x, X * X);
+    }
+    // register entries: every later entry of the same voxel is added to the first one and retired
+#pragma unroll
+    for (int k = 0; k < kHbhReg; ++k) {
+        if (vx[k] == kNone) continue;
+        float X = ex[k];
+#pragma unroll
+        for (int m = k + 1; m < kHbhReg; ++m)
+            if (vx[m] == vx[k]) { X += ex[m]; vx[m] = kNone; }
+        atomicAdd(tally + vx[k], X);
+        atomicAdd(p.hbh_sq + vx[k], X * X);
+    }
 }
 
 __device__ __forceinline__ void hbh_push(const TransportParams& p, float* __restrict__ tally, unsigned gslot, unsigned& hl, unsigned vox, float e, unsigned& overflow) {
@@ -729,7 +759,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
     const float t_max = (float)(p.ne - 1) - 1.0f / 1024.0f;
 
     float esc = 0.0f;
-    unsigned c_pe = 0, c_co = 0, c_ra = 0, c_esc = 0, c_cut = 0, c_el = 0, c_ovf = 0;
+    unsigned c_pe = 0, c_co = 0, c_ra = 0, c_esc = 0, c_cut = 0, c_el = 0, c_ovf = 0, c_fly = 0, c_ctry = 0, c_rtry = 0;
     FlyCounters fc = {0u, 0u};
     const unsigned gslot0 = (blockIdx.x * (unsigned)kPoolWarps + (threadIdx.x >> 5)) * (unsigned)kSlots;   // HBH: this warp's lists
 
@@ -857,6 +887,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                 unsigned vox = 0, hb = (meta >> 1) & 3u;
                 int mat = 0;
                 const int code = fly_two<STATS, T16>(p, s_tot, s_pec, x, y, z, u, v, w, ie, fe, maj, inv_maj, majo, inv_majo, r, hb, vox, mat, fc);
+                if (STATS) ++c_fly;
                 ANM_TR("S2 h=%llu ph=%u blk=%u FLY code=%d t=%d+%.9g pos=%.9g %.9g %.9g vox=%u hb=%u\n", h, ph, meta >> 16, code, ie, fe, x, y, z, vox, hb);
                 Bk[F_X * kSlots] = x; Bk[F_Y * kSlots] = y; Bk[F_Z * kSlots] = z;
                 // next event and slot header, branch-free: GO -> FLY; COMPTON / RAYLEIGH -> their queues, the voxel in
@@ -893,6 +924,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                 float* Bk = S + ph * (kBankFields * kSlots);
                 float E = Bk[F_E * kSlots];
                 float eps, t;
+                if (STATS) ++c_ctry;
                 if (compton_try(E, r, eps, t)) {
                     if (STATS) ++c_co;
                     const unsigned vox = reinterpret_cast<unsigned*>(Bk)[F_TV * kSlots];
@@ -973,6 +1005,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                 float* Bk = S + ph * (kBankFields * kSlots);
                 const float E = Bk[F_E * kSlots];
                 float c;
+                if (STATS) ++c_rtry;
                 if (rayleigh_try(E, r, s_x2, s_cum + ((meta >> 4) & 7u) * p.n_x2, p.n_x2, c)) {
                     if (STATS) ++c_ra;
                     float u = Bk[F_U * kSlots], v = Bk[F_V * kSlots], w = Bk[F_W * kSlots];
@@ -1011,6 +1044,9 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
             c_cut += __shfl_xor_sync(0xffffffffu, c_cut, o);
             c_el += __shfl_xor_sync(0xffffffffu, c_el, o);
             c_ovf += __shfl_xor_sync(0xffffffffu, c_ovf, o);
+            c_fly += __shfl_xor_sync(0xffffffffu, c_fly, o);
+            c_ctry += __shfl_xor_sync(0xffffffffu, c_ctry, o);
+            c_rtry += __shfl_xor_sync(0xffffffffu, c_rtry, o);
         }
         if (lane == 0) {
             atomicAdd(&p.stats->escaped_MeV, (double)esc);
@@ -1023,6 +1059,9 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
             atomicAdd(&p.stats->n_cutoff, (unsigned long long)c_cut);
             atomicAdd(&p.stats->n_electrons, (unsigned long long)c_el);
             atomicAdd(&p.stats->n_hbh_overflow, (unsigned long long)c_ovf);
+            atomicAdd(&p.stats->n_fly_trips, (unsigned long long)c_fly);
+            atomicAdd(&p.stats->n_compton_tries, (unsigned long long)c_ctry);
+            atomicAdd(&p.stats->n_rayleigh_tries, (unsigned long long)c_rtry);
         }
     }
 }
@@ -1084,6 +1123,85 @@ fold_kernel(float4* __restrict__ batch, float4* __restrict__ sum, float4* __rest
         __syncthreads();
         if ((int)threadIdx.x <= n_organs && threadIdx.x > 0 && s_org[threadIdx.x] != 0.0)
             atomicAdd(organ_row + threadIdx.x, s_org[threadIdx.x]);
+    }
+}
+
+// A10 for a batch group (anm_options.batches_per_launch): the G per-batch tallies of one launch folded in ONE pass.
+// A thread takes a group of four voxels and reads it from all G tallies (independent loads, kFoldMlp in flight), adds
+// what it finds to register accumulators, zeroes the touched words, and updates sum / sumsq once -- per touched voxel the
+// run sums are read and written once per GROUP instead of once per batch, and the untouched (air) part of the volume is
+// streamed with G loads in flight per thread.  Organ partials stay per batch: s_org[j][label], rows row0 + j.
+// The same arithmetic per batch as fold_kernel (x, x^2 in fp32; x / (rho V) in fp32, summed in fp64); the G values of a
+// voxel are summed before they are added to the run sum (fp32, <= 256 terms of the same sign).
+constexpr int kFoldMlp = 8;
+__global__ void __launch_bounds__(kFoldThreads)
+fold_group_kernel(float4* __restrict__ batch, size_t stride4, int G, float4* __restrict__ sum, float4* __restrict__ sumsq,
+                  const uint32_t* __restrict__ labels4, const uint4* __restrict__ texels4, double* __restrict__ organ_rows,
+                  int n_organs, size_t n4, float inv_vox_cm3) {
+    extern __shared__ double s_orgs[];                 // [G][n_organs + 1]
+    const bool organs = (labels4 != nullptr);
+    const int n1 = n_organs + 1;
+    if (organs) { for (int k = threadIdx.x; k < G * n1; k += kFoldThreads) s_orgs[k] = 0.0; __syncthreads(); }
+    for (size_t i = (size_t)blockIdx.x * kFoldThreads + threadIdx.x; i < n4; i += (size_t)gridDim.x * kFoldThreads) {
+        float4 s = make_float4(0.f, 0.f, 0.f, 0.f), q = s;
+        bool any = false;
+        uint32_t l4 = 0;
+        float w[4] = {1.f, 1.f, 1.f, 1.f};             // densities of the four voxels, loaded when first needed
+        for (int j0 = 0; j0 < G; j0 += kFoldMlp) {
+            float4 xv[kFoldMlp];
+#pragma unroll
+            for (int k = 0; k < kFoldMlp; ++k) xv[k] = j0 + k < G ? batch[(size_t)(j0 + k) * stride4 + i] : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+            for (int k = 0; k < kFoldMlp; ++k) {
+                const float4 x = xv[k];
+                if (x.x == 0.0f && x.y == 0.0f && x.z == 0.0f && x.w == 0.0f) continue;
+                batch[(size_t)(j0 + k) * stride4 + i] = make_float4(0.f, 0.f, 0.f, 0.f);
+                s.x += x.x; s.y += x.y; s.z += x.z; s.w += x.w;
+                q.x = fmaf(x.x, x.x, q.x); q.y = fmaf(x.y, x.y, q.y); q.z = fmaf(x.z, x.z, q.z); q.w = fmaf(x.w, x.w, q.w);
+                if (organs) {
+                    if (!any) {
+                        l4 = labels4[i];
+                        if (l4) {
+                            const uint4 t = texels4[i];
+                            const unsigned ts[4] = {t.x, t.y, t.z, t.w};
+#pragma unroll
+                            for (int v = 0; v < 4; ++v) w[v] = (float)(ts[v] & 0xffffffu) * kDensityStep;
+                        }
+                    }
+                    if (l4) {
+                        double* so = s_orgs + (size_t)(j0 + k) * n1;
+                        const float xs[4] = {x.x, x.y, x.z, x.w};
+                        const unsigned l0 = l4 & 0xffu;
+                        if (l4 == l0 * 0x01010101u) {
+                            double acc = 0.0;
+#pragma unroll
+                            for (int v = 0; v < 4; ++v) if (xs[v] != 0.0f) acc += (double)__fdividef(xs[v] * inv_vox_cm3, w[v]);
+                            if (acc != 0.0) atomicAdd(&so[l0], acc);
+                        } else {
+#pragma unroll
+                            for (int v = 0; v < 4; ++v) {
+                                const unsigned l = (l4 >> (8 * v)) & 0xffu;
+                                if (l && xs[v] != 0.0f) atomicAdd(&so[l], (double)__fdividef(xs[v] * inv_vox_cm3, w[v]));
+                            }
+                        }
+                    }
+                }
+                any = true;
+            }
+        }
+        if (any) {
+            float4 S = sum[i], Q = sumsq[i];
+            S.x += s.x; S.y += s.y; S.z += s.z; S.w += s.w;
+            Q.x += q.x; Q.y += q.y; Q.z += q.z; Q.w += q.w;
+            sum[i] = S; sumsq[i] = Q;
+        }
+    }
+    if (organs) {
+        __syncthreads();
+        for (int k = threadIdx.x; k < G * n1; k += kFoldThreads) {
+            const int j = k / n1, l = k - j * n1;
+            if (l > 0 && s_orgs[k] != 0.0) atomicAdd(organ_rows + (size_t)j * 256 + l, s_orgs[k]);
+        }
     }
 }
 

@@ -12,7 +12,8 @@ from dataclasses import dataclass
 # every additive field of anm_stats (tests/test_multi_gpu_host.py checks that no uint64 counter of the struct is left out;
 # n_decays is set by anm_merge from the logical run, tally_binned is a flag)
 STAT_SUM_KEYS = ("escaped_MeV", "n_steps", "n_real", "n_pe", "n_compton", "n_rayleigh", "n_escaped", "n_cutoff", "n_launches",
-                 "n_electrons", "n_hbh_overflow", "n_tally_overflow")
+                 "n_electrons", "n_hbh_overflow", "n_tally_overflow", "n_fly_trips", "n_compton_tries", "n_rayleigh_tries",
+                 "n_check_violations")
 STAT_MAX_KEYS = ("ms_transport", "ms_fold", "ms_finalize", "ms_setup")
 
 

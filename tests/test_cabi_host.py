@@ -38,7 +38,7 @@ def test_struct_sizes_match_header():
     assert C.sizeof(binding.anm_options) == 16 + 16 + 16 + 8 + 8 + 8 + 8
     assert C.sizeof(binding.anm_electron_tables) == 8 + 16 + 8
     assert C.sizeof(binding.anm_organ) == 5 * 8 + 2 * 8
-    assert C.sizeof(binding.anm_stats) == 3 * 8 + 10 * 8 + 4 * 8 + 8 + 2 * 8 + 2 * 8 + 8 * 8
+    assert C.sizeof(binding.anm_stats) == 3 * 8 + 10 * 8 + 4 * 8 + 8 + 2 * 8 + 2 * 8 + 11 * 8
     assert C.sizeof(binding.anm_hu_ramp) == 8 + 16 * 8 + 16 * 8 + 16 * 4 + 8
 
 

@@ -307,7 +307,7 @@ def test_batch_groups_keep_every_batch_apart(anm, tables, case):
             s_, q_, rows = sim.get_tally_buffers()
             out[G] = (st, sim.get_energy().astype(np.float64), q_.cpu().numpy().astype(np.float64), rows.cpu().numpy().copy())
     assert out[1][0]["batches_per_launch"] == 1 and out[7][0]["batches_per_launch"] == 6 and out[0][0]["batches_per_launch"] == B
-    assert out[1][0]["n_launches"] == 2 * B + 3 and out[0][0]["n_launches"] == 1 + B + 3       # (even groups: 24 = 4 x 6)
+    assert out[1][0]["n_launches"] == 2 * B + 3 and out[0][0]["n_launches"] == 1 + 1 + 3       # one launch, one fused fold, finalize x 3
     ref = out[1]
     for G in (7, 0):
         st, e, q, rows = out[G]

@@ -93,3 +93,20 @@ def test_merge_tallies_checks_row_count():
     from paper_2111_11687_b200.multi_gpu import merge_tallies
     with pytest.raises(ValueError):
         merge_tallies(torch.zeros(4), torch.zeros(4), torch.zeros(3, 256), Shard(0, 0, 2, 0, 20), 4)
+
+
+def test_every_counter_of_anm_stats_is_merged():
+    """merge_stats must sum every additive uint64 counter of anm_stats over the ranks (a counter left out would report
+    one rank's value beside globally summed ones); the few that are not additive are named here."""
+    import ctypes as C
+    from paper_2111_11687_b200 import binding
+    from paper_2111_11687_b200.multi_gpu import STAT_MAX_KEYS, STAT_SUM_KEYS
+    not_additive = {"n_decays",                    # set by anm_merge from the logical run
+                    "tally_binned", "batches_per_launch", "texel_bits",      # how the run was made, the same on every rank
+                    "n_voxels_gt10", "n_voxels_gt50"}                        # recomputed by anm_merge on the merged volumes
+    fields = dict(binding.anm_stats._fields_)
+    for name, typ in fields.items():
+        if typ is C.c_uint64:
+            assert name in STAT_SUM_KEYS or name in not_additive, name
+    assert set(STAT_SUM_KEYS) <= set(fields) and set(STAT_MAX_KEYS) <= set(fields)
+    assert not (set(STAT_SUM_KEYS) & not_additive)
