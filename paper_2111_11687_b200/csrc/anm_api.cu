@@ -686,9 +686,11 @@ static int resample_blocks(const anm_ctx* c) {
     return (int)std::max<size_t>(1, std::min<size_t>((size_t)c->ny * c->nz, (size_t)c->num_sms * 16));
 }
 
-static int upload_overlap_tables(anm_ctx* c, const ResampleParams& p, DevBuf<AxisOverlap>& tab) {
+// kx_max (if not null) = the largest number of source voxels a destination voxel overlaps along x
+static int upload_overlap_tables(anm_ctx* c, const ResampleParams& p, DevBuf<AxisOverlap>& tab, int* kx_max = nullptr) {
     std::vector<AxisOverlap> h((size_t)p.nx + p.ny + p.nz);
     axis_overlap_table(h.data(), p.nx, p.dx, p.snx, p.sdx, p.ox);
+    if (kx_max) { *kx_max = 0; for (int i = 0; i < p.nx; ++i) *kx_max = std::max(*kx_max, h[(size_t)i].j1 - h[(size_t)i].j0 + 1); }
     axis_overlap_table(h.data() + p.nx, p.ny, p.dy, p.sny, p.sdy, p.oy);
     axis_overlap_table(h.data() + p.nx + p.ny, p.nz, p.dz, p.snz, p.sdz, p.oz);
     ANM_CUDA(c, tab.alloc(h.size()));
@@ -734,10 +736,17 @@ int anm_load_ct(anm_ctx* c, const int16_t* hu, int cnx, int cny, int cnz, double
     ANM_CUDA(c, cudaMemsetAsync(c->d_flags.p, 0, (2 + ANM_MAX_MATERIALS + 6 + ANM_MAX_MATERIALS) * 4, c->stream));
     const ResampleParams p = resample_params(c, cnx, cny, cnz, cdx_mm, cdy_mm, cdz_mm, ox_mm, oy_mm, oz_mm, ramp->hu_outside, 1.0);
     DevBuf<AxisOverlap> tab;
-    { const int rc = upload_overlap_tables(c, p, tab); if (rc != ANM_OK) { stage.release(); tab.release(); return rc; } }
+    int kx = 0;
+    { const int rc = upload_overlap_tables(c, p, tab, &kx); if (rc != ANM_OK) { stage.release(); tab.release(); return rc; } }
     ANM_CUDA(c, cudaEventRecord(e0, c->stream));
-    resample_kernel<int16_t, RS_CT><<<resample_blocks(c), kResampleThreads, 0, c->stream>>>(
-        d_src, tab.p, p, rp, c->texels.p, nullptr, nullptr, nullptr, c->d_flags.p, c->d_flags.p + 1);
+    // resample_fast_kernel where a destination voxel overlaps <= 4 source voxels along x and the image indexes in 32 bits
+    const bool fast = n_src < 0x7fffffffull && kx <= 4;
+#define ANM_RS_ARGS d_src, tab.p, p, rp, c->texels.p, nullptr, nullptr, nullptr, c->d_flags.p, c->d_flags.p + 1
+    if (fast && kx <= 2) resample_fast_kernel<int16_t, RS_CT, 2><<<resample_blocks(c), kResampleThreads, 0, c->stream>>>(ANM_RS_ARGS);
+    else if (fast && kx == 3) resample_fast_kernel<int16_t, RS_CT, 3><<<resample_blocks(c), kResampleThreads, 0, c->stream>>>(ANM_RS_ARGS);
+    else if (fast) resample_fast_kernel<int16_t, RS_CT, 4><<<resample_blocks(c), kResampleThreads, 0, c->stream>>>(ANM_RS_ARGS);
+    else resample_kernel<int16_t, RS_CT><<<resample_blocks(c), kResampleThreads, 0, c->stream>>>(ANM_RS_ARGS);
+#undef ANM_RS_ARGS
     ANM_CUDA(c, cudaGetLastError());
     ANM_CUDA(c, cudaEventRecord(e1, c->stream));
     unsigned flags[2] = {0, 0};
@@ -813,10 +822,16 @@ int anm_load_pet(anm_ctx* c, const float* bq_per_ml, int pnx, int pny, int pnz, 
         pet_same_grid_kernel<<<grid_blocks(c, c->V / 4 + 1, kResampleThreads), kResampleThreads, 0, c->stream>>>(
             d_src, vox_ml, c->scratch.p, d_copy, c->V, d_total.p, c->d_flags.p);
     } else {
-        { const int rc = upload_overlap_tables(c, p, tab); if (rc != ANM_OK) { stage.release(); tab.release(); d_total.release(); return rc; } }
+        int kx = 0;
+        { const int rc = upload_overlap_tables(c, p, tab, &kx); if (rc != ANM_OK) { stage.release(); tab.release(); d_total.release(); return rc; } }
         cudaEventRecord(e0, c->stream);
-        resample_kernel<float, RS_PET><<<resample_blocks(c), kResampleThreads, 0, c->stream>>>(
-            d_src, tab.p, p, rp, nullptr, c->scratch.p, d_copy, d_total.p, c->d_flags.p, c->d_flags.p + 1);
+        const bool fast = (unsigned long long)pnx * pny * pnz < 0x7fffffffull && kx <= 4;
+#define ANM_RS_ARGS d_src, tab.p, p, rp, nullptr, c->scratch.p, d_copy, d_total.p, c->d_flags.p, c->d_flags.p + 1
+        if (fast && kx <= 2) resample_fast_kernel<float, RS_PET, 2><<<resample_blocks(c), kResampleThreads, 0, c->stream>>>(ANM_RS_ARGS);
+        else if (fast && kx == 3) resample_fast_kernel<float, RS_PET, 3><<<resample_blocks(c), kResampleThreads, 0, c->stream>>>(ANM_RS_ARGS);
+        else if (fast) resample_fast_kernel<float, RS_PET, 4><<<resample_blocks(c), kResampleThreads, 0, c->stream>>>(ANM_RS_ARGS);
+        else resample_kernel<float, RS_PET><<<resample_blocks(c), kResampleThreads, 0, c->stream>>>(ANM_RS_ARGS);
+#undef ANM_RS_ARGS
     }
     ANM_CUDA(c, cudaGetLastError());
     cudaEventRecord(e1, c->stream);
