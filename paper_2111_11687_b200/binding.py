@@ -109,7 +109,9 @@ class anm_hu_ramp(C.Structure):
 
 
 def lib_path() -> str:
-    return os.path.join(_PKG, "libanm.so")
+    """The library to load: paper_2111_11687_b200/libanm.so, or the build named by ANM_LIBRARY (e.g. the bounds-checking
+    build of tests/test_gpu_bounds_check.py)."""
+    return os.environ.get("ANM_LIBRARY") or os.path.join(_PKG, "libanm.so")
 
 
 _lib = None

@@ -28,7 +28,12 @@ def needs_build() -> bool:
     return any(os.path.getmtime(d) > t for d in DEPENDS)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, out: str | None = None, extra: list | None = None) -> str:
+    """Builds libanm.so in-tree; or, with `out`, a variant (e.g. extra = ["-DANM_BOUNDS_CHECK"]) into another file."""
+    if out is not None:
+        cmd = [nvcc()] + NVCC_FLAGS + list(extra or []) + ["-o", out] + SOURCES
+        subprocess.check_call(cmd)
+        return out
     if force or needs_build():
         tmp = LIB + ".tmp.%d" % os.getpid()
         extra = os.environ.get("ANM_NVCC_EXTRA", "").split()      # e.g. -DANM_POOL_THREADS=768 -DANM_CHUNK=64 (tuning experiments)
