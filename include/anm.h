@@ -133,7 +133,7 @@ typedef struct {
                                    launch (its last decays draining, ~0.25 ms) is paid n_batches / G times instead of
                                    n_batches times.  0 auto: as many as keep the tallies in flight within 4 GiB (at most
                                    256, and below 2^32 histories per launch); 1..256: at most that many.  Always 1 with
-                                   schedule 1, electron_transport or tally = 2.  Same histories, same per-batch tallies.
+                                   schedule 1 or tally = 2.  Same histories, same per-batch tallies.
                                    The ctx then owns pipeline depth x G tally volumes (anm_stats.batches_per_launch = G). */
     int32_t texel_bits;         /* width of the (material, density) texel the Woodcock flight reads at random: 32 =
                                    material<<24 | density / 2^-20 g/cm^3 (every phantom); 16 = material<<13 | density / 2^-12,

@@ -1171,11 +1171,10 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     // folds follow the launch.  A launch is one resident wave of persistent CTAs whose tail (the last decays draining,
     // queues below 32 entries in every warp at the same time) costs ~0.25 ms whatever its size; with G batches per launch
     // that cost is paid B / G times instead of B times.  Same histories, same per-batch tallies.
-    // G = 1 for the history-based schedule, electron transport and the tile-binned tally (their per-launch scratch is
-    // per batch); else the largest group that keeps depth * G tally volumes within the memory budget, at most 256
+    // G = 1 for the history-based schedule and the tile-binned tally (its per-launch lists are per batch); else the largest group that keeps depth * G tally volumes within the memory budget, at most 256
     // (8 bits of the meta word), G * nb < 2^32 histories per launch (2^26 with history-by-history scoring).
     int G = 1;
-    if (schedule == 2 && !EL && !BIN) {
+    if (schedule == 2 && !BIN) {
         const uint64_t hist_cap = HB ? (uint64_t)kHbhHistMask : 0xffffffffull;
         uint64_t gmax = std::min<uint64_t>({(uint64_t)B, (uint64_t)kMaxGroup, std::max<uint64_t>(1, hist_cap / nb)});
         if (c->opt.batches_per_launch > 0) gmax = std::min<uint64_t>(gmax, (uint64_t)c->opt.batches_per_launch);
@@ -1208,7 +1207,7 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     const uint64_t per_block = schedule == 2 ? (uint64_t)kPoolWarps * kSlots : (uint64_t)kThreads;
     const int blocks = (int)std::max<uint64_t>(1, std::min<uint64_t>((uint64_t)c->num_sms * per_sm, (nb * (uint64_t)G + per_block - 1) / per_block));
     if (EL) {   // per-warp arrays of electrons waiting for their walk, one per launch in flight
-        ANM_CUDA(c, c->e_ring.alloc((size_t)depth * blocks * kPoolWarps * 8 * kPend));
+        ANM_CUDA(c, c->e_ring.alloc((size_t)depth * blocks * kPoolWarps * kEFields * kPend));
         p.e_ring = c->e_ring.p;
     }
     if (HB) {   // history-by-history scoring: sum of X_h^2 over the whole run + one deposit list per decay slot
@@ -1259,7 +1258,7 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
             p.bin_cnt = c->bin_cnt.p + (size_t)set * n_lists;
             p.bin_rec = c->bin_rec.p ? c->bin_rec.p + (size_t)set * bin_total : nullptr;
         }
-        if (EL) p.e_ring = c->e_ring.p + (size_t)set * blocks * kPoolWarps * 8 * kPend;
+        if (EL) p.e_ring = c->e_ring.p + (size_t)set * blocks * kPoolWarps * kEFields * kPend;
         if (HB) p.hbh_list = c->hbh_list.p + (size_t)set * kHbhCap * p.hbh_nslots;
         p.counter = c->counters.p + g;
         p.hist_base = c->opt.history_offset + (unsigned long long)b0 * nb;

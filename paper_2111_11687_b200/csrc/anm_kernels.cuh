@@ -115,7 +115,7 @@ struct TransportParams {
     // the electron cutoff, [nm][n_t] g/cm^2 on the kinetic-energy grid t_min + k dt; t_min = the cutoff
     const float* e_range;
     int n_t, e_nm;               // e_nm materials in the electron tables
-    float* e_ring;               // [warps of the launch][8][kPend] electrons waiting for their walk (event pool)
+    float* e_ring;               // [warps of the launch][kEFields][kPend] electrons waiting for their walk (event pool)
     float t_min, e_dt, e_inv_dt;
     // history-by-history scoring (anm_options.uncertainty = 1, Walters et al. 2002): per decay slot a
     // list of the decay's deposits {voxel, energy} in global scratch, hbh_list[i * hbh_nslots + slot] (its length in the
@@ -446,9 +446,10 @@ __device__ __forceinline__ float electron_walk_to(const TransportParams& p, cons
     }
 }
 
-__device__ __forceinline__ float electron_walk(const TransportParams& p, const float* __restrict__ er, float x, float y, float z,
-                                            float ex, float ey, float ez, unsigned vox, float T) {
-    return electron_walk_to(p, er, x, y, z, ex, ey, ez, vox, T, [&](unsigned v, float e) { atomicAdd(p.batch + v, e); });
+// `tally`: the energy volume of the batch the electron's decay belongs to
+__device__ __forceinline__ float electron_walk(const TransportParams& p, float* __restrict__ tally, const float* __restrict__ er, float x, float y,
+                                            float z, float ex, float ey, float ez, unsigned vox, float T) {
+    return electron_walk_to(p, er, x, y, z, ex, ey, ez, vox, T, [&](unsigned v, float e) { atomicAdd(tally + v, e); });
 }
 
 // inspection / parity hook (anm_trace_electrons): one given electron per thread, in = {x, y, z (cm), ex, ey, ez, T}
@@ -460,7 +461,7 @@ __global__ void electron_trace_kernel(const __grid_constant__ TransportParams p,
     const float x = e[0], y = e[1], z = e[2];
     const int ix = __float2int_rd(x * p.inv_dx), iy = __float2int_rd(y * p.inv_dy), iz = __float2int_rd(z * p.inv_dz);
     const unsigned vox = (unsigned)ix + (unsigned)p.nx * ((unsigned)iy + (unsigned)p.ny * (unsigned)iz);
-    const float out = electron_walk(p, p.e_range, x, y, z, e[3], e[4], e[5], vox, e[6]);
+    const float out = electron_walk(p, p.batch, p.e_range, x, y, z, e[3], e[4], e[5], vox, e[6]);
     if (out > 0.0f) atomicAdd(escaped, (double)out);
 }
 
@@ -701,6 +702,7 @@ constexpr int kPoolWarps = kPoolThreads / 32;
 constexpr int kPoolMinBlocksPerSM = ANM_POOL_MIN_BLOCKS;
 constexpr int kSlots = 64;                  // per warp (a power of two: the queues are rings)
 constexpr unsigned kPend = 64;              // capacity of a warp's array of waiting electrons (ELEC)
+constexpr unsigned kEFields = 9;            // x, y, z, ex, ey, ez, T, voxel, local batch of the decay
 #ifndef ANM_RAYBATCH
 #define ANM_RAYBATCH 8
 #endif
@@ -782,10 +784,10 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
     // walked 32 at a time by all lanes -- inside the COMPTON event only the quarter of the lanes whose recoil electron
     // exceeds the cutoff would walk while the others wait.  pend < 32 between trips, so an event adds at most 32 more.
     unsigned pend = 0;                      // warp-uniform
-    float* ering = ELEC ? p.e_ring + (size_t)(gslot0 / (unsigned)kSlots) * (8u * kPend) : nullptr;
+    float* ering = ELEC ? p.e_ring + (size_t)(gslot0 / (unsigned)kSlots) * (kEFields * kPend) : nullptr;
     bool e_want = false;
     float e_x = 0, e_y = 0, e_z = 0, e_ex = 0, e_ey = 0, e_ez = 1, e_T = 0;
-    unsigned e_vox = 0;
+    unsigned e_vox = 0, e_bl = 0;
     auto e_append = [&]() {                 // all 32 lanes call it
         const unsigned b = __ballot_sync(0xffffffffu, e_want);
         if (b) {
@@ -794,7 +796,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                 float* E = ering + pend + __popc(b & lanemask_lt);
                 E[0 * kPend] = e_x; E[1 * kPend] = e_y; E[2 * kPend] = e_z;
                 E[3 * kPend] = e_ex; E[4 * kPend] = e_ey; E[5 * kPend] = e_ez;
-                E[6 * kPend] = e_T; E[7 * kPend] = __uint_as_float(e_vox);
+                E[6 * kPend] = e_T; E[7 * kPend] = __uint_as_float(e_vox); E[8 * kPend] = __uint_as_float(e_bl);
             }
             pend += __popc(b);
             e_want = false;
@@ -807,8 +809,9 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
             pend -= n;
             if (lane < n) {
                 const float* E = ering + pend + lane;
-                const float out = electron_walk(p, s_er, E[0 * kPend], E[1 * kPend], E[2 * kPend], E[3 * kPend], E[4 * kPend],
-                                                E[5 * kPend], __float_as_uint(E[7 * kPend]), E[6 * kPend]);
+                const float out = electron_walk(p, p.batch + (size_t)__float_as_uint(E[8 * kPend]) * p.batch_stride, s_er, E[0 * kPend],
+                                                E[1 * kPend], E[2 * kPend], E[3 * kPend], E[4 * kPend], E[5 * kPend],
+                                                __float_as_uint(E[7 * kPend]), E[6 * kPend]);
                 if (STATS) { esc += out; ++c_el; }
             }
             __syncwarp();
@@ -907,7 +910,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                     if (ELEC && Epe > p.t_min) {          // rare (0.002 per decay): walked on the spot, not queued
                         const float out = HBH ? electron_walk_to(p, s_er, x, y, z, u, v, w, vox, Epe, [&](unsigned vv, float ee) {
                                                     hbh_push(p, tally_of(meta), gslot0 + slot, SU[F_HL * kSlots], vv, ee, c_ovf); })
-                                              : electron_walk(p, s_er, x, y, z, u, v, w, vox, Epe);
+                                              : electron_walk(p, tally_of(meta), s_er, x, y, z, u, v, w, vox, Epe);
                         if (STATS) { esc += out; ++c_el; }
                     } else if (HBH) hbh_push(p, tally_of(meta), gslot0 + slot, SU[F_HL * kSlots], vox, Epe, c_ovf);
                     else deposit<TALLY>(p, tally_of(meta), vox, Epe);
@@ -948,7 +951,7 @@ transport_pool_kernel(const __grid_constant__ TransportParams p) {
                                 if (STATS) { esc += out; ++c_el; }
                             } else {
                                 e_want = true; e_x = Bk[F_X * kSlots]; e_y = Bk[F_Y * kSlots]; e_z = Bk[F_Z * kSlots];
-                                e_ex = ex; e_ey = ey; e_ez = ez; e_T = dep; e_vox = vox;
+                                e_ex = ex; e_ey = ey; e_ez = ez; e_T = dep; e_vox = vox; e_bl = (meta >> 8) & 0xffu;
                             }
                             dep = 0.0f;
                         }

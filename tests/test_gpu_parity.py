@@ -284,24 +284,27 @@ def test_schedules_and_hull_run_the_same_histories(anm, tables, k, scale, n, B):
     assert np.allclose(hs[0]["energy"], hs[1]["energy"], rtol=1e-4, atol=1e-3)
 
 
-@pytest.mark.parametrize("case", ["patient", "point_wagg", "hbh"])
+@pytest.mark.parametrize("case", ["patient", "point_wagg", "hbh", "electrons"])
 def test_batch_groups_keep_every_batch_apart(anm, tables, case):
     """anm_options.batches_per_launch: one launch covers G batches, every deposit tagged with its decay's batch.  The
     histories and the per-batch tallies must not depend on G: the per-batch organ rows (a sum over the batch's own
     tally), the energy map, the batch sum of squares and every counter agree between G = 1 (one launch per batch) and
     grouped launches -- also with a ragged last group, with the warp-aggregated atomics of a point source (lanes of
-    DIFFERENT batches hit the same voxel in one trip) and with the history-by-history deposit lists."""
+    DIFFERENT batches hit the same voxel in one trip), with the history-by-history deposit lists and with transported
+    electrons (the waiting-electron arrays carry each electron's batch)."""
     n, B = 240_000, 24
     if case == "point_wagg":
         cfg = dict(anm_inputs.make_config(0, 2), positron_ke_mev=0.2498)
         kw = dict(warp_aggregate=1)
     else:
         cfg = anm_inputs.make_config(3, 4)
-        kw = dict(uncertainty=1) if case == "hbh" else {}
+        kw = dict(uncertainty=1) if case == "hbh" else (dict(electron_transport=1) if case == "electrons" else {})
     out = {}
     for G in (1, 7, 0):
         with anm.Simulation(0) as sim:
             sim.load_config(cfg, tables, n_batches=B, collect_stats=1, batches_per_launch=G, **kw)
+            if case == "electrons":
+                sim.set_electron_tables(anm_inputs.make_electron_tables())
             sim.run(n, 11)
             st = sim.get_stats()
             s_, q_, rows = sim.get_tally_buffers()
@@ -311,7 +314,7 @@ def test_batch_groups_keep_every_batch_apart(anm, tables, case):
     ref = out[1]
     for G in (7, 0):
         st, e, q, rows = out[G]
-        for key in ("n_steps", "n_real", "n_pe", "n_compton", "n_rayleigh", "n_escaped", "n_cutoff"):
+        for key in ("n_steps", "n_real", "n_pe", "n_compton", "n_rayleigh", "n_escaped", "n_cutoff", "n_electrons"):
             assert st[key] == ref[0][key], (G, key)
         assert np.allclose(e, ref[1], rtol=2e-5, atol=1e-4)                  # fp32 atomic order only
         assert np.allclose(q, ref[2], rtol=1e-4, atol=1e-3)
