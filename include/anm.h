@@ -107,7 +107,13 @@ typedef struct {
                                       s^2 of the mean = (sum X_h^2 / N - (sum X_h / N)^2) / (N - 1).  anm_get_uncertainty
                                       and the organs' Eq. 3 value then use it; the organ sigma_mean stays the batch
                                       one.  Schedule 0 or 2.  With electron_transport the
-                                      electrons are walked inside the events (their deposits belong to the decay). */
+                                      electrons are walked inside the events (their deposits belong to the decay).
+                                      Limits of this mode: at most 2^26 decays per launch (ANM_E_UNSUPPORTED beyond); a
+                                      decay with more than 63 deposits is merged early (anm_stats.n_hbh_overflow); the sum
+                                      of X_h^2 is ONE fp32 volume accumulated over the whole run, so a voxel that receives
+                                      more than ~1e7 similar contributions (a point source with positron energy at 1e8
+                                      decays; not a patient activity map) stops resolving further ones and reports
+                                      sigma = 0 there -- use the batch method for such sources.                       */
     int32_t batch_pipeline;     /* launch pipeline over batches: 0 auto (3), 1 serial (one launch at a time on the ctx
                                    stream; per-launch ms_transport / ms_fold), 2 | 3: that many batch tallies and
                                    internal streams, so that the CTAs of batch b+1 take over the SMs as those of batch
