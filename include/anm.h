@@ -233,6 +233,11 @@ const char* anm_last_error(const anm_ctx* c);
 int anm_set_stream(anm_ctx* c, void* cuda_stream); /* cudaStream_t; NULL = the default stream          */
 
 /* --- inputs (any order; set_grid first) -------------------------------------------------------- */
+/* Sets the voxel grid (origin = grid corner, linear index = ix + nx*(iy + ny*iz)) and allocates the ctx's volumes: texels,
+ * the run sums, and the per-batch energy tallies of the launches in flight -- two sets of as many volumes of nx*ny*nz
+ * floats as fit 4 GiB (at least one per set, at most 256; anm_options.batches_per_launch), zeroed on an internal stream
+ * while the caller goes on loading inputs.  Drops the phantom, the activity map and the organ labels of a previous
+ * grid; a point source is kept only if it still lies inside the new extents.  ANM_E_ARG, ANM_E_NOMEM. */
 int anm_set_grid(anm_ctx* c, int nx, int ny, int nz, double dx_mm, double dy_mm, double dz_mm);
 /* material[V] < n_materials (checked at run), density[V] in [0, 16) g/cm^3, stored on a 2^-20 grid. */
 int anm_load_phantom(anm_ctx* c, const uint8_t* material, const float* density_g_cm3, int on_device);

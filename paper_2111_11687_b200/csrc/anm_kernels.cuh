@@ -1130,14 +1130,14 @@ fold_kernel(float4* __restrict__ batch, float4* __restrict__ sum, float4* __rest
 }
 
 // A10 for a batch group (anm_options.batches_per_launch): the G per-batch tallies of one launch folded in ONE pass.
-// A thread takes a group of four voxels and reads it from all G tallies (independent loads, kFoldMlp in flight), adds
+// A thread takes a group of four voxels and reads it from all G tallies (independent loads, kFoldMlp at a time), adds
 // what it finds to register accumulators, zeroes the touched words, and updates sum / sumsq once -- per touched voxel the
 // run sums are read and written once per GROUP instead of once per batch, and the untouched (air) part of the volume is
 // streamed with G loads in flight per thread.  Organ partials stay per batch: s_org[j][label], rows row0 + j.
 // The same arithmetic per batch as fold_kernel (x, x^2 in fp32; x / (rho V) in fp32, summed in fp64); the G values of a
 // voxel are summed before they are added to the run sum (fp32, <= 256 terms of the same sign).
-constexpr int kFoldMlp = 8;
-__global__ void __launch_bounds__(kFoldThreads)
+constexpr int kFoldMlp = 4;                 // measured: 4 loads in flight at 4 CTAs per SM (64 registers) beat 8 at 3 CTAs (79 registers) by 24 %
+__global__ void __launch_bounds__(kFoldThreads, 4)
 fold_group_kernel(float4* __restrict__ batch, size_t stride4, int G, float4* __restrict__ sum, float4* __restrict__ sumsq,
                   const uint32_t* __restrict__ labels4, const uint4* __restrict__ texels4, double* __restrict__ organ_rows,
                   int n_organs, size_t n4, float inv_vox_cm3) {
