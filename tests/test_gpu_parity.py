@@ -322,6 +322,51 @@ def test_batch_groups_keep_every_batch_apart(anm, tables, case):
     assert np.count_nonzero(ref[3].sum(1)) == B
 
 
+def test_one_context_many_runs_with_changing_options(anm, tables):
+    """The ctx keeps its per-batch tallies between runs (the folds leave them zero) and re-sizes them only when a run
+    needs more: a sequence of runs with different kernels, group sizes, pipelines and a grid change in ONE context must
+    give what a fresh context gives for each of them -- counters equal, energy map equal up to fp32 atomic order."""
+    cfg = anm_inputs.make_config(3, 8)
+    et = anm_inputs.make_electron_tables()
+    n, B = 60_000, 12
+    base = dict(n_batches=B, photons_per_decay=2, rayleigh_on=1, positron_ke_MeV=cfg["positron_ke_mev"], collect_stats=1)
+    seq = [dict(), dict(batches_per_launch=1), dict(uncertainty=1), dict(electron_transport=1), dict(tally=2), dict(schedule=1),
+           dict(batches_per_launch=5, batch_pipeline=1), dict(electron_transport=1, uncertainty=1), dict(warp_aggregate=1), dict()]
+
+    def one(sim, kw):
+        sim.set_options(**dict(base, **kw))
+        sim.run(n, 9)
+        return sim.get_stats(), sim.get_energy().astype(np.float64), sim.get_uncertainty().astype(np.float64)
+
+    with anm.Simulation(0) as reused:
+        reused.load_config(cfg, tables, **base)
+        reused.set_electron_tables(et)
+        for i, kw in enumerate(seq):
+            st_r, e_r, u_r = one(reused, kw)
+            with anm.Simulation(0) as fresh:
+                fresh.load_config(cfg, tables, **base)
+                fresh.set_electron_tables(et)
+                st_f, e_f, u_f = one(fresh, kw)
+            for key in ("n_steps", "n_real", "n_pe", "n_compton", "n_rayleigh", "n_escaped", "n_cutoff", "n_electrons"):
+                assert st_r[key] == st_f[key], (i, kw, key)
+            assert np.allclose(e_r, e_f, rtol=2e-5, atol=1e-4), (i, kw)
+            assert np.allclose(u_r, u_f, rtol=1e-3, atol=1e-4), (i, kw)
+            if i == 4:      # in between: a run that is refused (N not a multiple of B) must leave the ctx usable
+                with pytest.raises(anm.AnmError):
+                    reused.run(n + 1, 9)
+        # a grid change re-allocates the tallies; the same phantom again afterwards
+        small = anm_inputs.make_config(0, 4)
+        reused.load_config(small, tables, n_batches=10, collect_stats=1)
+        reused.run(20_000, 1)
+        assert reused.get_energy().sum() > 0
+        reused.load_config(cfg, tables, **base)
+        st_r, e_r, _ = one(reused, {})
+        with anm.Simulation(0) as fresh:
+            fresh.load_config(cfg, tables, **base)
+            st_f, e_f, _ = one(fresh, {})
+        assert st_r["n_compton"] == st_f["n_compton"] and np.allclose(e_r, e_f, rtol=2e-5, atol=1e-4)
+
+
 def test_16_bit_texels_are_the_same_phantom(anm, tables):
     """anm_options.texel_bits (reading C18): the Woodcock flight reads a 16-bit copy of the texels only when it
     holds exactly the values of the 32-bit one (cfg4's generator puts every density on the 2^-12 grid), so the histories
