@@ -360,6 +360,46 @@ int anm_measure_peaks(anm_ctx* c, uint64_t small_bytes, uint64_t large_bytes, an
 int anm_get_tally_buffers(anm_ctx* c, float** d_sum, float** d_sumsq, size_t* n_floats, double** d_organ_rows, int* n_rows);
 int anm_merge(anm_ctx* c, uint64_t total_decays, int total_batches, const double* organ_rows_all, const anm_stats* summed);
 
+/* --- per-organ summary without any allocation by the library (csrc/anm_static.cu) ----------------------------------
+ * For callers that cannot let this library allocate device memory: a process whose own allocator already owns the
+ * whole HBM (a PyTorch job whose caching allocator holds the card, a server working out of one fixed arena), where a
+ * cudaMalloc behind its back fails or eats into the arena; and a host thread on a deadline, which must stay away
+ * from cudaMalloc / cudaFree because they take driver locks and can wait for the device.  Every other call of this
+ * header needs an anm_ctx, and a ctx allocates.  This one needs none: it takes tally volumes the caller already holds
+ * on the device (its own, or the ones anm_get_tally_buffers returns) and computes, per organ label, what A11's
+ * finalize pass computes (Eq. 3), with the same arithmetic:
+ *
+ *   d_out[3 o + 0]  RMS over the organ's voxels with energy of the voxel's relative sigma
+ *                   sqrt((n_samples Q / S^2 - 1) / (n_samples - 1)),  S = d_sum[v], Q = d_sumsq[v]     (o = 1..n_organs)
+ *   d_out[3 o + 1]  how many of the organ's voxels hold energy (S != 0), as a double
+ *   d_out[3 o + 2]  the organ's energy, sum of S (MeV)
+ *   d_out[0], d_out[1] = 0;  d_out[2] = sum of S over ALL n_voxels voxels (the total deposited energy)
+ *
+ * d_sum, d_sumsq: DEVICE, n_voxels fp32 each.  d_labels: DEVICE, n_voxels uint8, 0 = no organ, labels above
+ * n_organs are ignored; may be NULL when n_organs = 0 (then only d_out[2] is of interest).  d_out: DEVICE, caller-
+ * owned, 3 (n_organs + 1) fp64, overwritten.  n_samples: the batches behind the sums (or the histories, for history-
+ * by-history sums), >= 2.  All pointers belong to the CURRENT device (cudaSetDevice is the caller's business); the
+ * work is queued on cuda_stream (a cudaStream_t, NULL = default stream) and the call returns without waiting.
+ *
+ * Where the accumulators live: in an array that is part of the library image, 3 (ANM_STATIC_MAX_ORGANS + 1) fp64
+ * = 6144 bytes, present on every GPU that loads libanm.so until the process ends.  n_organs above
+ * ANM_STATIC_MAX_ORGANS is refused with ANM_E_ARG and a message saying so.  The call makes no cudaMalloc / cudaFree
+ * and uses no routine that allocates.  The first call on a device looks up where that device keeps the array
+ * (cudaGetSymbolAddress; the driver may load the module at that point): make that first call during start-up, not
+ * on the deadline path, and before any stream capture begins.  Later calls only queue a memset and two kernels.
+ * There is ONE such array per device and every call uses it: it is cleared at the start of each call, so results
+ * never carry over, but two calls whose GPU work can overlap (different streams without an ordering between them,
+ * or two host threads on the same device) race on it and both results are garbage.  Keep calls on one stream, or
+ * order them with events.
+ *
+ * errbuf (may be NULL) receives the message of a failed call, at most errbuf_len bytes with the terminator -- there
+ * is no ctx to keep it.  ANM_E_ARG: NULL pointer, n_voxels = 0, n_samples < 2, n_organs out of range;
+ * ANM_E_UNSUPPORTED: device ordinal >= 64;  ANM_E_CUDA: the runtime refused a step. */
+#define ANM_STATIC_MAX_ORGANS 255
+int anm_organ_summary_static(const float* d_sum, const float* d_sumsq, const uint8_t* d_labels, size_t n_voxels,
+                             int n_organs, double n_samples, double* d_out, void* cuda_stream,
+                             char* errbuf, size_t errbuf_len);
+
 #ifdef __cplusplus
 }
 #endif

@@ -2,4 +2,4 @@
 (the hot path of ARCHER-NM, arxiv 2111.11687).  The product is libanm.so (include/anm.h, csrc/);
 this package is its thin Python binding.  There is no CPU fallback: `load()` raises if the CUDA
 library is missing or no GPU is usable."""
-from .binding import Simulation, AnmError, load, lib_path, ANM_SYMBOLS  # noqa: F401
+from .binding import Simulation, AnmError, load, lib_path, ANM_SYMBOLS, organ_summary_static  # noqa: F401

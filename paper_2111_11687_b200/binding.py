@@ -22,6 +22,7 @@ ANM_SYMBOLS = [
     "anm_get_organ_doses", "anm_get_stats", "anm_get_tally_buffers", "anm_merge", "anm_get_alias_table",
     "anm_default_hu_ramp", "anm_load_ct", "anm_get_phantom", "anm_load_pet",
     "anm_set_electron_tables", "anm_trace_electrons", "anm_philox_blocks", "anm_measure_peaks",
+    "anm_organ_summary_static",
 ]
 
 STATUS = {0: "ANM_OK", -1: "ANM_E_ARG", -2: "ANM_E_STATE", -3: "ANM_E_CUDA", -4: "ANM_E_NOMEM", -5: "ANM_E_UNSUPPORTED"}
@@ -153,12 +154,41 @@ def load(build_if_missing: bool = True):
         "anm_load_ct": (i32, [vp, vp, i32, i32, i32, dbl, dbl, dbl, dbl, dbl, dbl, C.POINTER(anm_hu_ramp), i32]),
         "anm_get_phantom": (i32, [vp, vp, vp, sz, i32]),
         "anm_load_pet": (i32, [vp, vp, i32, i32, i32, dbl, dbl, dbl, dbl, dbl, dbl, i32, C.POINTER(dbl), vp, sz]),
+        "anm_organ_summary_static": (i32, [vp, vp, vp, sz, i32, dbl, vp, vp, C.c_char_p, sz]),
     }
     for name, (res, args) in protos.items():
         f = getattr(L, name)
         f.restype, f.argtypes = res, args
     _lib = L
     return L
+
+
+def organ_summary_static(d_sum, d_sumsq, d_labels, n_organs: int, n_samples: float, d_out, stream=None, n_voxels=None):
+    """anm_organ_summary_static (include/anm.h): the per-organ summary for callers that cannot let the library allocate
+    device memory (their own allocator owns the card, or they are on a thread that must not call cudaMalloc).  No
+    anm_ctx, no allocation: every argument is a CUDA torch tensor the caller already owns -- d_sum / d_sumsq float32,
+    d_labels uint8 (None with n_organs = 0), d_out float64 with 3 * (n_organs + 1) elements, overwritten with
+    {RMS relative sigma, voxels with energy, energy in MeV} per label (row 0: total energy in its third word).  The
+    work is queued on `stream` (torch stream, raw handle or None); all calls on a device share one built-in scratch
+    array, so keep them ordered on the GPU.  Marshalling only: this wrapper creates no tensor."""
+    L = load()
+    for t in (d_sum, d_sumsq, d_out) + ((d_labels,) if d_labels is not None else ()):
+        if not (_is_torch(t) and t.is_cuda and t.is_contiguous()):
+            raise ValueError("organ_summary_static takes contiguous CUDA tensors")
+    if d_sum.dtype.itemsize != 4 or d_sumsq.dtype.itemsize != 4 or d_out.dtype.itemsize != 8 or (d_labels is not None and d_labels.dtype.itemsize != 1):
+        raise ValueError("organ_summary_static: float32 sums, uint8 labels, float64 out")
+    n = int(n_voxels) if n_voxels is not None else int(d_sum.numel())
+    if d_sumsq.numel() < n or d_sum.numel() < n or (d_labels is not None and d_labels.numel() < n):
+        raise ValueError("organ_summary_static: a volume is shorter than n_voxels")
+    if 0 <= int(n_organs) <= 255 and d_out.numel() < 3 * (int(n_organs) + 1):
+        raise ValueError("organ_summary_static: d_out needs 3 * (n_organs + 1) float64")
+    h = getattr(stream, "cuda_stream", stream)
+    err = C.create_string_buffer(512)
+    rc = L.anm_organ_summary_static(C.c_void_p(d_sum.data_ptr()), C.c_void_p(d_sumsq.data_ptr()),
+                                    C.c_void_p(d_labels.data_ptr()) if d_labels is not None else None, n, int(n_organs),
+                                    float(n_samples), C.c_void_p(d_out.data_ptr()), C.c_void_p(int(h) if h else None), err, len(err))
+    if rc != 0:
+        raise AnmError(rc, err.value.decode())
 
 
 def _is_torch(a) -> bool:

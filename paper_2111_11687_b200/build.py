@@ -8,7 +8,7 @@ import sys
 PKG = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libanm.so")
-SOURCES = [os.path.join(CSRC, "anm_api.cu")]
+SOURCES = [os.path.join(CSRC, "anm_api.cu"), os.path.join(CSRC, "anm_static.cu")]
 DEPENDS = SOURCES + [os.path.join(CSRC, "anm_kernels.cuh"), os.path.join(CSRC, "anm_alias.cuh"), os.path.join(CSRC, "anm_frontend.cuh"), os.path.join(CSRC, "anm_peaks.cuh"), os.path.join(os.path.dirname(PKG), "include", "anm.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-fmad=false", "-ftz=true", "-prec-div=false", "-prec-sqrt=false",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
