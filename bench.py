@@ -265,13 +265,16 @@ def main():
         peak_source = ("anm_measure_peaks: %.1f Gthread-instr/s at %.0f MHz (power-limited) = %.3f of the issue slots per clock, "
                        "x 148 SM x 128 lanes x %.0f MHz held during the timed region" % (peaks_dev["issue_gtis"], peaks_dev["issue_sm_mhz"], slots_per_clk, sm_run))
         g_peak, r_peak = peaks_dev["gather_gps"][1 if big else 0], peaks_dev["red_gps"][1 if big else 0]
+        m_peak = peaks_dev["mix_gps"][1 if big else 0]
     else:
+        m_peak = None
         peak, peak_source = nominal, "nominal 148 SM x 4 SMSP x 32 lanes x %.0f MHz (clocks.max.sm); --no-peaks" % sm_max
         g_peak = r_peak = None
     g_ach = per_decay["n_steps"] * decays_per_s_kernel / 1e9
     r_ach = deposits * decays_per_s_kernel / 1e9
     h_ach = alg_bytes * decays_per_s_kernel / 1e9
     traffic, traffic_source = None, None   # dram__bytes_read.sum + dram__bytes_write.sum per launch, from the committed ncu capture
+    instr_executed, instr_executed_source = None, None   # thread-instructions the kernel EXECUTES per decay, same capture
     tdir = os.path.join(ROOT, "profiles")
     for name in sorted(os.listdir(tdir) if os.path.isdir(tdir) else [], reverse=True):
         if name.endswith("_transport_traffic.csv"):
@@ -280,18 +283,34 @@ def main():
             if rows and int(rows[-1]["decays_per_launch"]) == D // n_groups and args.config == 3:
                 traffic = int(rows[-1]["dram_bytes_read"]) + int(rows[-1]["dram_bytes_write"])
                 traffic_source = "profiles/%s (ncu --set full capture of this kernel and launch size; not measured in this run)" % name
+                if rows[-1].get("warp_instr_executed") and rows[-1].get("lanes_per_warp_instr"):
+                    # smsp__inst_executed.sum x smsp__thread_inst_executed_per_inst_executed.ratio / decays of the launch
+                    instr_executed = float(rows[-1]["warp_instr_executed"]) * float(rows[-1]["lanes_per_warp_instr"]) / float(rows[-1]["decays_per_launch"])
+                    instr_executed_source = "profiles/%s (same capture; goes stale with the next kernel edit until re-captured)" % name
             break
     roofline = {"bound": "alu", "kernel": "transport_pool_kernel", "achieved": achieved, "peak": peak, "unit": "Gthread-instr/s",
                 "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_source, "peak_source": peak_source,
                 "alu": {"achieved": achieved, "peak": peak, "frac": achieved / peak, "unit": "Gthread-instr/s",
-                        "peak_nominal": nominal, "peak_power_limited": peaks_dev["issue_gtis"] if peaks_dev else None},
+                        "numerator": "SASS-issued work: this build's instruction counts of the per-event device functions x the events a "
+                                     "counted run measures (profiles/r2_event_instr.md) -- not a count derived from the method alone, so "
+                                     "compare rounds on decays/s and on instr_per_decay_executed, not on this fraction",
+                        "peak_nominal": nominal, "frac_nominal": achieved / nominal,
+                        "peak_power_limited": peaks_dev["issue_gtis"] if peaks_dev else None},
                 "l2_gather": {"achieved": g_ach, "peak": g_peak, "frac": g_ach / g_peak if g_peak else None, "unit": "G loads/s",
                               "array_bytes": peaks_dev["bytes"][1 if big else 0] if peaks_dev else None},
                 "red": {"achieved": r_ach, "peak": r_peak, "frac": r_ach / r_peak if r_peak else None, "unit": "G atomics/s"},
+                # both streams at once (loads 5 : REDs 2, UNIFORMLY random over two arrays of the volume's size).  A reference
+                # point, not a ceiling: two 105 MB arrays no longer fit the L2 together, whereas the transport's accesses
+                # are concentrated on the body (its hot part does fit), so the kernel can exceed it -- ratio > 1 measures
+                # that locality.  The separate gather / red fractions share the L2 and the HBM and must not be added up.
+                "mem_mix_uniform": {"achieved": g_ach + r_ach, "reference": m_peak, "ratio": (g_ach + r_ach) / m_peak if m_peak else None,
+                                    "unit": "G accesses/s (texel loads + tally REDs)",
+                                    "note": "uniform-random reference over 2 arrays, not a peak: the kernel's accesses have locality"},
                 "hbm": {"achieved": h_ach, "peak": hbm_peak, "frac": h_ach / hbm_peak, "unit": "GB/s",
                         "peak_source": "MEASURED_PEAKS.json hbm_gbs" if file_peaks else "fallback 6500 GB/s"},
                 "peaks_measured": peaks_dev,
-                "instr_per_decay_algorithmic": instr_per_decay, "events_per_decay": per_decay,
+                "instr_per_decay_algorithmic": instr_per_decay, "instr_per_decay_executed": instr_executed,
+                "instr_per_decay_executed_source": instr_executed_source, "events_per_decay": per_decay,
                 "avg_launch_ms": sec_per_launch * 1e3, "batches_per_launch": G, "transport_launches_per_step": n_groups,
                 "decays_per_launch": D // n_groups, "share_of_step": ms_t / max(ms_t + ms_f + ms_fin, 1e-9),
                 "texel_bytes_per_decay": 4.0 * per_decay["n_steps"], "tally_bytes_per_decay": 8.0 * deposits,
@@ -415,6 +434,18 @@ def main():
                       "decays": n4, "ms": ms4, "value": dps4, "unit": "decays/s", "texel_bits": int(st4["texel_bits"]),
                       "batches_per_launch": int(st4["batches_per_launch"]),
                       "events_per_decay": {"n_steps": steps4, "deposits": dep4}}
+                # the same phantom through the 32-bit texels: what a phantom that is NOT on the 2^-12 g/cm^3 density grid
+                # gets -- every phantom loaded from a CT image (anm_load_ct stores densities on the 2^-20 grid), and cfg4
+                # itself before its generator was put on the coarse grid (reading C18)
+                s4.set_options(n_batches=100, positron_ke_MeV=cfg4["positron_ke_mev"], texel_bits=32)
+                s4.run(n4, cfg4["seed"])
+                s4.run(n4, cfg4["seed"])
+                st32 = s4.get_stats()
+                ms32 = st32["ms_transport"] + st32["ms_fold"] + st32["ms_finalize"]
+                v4["texel_bits_32"] = {"decays": n4, "ms": ms32, "value": n4 / (ms32 * 1e-3), "unit": "decays/s",
+                                       "texel_bits": int(st32["texel_bits"]),
+                                       "note": "same phantom, 32-bit texels: the path of any phantom off the 2^-12 density grid (every CT-loaded one)"}
+                s4.set_options(n_batches=100, positron_ke_MeV=cfg4["positron_ke_mev"])
                 if D >= 1_000_000_000:      # the config's own size (BASELINE.json configs[4]: "Run 1e10 decays"), once
                     s4.run(10_000_000_000, cfg4["seed"])
                     st10 = s4.get_stats()
@@ -426,6 +457,7 @@ def main():
                     t_model = steps4 / (peaks_dev["gather_gps"][1] * 1e9) + dep4 / (peaks_dev["red_gps"][1] * 1e9)
                     v4["roofline"] = {"bound": "hbm random access", "gather_frac": steps4 * dps4 / 1e9 / peaks_dev["gather_gps"][1],
                                       "red_frac": dep4 * dps4 / 1e9 / peaks_dev["red_gps"][1],
+                                      "mem_mix_uniform_ratio": (steps4 + dep4) * dps4 / 1e9 / peaks_dev["mix_gps"][1],   # > 1: locality (see roofline.mem_mix_uniform)
                                       "decays_per_s_if_gathers_and_reds_were_serial_at_peak": 1.0 / t_model}
             variants["cfg4_fullres"] = v4
             del cfg4

@@ -91,7 +91,8 @@ typedef struct {
     int32_t warp_aggregate;     /* deposits of the lanes of a warp that hit the same voxel in one trip are merged
                                    (__match_any_sync) into one atomic.  Pays only where deposits pile onto few voxels
                                    (DESIGN.md §5.1 has the measurement): 0 auto = on iff positron energy is deposited and
-                                   the source is a point or fewer than 1024 active voxels; 1 on; 2 off.  Same tallies up
+                                   the source is a point or fewer than 1024 active voxels, and tally is not 2 (the tile-binned
+                                   tally was asked for: it wins over the automatic choice); 1 on; 2 off.  Same tallies up
                                    to fp32 atomic order.  1 with electron_transport or uncertainty = 1: ANM_E_UNSUPPORTED */
     int32_t hull_majorant;      /* 0 auto / 1 on: a photon that has left the bounding box of the dense voxels on a
                                    straight line (it cannot re-enter a convex box) flies against the majorant of
@@ -114,11 +115,12 @@ typedef struct {
                                       more than ~1e7 similar contributions (a point source with positron energy at 1e8
                                       decays; not a patient activity map) stops resolving further ones and reports
                                       sigma = 0 there -- use the batch method for such sources.                       */
-    int32_t batch_pipeline;     /* launch pipeline over batches: 0 auto (3), 1 serial (one launch at a time on the ctx
-                                   stream; per-launch ms_transport / ms_fold), 2 | 3: that many batch tallies and
-                                   internal streams, so that the CTAs of batch b+1 take over the SMs as those of batch
-                                   b drain; the same histories and tallies; then ms_transport covers the whole
-                                   pipeline (folds inside it) and ms_fold is 0.                                    */
+    int32_t batch_pipeline;     /* launch pipeline over batch groups: 0 auto (2 sets of tallies when a launch covers more
+                                   than one batch, see batches_per_launch; 3 when it covers one), 1 serial (one launch at
+                                   a time on the ctx stream; per-launch ms_transport / ms_fold), 2 | 3: that many sets of
+                                   batch tallies and internal streams, so that the CTAs of launch g+1 take over the SMs as
+                                   those of launch g drain; never more than there are launches; the same histories and
+                                   tallies; then ms_transport covers the whole pipeline (folds inside it) and ms_fold is 0. */
     int32_t tally;              /* how deposits reach the per-batch tally: 1 = one fp32 atomic (RED) per
                                    deposit into the batch volume; 2 = tile-binned: a deposit is appended as an 8-byte record
                                    {voxel, energy} to the list of the voxel's tile (2^14 consecutive voxels; position from
@@ -138,7 +140,8 @@ typedef struct {
                                    tally volume (deposits are batch-tagged), followed by their folds -- the fixed cost of a
                                    launch (its last decays draining, ~0.25 ms) is paid n_batches / G times instead of
                                    n_batches times.  0 auto: as many as keep the tallies in flight within 4 GiB (at most
-                                   256, and below 2^32 histories per launch); 1..256: at most that many.  Always 1 with
+                                   256, and at most 0xF0000000 histories per launch, which keeps the launch's 32-bit history counter
+                                   from wrapping); 1..256: at most that many.  Always 1 with
                                    schedule 1 or tally = 2.  Same histories, same per-batch tallies.
                                    The ctx then owns pipeline depth x G tally volumes (anm_stats.batches_per_launch = G). */
     int32_t texel_bits;         /* width of the (material, density) texel the Woodcock flight reads at random: 32 =
@@ -231,12 +234,19 @@ int anm_create(anm_ctx** out, int cuda_device);    /* ANM_E_CUDA if the device c
 int anm_destroy(anm_ctx* c);                       /* frees everything the ctx allocated; NULL is ok   */
 const char* anm_last_error(const anm_ctx* c);
 int anm_set_stream(anm_ctx* c, void* cuda_stream); /* cudaStream_t; NULL = the default stream          */
+/* How many bytes of per-batch energy tallies this ctx may keep in flight (default, and bytes = 0: 4 GiB).  Call it BEFORE
+ * anm_set_grid, which allocates them: several ctxs on one device (one per rank sharing a GPU, one per worker thread)
+ * each pay this amount.  A smaller budget means fewer batches per launch (anm_options.batches_per_launch = 0 follows it;
+ * an explicit batches_per_launch may still ask anm_run for more), never different results; the floor is two volumes of
+ * nx*ny*nz floats.  Takes effect at the next anm_set_grid.  ANM_E_ARG for a NULL ctx. */
+int anm_set_tally_budget(anm_ctx* c, uint64_t bytes);
 
 /* --- inputs (any order; set_grid first) -------------------------------------------------------- */
 /* Sets the voxel grid (origin = grid corner, linear index = ix + nx*(iy + ny*iz)) and allocates the ctx's volumes: texels,
  * the run sums, and the per-batch energy tallies of the launches in flight -- two sets of as many volumes of nx*ny*nz
- * floats as fit 4 GiB (at least one per set, at most 256; anm_options.batches_per_launch), zeroed on an internal stream
- * while the caller goes on loading inputs.  Drops the phantom, the activity map and the organ labels of a previous
+ * floats as fit the tally budget (4 GiB unless anm_set_tally_budget said otherwise; at least one per set, at most 256;
+ * anm_options.batches_per_launch), zeroed on an internal stream while the caller goes on loading inputs.  If the device
+ * cannot give that much the number of volumes per set is halved, down to one, before the call fails with ANM_E_NOMEM.  Drops the phantom, the activity map and the organ labels of a previous
  * grid; a point source is kept only if it still lies inside the new extents.  ANM_E_ARG, ANM_E_NOMEM. */
 int anm_set_grid(anm_ctx* c, int nx, int ny, int nz, double dx_mm, double dy_mm, double dz_mm);
 /* material[V] < n_materials (checked at run), density[V] in [0, 16) g/cm^3, stored on a 2^-20 grid. */
@@ -324,9 +334,16 @@ int anm_trace_electrons(anm_ctx* c, const float* electrons, size_t n, float* out
  *   philox_gblocks  1e9 Philox4x32-10 blocks/s, back to back (the generator the kernels call)
  *   gather_gps[k]   1e9 random 4-byte ld.global.nc per second over an array of bytes[k] (the texel fetch)
  *   red_gps[k]      1e9 random fp32 RED.ADD per second over an array of bytes[k] (the tally)
+ *   mix_gps[k]      1e9 accesses per second of both together, 5 loads : 2 REDs (cfg3's sub-steps : deposits) over TWO arrays
+ *                   of bytes[k], uniformly random: the two streams share the L2 and the HBM, so the separate gather and
+ *                   RED fractions must not be added up.  A reference point rather than a ceiling: the transport kernel's
+ *                   accesses are concentrated on the body, which fits the L2 where two whole volumes do not, and it
+ *                   exceeds this rate (measured 1.36x on cfg3, 1.5x on cfg4)
+ * gather_gps and red_gps are the best of a sweep over 4, 8, 16 and 32 independent accesses in flight per thread at full
+ * occupancy (64 warps per SM); gather_in_flight / red_in_flight say where the best was.
  * k = 0: small_bytes (choose a size that fits the L2, e.g. cfg3's 105 MB volume), k = 1: large_bytes (one that does not,
- * e.g. cfg4's 630 MB).  Sizes are rounded down to a multiple of 4, must be >= 4096 and < 16 GiB.  Scratch memory is
- * allocated for the call and released.  Needs only a ctx.  ANM_E_ARG for bad sizes, ANM_E_NOMEM / ANM_E_CUDA. */
+ * e.g. cfg4's 630 MB).  Sizes are rounded down to a multiple of 4, must be >= 4096 and < 16 GiB.  Scratch memory (two
+ * arrays of the size under test) is allocated for the call and released.  Needs only a ctx.  ANM_E_ARG for bad sizes, ANM_E_NOMEM / ANM_E_CUDA. */
 typedef struct {
     double issue_gtis;
     double issue_sm_mhz;      /* SM clock held during the issue stream (clock64 over the launch / its duration): a pure
@@ -336,6 +353,8 @@ typedef struct {
     double gather_gps[2];
     double red_gps[2];
     uint64_t bytes[2];
+    double mix_gps[2];        /* loads + REDs per second (1e9) with both in flight */
+    int32_t gather_in_flight[2], red_in_flight[2];   /* the depth per thread at which the best rate was seen */
 } anm_peaks;
 int anm_measure_peaks(anm_ctx* c, uint64_t small_bytes, uint64_t large_bytes, anm_peaks* out);
 

@@ -22,7 +22,7 @@ ANM_SYMBOLS = [
     "anm_get_organ_doses", "anm_get_stats", "anm_get_tally_buffers", "anm_merge", "anm_get_alias_table",
     "anm_default_hu_ramp", "anm_load_ct", "anm_get_phantom", "anm_load_pet",
     "anm_set_electron_tables", "anm_trace_electrons", "anm_philox_blocks", "anm_measure_peaks",
-    "anm_organ_summary_static",
+    "anm_organ_summary_static", "anm_set_tally_budget",
 ]
 
 STATUS = {0: "ANM_OK", -1: "ANM_E_ARG", -2: "ANM_E_STATE", -3: "ANM_E_CUDA", -4: "ANM_E_NOMEM", -5: "ANM_E_UNSUPPORTED"}
@@ -78,7 +78,8 @@ class anm_stats(C.Structure):
 
 class anm_peaks(C.Structure):
     _fields_ = [("issue_gtis", C.c_double), ("issue_sm_mhz", C.c_double), ("philox_gblocks", C.c_double), ("gather_gps", C.c_double * 2),
-                ("red_gps", C.c_double * 2), ("bytes", C.c_uint64 * 2)]
+                ("red_gps", C.c_double * 2), ("bytes", C.c_uint64 * 2), ("mix_gps", C.c_double * 2),
+                ("gather_in_flight", C.c_int32 * 2), ("red_in_flight", C.c_int32 * 2)]
 
 
 ANM_MAX_RAMP_NODES = 16
@@ -154,6 +155,7 @@ def load(build_if_missing: bool = True):
         "anm_load_ct": (i32, [vp, vp, i32, i32, i32, dbl, dbl, dbl, dbl, dbl, dbl, C.POINTER(anm_hu_ramp), i32]),
         "anm_get_phantom": (i32, [vp, vp, vp, sz, i32]),
         "anm_load_pet": (i32, [vp, vp, i32, i32, i32, dbl, dbl, dbl, dbl, dbl, dbl, i32, C.POINTER(dbl), vp, sz]),
+        "anm_set_tally_budget": (i32, [vp, u64]),
         "anm_organ_summary_static": (i32, [vp, vp, vp, sz, i32, dbl, vp, vp, C.c_char_p, sz]),
     }
     for name, (res, args) in protos.items():
@@ -255,6 +257,10 @@ class Simulation:
         nx, ny, nz = (int(v) for v in shape)
         self._ck(self._L.anm_set_grid(self._ctx, nx, ny, nz, *(float(s) for s in spacing_mm)))
         self.shape, self.V = (nx, ny, nz), nx * ny * nz
+
+    def set_tally_budget(self, n_bytes: int):
+        """Bytes of per-batch tallies this ctx may keep in flight (default 4 GiB); call before set_grid (anm_set_tally_budget)."""
+        self._ck(self._L.anm_set_tally_budget(self._ctx, int(n_bytes)))
 
     def load_phantom(self, material, density):
         keep = []
@@ -430,7 +436,9 @@ class Simulation:
         self._ck(self._L.anm_measure_peaks(self._ctx, int(small_bytes), int(large_bytes), C.byref(pk)))
         return {"issue_gtis": pk.issue_gtis, "issue_sm_mhz": pk.issue_sm_mhz, "philox_gblocks": pk.philox_gblocks,
                 "gather_gps": [pk.gather_gps[0], pk.gather_gps[1]], "red_gps": [pk.red_gps[0], pk.red_gps[1]],
-                "bytes": [int(pk.bytes[0]), int(pk.bytes[1])]}
+                "bytes": [int(pk.bytes[0]), int(pk.bytes[1])], "mix_gps": [pk.mix_gps[0], pk.mix_gps[1]],
+                "gather_in_flight": [pk.gather_in_flight[0], pk.gather_in_flight[1]],
+                "red_in_flight": [pk.red_in_flight[0], pk.red_in_flight[1]]}
 
     def get_alias_table(self) -> np.ndarray:
         """uint32 [n_entries][4] = {threshold, own voxel, alias voxel, 0} of the loaded activity map."""

@@ -27,6 +27,7 @@ namespace {
 
 constexpr double kGyPerMeVPerGram = 1.602176634e-10;
 constexpr uint64_t kBatchBudget = 4ull << 30;   // bytes of per-batch tallies in flight (anm_options.batches_per_launch = 0)
+constexpr uint64_t kLaunchHistCap = 0xF0000000ull;   // histories one transport launch may cover (anm_options.batches_per_launch)
 constexpr int kAutoSchedule = 2;   // anm_options.schedule = 0: the warp event pool (1.4x schedule 1 on cfg3, profiles/)
 
 // Device buffers come from the device's default stream-ordered memory pool (its release threshold is raised in
@@ -50,6 +51,28 @@ struct DevBuf {
         if (p) { if (!synced) cudaDeviceSynchronize(); cudaFreeAsync(p, (cudaStream_t)0); }
         p = nullptr; n = 0;
     }
+    // a local buffer is given back on every return path, the early error returns included
+    DevBuf() = default;
+    DevBuf(const DevBuf&) = delete;
+    DevBuf& operator=(const DevBuf&) = delete;
+    ~DevBuf() { release(); }
+};
+
+// cudaEvent_t locals that are destroyed on every return path
+template <int N>
+struct Events {
+    cudaEvent_t e[N] = {};
+    Events() = default;
+    Events(const Events&) = delete;
+    Events& operator=(const Events&) = delete;
+    cudaError_t create() {
+        for (auto& x : e) {
+            const cudaError_t r = cudaEventCreate(&x);
+            if (r != cudaSuccess) { x = nullptr; return r; }
+        }
+        return cudaSuccess;
+    }
+    ~Events() { for (auto x : e) if (x) cudaEventDestroy(x); }
 };
 
 }  // namespace
@@ -97,6 +120,8 @@ struct anm_ctx {
     bool tex16_ok = false;
     DevBuf<float> batch, sum, sumsq, scratch;   // batch: [pipeline depth][batches per launch][Vpad] per-batch tallies
     bool batch_clean = false;             // `batch` holds zeros (the folds of a completed run leave it so)
+    uint64_t batch_budget = kBatchBudget; // bytes of per-batch tallies a ctx may hold in flight (anm_set_tally_budget)
+    size_t auto_group = 1;                // batches per launch that anm_set_grid found room for (<= the budget's figure)
     cudaEvent_t batch_zero_ev = nullptr;  // the memset of anm_set_grid (internal stream) has completed
     cudaStream_t pipe[3] = {nullptr, nullptr, nullptr};   // internal streams of the pipeline, created on first use
     DevBuf<float> e_ring;                 // waiting electrons of the event pool (electron_transport)
@@ -449,6 +474,12 @@ int anm_set_stream(anm_ctx* c, void* cuda_stream) {
     return ANM_OK;
 }
 
+int anm_set_tally_budget(anm_ctx* c, uint64_t bytes) {
+    if (!c) return ANM_E_ARG;
+    c->batch_budget = bytes == 0 ? kBatchBudget : bytes;
+    return ANM_OK;
+}
+
 int anm_set_grid(anm_ctx* c, int nx, int ny, int nz, double dx_mm, double dy_mm, double dz_mm) {
     if (!c) return ANM_E_ARG;
     if (nx < 1 || ny < 1 || nz < 1 || !(dx_mm > 0) || !(dy_mm > 0) || !(dz_mm > 0) ||
@@ -476,8 +507,19 @@ int anm_set_grid(anm_ctx* c, int nx, int ny, int nz, double dx_mm, double dy_mm,
     {   // per-batch tallies of the launches in flight (anm_options.batches_per_launch): the auto size -- 2 sets of as many
         // volumes as fit kBatchBudget -- is allocated here and zeroed on an internal stream, so that the memset overlaps
         // the uploads that follow; anm_run re-sizes it only when the options ask for more
-        const size_t g_auto = std::max<size_t>(1, std::min<size_t>(kMaxGroup, kBatchBudget / (c->Vpad * 4 * 2)));
-        ANM_CUDA(c, c->batch.alloc(2 * g_auto * c->Vpad));
+        // If the device cannot give that much, the group is halved down to one volume per set before the call gives up
+        // (ANM_E_NOMEM): a smaller group only costs launch tails, the results are the same.
+        size_t g_auto = std::max<size_t>(1, std::min<size_t>(kMaxGroup, c->batch_budget / (c->Vpad * 4 * 2)));
+        for (;;) {
+            const cudaError_t e = c->batch.alloc(2 * g_auto * c->Vpad);
+            if (e == cudaSuccess) break;
+            cudaGetLastError();
+            if (e != cudaErrorMemoryAllocation || g_auto == 1)
+                return fail(c, e == cudaErrorMemoryAllocation ? ANM_E_NOMEM : ANM_E_CUDA, "grid: per-batch tallies (2 x %zu volumes of %zu bytes): %s",
+                            g_auto, c->Vpad * 4, cudaGetErrorString(e));
+            g_auto = (g_auto + 1) / 2;
+        }
+        c->auto_group = g_auto;
         if (!c->pipe[0]) ANM_CUDA(c, cudaStreamCreateWithFlags(&c->pipe[0], cudaStreamNonBlocking));
         if (!c->batch_zero_ev) ANM_CUDA(c, cudaEventCreateWithFlags(&c->batch_zero_ev, cudaEventDisableTiming));
         ANM_CUDA(c, cudaMemsetAsync(c->batch.p, 0, c->batch.n * 4, c->pipe[0]));
@@ -500,9 +542,9 @@ int anm_load_phantom(anm_ctx* c, const uint8_t* material, const float* density, 
     if (!material || !density) return fail(c, ANM_E_ARG, "phantom: null pointer");
     if (!c->have_grid) return fail(c, ANM_E_STATE, "phantom: set the grid first");
     ANM_CUDA(c, cudaSetDevice(c->device));
-    cudaEvent_t e0, e1;
-    ANM_CUDA(c, cudaEventCreate(&e0));
-    ANM_CUDA(c, cudaEventCreate(&e1));
+    Events<2> evs;
+    ANM_CUDA(c, evs.create());
+    const cudaEvent_t e0 = evs.e[0], e1 = evs.e[1];
     ANM_CUDA(c, cudaEventRecord(e0, c->stream));
     const uint8_t* d_mat = material;
     const float* d_rho = density;
@@ -525,7 +567,6 @@ int anm_load_phantom(anm_ctx* c, const uint8_t* material, const float* density, 
     stage_m.release();
     float ms = 0;
     cudaEventElapsedTime(&ms, e0, e1);
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
     c->ms_setup += ms;
     c->have_phantom = false;
     if (flags[0] & 1u) return fail(c, ANM_E_ARG, "phantom: density must be finite and in [0, 16) g/cm^3");
@@ -601,9 +642,9 @@ int anm_load_activity(anm_ctx* c, const float* activity, int on_device) {
         d_act = c->scratch.p;
     }
     c->have_source = false;
-    cudaEvent_t e0, e1;
-    ANM_CUDA(c, cudaEventCreate(&e0));
-    ANM_CUDA(c, cudaEventCreate(&e1));
+    Events<2> evs;
+    ANM_CUDA(c, evs.create());
+    const cudaEvent_t e0 = evs.e[0], e1 = evs.e[1];
     cudaEventRecord(e0, c->stream);
     int rc;
     try {
@@ -615,7 +656,6 @@ int anm_load_activity(anm_ctx* c, const float* activity, int on_device) {
     cudaEventSynchronize(e1);
     float ms = 0;
     cudaEventElapsedTime(&ms, e0, e1);
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
     c->ms_setup += ms;
     if (rc != ANM_OK) return rc;
     c->point_source = false;
@@ -730,9 +770,9 @@ int anm_load_ct(anm_ctx* c, const int16_t* hu, int cnx, int cny, int cnz, double
         d_src = stage.p;
     }
     c->have_phantom = false;
-    cudaEvent_t e0, e1;
-    ANM_CUDA(c, cudaEventCreate(&e0));
-    ANM_CUDA(c, cudaEventCreate(&e1));
+    Events<2> evs;
+    ANM_CUDA(c, evs.create());
+    const cudaEvent_t e0 = evs.e[0], e1 = evs.e[1];
     ANM_CUDA(c, cudaMemsetAsync(c->d_flags.p, 0, (2 + ANM_MAX_MATERIALS + 6 + ANM_MAX_MATERIALS) * 4, c->stream));
     const ResampleParams p = resample_params(c, cnx, cny, cnz, cdx_mm, cdy_mm, cdz_mm, ox_mm, oy_mm, oz_mm, ramp->hu_outside, 1.0);
     DevBuf<AxisOverlap> tab;
@@ -755,7 +795,6 @@ int anm_load_ct(anm_ctx* c, const int16_t* hu, int cnx, int cny, int cnz, double
     stage.release(); tab.release();
     float ms = 0;
     cudaEventElapsedTime(&ms, e0, e1);
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
     c->ms_setup += ms; c->ms_load_ct = ms;
     c->max_material = flags[1];
     return phantom_setup(c);
@@ -805,10 +844,9 @@ int anm_load_pet(anm_ctx* c, const float* bq_per_ml, int pnx, int pny, int pnz, 
     ANM_CUDA(c, cudaMemsetAsync(d_total.p, 0, 8, c->stream));
     ANM_CUDA(c, cudaMemsetAsync(c->d_flags.p, 0, 8, c->stream));
     c->have_source = false;
-    cudaEvent_t e0, e1, e2;
-    ANM_CUDA(c, cudaEventCreate(&e0));
-    ANM_CUDA(c, cudaEventCreate(&e1));
-    ANM_CUDA(c, cudaEventCreate(&e2));
+    Events<3> evs;
+    ANM_CUDA(c, evs.create());
+    const cudaEvent_t e0 = evs.e[0], e1 = evs.e[1], e2 = evs.e[2];
     const double vox_ml = c->dx * c->dy * c->dz;     // cm^3 = mL
     const ResampleParams p = resample_params(c, pnx, pny, pnz, pdx_mm, pdy_mm, pdz_mm, ox_mm, oy_mm, oz_mm, 0.0, vox_ml);
     RampParams rp;
@@ -846,7 +884,7 @@ int anm_load_pet(anm_ctx* c, const float* bq_per_ml, int pnx, int pny, int pnz, 
     float ms = 0;
     cudaEventElapsedTime(&ms, e0, e1);
     c->ms_load_pet = ms;
-    if (flags & 1u) { cudaEventDestroy(e0); cudaEventDestroy(e1); cudaEventDestroy(e2); return fail(c, ANM_E_ARG, "pet: values must be finite and >= 0"); }
+    if (flags & 1u) return fail(c, ANM_E_ARG, "pet: values must be finite and >= 0");
     int rc;
     try {
         rc = build_alias(c, c->scratch.p);
@@ -856,7 +894,6 @@ int anm_load_pet(anm_ctx* c, const float* bq_per_ml, int pnx, int pny, int pnz, 
     cudaEventRecord(e2, c->stream);
     cudaEventSynchronize(e2);
     cudaEventElapsedTime(&ms, e0, e2);
-    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaEventDestroy(e2);
     c->ms_setup += ms;
     if (rc != ANM_OK) return rc;
     if (total_activity_Bq) *total_activity_Bq = total;
@@ -1141,7 +1178,8 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     // voxels -- a point source or a handful of active voxels -- and 32 same-address atomics per SOURCE trip would
     // serialise at the L2 (measured: 160 ms -> 18 ms per 1e8 histories on cfg1 with positron energy)
     const bool hot_source = c->opt.positron_ke_MeV > 0 && (c->point_source || c->n_alias < 1024u);
-    const bool S = c->opt.collect_stats != 0, W = c->opt.warp_aggregate == 1 || (c->opt.warp_aggregate == 0 && hot_source && !EL && !HB);
+    // (an explicit tally = 2 is a request too: it keeps the automatic aggregation off; tally = 2 with warp_aggregate = 1 is refused in anm_set_options)
+    const bool S = c->opt.collect_stats != 0, W = c->opt.warp_aggregate == 1 || (c->opt.warp_aggregate == 0 && hot_source && !EL && !HB && c->opt.tally != 2);
     // tile-binned tally: on request only -- measured +3 % on cfg4 (630 MB volumes) and 0.43x on cfg3, the
     // tile counters' same-address atomics bound it; needs the event pool, the batch estimator and local electrons
     const bool can_bin = schedule == 2 && !EL && !HB && !W;
@@ -1172,14 +1210,17 @@ int anm_run(anm_ctx* c, uint64_t n_decays, uint64_t seed) {
     // queues below 32 entries in every warp at the same time) costs ~0.25 ms whatever its size; with G batches per launch
     // that cost is paid B / G times instead of B times.  Same histories, same per-batch tallies.
     // G = 1 for the history-based schedule and the tile-binned tally (its per-launch lists are per batch); else the largest group that keeps depth * G tally volumes within the memory budget, at most 256
-    // (8 bits of the meta word), G * nb < 2^32 histories per launch (2^26 with history-by-history scoring).
+    // (8 bits of the meta word), G * nb <= 0xF0000000 histories per launch (2^26 with history-by-history scoring).
     int G = 1;
     if (schedule == 2 && !BIN) {
-        const uint64_t hist_cap = HB ? (uint64_t)kHbhHistMask : 0xffffffffull;
+        // The launch's history counter is a 32-bit atomicAdd, and every warp adds to it a little past n_hist (its last
+        // request plus the one it has asked for ahead: <= 2 kChunk per warp, a few million over the whole grid).  The cap
+        // leaves 2^28 of headroom so that the counter can never wrap and hand out history 0 a second time.
+        const uint64_t hist_cap = HB ? (uint64_t)kHbhHistMask : kLaunchHistCap;
         uint64_t gmax = std::min<uint64_t>({(uint64_t)B, (uint64_t)kMaxGroup, std::max<uint64_t>(1, hist_cap / nb)});
         if (c->opt.batches_per_launch > 0) gmax = std::min<uint64_t>(gmax, (uint64_t)c->opt.batches_per_launch);
         else {
-            gmax = std::min<uint64_t>(gmax, std::max<uint64_t>(1, kBatchBudget / ((uint64_t)c->Vpad * 4 * 2)));      // auto
+            gmax = std::min<uint64_t>(gmax, (uint64_t)c->auto_group);      // auto: what anm_set_grid sized the tallies for
         }
         const int n_groups0 = (int)(((uint64_t)B + gmax - 1) / gmax);
         G = (B + n_groups0 - 1) / n_groups0;                           // even groups
@@ -1480,11 +1521,10 @@ int anm_measure_peaks(anm_ctx* c, uint64_t small_bytes, uint64_t large_bytes, an
     ANM_CUDA(c, cudaSetDevice(c->device));
     std::memset(out, 0, sizeof *out);
     cudaStream_t st = c->stream;
-    cudaEvent_t e0, e1;
-    ANM_CUDA(c, cudaEventCreate(&e0));
-    ANM_CUDA(c, cudaEventCreate(&e1));
+    Events<2> evs;
+    ANM_CUDA(c, evs.create());
+    const cudaEvent_t e0 = evs.e[0], e1 = evs.e[1];
     DevBuf<float> arr, sink;
-    struct Cleanup { DevBuf<float>&a, &b; cudaEvent_t &e0, &e1; ~Cleanup() { a.release(); b.release(); cudaEventDestroy(e0); cudaEventDestroy(e1); } } cleanup{arr, sink, e0, e1};
     ANM_CUDA(c, sink.alloc(4));
     const int blocks = c->num_sms * 2;            // 64 resident warps per SM
     const double threads = (double)blocks * kPeakThreads;
@@ -1528,19 +1568,50 @@ int anm_measure_peaks(anm_ctx* c, uint64_t small_bytes, uint64_t large_bytes, an
         if (rc != ANM_OK) return rc;
         out->philox_gblocks = threads * nb / sec * 1e-9;
     }
+    DevBuf<float> arr2;
     for (int k = 0; k < 2; ++k) {
         const size_t n = (size_t)(sizes[k] / 4);
         out->bytes[k] = sizes[k];
         ANM_CUDA(c, arr.alloc(n));
         ANM_CUDA(c, cudaMemsetAsync(arr.p, 0, n * 4, st));
         const unsigned n32 = (unsigned)std::min<size_t>(n, 0xffffffffu);
-        const int trips = 256;
-        rc = timed([&] { gather_kernel<<<blocks, kPeakThreads, 0, st>>>((const uint32_t*)arr.p, n32, trips, (unsigned*)sink.p); }, &sec);
+        const int accesses = 2048;                 // per thread and launch, whatever the depth
+        // sweep of the accesses in flight per thread (full occupancy throughout): the best rate is the denominator
+        const int depths[4] = {4, 8, 16, 32};
+        for (int d = 0; d < 4; ++d) {
+            const int trips = accesses / depths[d];
+            rc = timed([&] {
+                const uint32_t* a = (const uint32_t*)arr.p; unsigned* o = (unsigned*)sink.p;
+                switch (depths[d]) {
+                    case 4: gather_kernel<4><<<blocks, kPeakThreads, 0, st>>>(a, n32, trips, o); break;
+                    case 8: gather_kernel<8><<<blocks, kPeakThreads, 0, st>>>(a, n32, trips, o); break;
+                    case 16: gather_kernel<16><<<blocks, kPeakThreads, 0, st>>>(a, n32, trips, o); break;
+                    default: gather_kernel<32><<<blocks, kPeakThreads, 0, st>>>(a, n32, trips, o); break;
+                } }, &sec);
+            if (rc != ANM_OK) return rc;
+            const double g = threads * trips * depths[d] / sec * 1e-9;
+            if (g > out->gather_gps[k]) { out->gather_gps[k] = g; out->gather_in_flight[k] = depths[d]; }
+        }
+        for (int d = 0; d < 4; ++d) {
+            const int trips = accesses / 4 / depths[d];
+            rc = timed([&] {
+                switch (depths[d]) {
+                    case 4: red_kernel<4><<<blocks, kPeakThreads, 0, st>>>(arr.p, n32, trips); break;
+                    case 8: red_kernel<8><<<blocks, kPeakThreads, 0, st>>>(arr.p, n32, trips); break;
+                    case 16: red_kernel<16><<<blocks, kPeakThreads, 0, st>>>(arr.p, n32, trips); break;
+                    default: red_kernel<32><<<blocks, kPeakThreads, 0, st>>>(arr.p, n32, trips); break;
+                } }, &sec);
+            if (rc != ANM_OK) return rc;
+            const double r = threads * trips * depths[d] / sec * 1e-9;
+            if (r > out->red_gps[k]) { out->red_gps[k] = r; out->red_in_flight[k] = depths[d]; }
+        }
+        // both at once over two arrays of this size (loads from one, REDs into the other)
+        ANM_CUDA(c, arr2.alloc(n));
+        ANM_CUDA(c, cudaMemsetAsync(arr2.p, 0, n * 4, st));
+        const int mtrips = 64;
+        rc = timed([&] { mix_kernel<<<blocks, kPeakThreads, 0, st>>>((const uint32_t*)arr.p, arr2.p, n32, mtrips, (unsigned*)sink.p); }, &sec);
         if (rc != ANM_OK) return rc;
-        out->gather_gps[k] = threads * trips * kGatherInFlight / sec * 1e-9;
-        rc = timed([&] { red_kernel<<<blocks, kPeakThreads, 0, st>>>(arr.p, n32, trips / 4); }, &sec);
-        if (rc != ANM_OK) return rc;
-        out->red_gps[k] = threads * (trips / 4) * kGatherInFlight / sec * 1e-9;
+        out->mix_gps[k] = threads * mtrips * (kMixGathers + kMixReds) / sec * 1e-9;
     }
     return ANM_OK;
 }

@@ -1,12 +1,16 @@
 // anm_kernels.cuh -- device code of libanm.so (sm_100a).  Hand-written CUDA; no oracle code is shared.
 //
 // Kernels
-//   transport_kernel : source sampling + Woodcock photon transport + fp32 RED tally
-//   fold_kernel      : per-batch fold  sum += x, sumsq += x^2, x = 0, organ partial sums   (A10)
+//   transport_pool_kernel / transport_kernel : source sampling + Woodcock photon transport + fp32 RED tally
+//                      (the two schedules below)
+//   fold_group_kernel : the G per-batch tallies of one launch folded in one pass: sum += x, sumsq += x^2, x = 0,
+//                      organ partial sums per batch (A10);  fold_kernel: the same for a single batch tally;
+//                      bin_fold_kernel: the same from the tile-binned deposit lists (anm_options.tally = 2)
 //   finalize_kernel  : organ Eq. 3 accumulators, organ energy / mass / counts, total energy (A11)
 //   readout_kernel   : dose / dose rate / relative sigma read-out                           (A11)
 //   dose_max_kernel, run_sigma_kernel : run-level RMS relative sigma above 10 % / 50 % of the maximum dose (A11)
-//   pack_texels / rho_max / hull_box / organ_mass kernels : set-up (A0); the alias table is in anm_alias.cuh,
+//   pack_texels / pack_texels16 (the exact 16-bit texel copy, anm_options.texel_bits) / rho_max / rho_max_outside /
+//   hull_box / organ_mass kernels : set-up (A0); the alias table is in anm_alias.cuh,
 //                      the image front end in anm_frontend.cuh
 //   electron_walk (device function) + electron_trace_kernel : secondary electrons
 //   hbh_push / hbh_flush (device functions)                 : history-by-history scoring (NEXT-4)

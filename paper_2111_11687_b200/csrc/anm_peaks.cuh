@@ -5,6 +5,7 @@
 //   philox_kernel  back-to-back Philox4x32-10 blocks (the generator of the kernels)        -> blocks / s
 //   gather_kernel  random 4-byte ld.global.nc over an array (the texel fetch)              -> loads / s
 //   red_kernel     random fp32 RED.ADD over an array (the tally)                          -> atomics / s
+//   mix_kernel     both at once, 5 loads : 2 REDs over two arrays (the transport's mix)    -> accesses / s
 // each at two array sizes: one that fits the 126 MB L2 (cfg3's 105 MB volumes) and one that does not (cfg4's 630 MB).
 #pragma once
 #include <cstdint>
@@ -53,29 +54,53 @@ philox_chain_kernel(const __grid_constant__ TransportParams p, unsigned* __restr
     if ((c.x ^ c.y ^ c.z ^ c.w) == 0x12345678u) out[0] = c.x;
 }
 
-// kGatherInFlight independent random loads per thread per trip
-constexpr int kGatherInFlight = 8;
+// IF independent random accesses per thread per trip.  The host sweeps IF over {4, 8, 16, 32} at full occupancy
+// (64 resident warps per SM) and keeps the best rate: the denominators are then what the memory system gives when it
+// is saturated, not what one arbitrary depth happens to reach.
+template <int IF>
 __global__ void __launch_bounds__(kPeakThreads)
 gather_kernel(const uint32_t* __restrict__ a, unsigned n, int trips, unsigned* __restrict__ out) {
     unsigned s = (blockIdx.x * kPeakThreads + threadIdx.x) * 2654435761u + 0x9E3779B9u;
     unsigned acc = 0;
     for (int t = 0; t < trips; ++t) {
-        unsigned v[kGatherInFlight];
+        unsigned v[IF];
 #pragma unroll
-        for (int k = 0; k < kGatherInFlight; ++k) v[k] = __ldg(a + __umulhi(peak_next(s), n));
+        for (int k = 0; k < IF; ++k) v[k] = __ldg(a + __umulhi(peak_next(s), n));
 #pragma unroll
-        for (int k = 0; k < kGatherInFlight; ++k) acc += v[k];
+        for (int k = 0; k < IF; ++k) acc += v[k];
     }
     if (acc == 0x12345678u) out[0] = acc;
 }
 
+template <int IF>
 __global__ void __launch_bounds__(kPeakThreads)
 red_kernel(float* __restrict__ a, unsigned n, int trips) {
     unsigned s = (blockIdx.x * kPeakThreads + threadIdx.x) * 2654435761u + 0x9E3779B9u;
     for (int t = 0; t < trips; ++t) {
 #pragma unroll
-        for (int k = 0; k < kGatherInFlight; ++k) atomicAdd(a + __umulhi(peak_next(s), n), 1.0f);
+        for (int k = 0; k < IF; ++k) atomicAdd(a + __umulhi(peak_next(s), n), 1.0f);
     }
+}
+
+// The transport kernel's mix: per trip kMixGathers random 4-byte loads from one array (texels) and kMixReds fp32 REDs
+// into ANOTHER array of the same size (the tally) -- 5 : 2, cfg3's 15.6 sub-steps : 6.2 deposits per decay.  Both
+// streams compete for the same L2 / HBM, so the sum of the separate gather and RED fractions overstates the headroom;
+// this is the rate (loads + REDs per second) with both in flight.
+constexpr int kMixGathers = 10, kMixReds = 4;
+__global__ void __launch_bounds__(kPeakThreads)
+mix_kernel(const uint32_t* __restrict__ a, float* __restrict__ b, unsigned n, int trips, unsigned* __restrict__ out) {
+    unsigned s = (blockIdx.x * kPeakThreads + threadIdx.x) * 2654435761u + 0x9E3779B9u;
+    unsigned acc = 0;
+    for (int t = 0; t < trips; ++t) {
+        unsigned v[kMixGathers];
+#pragma unroll
+        for (int k = 0; k < kMixGathers; ++k) v[k] = __ldg(a + __umulhi(peak_next(s), n));
+#pragma unroll
+        for (int k = 0; k < kMixReds; ++k) atomicAdd(b + __umulhi(peak_next(s), n), 1.0f);
+#pragma unroll
+        for (int k = 0; k < kMixGathers; ++k) acc += v[k];
+    }
+    if (acc == 0x12345678u) out[0] = acc;
 }
 
 }  // namespace anm

@@ -77,7 +77,8 @@ def merge_stats(stats: dict, device, group=None) -> dict:
 def run_sharded(sim, n_decays: int, seed: int, n_batches: int, options: dict, group=None) -> Shard:
     """Run this rank's shard of the logical run (n_decays, n_batches, seed) on `sim` (inputs already loaded) and merge:
     afterwards every rank's `sim.get_*` returns the result of the whole run.  `options`: the anm_options fields other
-    than n_batches / history_offset."""
+    than n_batches / history_offset.  Where several ranks share one device (or one process holds several contexts), give
+    each `sim.set_tally_budget(...)` before `set_grid`: every context otherwise sets 4 GiB of batch tallies aside."""
     import torch.distributed as dist
     rank, world = dist.get_rank(group), dist.get_world_size(group)
     shard = plan_shards(n_decays, n_batches, world)[rank]

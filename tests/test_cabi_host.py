@@ -40,6 +40,7 @@ def test_struct_sizes_match_header():
     assert C.sizeof(binding.anm_organ) == 5 * 8 + 2 * 8
     assert C.sizeof(binding.anm_stats) == 3 * 8 + 10 * 8 + 4 * 8 + 8 + 2 * 8 + 2 * 8 + 11 * 8
     assert C.sizeof(binding.anm_hu_ramp) == 8 + 16 * 8 + 16 * 8 + 16 * 4 + 8
+    assert C.sizeof(binding.anm_peaks) == 3 * 8 + 2 * 8 + 2 * 8 + 2 * 8 + 2 * 8 + 4 * 4
 
 
 def test_default_options():
@@ -77,6 +78,18 @@ def test_null_ctx_calls_do_not_crash():
     assert lib.anm_destroy(None) == 0
     assert lib.anm_run(None, 10, 1) == -1
     assert lib.anm_last_error(None) == b"null context"
+    assert lib.anm_set_tally_budget(None, 1 << 30) == -1
+
+
+def test_static_summary_checks_its_arguments_before_it_touches_the_gpu():
+    """anm_organ_summary_static validates sizes and pointers first: these refusals need no device."""
+    lib = binding.load()
+    err = C.create_string_buffer(256)
+    assert lib.anm_organ_summary_static(None, None, None, 16, 256, 10.0, None, None, err, len(err)) == -1
+    assert b"at most 255 organs" in err.value
+    assert lib.anm_organ_summary_static(None, None, None, 16, 4, 10.0, None, None, err, len(err)) == -1
+    assert b"must not be NULL" in err.value
+    assert lib.anm_organ_summary_static(None, None, None, 16, 4, 10.0, None, None, None, 0) == -1     # no buffer: still no crash
 
 
 def test_product_does_not_import_oracle():

@@ -322,6 +322,48 @@ def test_batch_groups_keep_every_batch_apart(anm, tables, case):
     assert np.count_nonzero(ref[3].sum(1)) == B
 
 
+def test_launch_history_cap_leaves_the_counter_headroom(anm, tables):
+    """A launch hands out history indices from a 32-bit counter that every warp overshoots a little at the end, so a
+    batch group may cover at most 0xF0000000 histories (include/anm.h, batches_per_launch): two batches of 0x78000000
+    share a launch, two of one more do not.  At the cap every history must still run exactly once: each photon ends
+    in exactly one of escape / photoelectric absorption / cutoff, so a wrapped counter (histories handed out twice)
+    would show as more endings than photons."""
+    cfg = anm_inputs.make_config(0, 2)                # single photon per history, 16^3 voxels of water
+    half = 0x78000000
+    for nb, want_g in ((half, 2), (half + 1, 1)):
+        with anm.Simulation(0) as sim:
+            sim.load_config(cfg, tables, n_batches=2, collect_stats=1)
+            sim.run(2 * nb, 3)
+            st = sim.get_stats()
+        assert st["batches_per_launch"] == want_g, (nb, st["batches_per_launch"])
+        assert st["n_decays"] == 2 * nb
+        assert st["n_escaped"] + st["n_pe"] + st["n_cutoff"] == 2 * nb * cfg["photons_per_decay"], st
+
+
+def test_tally_budget_sizes_the_batch_groups(anm, tables):
+    """anm_set_tally_budget before anm_set_grid: the automatic batches per launch follow the budget (two sets of G
+    volumes must fit it), the floor is one volume per set, and the results do not depend on it."""
+    cfg = anm_inputs.make_config(3, 4)
+    vol = (int(np.prod(cfg["shape"])) + 3) // 4 * 4 * 4          # bytes of one tally volume
+    n, B = 240_000, 24
+    out = {}
+    for budget, want_g in ((0, B), (2 * 6 * vol, 6), (1, 1)):
+        with anm.Simulation(0) as sim:
+            sim.set_tally_budget(budget)
+            sim.load_config(cfg, tables, n_batches=B, collect_stats=1)
+            sim.run(n, 5)
+            st = sim.get_stats()
+            assert st["batches_per_launch"] == want_g, (budget, st["batches_per_launch"])
+            out[budget] = (st, sim.get_energy().astype(np.float64), sim.get_organ_doses())
+    ref = out[0]
+    for budget in (2 * 6 * vol, 1):
+        st, e, org = out[budget]
+        for key in ("n_steps", "n_real", "n_pe", "n_compton", "n_rayleigh", "n_escaped", "n_cutoff"):
+            assert st[key] == ref[0][key], (budget, key)
+        assert np.allclose(e, ref[1], rtol=2e-5, atol=1e-4)
+        assert np.allclose(org["mean_Gy_per_decay"], ref[2]["mean_Gy_per_decay"], rtol=1e-6)
+
+
 def test_one_context_many_runs_with_changing_options(anm, tables):
     """The ctx keeps its per-batch tallies between runs (the folds leave them zero) and re-sizes them only when a run
     needs more: a sequence of runs with different kernels, group sizes, pipelines and a grid change in ONE context must

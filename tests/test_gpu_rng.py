@@ -33,3 +33,18 @@ def test_device_philox_known_answers_and_oracle():
             key = [seed & 0xffffffff, seed >> 32]
             want = np.array([O.philox4x32_10(c, key) for c in ctr])
             assert np.array_equal(got, want)
+
+
+def test_peaks_sweep_reports_saturated_rates():
+    """anm_measure_peaks (include/anm.h): the gather / RED denominators are the best of a depth sweep, and the combined
+    loads + REDs rate cannot beat the faster of the two alone and stays within a small factor of the slower one."""
+    import paper_2111_11687_b200 as pkg
+    with pkg.Simulation(0) as sim:
+        p = sim.measure_peaks(64 << 20, 512 << 20)
+    for k in range(2):
+        assert p["gather_in_flight"][k] in (4, 8, 16, 32) and p["red_in_flight"][k] in (4, 8, 16, 32)
+        assert p["gather_gps"][k] > 0 and p["red_gps"][k] > 0 and p["mix_gps"][k] > 0
+        # (two arrays: twice the footprint of the single-array runs, so the mix may sit well below either of them)
+        assert 0.2 * min(p["gather_gps"][k], p["red_gps"][k]) < p["mix_gps"][k] < 1.05 * max(p["gather_gps"][k], p["red_gps"][k])
+    assert p["gather_gps"][0] > p["gather_gps"][1] and p["red_gps"][0] > p["red_gps"][1]     # L2-resident beats HBM
+    assert p["issue_gtis"] > 1e3 and p["philox_gblocks"] > 10
