@@ -222,7 +222,12 @@ typedef struct {
 #define ANM_MAX_RAMP_NODES 16
 typedef struct {
     int32_t n_nodes;          /* 2..ANM_MAX_RAMP_NODES */
-    int32_t reserved0;
+    int32_t density_bits;     /* the grid the densities are rounded to (to nearest): 0 or 20 = 2^-20 g/cm^3, the 32-bit
+                                 texel's (every phantom); 12 = 2^-12 g/cm^3, on which the exact 16-bit texel copy exists
+                                 (anm_options.texel_bits) as long as every density is below 2 g/cm^3 -- HU < 1809 on the
+                                 default ramp; otherwise the run uses the 32-bit texels as before.  The rounding error,
+                                 <= 1.2e-4 g/cm^3, is a quarter of what one HU step resolves (reading C30).
+                                 anm_default_hu_ramp sets 0.  Other values: ANM_E_ARG */
     double hu[ANM_MAX_RAMP_NODES];
     double rho[ANM_MAX_RAMP_NODES];
     int32_t material[ANM_MAX_RAMP_NODES];
@@ -257,7 +262,8 @@ int anm_load_phantom(anm_ctx* c, const uint8_t* material, const float* density_g
  * simulation grid ("The CT images are resampled to obtain the same size as the PET images") -- the
  * value of a simulation voxel is the volume-weighted MEAN of the piecewise-constant HU image over that voxel, with
  * ramp->hu_outside wherever the voxel reaches beyond the image -- and converted to (material, density) by `ramp`
- * (NULL = anm_default_hu_ramp), densities rounded to the 2^-20 g/cm^3 texel grid.  One fused kernel; fp64 weights
+ * (NULL = anm_default_hu_ramp), densities rounded to the 2^-20 g/cm^3 texel grid, or to the 2^-12 grid on request
+ * (anm_hu_ramp.density_bits = 12: the phantom can then use the 16-bit texels).  One fused kernel; fp64 weights
  * and accumulation.  ANM_E_ARG for a bad ramp or sizes; ANM_E_STATE before anm_set_grid.
  * anm_get_phantom returns the (material, density) volumes the ctx holds (after anm_load_ct or anm_load_phantom). */
 int anm_default_hu_ramp(anm_hu_ramp* r);   /* air / lung / water / compact bone; numbers approximate */

@@ -83,18 +83,23 @@ def hu_to_material_density(hu, ramp: dict):
     return mats[k].astype(np.uint8), rho
 
 
-def quantize_density(rho) -> np.ndarray:
-    """DESIGN.md reading C18: densities live on the 2^-20 g/cm^3 texel grid (round to nearest, at most 2^24 - 1)."""
-    counts = np.minimum(np.rint(np.asarray(rho, np.float64) / DENSITY_STEP), float(2 ** 24 - 1))
-    return (counts * DENSITY_STEP).astype(np.float32)
+def quantize_density(rho, bits: int = 20) -> np.ndarray:
+    """DESIGN.md reading C18: densities live on the 2^-20 g/cm^3 texel grid (round to nearest, at most 2^24 - 1 counts).
+    Reading C30: bits = 12 rounds to the 2^-12 g/cm^3 grid instead (to nearest, at most 2^16 - 1 steps) -- every value is
+    then also on the 2^-20 grid, with its low 8 bits zero."""
+    assert bits in (12, 20)
+    step = 2.0 ** -bits
+    counts = np.minimum(np.rint(np.asarray(rho, np.float64) / step), float(2 ** (bits + 4) - 1))
+    return (counts * step).astype(np.float32)
 
 
 def ct_to_phantom(hu_ct, ct_spacing, ct_offset, shape, spacing, ramp: dict):
     """PAPER.md:L81 then L65: resample the CT to the simulation grid, then HU -> (material, density).
+    ramp["density_bits"] (absent or 0: 20) chooses the density grid, reading C30.
     Returns (material uint8 [nz][ny][nx], density float32 on the texel grid, resampled HU float64)."""
     hu = resample_mean(hu_ct, ct_spacing, ct_offset, shape, spacing, float(ramp["hu_outside"]))
     mat, rho = hu_to_material_density(hu, ramp)
-    return mat, quantize_density(rho), hu
+    return mat, quantize_density(rho, int(ramp.get("density_bits", 0)) or 20), hu
 
 
 def pet_to_activity(bqml_pet, pet_spacing, pet_offset, shape, spacing):

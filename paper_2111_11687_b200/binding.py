@@ -86,7 +86,7 @@ ANM_MAX_RAMP_NODES = 16
 
 
 class anm_hu_ramp(C.Structure):
-    _fields_ = [("n_nodes", C.c_int32), ("reserved0", C.c_int32), ("hu", C.c_double * ANM_MAX_RAMP_NODES),
+    _fields_ = [("n_nodes", C.c_int32), ("density_bits", C.c_int32), ("hu", C.c_double * ANM_MAX_RAMP_NODES),
                 ("rho", C.c_double * ANM_MAX_RAMP_NODES), ("material", C.c_int32 * ANM_MAX_RAMP_NODES),
                 ("hu_outside", C.c_double)]
 
@@ -102,12 +102,16 @@ class anm_hu_ramp(C.Structure):
         for k in range(n - 1):
             r.material[k] = int(ramp["material"][k])
         r.hu_outside = float(ramp["hu_outside"])
+        r.density_bits = int(ramp.get("density_bits", 0))
         return r
 
     def as_dict(self) -> dict:
         n = self.n_nodes
-        return {"hu": [self.hu[k] for k in range(n)], "rho": [self.rho[k] for k in range(n)],
-                "material": [self.material[k] for k in range(n - 1)], "hu_outside": self.hu_outside}
+        d = {"hu": [self.hu[k] for k in range(n)], "rho": [self.rho[k] for k in range(n)],
+             "material": [self.material[k] for k in range(n - 1)], "hu_outside": self.hu_outside}
+        if self.density_bits:
+            d["density_bits"] = int(self.density_bits)
+        return d
 
 
 def lib_path() -> str:

@@ -758,6 +758,9 @@ int anm_load_ct(anm_ctx* c, const int16_t* hu, int cnx, int cny, int cnz, double
         rp.hu[k] = ramp->hu[k]; rp.rho[k] = ramp->rho[k]; rp.material[k] = ramp->material[k];
     }
     if (!std::isfinite(ramp->hu_outside)) return fail(c, ANM_E_ARG, "ct: hu_outside must be finite");
+    if (ramp->density_bits != 0 && ramp->density_bits != 12 && ramp->density_bits != 20) return fail(c, ANM_E_ARG, "ct: ramp density_bits must be 0 (= 20), 12 or 20");
+    if (ramp->density_bits == 12) { rp.q_scale = 4096.0; rp.q_cap = 65535.0; rp.q_mult = 256.0; }
+    else { rp.q_scale = 1048576.0; rp.q_cap = 16777215.0; rp.q_mult = 1.0; }
     rp.hu_outside = ramp->hu_outside;
     for (int k = 0; k + 1 < ramp->n_nodes; ++k) rp.inv_dhu[k] = 1.0 / (ramp->hu[k + 1] - ramp->hu[k]);
     ANM_CUDA(c, cudaSetDevice(c->device));

@@ -31,6 +31,9 @@ struct RampParams {
     double inv_dhu[kMaxRampNodes];      // 1 / (hu[k+1] - hu[k])
     int material[kMaxRampNodes];
     double hu_outside;
+    // density grid (readings C18, C30): texel counts = min(rint(rho * q_scale), q_cap) * q_mult
+    // 2^-20 grid: 1048576, 16777215, 1;  2^-12 grid: 4096, 65535, 256 (the same word with its low 8 bits zero)
+    double q_scale, q_cap, q_mult;
 };
 
 struct ResampleParams {
@@ -109,7 +112,7 @@ resample_kernel(const T* __restrict__ src, const AxisOverlap* __restrict__ tab, 
             const double f = (hc - ramp.hu[k]) * ramp.inv_dhu[k];
             const double rho = ramp.rho[k] + f * (ramp.rho[k + 1] - ramp.rho[k]);
             const unsigned m = (unsigned)ramp.material[k];
-            const double counts = fmin(rint(rho * 1048576.0), 16777215.0);
+            const double counts = fmin(rint(rho * ramp.q_scale), ramp.q_cap) * ramp.q_mult;
             out_texels[idx] = (m << 24) | (unsigned)counts;
             mm = max(mm, m);
         } else {
@@ -198,7 +201,7 @@ resample_fast_kernel(const T* __restrict__ src, const AxisOverlap* __restrict__ 
                 const double f = (hc - ramp.hu[k]) * ramp.inv_dhu[k];
                 const double rho = ramp.rho[k] + f * (ramp.rho[k + 1] - ramp.rho[k]);
                 const unsigned m = (unsigned)ramp.material[k];
-                const double counts = fmin(rint(rho * 1048576.0), 16777215.0);
+                const double counts = fmin(rint(rho * ramp.q_scale), ramp.q_cap) * ramp.q_mult;
                 out_texels[idx] = (m << 24) | (unsigned)counts;
                 mm = max(mm, m);
             } else {

@@ -114,3 +114,29 @@ def test_round_trip_recovers_the_phantom():
     act, tot = fe.pet_to_activity(img["pet_bqml"], img["pet_spacing_mm"], img["pet_offset_mm"], cfg["shape"], cfg["spacing_mm"])
     assert tot == pytest.approx(anm_inputs.phantoms.TOTAL_ACTIVITY_BQ, rel=1e-6)
     assert np.allclose(act / act.sum(), cfg["activity"].astype(np.float64) / cfg["activity"].astype(np.float64).sum(), rtol=1e-6, atol=0)
+
+
+def test_density_grid_of_reading_c30():
+    """quantize_density(rho, 12): every value on the 2^-12 g/cm^3 grid (hence on the 2^-20 grid with the low 8 bits of its
+    count zero: the word the 16-bit texel holds exactly), to nearest (error <= 2^-13), ties and the cap as for 20 bits;
+    the default is unchanged; ct_to_phantom takes the choice from ramp["density_bits"] and changes nothing else."""
+    rho = np.concatenate([np.random.default_rng(5).uniform(0.0, 2.2, 20000), [0.0, 0.0012, 1.0, 1.0 + 0.4 * 2.0 ** -12, 1.0 + 0.6 * 2.0 ** -12, 40.0]])
+    q12 = fe.quantize_density(rho, 12).astype(np.float64)
+    c20 = q12 * 2.0 ** 20
+    assert np.array_equal(c20, np.rint(c20)) and np.all(c20.astype(np.int64) % 256 == 0)
+    inside = rho < 15.9
+    assert np.max(np.abs(q12[inside] - rho[inside])) <= 2.0 ** -13 + 1e-15
+    assert q12[-3] == 1.0 and q12[-2] == 1.0 + 2.0 ** -12 and q12[-1] == (2 ** 16 - 1) * 2.0 ** -12
+    assert q12[-5] == round(0.0012 * 4096) / 4096                       # air: 5 steps of 2^-12 = 0.00122 g/cm^3
+    assert np.array_equal(fe.quantize_density(rho), fe.quantize_density(rho, 20))
+    assert np.max(np.abs(fe.quantize_density(rho, 20).astype(np.float64)[inside] - rho[inside])) <= 2.0 ** -21 + 2.0 ** -24   # + float32 storage
+    # through ct_to_phantom: same materials, same resampled HU, densities = the fine ones re-rounded from the SAME rho(HU)
+    hu = np.random.default_rng(6).integers(-1024, 1700, size=(7, 6, 5)).astype(np.int16)
+    ramp = {"hu": [-1024.0, -974.0, -724.0, 101.0, 1976.0], "rho": [0.001, 0.044, 0.302, 1.101, 2.088], "material": [0, 1, 2, 3], "hu_outside": -1024.0}
+    m20, r20, h20 = fe.ct_to_phantom(hu, (2.0, 2.0, 2.0), (0, 0, 0), (5, 6, 7), (2.0, 2.0, 2.0), ramp)
+    m12, r12, h12 = fe.ct_to_phantom(hu, (2.0, 2.0, 2.0), (0, 0, 0), (5, 6, 7), (2.0, 2.0, 2.0), dict(ramp, density_bits=12))
+    assert np.array_equal(m20, m12) and np.array_equal(h20, h12)
+    _, rho_exact = fe.hu_to_material_density(h12, ramp)
+    assert np.array_equal(r12, fe.quantize_density(rho_exact, 12))
+    assert np.max(np.abs(r12.astype(np.float64) - r20)) <= 2.0 ** -13 + 2.0 ** -20
+    assert abs(r12.astype(np.float64).sum() / r20.astype(np.float64).sum() - 1.0) < 2.0 ** -13      # total mass: within the per-voxel bound

@@ -52,8 +52,10 @@ def compare_front_end(anm, cfg, img, device_inputs=False):
     diff = mat_g != mat_o
     assert not (diff & ~near_node).any(), int((diff & ~near_node).sum())
     assert diff.sum() <= 4
-    counts_g = np.rint(rho_g.astype(np.float64) * 2 ** 20)
-    counts_o = np.rint(rho_o.astype(np.float64) * 2 ** 20)
+    bits = int(img["ramp"].get("density_bits", 0)) or 20       # the density grid (reading C30); counts in ITS steps
+    counts_g = rho_g.astype(np.float64) * 2 ** bits
+    counts_o = rho_o.astype(np.float64) * 2 ** bits
+    assert np.array_equal(counts_g, np.rint(counts_g)) and np.array_equal(counts_o, np.rint(counts_o))     # both on the grid
     assert np.max(np.abs(counts_g - counts_o)[~diff]) <= 1
     assert (counts_g != counts_o).mean() < 1e-3           # a 1-count difference needs rho*2^20 within ~1e-9 of a half-integer
     a32 = act_o.astype(np.float32).reshape(-1)
@@ -72,6 +74,35 @@ def test_front_end_small_ragged(anm, device_inputs):
     cfg = anm_inputs.make_config(3, 4)
     img = anm_inputs.make_ct_pet(cfg, ct_shape=(151, 131, 173), ct_margin_mm=(13.0, -9.0, 5.5))
     compare_front_end(anm, cfg, img, device_inputs)
+
+
+def test_front_end_on_the_coarse_density_grid_reaches_the_16_bit_texels(anm, tables):
+    """anm_hu_ramp.density_bits = 12 (reading C30): material ids as before, densities exactly the oracle's on the
+    2^-12 g/cm^3 grid -- and a phantom made from a CT image then runs on the exact 16-bit texel copy
+    (anm_stats.texel_bits), which the 2^-20 grid never allows.  The synthetic patient stays below 2 g/cm^3."""
+    cfg = anm_inputs.make_config(3, 4)
+    img = anm_inputs.make_ct_pet(cfg, ct_shape=(151, 131, 173), ct_margin_mm=(13.0, -9.0, 5.5))
+    img12 = dict(img, ramp=dict(img["ramp"], density_bits=12))
+    _, rho_o, _, _, _ = compare_front_end(anm, cfg, img12)
+    assert float(np.max(rho_o)) < 2.0
+    bits = {}
+    for name, im in (("fine", img), ("coarse", img12)):
+        with anm.Simulation(0) as sim:
+            sim.set_grid(cfg["shape"], cfg["spacing_mm"])
+            sim.load_ct(im["ct_hu"], im["ct_shape"], im["ct_spacing_mm"], im["ct_offset_mm"], im["ramp"])
+            sim.load_pet(im["pet_bqml"], im["pet_shape"], im["pet_spacing_mm"], im["pet_offset_mm"])
+            sim.set_physics_tables(tables)
+            sim.set_options(n_batches=10, collect_stats=1, positron_ke_MeV=0.2498)
+            sim.run(200_000, 9)
+            st = sim.get_stats()
+            bits[name] = (int(st["texel_bits"]), st["deposited_MeV"])
+    assert bits["fine"][0] == 32 and bits["coarse"][0] == 16
+    assert abs(bits["coarse"][1] / bits["fine"][1] - 1.0) < 5e-3        # densities moved by <= 1.2e-4 g/cm^3: the same physics
+    with anm.Simulation(0) as sim:
+        sim.set_grid(cfg["shape"], cfg["spacing_mm"])
+        with pytest.raises(anm.AnmError) as ei:
+            sim.load_ct(img["ct_hu"], img["ct_shape"], img["ct_spacing_mm"], img["ct_offset_mm"], dict(img["ramp"], density_bits=16))
+        assert ei.value.code == -1
 
 
 def test_front_end_pet_on_its_own_grid(anm):
